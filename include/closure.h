@@ -1,0 +1,191 @@
+/*
+ * closure.h -- C ABI of libclosure_b200: the data-parallel hot path of CLOSURE
+ * (arXiv 2403.09990) on NVIDIA B200 (sm_100a).
+ *
+ * "PAPER.md:<n>" cites /root/reference/PAPER.md line n; "R-n" cites the numbered readings
+ * of silent / garbled passages in DESIGN.md.
+ *
+ * The path: boundary walks (Step II: Alg. 2, Alg. 3 PAPER.md:295-322,
+ * Alg. A8/A9 PAPER.md:1001-1099) -> stream compaction of boundary samples -> minimum
+ * enclosing geodesic ball (Step III).  Step I (initial poses S_0,
+ * PAPER.md:201, 217-219) is off the path and enters as data through closure_set_init.
+ *
+ * Conventions
+ *   - Plain C99, no exceptions cross the boundary.  Every call returns an int status:
+ *     CLOSURE_OK (0) or a negative CLOSURE_E* code; closure_last_error(h) gives the text of
+ *     the last failure on that handle (owned by the handle; valid until the next call on it).
+ *   - "host" pointers are ordinary CPU memory, "DEVICE" pointers are CUDA device memory of the
+ *     current device.  The caller owns every buffer it passes; inputs of closure_create /
+ *     closure_set_init are copied; outputs are written into caller-allocated buffers.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls marked
+ *     ASYNC only enqueue work on it and do not synchronise with the host.
+ *   - There is no CPU fallback and no other backend: without a usable CUDA device every
+ *     compute call returns CLOSURE_ECUDA.
+ *   - A pose is 12 doubles: R row-major (9) then t (3).  One sample record = 96 bytes.
+ */
+#ifndef CLOSURE_B200_H
+#define CLOSURE_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CLOSURE_ABI_VERSION 1
+
+/* status codes */
+#define CLOSURE_OK 0
+#define CLOSURE_EINVAL (-1)   /* bad enum / size / NULL / non-finite input / beta <= 0 / n_p_star > n_p */
+#define CLOSURE_EINIT (-2)    /* an initial pose is not inside the PURSE (PAPER.md:217-219 admit only such) */
+#define CLOSURE_ENOINIT (-3)  /* closure_sample before closure_set_init */
+#define CLOSURE_ECUDA (-4)    /* CUDA runtime failure (message in closure_last_error) */
+#define CLOSURE_ENOMEM (-5)
+#define CLOSURE_EUNSUPPORTED (-6) /* combination not built (e.g. n_p_star > 32) */
+
+/* residual g(x, y_i) -- eqs. (2)-(4).  Measurement row layouts (doubles):
+ *   CLOSURE_REPROJ_2D3D     [z(2) Z(3)]          g = z - Pi(K (R Z + t)), pixels; depth<=0 violates (R-10)
+ *   CLOSURE_REG_3D3D        [a(3) b(3)]          g = b - (R a + t)
+ *   CLOSURE_POSE_REG        [R_i(9 row-major) t_i(3)]   g = [vec(R)-vec(R_i); t-t_i], ONE bound per hypothesis
+ *   CLOSURE_POSE_REG_SPLIT  same rows; TWO bounds per hypothesis, betas[2i] on ||vec(R)-vec(R_i)||,
+ *                           betas[2i+1] on ||t-t_i||  (PURSEreg; R-13)
+ * Lambda_i = I throughout (R-14). */
+enum { CLOSURE_REPROJ_2D3D = 1, CLOSURE_REG_3D3D = 2, CLOSURE_POSE_REG = 3, CLOSURE_POSE_REG_SPLIT = 4 };
+
+/* which boundary is sampled: CLOSURE_MODE_ROT = Alg. 2 (fixed angular velocity, translation
+ * perturbations); CLOSURE_MODE_TRANS = Alg. A8 (fixed centre velocity, rotation perturbations). */
+enum { CLOSURE_MODE_ROT = 0, CLOSURE_MODE_TRANS = 1 };
+
+/* The paper's simulation-parameter tuple P (values PAPER.md:374, 440, 464). */
+typedef struct {
+    int mode;        /* CLOSURE_MODE_* */
+    int n_p;         /* N_P   perturbations per iteration, >= 1 */
+    int n_p_star;    /* N_P*  kept perturbations, 1..min(n_p, 32) */
+    int n_t;         /* N_T   ladder length, 1..64; Delta T_m = gamma^(m-1) */
+    double omega0;   /* base angular velocity magnitude (ROT) */
+    double v0;       /* base centre velocity magnitude (TRANS) */
+    double gamma;    /* time-step decay, in (0, 1] */
+    double t_p;      /* translation perturbation scale: uniform on [-t_p, t_p]^3 (R-6) */
+    double theta_p;  /* rotation perturbation scale (the paper's R_p): rotation vector uniform on
+                        [-theta_p, theta_p]^3 (R-6) */
+    int precision;   /* 64 (fp64, the parity path) or 32 (fp32 arithmetic, fp64 I/O) */
+    int reserved;
+} closure_params;
+
+typedef struct closure_s closure_t;   /* opaque; owns device copies of the instance and of S_0 */
+
+/* Fill *p with the defaults this build uses for `residual_type` (paper values where units carry
+ * over).  Returns CLOSURE_EINVAL on a bad type / NULL. */
+int closure_default_params(int residual_type, closure_params *p);
+
+/* Describe a PURSE  S = { (R,t) : ||g(x, y_i)|| <= beta_i } and upload it.
+ *   measurements  host, n rows in the layout of `residual_type`
+ *   betas         host, n bounds (2n for CLOSURE_POSE_REG_SPLIT), each finite and > 0
+ *   intrinsics    host, {fx, fy, cx, cy}; required for CLOSURE_REPROJ_2D3D, ignored (may be NULL) else
+ *   p             walk parameters (copied)
+ *   out           receives the handle; destroy with closure_destroy
+ * Synchronous (small H2D copy).  Errors: CLOSURE_EINVAL, CLOSURE_ECUDA, CLOSURE_ENOMEM. */
+int closure_create(int residual_type, const double *measurements, int n, const double *betas,
+                   const double *intrinsics, const closure_params *p, closure_t **out);
+
+/* Replace the walk parameters of an existing handle (same validation as closure_create). */
+int closure_set_params(closure_t *h, const closure_params *p);
+
+/* Give the initial pose set S_0 (output of Step I).  poses: host, n0 x 12.  Computes
+ * R_bar = proj_SO(3)(sum R_j) and t_bar = mean t_j on the host (Alg. 2 l.3-4),
+ * checks every pose against the PURSE (CLOSURE_EINIT if one is outside) and uploads.
+ * mean_out (host, 12 doubles, may be NULL) receives [R_bar, t_bar]. */
+int closure_set_init(closure_t *h, const double *poses, int n0, double *mean_out);
+
+/* Step II.  ASYNC.  Runs walkers w = walker_begin .. walker_begin + num_walkers - 1, each for
+ * exactly num_steps iterations of Alg. 2 (ROT) / Alg. A8 (TRANS) from S_0[w mod n0]
+ * (the paper's repeat(S_0, N_W)), with Philox4x32-10 randomness keyed by
+ * (seed; w, iteration, perturbation) (R-5) so that any walker can be replayed alone.
+ *   out_samples      DEVICE, num_walkers x 12 doubles: final (R*, t*)      (Alg. 2 l.30)
+ *   out_on_boundary  DEVICE, num_walkers bytes: 1 iff some iteration could not take the full
+ *                    step (m_0 > 1 or nothing feasible) (R-12)
+ *   out_trace        DEVICE or NULL, num_walkers x num_steps int32: per iteration
+ *                    m_0 | (j_{k_0} << 8), 0 when nothing was feasible (parity protocol)
+ * closure_sample(h, W, S, seed, samples, flags, stream) of the north star is the
+ * walker_begin = 0, out_trace = NULL case. */
+int closure_sample_range(closure_t *h, long long walker_begin, long long num_walkers, int num_steps,
+                         unsigned long long seed, double *out_samples, unsigned char *out_on_boundary,
+                         int *out_trace, void *cuda_stream);
+int closure_sample(closure_t *h, long long num_walkers, int num_steps, unsigned long long seed,
+                   double *out_samples, unsigned char *out_on_boundary, void *cuda_stream);
+
+/* Step II for a batch of independent instances in ONE launch (BASELINE config 5).  All handles
+ * must share residual type, walk parameters and precision; N and S_0 may differ.  Instance b runs
+ * walkers 0 .. walkers_per_instance-1 with seeds[b]; outputs are instance-major:
+ * out_samples[(b * walkers_per_instance + w) * 12], out_on_boundary[b * walkers_per_instance + w].
+ * handles / seeds: host arrays of n_instances.  ASYNC. */
+int closure_sample_batch(closure_t *const *handles, int n_instances, long long walkers_per_instance,
+                         int num_steps, const unsigned long long *seeds, double *out_samples,
+                         unsigned char *out_on_boundary, void *cuda_stream);
+
+/* Stable stream compaction of the samples whose flag is non-zero, in walker order.  ASYNC.
+ *   samples, flags   DEVICE, n x 12 doubles / n bytes
+ *   out_compacted    DEVICE, room for n x 12 doubles
+ *   out_count        DEVICE, one long long: number of kept samples */
+int closure_compact(closure_t *h, const double *samples, const unsigned char *flags, long long n,
+                    double *out_compacted, long long *out_count, void *cuda_stream);
+
+/* Step III result.  Geodesic distance on SO(3): arccos((tr(C^T R) - 1) / 2). */
+typedef struct {
+    double R[9];              /* centre rotation C^ (row-major) */
+    double t[3];              /* centre translation c^ */
+    double rot_radius;        /* D^ in radians */
+    double trans_radius;      /* d^ */
+    long long rot_support[5]; /* indices (into the given samples) of the rotation ball's support set */
+    long long trans_support[4];
+    int n_rot_support, n_trans_support;
+    double host_seconds;      /* wall time of the host miniball part (reported separately) */
+    double reserved;
+} closure_megb_result;
+
+/* Step III (Alg. 1 l.6-7): minimum enclosing ball of {t} in R^3 and of the
+ * sign-aligned unit quaternions {q(R)} in R^4 (R-15, R-16) by Gaertner's miniball.
+ *   samples  DEVICE, count x 12 (e.g. closure_compact's output)
+ * Synchronises `cuda_stream`, copies the samples to the host and solves there.
+ * Errors: CLOSURE_EINVAL (count <= 0), CLOSURE_ENOINIT (R_bar needed for the sign), CLOSURE_ECUDA. */
+int closure_megb(closure_t *h, const double *samples, long long count, closure_megb_result *out,
+                 void *cuda_stream);
+
+/* Whole path from host buffers: walk, compact, MEGB; samples never leave the device except the
+ * compacted cloud for the miniball.  out_count (host, may be NULL) receives the number of
+ * boundary samples.  Synchronous. */
+int closure_run(closure_t *h, long long num_walkers, int num_steps, unsigned long long seed,
+                closure_megb_result *out, long long *out_count, void *cuda_stream);
+
+/* Counters of the last closure_sample* launch on this handle when statistics were enabled with
+ * closure_enable_stats(h, 1): executed constraint evaluations per phase (for the roofline's
+ * executed-flop count).  closure_get_stats synchronises the stream of that launch. */
+typedef struct {
+    unsigned long long perturb_pairs;   /* (perturbation, constraint) pairs evaluated, step a3 */
+    unsigned long long ladder_pairs;    /* (candidate, constraint) pairs evaluated, step a5 */
+    unsigned long long perturb_setups;  /* per-constraint set-ups (R-dependent part), a3 */
+    unsigned long long ladder_setups;   /* per-(rung, constraint) set-ups, a5 */
+    unsigned long long accepted_steps;  /* iterations that moved the walker */
+    unsigned long long walker_steps;    /* walkers x iterations */
+} closure_stats;
+int closure_enable_stats(closure_t *h, int on);
+int closure_get_stats(closure_t *h, closure_stats *out);
+
+/* Measured CUDA-core peak of this device: a register-resident FMA chain, fp64 (precision = 64)
+ * or fp32 (32).  Returns FLOP/s (FMA = 2) in *flops_per_s and the kernel time in *seconds.
+ * Synchronous.  Used as the roofline denominator for the walker kernel. */
+int closure_alu_peak(int precision, double *flops_per_s, double *seconds, void *cuda_stream);
+
+/* The host solver of Step III on its own: exact smallest enclosing ball of n points in R^d
+ * (1 <= d <= 4), points row-major in HOST memory.  center (d doubles), radius, support (up to d+1
+ * indices, ascending) and n_support are written.  Pure host code: needs no device. */
+int closure_miniball_host(const double *points, long long n, int d, double *center, double *radius,
+                          long long *support, int *n_support);
+
+const char *closure_last_error(const closure_t *h);
+const char *closure_strerror(int status);
+int closure_abi_version(void);
+void closure_destroy(closure_t *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CLOSURE_B200_H */

@@ -1,0 +1,81 @@
+// Measured CUDA-core FMA peak of the device: the roofline denominator of the walker kernel.
+// MEASURED_PEAKS.json carries only HBM and bf16 tensor peaks; the walk is bound by the plain
+// FP64 (or FP32) pipes, so the library times a register-resident FMA chain itself
+// (DESIGN.md "Roofline").
+#include <cuda_runtime.h>
+
+#include "closure_internal.h"
+
+namespace closure {
+namespace {
+
+constexpr int kChains = 8;
+constexpr int kIters = 4096;
+constexpr int kUnroll = 16;
+
+template <typename T>
+__global__ void __launch_bounds__(256) fma_chain_kernel(T *sink, T a, T b)
+{
+    T x[kChains];
+#pragma unroll
+    for (int c = 0; c < kChains; ++c) x[c] = (T)(threadIdx.x + c) * (T)1e-3;
+    for (int it = 0; it < kIters / kUnroll; ++it) {
+#pragma unroll
+        for (int u = 0; u < kUnroll; ++u)
+#pragma unroll
+            for (int c = 0; c < kChains; ++c) x[c] = fma(x[c], a, b);
+    }
+    T s = 0;
+#pragma unroll
+    for (int c = 0; c < kChains; ++c) s += x[c];
+    if (s == (T)123456789) sink[0] = s;      // never true; keeps the chain live
+}
+
+template <typename T>
+cudaError_t run(double *flops_per_s, double *seconds, cudaStream_t stream)
+{
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    T *sink = nullptr;
+    e = cudaMalloc(&sink, sizeof(T));
+    if (e != cudaSuccess) return e;
+    cudaEvent_t t0, t1;
+    cudaEventCreate(&t0);
+    cudaEventCreate(&t1);
+    const int blocks = sms * 16;
+    float best_ms = 1e30f;
+    for (int rep = 0; rep < 5; ++rep) {      // first repetitions warm the clocks up
+        cudaEventRecord(t0, stream);
+        fma_chain_kernel<T><<<blocks, 256, 0, stream>>>(sink, (T)0.999, (T)1e-3);
+        cudaEventRecord(t1, stream);
+        e = cudaEventSynchronize(t1);
+        if (e != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, t0, t1);
+        if (rep >= 2 && ms < best_ms) best_ms = ms;
+    }
+    cudaEventDestroy(t0);
+    cudaEventDestroy(t1);
+    cudaFree(sink);
+    if (e != cudaSuccess) return e;
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    const double flops = 2.0 * (double)blocks * 256.0 * (double)kIters * (double)kChains;
+    *seconds = best_ms * 1e-3;
+    *flops_per_s = flops / (best_ms * 1e-3);
+    return cudaSuccess;
+}
+
+}  // namespace
+
+cudaError_t measure_alu_peak(int precision, double *flops_per_s, double *seconds, cudaStream_t stream)
+{
+    if (precision == 64) return run<double>(flops_per_s, seconds, stream);
+    if (precision == 32) return run<float>(flops_per_s, seconds, stream);
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace closure

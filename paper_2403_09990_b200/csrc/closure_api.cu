@@ -1,0 +1,548 @@
+// C ABI of libclosure_b200 (include/closure.h): argument validation, instance packing and
+// upload, launches of the walker / compaction kernels on the caller's stream, and the host
+// side of closure_megb.  No CPU fallback exists: every compute entry point needs a CUDA device.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <numeric>
+#include <string>
+#include <vector>
+
+#include "closure_internal.h"
+
+using namespace closure;
+
+struct closure_s {
+    int type = 0;
+    int n = 0;
+    closure_params P{};
+    std::vector<double> meas;        // as given (validation of S_0 on the host)
+    std::vector<double> betas;
+    double K[4] = { 0, 0, 0, 0 };
+    InstanceDesc h_desc{};
+    double *d_rows = nullptr;
+    InstanceDesc *d_desc = nullptr;
+    double *d_S0 = nullptr;
+    bool has_init = false;
+    void *d_scratch = nullptr;
+    size_t scratch_bytes = 0;
+    unsigned long long *d_stats = nullptr;
+    bool stats_on = false;
+    cudaStream_t last_stream = nullptr;
+    // buffers of closure_run
+    double *d_samples = nullptr, *d_compact = nullptr;
+    unsigned char *d_flags = nullptr;
+    long long *d_count = nullptr;
+    long long run_capacity = 0;
+    std::string err;
+};
+
+namespace {
+
+int fail(closure_t *h, int code, const std::string &msg)
+{
+    if (h) h->err = msg;
+    return code;
+}
+
+int cuda_fail(closure_t *h, cudaError_t e, const char *what)
+{
+    return fail(h, CLOSURE_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+bool all_finite(const double *p, size_t n)
+{
+    for (size_t i = 0; i < n; ++i)
+        if (!std::isfinite(p[i])) return false;
+    return true;
+}
+
+int meas_cols(int type)
+{
+    switch (type) {
+    case CLOSURE_REPROJ_2D3D: return 5;
+    case CLOSURE_REG_3D3D: return 6;
+    case CLOSURE_POSE_REG:
+    case CLOSURE_POSE_REG_SPLIT: return 12;
+    default: return 0;
+    }
+}
+
+int check_params(const closure_params *p, std::string *why)
+{
+    if (!p) { *why = "params is NULL"; return CLOSURE_EINVAL; }
+    if (p->mode != CLOSURE_MODE_ROT && p->mode != CLOSURE_MODE_TRANS) { *why = "bad mode"; return CLOSURE_EINVAL; }
+    if (p->n_p < 1 || p->n_p_star < 1 || p->n_p_star > p->n_p) { *why = "need 1 <= n_p_star <= n_p"; return CLOSURE_EINVAL; }
+    if (p->n_t < 1 || p->n_t > kMaxNT) { *why = "need 1 <= n_t <= 64"; return CLOSURE_EINVAL; }
+    if (p->n_p >= (1 << 23)) { *why = "n_p too large"; return CLOSURE_EINVAL; }
+    const double v[6] = { p->omega0, p->v0, p->gamma, p->t_p, p->theta_p, 0.0 };
+    if (!all_finite(v, 5)) { *why = "non-finite parameter"; return CLOSURE_EINVAL; }
+    if (!(p->gamma > 0.0 && p->gamma <= 1.0)) { *why = "need 0 < gamma <= 1"; return CLOSURE_EINVAL; }
+    if (p->omega0 < 0.0 || p->v0 < 0.0 || p->t_p < 0.0 || p->theta_p < 0.0) { *why = "negative scale"; return CLOSURE_EINVAL; }
+    if (p->precision != 64 && p->precision != 32) { *why = "precision must be 64 or 32"; return CLOSURE_EINVAL; }
+    if (p->n_p_star > kMaxKStar) { *why = "n_p_star > 20 is not built"; return CLOSURE_EUNSUPPORTED; }
+    if (p->precision == 32) { *why = "fp32 mode is not built yet"; return CLOSURE_EUNSUPPORTED; }
+    return CLOSURE_OK;
+}
+
+// PURSE membership on the host, used only to validate S_0 (squared form, R-9).
+bool host_in_purse(const closure_t *h, const double *pose)
+{
+    const double *R = pose, *t = pose + 9;
+    for (int i = 0; i < h->n; ++i) {
+        const double *m = h->meas.data() + (size_t)i * meas_cols(h->type);
+        if (h->type == CLOSURE_REG_3D3D) {
+            double sq = 0.0;
+            for (int r = 0; r < 3; ++r) {
+                const double g = m[3 + r] - ((R[3 * r] * m[0] + R[3 * r + 1] * m[1] + R[3 * r + 2] * m[2]) + t[r]);
+                sq += g * g;
+            }
+            if (!(sq <= h->betas[i] * h->betas[i])) return false;
+        } else if (h->type == CLOSURE_REPROJ_2D3D) {
+            double p[3];
+            for (int r = 0; r < 3; ++r) p[r] = (R[3 * r] * m[2] + R[3 * r + 1] * m[3] + R[3 * r + 2] * m[4]) + t[r];
+            if (!(p[2] > 0.0)) return false;
+            const double g0 = m[0] - (h->K[0] * (p[0] / p[2]) + h->K[2]);
+            const double g1 = m[1] - (h->K[1] * (p[1] / p[2]) + h->K[3]);
+            if (!(g0 * g0 + g1 * g1 <= h->betas[i] * h->betas[i])) return false;
+        } else {
+            double sr = 0.0, st = 0.0;
+            for (int e = 0; e < 9; ++e) sr += (R[e] - m[e]) * (R[e] - m[e]);
+            for (int r = 0; r < 3; ++r) st += (t[r] - m[9 + r]) * (t[r] - m[9 + r]);
+            if (h->type == CLOSURE_POSE_REG) {
+                if (!(sr + st <= h->betas[i] * h->betas[i])) return false;
+            } else {
+                if (!(sr <= h->betas[2 * i] * h->betas[2 * i])) return false;
+                if (!(st <= h->betas[2 * i + 1] * h->betas[2 * i + 1])) return false;
+            }
+        }
+    }
+    return true;
+}
+
+void free_run_buffers(closure_t *h)
+{
+    cudaFree(h->d_samples); cudaFree(h->d_compact); cudaFree(h->d_flags); cudaFree(h->d_count);
+    h->d_samples = h->d_compact = nullptr; h->d_flags = nullptr; h->d_count = nullptr;
+    h->run_capacity = 0;
+}
+
+int ensure_scratch(closure_t *h, long long n)
+{
+    const size_t need = compact_scratch_bytes(n);
+    if (need <= h->scratch_bytes) return CLOSURE_OK;
+    cudaFree(h->d_scratch);
+    h->d_scratch = nullptr;
+    h->scratch_bytes = 0;
+    cudaError_t e = cudaMalloc(&h->d_scratch, need);
+    if (e != cudaSuccess) return cuda_fail(h, e, "cudaMalloc(scratch)");
+    h->scratch_bytes = need;
+    return CLOSURE_OK;
+}
+
+void fill_launch(const closure_t *h, WalkLaunch &L)
+{
+    std::memset(&L, 0, sizeof(L));
+    L.n_p = h->P.n_p; L.n_p_star = h->P.n_p_star; L.n_t = h->P.n_t;
+    L.omega0 = h->P.omega0; L.v0 = h->P.v0; L.gamma = h->P.gamma; L.t_p = h->P.t_p; L.theta_p = h->P.theta_p;
+}
+
+bool same_params(const closure_params &a, const closure_params &b)
+{
+    return a.mode == b.mode && a.n_p == b.n_p && a.n_p_star == b.n_p_star && a.n_t == b.n_t && a.omega0 == b.omega0 &&
+           a.v0 == b.v0 && a.gamma == b.gamma && a.t_p == b.t_p && a.theta_p == b.theta_p && a.precision == b.precision;
+}
+
+}  // namespace
+
+extern "C" {
+
+int closure_abi_version(void) { return CLOSURE_ABI_VERSION; }
+
+const char *closure_strerror(int status)
+{
+    switch (status) {
+    case CLOSURE_OK: return "ok";
+    case CLOSURE_EINVAL: return "invalid argument";
+    case CLOSURE_EINIT: return "initial pose outside the PURSE";
+    case CLOSURE_ENOINIT: return "closure_set_init has not been called";
+    case CLOSURE_ECUDA: return "CUDA failure";
+    case CLOSURE_ENOMEM: return "out of memory";
+    case CLOSURE_EUNSUPPORTED: return "combination not built";
+    default: return "unknown status";
+    }
+}
+
+const char *closure_last_error(const closure_t *h) { return h ? h->err.c_str() : "null handle"; }
+
+int closure_default_params(int residual_type, closure_params *p)
+{
+    if (!p || meas_cols(residual_type) == 0) return CLOSURE_EINVAL;
+    std::memset(p, 0, sizeof(*p));
+    p->mode = CLOSURE_MODE_ROT;
+    p->n_p = 150; p->n_p_star = 10; p->n_t = 15;
+    p->gamma = 0.5;
+    p->precision = 64;
+    if (residual_type == CLOSURE_REPROJ_2D3D) {       // PAPER.md:374 (t_p rescaled to metres at ~1 m depth)
+        p->omega0 = 1.0; p->v0 = 2.0; p->theta_p = 0.2; p->t_p = 0.01;
+    } else {
+        p->omega0 = 0.5; p->v0 = 0.0; p->theta_p = 0.0; p->t_p = 0.1;
+        if (residual_type != CLOSURE_REG_3D3D) p->n_t = 10;
+    }
+    return CLOSURE_OK;
+}
+
+int closure_set_params(closure_t *h, const closure_params *p)
+{
+    if (!h) return CLOSURE_EINVAL;
+    std::string why;
+    const int rc = check_params(p, &why);
+    if (rc != CLOSURE_OK) return fail(h, rc, why);
+    h->P = *p;
+    return CLOSURE_OK;
+}
+
+int closure_create(int residual_type, const double *measurements, int n, const double *betas,
+                   const double *intrinsics, const closure_params *p, closure_t **out)
+{
+    if (!out) return CLOSURE_EINVAL;
+    *out = nullptr;
+    const int cols = meas_cols(residual_type);
+    if (cols == 0 || !measurements || !betas || n <= 0 || n > 4096) return CLOSURE_EINVAL;
+    std::string why;
+    int rc = check_params(p, &why);
+    if (rc != CLOSURE_OK) return rc;
+    const int nb = residual_type == CLOSURE_POSE_REG_SPLIT ? 2 * n : n;
+    if (!all_finite(measurements, (size_t)n * cols) || !all_finite(betas, nb)) return CLOSURE_EINVAL;
+    for (int i = 0; i < nb; ++i)
+        if (!(betas[i] > 0.0)) return CLOSURE_EINVAL;
+    if (residual_type == CLOSURE_REPROJ_2D3D) {
+        if (!intrinsics || !all_finite(intrinsics, 4) || !(intrinsics[0] > 0.0) || !(intrinsics[1] > 0.0))
+            return CLOSURE_EINVAL;
+    }
+    closure_t *h = new (std::nothrow) closure_s;
+    if (!h) return CLOSURE_ENOMEM;
+    h->type = residual_type;
+    h->n = n;
+    h->P = *p;
+    h->meas.assign(measurements, measurements + (size_t)n * cols);
+    h->betas.assign(betas, betas + nb);
+    if (residual_type == CLOSURE_REPROJ_2D3D) std::memcpy(h->K, intrinsics, sizeof(h->K));
+
+    // pack rows, sorted by the translation-side bound (stable)
+    const int row = row_doubles(residual_type);
+    auto key = [&](int i) { return residual_type == CLOSURE_POSE_REG_SPLIT ? betas[2 * i + 1] : betas[i]; };
+    std::vector<int> order(n);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return key(a) < key(b); });
+    std::vector<double> rows((size_t)n * row, 0.0);
+    for (int k = 0; k < n; ++k) {
+        const int i = order[k];
+        const double *m = measurements + (size_t)i * cols;
+        double *r = rows.data() + (size_t)k * row;
+        if (residual_type == CLOSURE_REG_3D3D) {
+            std::memcpy(r, m, 6 * sizeof(double));
+            r[6] = betas[i]; r[7] = betas[i] * betas[i];
+        } else if (residual_type == CLOSURE_REPROJ_2D3D) {
+            std::memcpy(r, m, 5 * sizeof(double));
+            r[5] = betas[i]; r[6] = betas[i] * betas[i];
+        } else if (residual_type == CLOSURE_POSE_REG) {
+            std::memcpy(r, m, 12 * sizeof(double));
+            r[12] = betas[i]; r[13] = betas[i] * betas[i];
+        } else {
+            std::memcpy(r, m, 12 * sizeof(double));
+            r[12] = betas[2 * i]; r[13] = betas[2 * i] * betas[2 * i];
+            r[14] = betas[2 * i + 1]; r[15] = betas[2 * i + 1] * betas[2 * i + 1];
+        }
+    }
+    const size_t bytes = rows.size() * sizeof(double);     // row is 8 or 16 doubles: multiple of 16 B
+    cudaError_t e = cudaMalloc(&h->d_rows, bytes);
+    if (e == cudaSuccess) e = cudaMemcpy(h->d_rows, rows.data(), bytes, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&h->d_desc, sizeof(InstanceDesc));
+    if (e == cudaSuccess) e = cudaMalloc(&h->d_stats, 6 * sizeof(unsigned long long));
+    if (e != cudaSuccess) {
+        // no handle is returned: the failure text can only be seen through the status code
+        cudaFree(h->d_rows); cudaFree(h->d_desc); cudaFree(h->d_stats);
+        delete h;
+        return CLOSURE_ECUDA;
+    }
+    h->h_desc.rows = h->d_rows;
+    h->h_desc.n = n;
+    h->h_desc.rows_bytes = (int)bytes;
+    std::memcpy(h->h_desc.K, h->K, sizeof(h->K));
+    *out = h;
+    return CLOSURE_OK;
+}
+
+int closure_set_init(closure_t *h, const double *poses, int n0, double *mean_out)
+{
+    if (!h) return CLOSURE_EINVAL;
+    if (!poses || n0 <= 0) return fail(h, CLOSURE_EINVAL, "poses is NULL or n0 <= 0");
+    if (!all_finite(poses, (size_t)n0 * 12)) return fail(h, CLOSURE_EINVAL, "non-finite initial pose");
+    for (int s = 0; s < n0; ++s)
+        if (!host_in_purse(h, poses + (size_t)s * 12))
+            return fail(h, CLOSURE_EINIT, "initial pose " + std::to_string(s) + " violates a constraint");
+    // Alg. 2 l.3-4: R_bar = proj_SO(3)(sum R_j), t_bar = mean t_j
+    double M[9] = { 0 }, tb[3] = { 0 };
+    for (int s = 0; s < n0; ++s) {
+        for (int e = 0; e < 9; ++e) M[e] += poses[(size_t)s * 12 + e];
+        for (int r = 0; r < 3; ++r) tb[r] += poses[(size_t)s * 12 + 9 + r];
+    }
+    for (int r = 0; r < 3; ++r) tb[r] /= (double)n0;
+    double Rb[9];
+    if (!project_so3(M, Rb)) return fail(h, CLOSURE_EINVAL, "sum of initial rotations has no projection onto SO(3)");
+    cudaFree(h->d_S0);
+    h->d_S0 = nullptr;
+    h->has_init = false;
+    cudaError_t e = cudaMalloc(&h->d_S0, (size_t)n0 * 12 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemcpy(h->d_S0, poses, (size_t)n0 * 12 * sizeof(double), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return cuda_fail(h, e, "upload of S_0");
+    h->h_desc.S0 = h->d_S0;
+    h->h_desc.n0 = n0;
+    std::memcpy(h->h_desc.Rbar, Rb, sizeof(Rb));
+    std::memcpy(h->h_desc.tbar, tb, sizeof(tb));
+    e = cudaMemcpy(h->d_desc, &h->h_desc, sizeof(InstanceDesc), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return cuda_fail(h, e, "upload of instance descriptor");
+    h->has_init = true;
+    if (mean_out) {
+        std::memcpy(mean_out, Rb, sizeof(Rb));
+        std::memcpy(mean_out + 9, tb, sizeof(tb));
+    }
+    return CLOSURE_OK;
+}
+
+int closure_sample_range(closure_t *h, long long walker_begin, long long num_walkers, int num_steps,
+                         unsigned long long seed, double *out_samples, unsigned char *out_on_boundary,
+                         int *out_trace, void *cuda_stream)
+{
+    if (!h) return CLOSURE_EINVAL;
+    if (!h->has_init) return fail(h, CLOSURE_ENOINIT, "closure_set_init has not been called");
+    if (walker_begin < 0 || num_walkers < 0 || num_steps < 0) return fail(h, CLOSURE_EINVAL, "negative size");
+    if (num_walkers == 0) return CLOSURE_OK;
+    if (!out_samples || !out_on_boundary) return fail(h, CLOSURE_EINVAL, "output buffer is NULL");
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    WalkLaunch L;
+    fill_launch(h, L);
+    L.desc[0] = h->d_desc;
+    L.seed[0] = seed;
+    L.walker_begin = walker_begin;
+    L.num_walkers = num_walkers;
+    L.num_steps = num_steps;
+    L.out_samples = out_samples;
+    L.out_flags = out_on_boundary;
+    L.out_trace = out_trace;
+    if (h->stats_on) {
+        cudaError_t e = cudaMemsetAsync(h->d_stats, 0, 6 * sizeof(unsigned long long), stream);
+        if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync(stats)");
+        L.stats = h->d_stats;
+    }
+    std::string why;
+    cudaError_t e = launch_walkers(h->type, h->P.mode, h->stats_on, L, 1, h->h_desc.rows_bytes, stream, &why);
+    h->last_stream = stream;
+    if (e != cudaSuccess) return cuda_fail(h, e, why.empty() ? "walker kernel launch" : why.c_str());
+    return CLOSURE_OK;
+}
+
+int closure_sample(closure_t *h, long long num_walkers, int num_steps, unsigned long long seed,
+                   double *out_samples, unsigned char *out_on_boundary, void *cuda_stream)
+{
+    return closure_sample_range(h, 0, num_walkers, num_steps, seed, out_samples, out_on_boundary, nullptr,
+                                cuda_stream);
+}
+
+int closure_sample_batch(closure_t *const *handles, int n_instances, long long walkers_per_instance,
+                         int num_steps, const unsigned long long *seeds, double *out_samples,
+                         unsigned char *out_on_boundary, void *cuda_stream)
+{
+    if (!handles || n_instances <= 0 || !handles[0]) return CLOSURE_EINVAL;
+    closure_t *h0 = handles[0];
+    if (!seeds || walkers_per_instance < 0 || num_steps < 0) return fail(h0, CLOSURE_EINVAL, "bad batch arguments");
+    for (int b = 0; b < n_instances; ++b) {
+        if (!handles[b]) return fail(h0, CLOSURE_EINVAL, "NULL handle in batch");
+        if (!handles[b]->has_init) return fail(h0, CLOSURE_ENOINIT, "batch member without S_0");
+        if (handles[b]->type != h0->type || !same_params(handles[b]->P, h0->P))
+            return fail(h0, CLOSURE_EINVAL, "batch members must share residual type and parameters");
+    }
+    if (walkers_per_instance == 0) return CLOSURE_OK;
+    if (!out_samples || !out_on_boundary) return fail(h0, CLOSURE_EINVAL, "output buffer is NULL");
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (h0->stats_on) {
+        cudaError_t e = cudaMemsetAsync(h0->d_stats, 0, 6 * sizeof(unsigned long long), stream);
+        if (e != cudaSuccess) return cuda_fail(h0, e, "cudaMemsetAsync(stats)");
+    }
+    for (int b0 = 0; b0 < n_instances; b0 += kMaxBatch) {
+        const int nb = std::min(kMaxBatch, n_instances - b0);
+        WalkLaunch L;
+        fill_launch(h0, L);
+        int max_bytes = 0;
+        for (int b = 0; b < nb; ++b) {
+            L.desc[b] = handles[b0 + b]->d_desc;
+            L.seed[b] = seeds[b0 + b];
+            max_bytes = std::max(max_bytes, handles[b0 + b]->h_desc.rows_bytes);
+        }
+        L.walker_begin = 0;
+        L.num_walkers = walkers_per_instance;
+        L.num_steps = num_steps;
+        L.out_samples = out_samples + (size_t)b0 * walkers_per_instance * 12;
+        L.out_flags = out_on_boundary + (size_t)b0 * walkers_per_instance;
+        L.out_trace = nullptr;
+        L.stats = h0->stats_on ? h0->d_stats : nullptr;
+        std::string why;
+        cudaError_t e = launch_walkers(h0->type, h0->P.mode, h0->stats_on, L, nb, max_bytes, stream, &why);
+        if (e != cudaSuccess) return cuda_fail(h0, e, why.empty() ? "walker kernel launch" : why.c_str());
+    }
+    h0->last_stream = stream;
+    return CLOSURE_OK;
+}
+
+int closure_compact(closure_t *h, const double *samples, const unsigned char *flags, long long n,
+                    double *out_compacted, long long *out_count, void *cuda_stream)
+{
+    if (!h) return CLOSURE_EINVAL;
+    if (n < 0 || !out_count || (n > 0 && (!samples || !flags || !out_compacted)))
+        return fail(h, CLOSURE_EINVAL, "bad compaction arguments");
+    if ((reinterpret_cast<uintptr_t>(samples) | reinterpret_cast<uintptr_t>(out_compacted)) & 15u)
+        return fail(h, CLOSURE_EINVAL, "sample buffers must be 16-byte aligned");
+    int rc = ensure_scratch(h, std::max<long long>(n, 1));
+    if (rc != CLOSURE_OK) return rc;
+    cudaError_t e = launch_compact(samples, flags, n, out_compacted, out_count, h->d_scratch,
+                                   static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(h, e, "compaction kernel launch");
+    return CLOSURE_OK;
+}
+
+int closure_megb(closure_t *h, const double *samples, long long count, closure_megb_result *out,
+                 void *cuda_stream)
+{
+    if (!h) return CLOSURE_EINVAL;
+    if (!out || !samples || count <= 0) return fail(h, CLOSURE_EINVAL, "closure_megb needs count > 0 samples");
+    if (!h->has_init) return fail(h, CLOSURE_ENOINIT, "R_bar (closure_set_init) is needed to align quaternion signs");
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    std::vector<double> host;
+    try {
+        host.resize((size_t)count * 12);
+    } catch (const std::bad_alloc &) {
+        return fail(h, CLOSURE_ENOMEM, "host buffer for samples");
+    }
+    cudaError_t e = cudaMemcpyAsync(host.data(), samples, host.size() * sizeof(double), cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "copy of samples to the host");
+
+    const auto t0 = std::chrono::steady_clock::now();
+    std::vector<double> tp((size_t)count * 3), qp((size_t)count * 4);
+    double qbar[4];
+    rotation_to_quat(h->h_desc.Rbar, qbar);
+    for (long long i = 0; i < count; ++i) {
+        const double *s = host.data() + (size_t)i * 12;
+        std::memcpy(tp.data() + (size_t)i * 3, s + 9, 3 * sizeof(double));
+        double q[4];
+        rotation_to_quat(s, q);
+        const double dot = q[0] * qbar[0] + q[1] * qbar[1] + q[2] * qbar[2] + q[3] * qbar[3];
+        const double sg = dot < 0.0 ? -1.0 : 1.0;                   // R-15
+        for (int k = 0; k < 4; ++k) qp[(size_t)i * 4 + k] = sg * q[k];
+    }
+    Ball bt, bq;
+    if (!miniball(tp.data(), count, 3, &bt) || !miniball(qp.data(), count, 4, &bq))
+        return fail(h, CLOSURE_EINVAL, "miniball failed");
+    std::memset(out, 0, sizeof(*out));
+    const double hn = std::sqrt(bq.center[0] * bq.center[0] + bq.center[1] * bq.center[1] +
+                                bq.center[2] * bq.center[2] + bq.center[3] * bq.center[3]);
+    if (!(hn > 0.0)) return fail(h, CLOSURE_EINVAL, "rotation samples span the whole quaternion sphere");
+    const double qc[4] = { bq.center[0] / hn, bq.center[1] / hn, bq.center[2] / hn, bq.center[3] / hn };
+    quat_to_rotation(qc, out->R);
+    std::memcpy(out->t, bt.center, 3 * sizeof(double));
+    double ca = (1.0 + hn * hn - bq.sq_radius) / (2.0 * hn);       // R-16
+    ca = std::min(1.0, std::max(-1.0, ca));
+    out->rot_radius = 2.0 * std::acos(ca);
+    out->trans_radius = std::sqrt(bt.sq_radius);
+    out->n_rot_support = bq.n_support;
+    out->n_trans_support = bt.n_support;
+    for (int k = 0; k < bq.n_support; ++k) out->rot_support[k] = bq.support[k];
+    for (int k = 0; k < bt.n_support; ++k) out->trans_support[k] = bt.support[k];
+    out->host_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    return CLOSURE_OK;
+}
+
+int closure_run(closure_t *h, long long num_walkers, int num_steps, unsigned long long seed,
+                closure_megb_result *out, long long *out_count, void *cuda_stream)
+{
+    if (!h) return CLOSURE_EINVAL;
+    if (!out || num_walkers <= 0) return fail(h, CLOSURE_EINVAL, "closure_run needs walkers and a result");
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (num_walkers > h->run_capacity) {
+        free_run_buffers(h);
+        cudaError_t e = cudaMalloc(&h->d_samples, (size_t)num_walkers * 96);
+        if (e == cudaSuccess) e = cudaMalloc(&h->d_compact, (size_t)num_walkers * 96);
+        if (e == cudaSuccess) e = cudaMalloc(&h->d_flags, (size_t)num_walkers);
+        if (e == cudaSuccess) e = cudaMalloc(&h->d_count, sizeof(long long));
+        if (e != cudaSuccess) { free_run_buffers(h); return cuda_fail(h, e, "cudaMalloc(run buffers)"); }
+        h->run_capacity = num_walkers;
+    }
+    int rc = closure_sample(h, num_walkers, num_steps, seed, h->d_samples, h->d_flags, cuda_stream);
+    if (rc != CLOSURE_OK) return rc;
+    rc = closure_compact(h, h->d_samples, h->d_flags, num_walkers, h->d_compact, h->d_count, cuda_stream);
+    if (rc != CLOSURE_OK) return rc;
+    long long count = 0;
+    cudaError_t e = cudaMemcpyAsync(&count, h->d_count, sizeof(count), cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) return cuda_fail(h, e, "walk / compaction");
+    if (out_count) *out_count = count;
+    if (count == 0) {
+        // no walker was stopped by the boundary: every final pose is still a valid subset of S (Prop. 4)
+        return closure_megb(h, h->d_samples, num_walkers, out, cuda_stream);
+    }
+    return closure_megb(h, h->d_compact, count, out, cuda_stream);
+}
+
+int closure_enable_stats(closure_t *h, int on)
+{
+    if (!h) return CLOSURE_EINVAL;
+    h->stats_on = on != 0;
+    return CLOSURE_OK;
+}
+
+int closure_get_stats(closure_t *h, closure_stats *out)
+{
+    if (!h || !out) return CLOSURE_EINVAL;
+    unsigned long long v[6];
+    cudaError_t e = cudaStreamSynchronize(h->last_stream);
+    if (e == cudaSuccess) e = cudaMemcpy(v, h->d_stats, sizeof(v), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(h, e, "read of statistics");
+    out->perturb_pairs = v[0]; out->ladder_pairs = v[1]; out->perturb_setups = v[2];
+    out->ladder_setups = v[3]; out->accepted_steps = v[4]; out->walker_steps = v[5];
+    return CLOSURE_OK;
+}
+
+int closure_alu_peak(int precision, double *flops_per_s, double *seconds, void *cuda_stream)
+{
+    if (!flops_per_s || !seconds || (precision != 64 && precision != 32)) return CLOSURE_EINVAL;
+    cudaError_t e = measure_alu_peak(precision, flops_per_s, seconds, static_cast<cudaStream_t>(cuda_stream));
+    return e == cudaSuccess ? CLOSURE_OK : CLOSURE_ECUDA;
+}
+
+int closure_miniball_host(const double *points, long long n, int d, double *center, double *radius,
+                          long long *support, int *n_support)
+{
+    if (!points || !center || !radius || !support || !n_support || n <= 0 || d < 1 || d > 4) return CLOSURE_EINVAL;
+    Ball b;
+    if (!miniball(points, n, d, &b)) return CLOSURE_EINVAL;
+    for (int a = 0; a < d; ++a) center[a] = b.center[a];
+    *radius = std::sqrt(b.sq_radius);
+    *n_support = b.n_support;
+    for (int k = 0; k < b.n_support; ++k) support[k] = b.support[k];
+    return CLOSURE_OK;
+}
+
+void closure_destroy(closure_t *h)
+{
+    if (!h) return;
+    cudaFree(h->d_rows); cudaFree(h->d_desc); cudaFree(h->d_S0); cudaFree(h->d_scratch); cudaFree(h->d_stats);
+    free_run_buffers(h);
+    delete h;
+}
+
+}  // extern "C"

@@ -1,0 +1,81 @@
+// Internal declarations shared by the translation units of libclosure_b200.
+// Not part of the C ABI (include/closure.h is).  Nothing here is seen by oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/closure.h"
+
+namespace closure {
+
+// Device-side description of one PURSE instance.  `rows` is the packed constraint table the
+// walker kernel stages into shared memory with one bulk copy (TMA, cp.async.bulk):
+//   REG_3D3D        row = [a0 a1 a2 b0 b1 b2 beta beta^2]                      (8 doubles)
+//   REPROJ_2D3D     row = [zx zy Z0 Z1 Z2 beta beta^2 0]                       (8 doubles)
+//   POSE_REG        row = [R_i(9) t_i(3) beta beta^2 0 0]                      (16 doubles)
+//   POSE_REG_SPLIT  row = [R_i(9) t_i(3) betaR betaR^2 betaT betaT^2]          (16 doubles)
+// Rows are sorted by the translation-side bound (beta / betaT) so that equal bounds are
+// adjacent: eq. (14)'s min_i(beta_i - ||g_i||) then needs one square root per run of equal
+// bounds instead of one per constraint (min/AND over constraints are order-free).
+struct InstanceDesc {
+    const double *rows;     // device
+    int n;                  // rows (= N hypotheses / correspondences)
+    int rows_bytes;         // n * ROW * 8, a multiple of 16
+    const double *S0;       // device, n0 x 12
+    int n0;
+    int pad_;
+    double Rbar[9];
+    double tbar[3];
+    double K[4];            // fx fy cx cy
+};
+
+constexpr int kMaxBatch = 96;
+constexpr int kBlock = 128;       // walkers per CTA (one per thread)
+constexpr int kMaxNT = 64;
+constexpr int kMaxKStar = 20;
+
+struct WalkLaunch {
+    const InstanceDesc *desc[kMaxBatch];      // device pointers, one per instance (gridDim.y)
+    unsigned long long seed[kMaxBatch];
+    long long walker_begin;
+    long long num_walkers;                    // per instance
+    int num_steps;
+    int n_p, n_p_star, n_t;
+    double omega0, v0, gamma, t_p, theta_p;
+    double *out_samples;
+    unsigned char *out_flags;
+    int *out_trace;                           // nullable
+    unsigned long long *stats;                // nullable, 6 counters
+};
+
+int row_doubles(int residual_type);
+
+// walker_kernel.cu
+cudaError_t launch_walkers(int residual_type, int mode, bool stats, const WalkLaunch &L, int n_instances,
+                           int max_rows_bytes, cudaStream_t stream, std::string *why);
+
+// compact_kernel.cu
+size_t compact_scratch_bytes(long long n);
+cudaError_t launch_compact(const double *samples, const unsigned char *flags, long long n, double *out,
+                           long long *out_count, void *scratch, cudaStream_t stream);
+
+// alu_peak.cu
+cudaError_t measure_alu_peak(int precision, double *flops_per_s, double *seconds, cudaStream_t stream);
+
+// miniball.cpp (host)
+struct Ball {
+    double center[4];
+    double sq_radius;
+    long long support[5];
+    int n_support;
+};
+// Gaertner-style exact smallest enclosing ball of n points in R^d (d <= 4), points row-major.
+bool miniball(const double *pts, long long n, int d, Ball *out);
+void rotation_to_quat(const double R[9], double q[4]);
+void quat_to_rotation(const double q[4], double R[9]);
+bool project_so3(const double M[9], double R[9]);   // nearest rotation to M (polar factor)
+
+}  // namespace closure

@@ -1,0 +1,138 @@
+"""-m gpu: the CUDA walker kernel against the oracle, through the C ABI.
+
+Protocol: identical per-iteration decisions (m_0, j_{k_0}) and on_boundary
+flags, final samples within 1e-9 relative, except walkers whose first differing decision has an
+oracle decision slack below 1e-9 (excluded, counted, bounded).
+"""
+import copy
+
+import numpy as np
+import pytest
+
+from paper_2403_09990_b200 import instances as I
+from tests.gpu_common import assert_parity, gpu_walk
+
+pytestmark = pytest.mark.gpu
+
+
+def _small(P, **kw):
+    P = copy.copy(P)
+    for k, v in kw.items():
+        setattr(P, k, v)
+    return P
+
+
+def test_c1_full_size_every_walker():
+    """BASELINE config 1 at its full size: 1024 walkers x 200 iterations, all compared."""
+    inst = I.make_instance(1)
+    S0 = I.make_init_poses(inst, 128)
+    n, div = assert_parity(inst, inst.params, S0, inst.num_walkers, inst.num_steps, 42)
+    assert n == 1024
+
+
+@pytest.mark.parametrize("config,walkers,steps", [(2, 384, 60), (3, 300, 60), (4, 300, 60), (5, 515, 120)])
+def test_configs_reduced(config, walkers, steps):
+    """Configs 2-5 with every walker compared; sizes span several CTAs and a ragged tail."""
+    inst = I.make_instance(config)
+    S0 = I.make_init_poses(inst, 128)
+    assert_parity(inst, inst.params, S0, walkers, steps, 42)
+
+
+def test_c3_translation_boundary_sampler():
+    """Alg. A8 (TRANS mode) on the reprojection residual: C3's second number."""
+    inst = I.make_instance(3)
+    P = _small(inst.params, mode=I.MODE_TRANS, v0=0.05, theta_p=0.02, n_p=40, n_p_star=5, n_t=10)
+    assert_parity(inst, P, I.make_init_poses(inst, 64), 200, 40, 7)
+
+
+@pytest.mark.parametrize("kind", ["reg", "posereg", "split"])
+def test_translation_boundary_sampler_other_residuals(kind):
+    if kind == "reg":
+        inst = I.make_instance(1)
+        P = _small(inst.params, mode=I.MODE_TRANS, v0=0.1, theta_p=0.02, n_p=30, n_p_star=4, n_t=8)
+    else:
+        inst = I.make_instance(4)
+        if kind == "split":
+            inst = I.to_split(inst)
+        P = _small(inst.params, mode=I.MODE_TRANS, v0=0.02, theta_p=0.02, n_p=20, n_p_star=3, n_t=8)
+    assert_parity(inst, P, I.make_init_poses(inst, 32), 160, 30, 11)
+
+
+def test_split_pose_regression_rot_mode():
+    inst = I.to_split(I.make_instance(4))
+    assert_parity(inst, inst.params, I.make_init_poses(inst, 64), 260, 50, 3)
+
+
+@pytest.mark.parametrize("n_p,n_p_star,n_t", [(1, 1, 1), (7, 1, 3), (37, 3, 5), (150, 10, 15), (23, 15, 4),
+                                              (64, 20, 6), (10, 10, 2)])
+def test_parameter_edges(n_p, n_p_star, n_t):
+    """Ragged perturbation tiles, every top-k capacity, degenerate N_P = N_P* = N_T = 1."""
+    inst = I.make_instance(1)
+    P = _small(inst.params, n_p=n_p, n_p_star=n_p_star, n_t=n_t)
+    assert_parity(inst, P, I.make_init_poses(inst, 16), 130, 25, 5)
+
+
+@pytest.mark.parametrize("n,distinct", [(1, False), (2, True), (7, True), (33, True), (200, False)])
+def test_constraint_count_edges(n, distinct):
+    """N = 1, odd N, every beta different (one sqrt per constraint), the maximum config size."""
+    inst = I.make_custom_reg(n, 100 + n, distinct_betas=distinct)
+    P = _small(inst.params, n_p=30, n_p_star=4, n_t=8, t_p=0.05)
+    assert_parity(inst, P, I.make_init_poses(inst, 8), 96, 20, 9)
+
+
+@pytest.mark.parametrize("walkers", [1, 31, 127, 128, 129])
+def test_walker_count_edges(walkers):
+    inst = I.make_instance(1)
+    P = _small(inst.params, n_p=20, n_p_star=2, n_t=6)
+    assert_parity(inst, P, I.make_init_poses(inst, 5), walkers, 15, 2)
+
+
+def test_single_initial_pose_and_zero_velocity():
+    """|S_0| = 1 (direction term undefined -> zero, R-3) and omega_0 = 0 (pure perturbation walk)."""
+    inst = I.make_instance(1)
+    S0 = I.make_init_poses(inst, 1)
+    assert_parity(inst, _small(inst.params, n_p=30, n_p_star=3, n_t=6), S0, 64, 20, 8)
+    assert_parity(inst, _small(inst.params, omega0=0.0, n_p=30, n_p_star=3, n_t=6), S0, 64, 20, 8)
+
+
+def test_zero_steps_returns_initial_poses():
+    inst = I.make_instance(1)
+    S0 = I.make_init_poses(inst, 16)
+    smp, flag = gpu_walk(inst, inst.params, S0, 40, 0, 1, trace=False)
+    assert np.array_equal(smp, S0[np.arange(40) % 16]) and not flag.any()
+
+
+def test_walker_range_and_replay_are_bit_identical():
+    """Philox keyed by walker id: a sub-range, a re-run and a high walker id reproduce exactly."""
+    inst = I.make_instance(1)
+    S0 = I.make_init_poses(inst, 32)
+    P = _small(inst.params, n_p=40, n_p_star=4, n_t=8)
+    full = gpu_walk(inst, P, S0, 300, 20, 77)
+    again = gpu_walk(inst, P, S0, 300, 20, 77)
+    part = gpu_walk(inst, P, S0, 100, 20, 77, walker_begin=150)
+    for a, b in zip(full, again):
+        assert np.array_equal(a, b)
+    for a, b in zip(full, part):
+        assert np.array_equal(a[150:250], b)
+    other = gpu_walk(inst, P, S0, 300, 20, 78)
+    assert not np.array_equal(full[0], other[0])
+    # walker ids beyond 2^32 use the high counter word
+    big = (1 << 32) + 5
+    hi = gpu_walk(inst, P, S0, 4, 20, 77, walker_begin=big)
+    import oracle
+    o_smp, o_flag = oracle.walk(inst, P, S0, big + np.arange(4), 20, 77)
+    assert np.allclose(hi[0], o_smp, rtol=1e-9, atol=1e-13)
+    assert not np.array_equal(hi[0][0], full[0][5])
+
+
+def test_samples_are_feasible_and_orthonormal():
+    """Invariant: every emitted pose is still in S (checked with the oracle's test)."""
+    import oracle
+    for config in (1, 3, 4):
+        inst = I.make_instance(config)
+        smp, flag, _ = gpu_walk(inst, inst.params, I.make_init_poses(inst, 64), 256, 40, 21)
+        for s in smp:
+            assert oracle.margin(inst, s[:9], s[9:]) >= -1e-12
+            R = s[:9].reshape(3, 3)
+            assert np.allclose(R.T @ R, np.eye(3), atol=1e-12)
+        assert flag.mean() > 0.9
