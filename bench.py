@@ -1,0 +1,330 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the CLOSURE hot path on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py --gpus N --steps K --warmup W            # this build (CUDA path via the C ABI)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle on the host cores
+
+A "step" is one pass of the whole hot path over one synthetic instance batch: walker kernel
+(a0-a7) + compaction kernel (a8), device-resident, timed with CUDA events; the host MEGB (a9)
+is timed separately and is inside the end-to-end number.  The workload at one
+GPU is BASELINE.json configs[1] (C2: 3D registration, N=50, 65,536 walkers x 1,000 iterations).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+from paper_2403_09990_b200 import instances as I
+
+METRIC = "walker_steps_per_sec"
+UNIT = "walker-steps/s"
+WALK_SEED = 42
+
+# Algorithmic flops of the walker kernel's inner loops (FMA = 2):
+#   one (pose, constraint) pair  = 3 FMA + 1 compare/max                      = 7
+#   one per-constraint set-up    = R a (6 FMA + 3 MUL) + 6 ADD/SUB + |u|^2 (2 FMA + MUL) = 26 (+1 on the ladder)
+FLOP_PAIR, FLOP_SETUP_A, FLOP_SETUP_L = 7.0, 26.0, 27.0
+
+
+def _params_dict(P) -> dict:
+    return dict(mode="ROT" if P.mode == 0 else "TRANS", N_P=P.n_p, N_P_star=P.n_p_star, N_T=P.n_t,
+                gamma=P.gamma, omega0=P.omega0, v0=P.v0, t_p=P.t_p, theta_p=P.theta_p)
+
+
+def _workload(config: int):
+    inst = I.make_instance(config)
+    S0 = I.make_init_poses(inst, 128)
+    return inst, S0
+
+
+# ------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._pump, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------- oracle legs
+def _oracle_leg(inst, S0, walkers: int, steps: int, threads: int, seed: int) -> float:
+    import oracle
+    ids = np.arange(walkers, dtype=np.int64) * max(1, inst.num_walkers // walkers)   # strided subset
+    t0 = time.perf_counter()
+    oracle.walk(inst, inst.params, S0, ids, steps, seed, n_threads=threads)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(inst, S0) -> dict:
+    """The oracle as it stands on the host cores, on a bounded sample of the same workload."""
+    import oracle
+    oracle.build()
+    threads = os.cpu_count() or 1
+    P = inst.params
+    per_ws = 2.5e-8 * (P.n_p + P.n_p_star * P.n_t) * inst.n * 1.4        # rough CPU-seconds per walker-step
+    walkers = int(min(256, max(threads, round(20.0 / (per_ws * inst.num_steps)))))
+    dt = _oracle_leg(inst, S0, walkers, inst.num_steps, threads, WALK_SEED)
+    return {"value": walkers * inst.num_steps / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": f"{walkers} strided walkers x {inst.num_steps} iterations of the same instance, "
+                      f"OpenMP over walkers, {dt:.2f} s wall"}
+
+
+def run_reference(args) -> None:
+    """--impl reference: the oracle timed on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+    oracle.build()
+    inst, S0 = _workload(args.config)
+    threads = os.cpu_count() or 1
+    P = inst.params
+    per_ws = 2.5e-8 * (P.n_p + P.n_p_star * P.n_t) * inst.n * 1.4
+    walkers = int(min(256, max(threads, round(20.0 / (per_ws * inst.num_steps)))))
+    for w in range(args.warmup):
+        _oracle_leg(inst, S0, max(threads, walkers // 8), max(1, inst.num_steps // 8), threads, WALK_SEED + w)
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        _oracle_leg(inst, S0, walkers, inst.num_steps, threads, WALK_SEED + k)
+    dt = time.perf_counter() - t0
+    value = args.steps * walkers * inst.num_steps / dt
+    sample = f"per step: {walkers} strided walkers x {inst.num_steps} iterations (of {inst.num_walkers} walkers)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": inst.name, "N": inst.n, "walkers": inst.num_walkers, "iterations": inst.num_steps,
+                   "params": _params_dict(P), "S0": 128},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ------------------------------------------------------------------------------- this build
+def run_cuda(args) -> None:
+    import torch
+    import torch.distributed as dist
+    from paper_2403_09990_b200 import binding as B
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.load_library()     # fails loudly if libclosure_b200.so is missing
+
+    inst, S0 = _workload(args.config)
+    P = inst.params
+    W, S, nb = inst.num_walkers, inst.num_steps, inst.batch
+    insts = [inst] if nb == 1 else [I.make_instance(args.config, b) for b in range(nb)]
+    S0s = [S0] if nb == 1 else [I.make_init_poses(it, 128) for it in insts]
+    # Weak scaling: every rank walks W walkers per instance with its own
+    # walker-id range [rank*W, (rank+1)*W); walkers are independent, no collective
+    # sits on the data path.
+    begin = rank * W
+    handles = []
+    for it, s0 in zip(insts, S0s):
+        h = B.Closure.closure_create(it)
+        h.closure_set_init(s0)
+        handles.append(h)
+    dev = torch.device("cuda", local)
+    samples = torch.empty((nb * W, 12), dtype=torch.float64, device=dev)
+    flags = torch.empty((nb * W,), dtype=torch.uint8, device=dev)
+    compacted = torch.empty((nb * W, 12), dtype=torch.float64, device=dev)
+    count = torch.zeros((1,), dtype=torch.int64, device=dev)
+    flush = torch.empty((256 << 20,), dtype=torch.uint8, device=dev)      # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def walk(seed):
+        if nb == 1:
+            handles[0].closure_sample(W, S, seed, samples, flags, stream, walker_begin=begin)
+        else:
+            B.closure_sample_batch(handles, W, S, [seed + 1000 * b for b in range(nb)],
+                                   samples.view(nb, W, 12), flags.view(nb, W), stream)
+
+    def step(seed, ev=None):
+        if ev:
+            ev[0].record(stream)
+        walk(seed)
+        if ev:
+            ev[1].record(stream)
+        handles[0].closure_compact(samples, flags, compacted, count, stream)
+        if ev:
+            ev[2].record(stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    peak64, _ = B.closure_alu_peak(64)
+    for w in range(args.warmup):
+        step(WALK_SEED + 100 + w)
+        flush.fill_(w)
+    barrier()
+    clocks = ClockSampler(local)
+    clocks.start()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_begin.record(stream)
+    for k in range(args.steps):
+        step(WALK_SEED + k, evs[k])
+        flush.fill_(k)                                                     # L2 flush between iterations
+    t_end.record(stream)
+    barrier()
+    clk = clocks.stop()
+    total_ms = t_begin.elapsed_time(t_end)
+    if world > 1:
+        tt = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms = float(tt.item())
+    walk_ms = [e[0].elapsed_time(e[1]) for e in evs]
+    comp_ms = [e[1].elapsed_time(e[2]) for e in evs]
+    units = float(world) * nb * W * S * args.steps
+    value = units / (total_ms * 1e-3)
+
+    out = None
+    if rank == 0:
+        # executed work of one step (deterministic: same seed as timed step 0), counted by an untimed launch
+        handles[0].closure_enable_stats(True)
+        walk(WALK_SEED)
+        st = handles[0].closure_get_stats()
+        handles[0].closure_enable_stats(False)
+        flops = FLOP_PAIR * (st["perturb_pairs"] + st["ladder_pairs"]) + FLOP_SETUP_A * st["perturb_setups"] \
+            + FLOP_SETUP_L * st["ladder_setups"]
+        walk_s = statistics.mean(walk_ms) * 1e-3
+        achieved = flops / walk_s / 1e12
+        nominal_pairs = (P.n_p + P.n_p_star * P.n_t) * inst.n
+        n_cnt = int(count.item())
+        comp_bytes = nb * W * 1 + n_cnt * 96 * 2
+        comp_s = statistics.mean(comp_ms) * 1e-3
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except OSError:
+            pass
+        hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+
+        # end to end through the C ABI with HOST buffers: create + set_init (H2D) + walk + compact +
+        # D2H of the compacted cloud + host MEGB, every step.
+        e2e_steps = max(1, min(args.steps, 3))
+        megb_s, d2h = [], 0
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for k in range(e2e_steps):
+            hs = []
+            for it, s0 in zip(insts, S0s):
+                h = B.Closure.closure_create(it)
+                h.closure_set_init(s0)
+                hs.append(h)
+            for b, h in enumerate(hs):
+                r = h.closure_run(W, S, WALK_SEED + k + 1000 * b, stream)
+                megb_s.append(r["host_seconds"])
+                d2h += r["count"] * 96 + 8
+                h.closure_destroy()
+        torch.cuda.synchronize()
+        e2e_dt = time.perf_counter() - t0
+        h2d = sum(it.measurements.nbytes + it.betas.nbytes + s0.nbytes + 256 for it, s0 in zip(insts, S0s))
+
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": inst.name, "residual": "3D registration" if inst.residual_type == 2 else
+                       ("2D reprojection" if inst.residual_type == 1 else "pose regression"),
+                       "N": inst.n, "walkers": W, "iterations": S, "instances": nb, "S0": 128,
+                       "params": _params_dict(P), "l2": "256 MiB buffer written between timed iterations",
+                       "sharding": "walker ranges per rank, no collective"},
+            "constraint_evals_per_sec_nominal": value * nominal_pairs,
+            "constraint_evals_per_sec_executed": (st["perturb_pairs"] + st["ladder_pairs"]) / walk_s * world,
+            "latency_ms": {"walker_kernel": statistics.mean(walk_ms), "compaction_kernel": statistics.mean(comp_ms),
+                           "host_megb": 1e3 * statistics.mean(megb_s), "e2e_per_instance": 1e3 * e2e_dt / (e2e_steps * nb)},
+            "boundary_fraction": n_cnt / float(nb * W),
+            "roofline": {"bound": "alu", "kernel": "walker_kernel", "achieved": achieved, "peak": peak64 / 1e12,
+                         "unit": "TFLOP/s", "frac": achieved / (peak64 / 1e12), "traffic": None,
+                         "peak_source": "closure_alu_peak(64): DFMA chain measured in this run",
+                         "flops_per_launch": flops, "executed_pairs_per_walker_step":
+                             (st["perturb_pairs"] + st["ladder_pairs"]) / st["walker_steps"]},
+            "roofline_compaction": {"bound": "hbm", "kernel": "compact_kernel", "achieved": comp_bytes / comp_s / 1e9,
+                                    "peak": hbm_peak, "unit": "GB/s", "frac": comp_bytes / comp_s / 1e9 / hbm_peak,
+                                    "bytes_per_launch": comp_bytes, "peak_source": "MEASURED_PEAKS.json hbm_gbs"
+                                    if peaks else "fallback 6650"},
+            "e2e": {"value": e2e_steps * nb * W * S / e2e_dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h // e2e_steps},
+            "gpu_launches": args.steps * (-(-nb // 96) + 1),     # walker launch(es) + compaction kernel per step
+            "clocks": clk,
+        }
+        if not args.no_cpu_baseline and world == 1:
+            out["cpu_baseline"] = cpu_baseline(inst, S0)
+    for h in handles:
+        h.closure_destroy()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if out is not None:
+        print(json.dumps(out))
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config 1..5 (default 2 = configs[1])")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()
