@@ -64,6 +64,11 @@ struct Rng {
     }
 };
 
+// max / min by compare-select: fmax()/fmin() on doubles compile to DSETP + FSEL + SEL + LOP3 + moves
+// (IEEE NaN handling); no NaN reaches these call sites (inf - inf never occurs: see margin paths).
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+
 // ---------------------------------------------------------------------------------- small math
 __device__ __forceinline__ void mat3_mul(const double (&A)[9], const double (&B)[9], double (&C)[9])
 {
@@ -398,11 +403,11 @@ __global__ void __launch_bounds__(kBlock, 2) walker_kernel(const __grid_constant
             if (RES == CLOSURE_POSE_REG_SPLIT) {
                 for (int i = 0; i < n; ++i) {
                     const double *row = rows + i * ROW;
-                    rot_margin = fmin(rot_margin, row[12] - sqrt(frob_sq(R, row)));
+                    rot_margin = dmin(rot_margin, row[12] - sqrt(frob_sq(R, row)));
                 }
             }
             for (int j0 = 0; j0 < n_p; j0 += kJT) {
-                double e0[kJT], e1[kJT], e2[kJT], dd[kJT], acc_mx[kJT], dmin[kJT];
+                double e0[kJT], e1[kJT], e2[kJT], dd[kJT], acc_mx[kJT], dmn[kJT];
 #pragma unroll
                 for (int jj = 0; jj < kJT; ++jj) {
                     double x, y, z;
@@ -411,7 +416,7 @@ __global__ void __launch_bounds__(kBlock, 2) walker_kernel(const __grid_constant
                     e0[jj] = d0; e1[jj] = d1; e2[jj] = d2;
                     dd[jj] = fma(d2, d2, fma(d1, d1, d0 * d0));
                     acc_mx[jj] = -CUDART_INF;
-                    dmin[jj] = rot_margin;
+                    dmn[jj] = rot_margin;
                 }
                 if (RS::AFFINE) {
 #pragma unroll
@@ -422,13 +427,13 @@ __global__ void __launch_bounds__(kBlock, 2) walker_kernel(const __grid_constant
                         affine_setup<RES>(R, t, row, u0, u1, u2, c);
 #pragma unroll
                         for (int jj = 0; jj < kJT; ++jj)
-                            acc_mx[jj] = fmax(acc_mx[jj], fma(u0, e0[jj], fma(u1, e1[jj], fma(u2, e2[jj], c))));
+                            acc_mx[jj] = dmax(acc_mx[jj], fma(u0, e0[jj], fma(u1, e1[jj], fma(u2, e2[jj], c))));
                         const double beta = row[RS::BETA];
                         const bool run_ends = (i == n - 1) || (rows[(i + 1) * ROW + RS::BETA] != beta);
                         if (run_ends) {                          // warp-uniform
 #pragma unroll
                             for (int jj = 0; jj < kJT; ++jj) {
-                                dmin[jj] = fmin(dmin[jj], beta - sqrt(fmax(acc_mx[jj] + dd[jj], 0.0)));
+                                dmn[jj] = dmin(dmn[jj], beta - sqrt(dmax(acc_mx[jj] + dd[jj], 0.0)));
                                 acc_mx[jj] = -CUDART_INF;
                             }
                         }
@@ -452,14 +457,14 @@ __global__ void __launch_bounds__(kBlock, 2) walker_kernel(const __grid_constant
                                 const double g1 = row[1] - (K[1] * (p1 / p2) + K[3]);
                                 sq = g0 * g0 + g1 * g1;
                             }
-                            dmin[jj] = fmin(dmin[jj], beta - sqrt(sq));
+                            dmn[jj] = dmin(dmn[jj], beta - sqrt(sq));
                         }
                     }
                     if (STATS) { st_pp += (unsigned long long)n * kJT; st_ps += n; }
                 }
 #pragma unroll
                 for (int jj = 0; jj < kJT; ++jj)
-                    if (j0 + jj < n_p) top.insert(dmin[jj], j0 + jj);
+                    if (j0 + jj < n_p) top.insert(dmn[jj], j0 + jj);
             }
         } else {
             // TRANS (A8 l.12-15, A9): R_j = Exp(theta_p xi_j) R*, t_j = t*
