@@ -67,8 +67,10 @@ typedef struct {
     double theta_p;  /* rotation perturbation scale (the paper's R_p): rotation vector uniform on
                         [-theta_p, theta_p]^3 (R-6) */
     int precision;   /* 64 (fp64, the parity path) or 32 (fp32 arithmetic, fp64 I/O) */
-    int reserved;
+    int flags;       /* bit 0 (CLOSURE_FLAG_EXACT_ONLY): run the plain fp64 kernel even where the fp32-screened
+                        kernel exists (same results bit for bit; for verification and timing) */
 } closure_params;
+#define CLOSURE_FLAG_EXACT_ONLY 1
 
 typedef struct closure_s closure_t;   /* opaque; owns device copies of the instance and of S_0 */
 
@@ -159,12 +161,16 @@ int closure_run(closure_t *h, long long num_walkers, int num_steps, unsigned lon
  * closure_enable_stats(h, 1): executed constraint evaluations per phase (for the roofline's
  * executed-flop count).  closure_get_stats synchronises the stream of that launch. */
 typedef struct {
-    unsigned long long perturb_pairs;   /* (perturbation, constraint) pairs evaluated, step a3 */
-    unsigned long long ladder_pairs;    /* (candidate, constraint) pairs evaluated, step a5 */
+    unsigned long long perturb_pairs;   /* (perturbation, constraint) pairs evaluated in fp64, step a3 */
+    unsigned long long ladder_pairs;    /* (candidate, constraint) pairs evaluated in fp64, step a5 */
     unsigned long long perturb_setups;  /* per-constraint set-ups (R-dependent part), a3 */
     unsigned long long ladder_setups;   /* per-(rung, constraint) set-ups, a5 */
     unsigned long long accepted_steps;  /* iterations that moved the walker */
     unsigned long long walker_steps;    /* walkers x iterations */
+    unsigned long long perturb_pairs_f32; /* pairs evaluated in fp32 by the screening pass, a3 */
+    unsigned long long ladder_pairs_f32;  /* pairs evaluated in fp32 by the lenient ladder pass, a5 */
+    unsigned long long fallback_steps;  /* iterations whose candidate list could not be proven complete */
+    unsigned long long verified_rungs;  /* ladder rungs re-run in fp64 */
 } closure_stats;
 int closure_enable_stats(closure_t *h, int on);
 int closure_get_stats(closure_t *h, closure_stats *out);

@@ -29,7 +29,7 @@ EXPORTS = [
 class ClosureParams(Structure):
     _fields_ = [("mode", c_int), ("n_p", c_int), ("n_p_star", c_int), ("n_t", c_int),
                 ("omega0", c_double), ("v0", c_double), ("gamma", c_double), ("t_p", c_double),
-                ("theta_p", c_double), ("precision", c_int), ("reserved", c_int)]
+                ("theta_p", c_double), ("precision", c_int), ("flags", c_int)]
 
 
 class MegbResult(Structure):
@@ -42,7 +42,9 @@ class MegbResult(Structure):
 class Stats(Structure):
     _fields_ = [("perturb_pairs", c_ulonglong), ("ladder_pairs", c_ulonglong),
                 ("perturb_setups", c_ulonglong), ("ladder_setups", c_ulonglong),
-                ("accepted_steps", c_ulonglong), ("walker_steps", c_ulonglong)]
+                ("accepted_steps", c_ulonglong), ("walker_steps", c_ulonglong),
+                ("perturb_pairs_f32", c_ulonglong), ("ladder_pairs_f32", c_ulonglong),
+                ("fallback_steps", c_ulonglong), ("verified_rungs", c_ulonglong)]
 
 
 class ClosureError(RuntimeError):
@@ -109,7 +111,7 @@ def make_params(p) -> ClosureParams:
     """From any object with the paper's parameter names (e.g. instances.WalkParams)."""
     return ClosureParams(int(p.mode), int(p.n_p), int(p.n_p_star), int(p.n_t), float(p.omega0),
                          float(p.v0), float(p.gamma), float(p.t_p), float(p.theta_p),
-                         int(getattr(p, "precision", 64)), 0)
+                         int(getattr(p, "precision", 64)), int(getattr(p, "flags", 0)))
 
 
 def closure_default_params(residual_type: int) -> ClosureParams:

@@ -149,12 +149,13 @@ void fill_launch(const closure_t *h, WalkLaunch &L)
     std::memset(&L, 0, sizeof(L));
     L.n_p = h->P.n_p; L.n_p_star = h->P.n_p_star; L.n_t = h->P.n_t;
     L.omega0 = h->P.omega0; L.v0 = h->P.v0; L.gamma = h->P.gamma; L.t_p = h->P.t_p; L.theta_p = h->P.theta_p;
+    L.exact_only = h->P.flags & 7;            // bit 0 documented; bits 1-2: debug switches of the screened kernel
 }
 
 bool same_params(const closure_params &a, const closure_params &b)
 {
     return a.mode == b.mode && a.n_p == b.n_p && a.n_p_star == b.n_p_star && a.n_t == b.n_t && a.omega0 == b.omega0 &&
-           a.v0 == b.v0 && a.gamma == b.gamma && a.t_p == b.t_p && a.theta_p == b.theta_p && a.precision == b.precision;
+           a.v0 == b.v0 && a.gamma == b.gamma && a.t_p == b.t_p && a.theta_p == b.theta_p && a.precision == b.precision && a.flags == b.flags;
 }
 
 }  // namespace
@@ -263,7 +264,7 @@ int closure_create(int residual_type, const double *measurements, int n, const d
     cudaError_t e = cudaMalloc(&h->d_rows, bytes);
     if (e == cudaSuccess) e = cudaMemcpy(h->d_rows, rows.data(), bytes, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc(&h->d_desc, sizeof(InstanceDesc));
-    if (e == cudaSuccess) e = cudaMalloc(&h->d_stats, 6 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(&h->d_stats, kNumStats * sizeof(unsigned long long));
     if (e != cudaSuccess) {
         // no handle is returned: the failure text can only be seen through the status code
         cudaFree(h->d_rows); cudaFree(h->d_desc); cudaFree(h->d_stats);
@@ -336,7 +337,7 @@ int closure_sample_range(closure_t *h, long long walker_begin, long long num_wal
     L.out_flags = out_on_boundary;
     L.out_trace = out_trace;
     if (h->stats_on) {
-        cudaError_t e = cudaMemsetAsync(h->d_stats, 0, 6 * sizeof(unsigned long long), stream);
+        cudaError_t e = cudaMemsetAsync(h->d_stats, 0, kNumStats * sizeof(unsigned long long), stream);
         if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync(stats)");
         L.stats = h->d_stats;
     }
@@ -371,7 +372,7 @@ int closure_sample_batch(closure_t *const *handles, int n_instances, long long w
     if (!out_samples || !out_on_boundary) return fail(h0, CLOSURE_EINVAL, "output buffer is NULL");
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     if (h0->stats_on) {
-        cudaError_t e = cudaMemsetAsync(h0->d_stats, 0, 6 * sizeof(unsigned long long), stream);
+        cudaError_t e = cudaMemsetAsync(h0->d_stats, 0, kNumStats * sizeof(unsigned long long), stream);
         if (e != cudaSuccess) return cuda_fail(h0, e, "cudaMemsetAsync(stats)");
     }
     for (int b0 = 0; b0 < n_instances; b0 += kMaxBatch) {
@@ -508,12 +509,14 @@ int closure_enable_stats(closure_t *h, int on)
 int closure_get_stats(closure_t *h, closure_stats *out)
 {
     if (!h || !out) return CLOSURE_EINVAL;
-    unsigned long long v[6];
+    unsigned long long v[kNumStats];
     cudaError_t e = cudaStreamSynchronize(h->last_stream);
     if (e == cudaSuccess) e = cudaMemcpy(v, h->d_stats, sizeof(v), cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) return cuda_fail(h, e, "read of statistics");
     out->perturb_pairs = v[0]; out->ladder_pairs = v[1]; out->perturb_setups = v[2];
     out->ladder_setups = v[3]; out->accepted_steps = v[4]; out->walker_steps = v[5];
+    out->perturb_pairs_f32 = v[6]; out->ladder_pairs_f32 = v[7]; out->fallback_steps = v[8];
+    out->verified_rungs = v[9];
     return CLOSURE_OK;
 }
 

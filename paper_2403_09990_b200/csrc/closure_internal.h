@@ -36,6 +36,7 @@ constexpr int kMaxBatch = 96;
 constexpr int kBlock = 128;       // walkers per CTA (one per thread)
 constexpr int kMaxNT = 64;
 constexpr int kMaxKStar = 20;
+constexpr int kNumStats = 10;
 
 struct WalkLaunch {
     const InstanceDesc *desc[kMaxBatch];      // device pointers, one per instance (gridDim.y)
@@ -48,7 +49,8 @@ struct WalkLaunch {
     double *out_samples;
     unsigned char *out_flags;
     int *out_trace;                           // nullable
-    unsigned long long *stats;                // nullable, 6 counters
+    unsigned long long *stats;                // nullable, kNumStats counters
+    int exact_only;                           // 1: plain fp64 kernel even where the screened kernel exists
 };
 
 int row_doubles(int residual_type);
@@ -56,6 +58,11 @@ int row_doubles(int residual_type);
 // walker_kernel.cu
 cudaError_t launch_walkers(int residual_type, int mode, bool stats, const WalkLaunch &L, int n_instances,
                            int max_rows_bytes, cudaStream_t stream, std::string *why);
+
+// walker_rot_kernel.cu: fp32-screened kernel for ROT mode on REG / POSE_REG / POSE_REG_SPLIT
+bool rot_fast_path_available(int residual_type, int mode);
+cudaError_t launch_walkers_rot_fast(int residual_type, bool stats, const WalkLaunch &L, dim3 grid,
+                                    int max_rows_bytes, cudaStream_t stream);
 
 // compact_kernel.cu
 size_t compact_scratch_bytes(long long n);

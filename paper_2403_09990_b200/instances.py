@@ -40,6 +40,7 @@ class WalkParams:
     gamma: float = 0.5
     t_p: float = 0.1
     theta_p: float = 0.0    # the paper's R_p
+    flags: int = 0          # include/closure.h CLOSURE_FLAG_* (1 = plain fp64 kernel only)
 
 
 @dataclass

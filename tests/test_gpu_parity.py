@@ -136,3 +136,28 @@ def test_samples_are_feasible_and_orthonormal():
             R = s[:9].reshape(3, 3)
             assert np.allclose(R.T @ R, np.eye(3), atol=1e-12)
         assert flag.mean() > 0.9
+
+
+@pytest.mark.parametrize("config,walkers,steps", [(2, 4096, 150), (1, 1024, 200), (4, 2048, 120), (5, 2048, 150)])
+def test_screened_kernel_is_bit_identical_to_exact_kernel(config, walkers, steps):
+    """The fp32-screened kernel takes every decision on fp64 values: outputs and traces must equal the
+    plain fp64 kernel's (CLOSURE_FLAG_EXACT_ONLY) bit for bit, on far more walkers than the oracle replays."""
+    inst = I.make_instance(config)
+    S0 = I.make_init_poses(inst, 128)
+    fast = gpu_walk(inst, inst.params, S0, walkers, steps, 4242)
+    plain = gpu_walk(inst, _small(inst.params, flags=1), S0, walkers, steps, 4242)
+    for a, b in zip(fast, plain):
+        assert np.array_equal(a, b)
+
+
+def test_screened_kernel_falls_back_on_ties():
+    """t_p = 0 makes all N_P distances equal: the candidate list cannot be proven complete, the warp must
+    take the exact path, and results still match the oracle."""
+    inst = I.make_instance(1)
+    P = _small(inst.params, t_p=0.0, n_p=40, n_p_star=4, n_t=10)
+    assert_parity(inst, P, I.make_init_poses(inst, 16), 96, 20, 13)
+    sp = I.to_split(I.make_instance(4))
+    fast = gpu_walk(sp, sp.params, I.make_init_poses(sp, 32), 512, 60, 5)
+    plain = gpu_walk(sp, _small(sp.params, flags=1), I.make_init_poses(sp, 32), 512, 60, 5)
+    for a, b in zip(fast, plain):
+        assert np.array_equal(a, b)
