@@ -64,6 +64,11 @@ bool rot_fast_path_available(int residual_type, int mode);
 cudaError_t launch_walkers_rot_fast(int residual_type, bool stats, const WalkLaunch &L, dim3 grid,
                                     int max_rows_bytes, cudaStream_t stream);
 
+// walker_coop_kernel.cu: warp-cooperative, fp32-certified kernel for ROT mode on REG / POSE_REG / POSE_REG_SPLIT
+bool coop_path_available(int residual_type, int mode, int n_p, int max_n);
+cudaError_t launch_walkers_coop(int residual_type, const WalkLaunch &L, int n_instances, int max_rows_bytes,
+                                cudaStream_t stream);
+
 // compact_kernel.cu
 size_t compact_scratch_bytes(long long n);
 cudaError_t launch_compact(const double *samples, const unsigned char *flags, long long n, double *out,

@@ -1,0 +1,697 @@
+// Warp-cooperative walker kernel for the rotation-boundary sampler (Alg. 2) on
+// the residuals whose squared norm is quadratic in the translation perturbation (Ex.2 registration,
+// Ex.3 pose regression, stacked or split).  One WARP owns one walker; the 32 lanes split the work
+// that Alg. 3 tensorises per walker:
+//
+//   a2-a4  the N_P perturbations are dealt to the lanes (j = lane + 32 q); the per-constraint
+//          set-up u_i = b_i - (R* a_i + t*) is computed ONCE per accepted move (lane i mod 32)
+//          and broadcast through shared memory; a pair costs 3 FFMA + 1 FMNMX in fp32
+//          (packed FFMA2 + FMNMX3 in SASS).  eq. (14)'s values d~_j carry a rigorous error bound
+//          `unc`; the top-N_P* are extracted with warp reductions and the ranking is accepted only
+//          if consecutive values (and the N_P*-th against the next) are more than 2 unc apart.
+//          Otherwise the step falls back to the fp64 evaluation of the plain kernel.
+//   a5-a6  every rung m = 1..N_T is screened first against the two tightest constraints (lane =
+//          (rung, constraint)); rungs with a surviving candidate are then evaluated in full, lane =
+//          (candidate, constraint chunk), in fp32 with a three-way outcome per candidate: violated
+//          for sure / satisfied for sure / undecided -> fp64.
+//
+// Every accept/reject decision is therefore the decision the fp64 arithmetic of walker_kernel.cu
+// takes (DESIGN.md 6.1 "Certified fp32 evaluation"); the pose itself is only ever updated in fp64.
+// Unlike the one-walker-per-thread kernels all lanes of a warp follow the same walker: no
+// divergence between walkers, the set-up is not repeated per register tile, ~100 registers.
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include <stdint.h>
+
+#include "closure_internal.h"
+#include "walker_common.cuh"
+
+namespace closure {
+namespace {
+
+constexpr int kCoopWarps = 4;                 // walkers per CTA
+constexpr int kCoopThreads = 32 * kCoopWarps;
+constexpr unsigned FULL = 0xffffffffu;
+constexpr float kMu19 = 1.9073486328125e-06f;   // 2^-19
+
+// ---------------------------------------------------------------------------------- small helpers
+// order-preserving maps to unsigned keys
+__device__ __forceinline__ uint32_t fkey(float x)
+{
+    const uint32_t b = __float_as_uint(x);
+    return b ^ ((uint32_t)((int32_t)b >> 31) | 0x80000000u);
+}
+__device__ __forceinline__ float fkey_inv(uint32_t k)
+{
+    return __uint_as_float((k & 0x80000000u) ? (k ^ 0x80000000u) : ~k);
+}
+__device__ __forceinline__ unsigned long long dkey(double x)
+{
+    const unsigned long long b = (unsigned long long)__double_as_longlong(x);
+    return b ^ ((unsigned long long)((long long)b >> 63) | 0x8000000000000000ull);
+}
+__device__ __forceinline__ float wmax_nonneg(float v)      // v >= 0 (or NaN, which wins: callers then fall back)
+{
+    return __uint_as_float(__reduce_max_sync(FULL, __float_as_uint(v)));
+}
+__device__ __forceinline__ double wmin_f64(double v)
+{
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) v = dmin(v, __shfl_xor_sync(FULL, v, o));
+    return v;
+}
+
+// packed fp32 pairs (FFMA2 on sm_100a)
+__device__ __forceinline__ unsigned long long pk2(float lo, float hi)
+{
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk2(unsigned long long v, float &lo, float &hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c)
+{
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+
+// Philox4x32-10 for NJ counters that differ only in word 2 (= perturbation index): rolled rounds,
+// NJ independent dependency chains.
+template <int NJ>
+__device__ __forceinline__ void philox_batch(const Rng &rng, uint32_t s, const int (&j)[NJ], uint32_t (&x)[NJ],
+                                             uint32_t (&y)[NJ], uint32_t (&z)[NJ])
+{
+    uint32_t c0[NJ], c1[NJ], c2[NJ], c3[NJ];
+#pragma unroll
+    for (int q = 0; q < NJ; ++q) { c0[q] = rng.w_lo; c1[q] = s; c2[q] = (uint32_t)j[q]; c3[q] = 1u | rng.w_hi8; }
+    uint32_t k0 = rng.k0, k1 = rng.k1;
+#pragma unroll 1
+    for (int r = 0; r < 10; ++r) {
+#pragma unroll
+        for (int q = 0; q < NJ; ++q) {
+            const uint32_t hi0 = __umulhi(0xD2511F53u, c0[q]), lo0 = 0xD2511F53u * c0[q];
+            const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2[q]), lo1 = 0xCD9E8D57u * c2[q];
+            c0[q] = hi1 ^ c1[q] ^ k0;
+            c1[q] = lo1;
+            c2[q] = hi0 ^ c3[q] ^ k1;
+            c3[q] = lo0;
+        }
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+#pragma unroll
+    for (int q = 0; q < NJ; ++q) { x[q] = c0[q]; y[q] = c1[q]; z[q] = c2[q]; }
+}
+
+// fp32 image of pm1(): |pm1f(x) - pm1(x)| <= 2^-22.
+__device__ __forceinline__ float pm1f(uint32_t x)
+{
+    return fmaf((float)x, 4.656612873077392578125e-10f, 2.3283064365386962890625e-10f - 1.0f);
+}
+
+// fp32 image of one set-up row and the bound eps on |v32 - v64| for ANY perturbation with
+// |d_c| <= t_p, where v = c - 2 u.d is evaluated as three chained FMAs:
+//   inputs: (u, c) rounded to fp32 (relative 2^-24 each); e = -2 d from pm1f (absolute 6 * 2^-24 * 2 t_p);
+//   three FFMA roundings (2^-24 of the partial sums, each <= |c| + 2 t_p |u|_1)
+//   =>  |v32 - v64| <= 2^-24 (4 |c| + 10 * 2 t_p |u|_1).
+// eps = 2^-19 (|c| + 2 t_p |u|_1 + 3 t_p^2) leaves a factor > 3 for the roundings of eps itself,
+// of the threshold -|d|^2 in fp32 (<= 15 * 2^-24 * 3 t_p^2) and of the shifted constants c -+ eps.
+__device__ __forceinline__ void screen_row(double u0, double u1, double u2, double c, float tp2, float tp2sq3,
+                                           float &f0, float &f1, float &f2, float &fc, float &eps)
+{
+    f0 = (float)u0; f1 = (float)u1; f2 = (float)u2; fc = (float)c;
+    const float mag = fabsf(fc) + tp2 * (fabsf(f0) + fabsf(f1) + fabsf(f2)) + tp2sq3;
+    eps = mag * (kMu19 * 1.001f);
+}
+
+// The plain kernel's phase A for the NQ perturbations of this lane (same arithmetic as
+// walker_kernel.cu): exact eq. (14) margins, one sqrt per run of equal bounds.  jv[q] < 0: empty.
+template <int RES, int NJ>
+__device__ __forceinline__ void exact_margins(const double (&R)[9], const double (&t)[3], const double *rows, int n,
+                                              const Rng &rng, uint32_t s, double t_p, double rot_margin,
+                                              const int (&jv)[NJ], double (&d)[NJ])
+{
+    using RS = Res<RES>;
+    constexpr int ROW = RS::ROW;
+    uint32_t x[NJ], y[NJ], z[NJ];
+    philox_batch<NJ>(rng, s, jv, x, y, z);
+    double e0[NJ], e1[NJ], e2[NJ], dd[NJ], acc_mx[NJ];
+#pragma unroll
+    for (int q = 0; q < NJ; ++q) {
+        const double d0 = t_p * pm1(x[q]), d1 = t_p * pm1(y[q]), d2 = t_p * pm1(z[q]);
+        dd[q] = fma(d2, d2, fma(d1, d1, d0 * d0));
+        e0[q] = d0 * -2.0; e1[q] = d1 * -2.0; e2[q] = d2 * -2.0;
+        acc_mx[q] = -CUDART_INF;
+        d[q] = rot_margin;
+    }
+#pragma unroll 1
+    for (int i = 0; i < n; ++i) {
+        const double *row = rows + i * ROW;
+        double u0, u1, u2, c;
+        affine_setup<RES>(R, t, row, u0, u1, u2, c);
+#pragma unroll
+        for (int q = 0; q < NJ; ++q)
+            acc_mx[q] = dmax(acc_mx[q], fma(u0, e0[q], fma(u1, e1[q], fma(u2, e2[q], c))));
+        const double beta = row[RS::BETA];
+        const bool run_ends = (i == n - 1) || (rows[(i + 1) * ROW + RS::BETA] != beta);
+        if (run_ends) {                          // warp-uniform
+#pragma unroll
+            for (int q = 0; q < NJ; ++q) {
+                d[q] = dmin(d[q], beta - sqrt(dmax(acc_mx[q] + dd[q], 0.0)));
+                acc_mx[q] = -CUDART_INF;
+            }
+        }
+    }
+}
+
+// fp64 in_purse of ladder candidate (Rm, t* + d_j), constraints dealt to the lanes; the arithmetic
+// of the plain kernel's ladder.  Warp-uniform result.
+template <int RES>
+__device__ __forceinline__ bool exact_candidate_feasible(const double (&Rm)[9], const double (&t)[3], const double *rows,
+                                                         int n, const Rng &rng, uint32_t s, int j, double t_p, int lane)
+{
+    using RS = Res<RES>;
+    constexpr int ROW = RS::ROW;
+    double x, y, z;
+    rng.xi3(s, (uint32_t)j, 1u, x, y, z);
+    const double d0 = t_p * x, d1 = t_p * y, d2 = t_p * z;
+    const double kdd = -fma(d2, d2, fma(d1, d1, d0 * d0));
+    const double k0 = -2.0 * d0, k1 = -2.0 * d1, k2 = -2.0 * d2;
+    bool ok = true;
+    for (int i = lane; i < n; i += 32) {
+        const double *row = rows + i * ROW;
+        double u0, u1, u2, c;
+        affine_setup<RES>(Rm, t, row, u0, u1, u2, c);
+        if (RES == CLOSURE_POSE_REG_SPLIT) {
+            if (!(frob_sq(Rm, row) <= row[13])) ok = false;
+        }
+        const double cb = c - row[RS::BETA + 1];
+        const double v = fma(u0, k0, fma(u1, k1, fma(u2, k2, cb)));
+        if (!(v <= kdd)) ok = false;
+    }
+    return __all_sync(FULL, ok);
+}
+
+struct CoopSmem {
+    size_t run_end, run_bf, warp0, per_warp, rowsA, rowsL, pert, ab, RmS, dex, candj, total;
+};
+
+__host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, int nq)
+{
+    CoopSmem s;
+    size_t o = 16 + (size_t)((rows_bytes + 15) & ~15);
+    s.run_end = o; o += (size_t)((n * 4 + 15) & ~15);
+    s.run_bf = o;  o += (size_t)((n * 4 + 15) & ~15);
+    s.warp0 = o;
+    size_t w = 0;
+    s.rowsA = w; w += (size_t)n * 16;
+    s.rowsL = w; w += (size_t)n * 16;
+    s.pert = w;  w += (size_t)nq * 32 * 16;
+    s.ab = w;    w += (size_t)n_t * 16;
+    s.RmS = w;   w += (size_t)((n_t * 72 + 15) & ~15);
+    s.dex = w;   w += (size_t)nq * 32 * 8;
+    s.candj = w; w += 32 * 4;
+    s.per_warp = w;
+    s.total = o + (size_t)kCoopWarps * w;
+    return s;
+}
+
+// ---------------------------------------------------------------------------------- the kernel
+template <int RES, int NQ>
+__global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __grid_constant__ WalkLaunch L)
+{
+    using RS = Res<RES>;
+    constexpr int ROW = RS::ROW;
+    constexpr int NPK = NQ / 2;            // packed pairs of perturbations
+    constexpr bool ODD = (NQ & 1) != 0;    // plus one scalar slot
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ int n_runs_s;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const InstanceDesc *__restrict__ D = L.desc[blockIdx.y];
+    const int n = D->n;
+    const int rows_bytes = D->rows_bytes;
+    const int n_p = L.n_p, n_ps = L.n_p_star, n_t = L.n_t;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
+    double *rows = reinterpret_cast<double *>(smem_raw + 16);
+    stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ);
+    int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
+    float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
+    if (warp == 0) {                                   // runs of equal bounds (rows are sorted by bound)
+        int cnt = 0;
+        for (int base = 0; base < n; base += 32) {
+            const int i = base + lane;
+            bool end = false;
+            double beta = 0.0;
+            if (i < n) {
+                beta = rows[i * ROW + RS::BETA];
+                end = (i == n - 1) || (rows[(i + 1) * ROW + RS::BETA] != beta);
+            }
+            const unsigned m = __ballot_sync(FULL, end);
+            if (end) {
+                const int r = cnt + __popc(m & ((1u << lane) - 1u));
+                run_end[r] = i;
+                run_bf[r] = (float)beta;
+            }
+            cnt += __popc(m);
+        }
+        if (lane == 0) n_runs_s = cnt;
+    }
+    __syncthreads();
+    const int n_runs = n_runs_s;
+
+    const long long local = (long long)blockIdx.x * kCoopWarps + warp;
+    if (local >= L.num_walkers) return;                // no block-wide barrier below this line
+    unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
+    float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);
+    float4 *rowsL = reinterpret_cast<float4 *>(wp + lay.rowsL);
+    float4 *pert = reinterpret_cast<float4 *>(wp + lay.pert);
+    double2 *ab = reinterpret_cast<double2 *>(wp + lay.ab);
+    double *RmS = reinterpret_cast<double *>(wp + lay.RmS);
+    double *dex = reinterpret_cast<double *>(wp + lay.dex);      // fp64 fallback: exact d_j, [q][lane]
+    int *candj = reinterpret_cast<int *>(wp + lay.candj);
+
+    const unsigned long long w = (unsigned long long)(L.walker_begin + local);
+    const unsigned long long seed = L.seed[blockIdx.y];
+    Rng rng;
+    rng.w_lo = (uint32_t)w;
+    rng.w_hi8 = (uint32_t)(w >> 32) << 8;
+    rng.k0 = (uint32_t)seed;
+    rng.k1 = (uint32_t)(seed >> 32);
+
+    // ---- a1: walker init, replicated on the lanes (Alg. 2 l.8-9)
+    double R[9], t[3], vel[3];
+    init_walker<CLOSURE_MODE_ROT>(D, L, rng, w, R, t, vel);
+    for (int m = lane; m < n_t; m += 32) {             // ladder dT_m = gamma^(m-1) by repeated multiplication
+        double dT = 1.0;
+        for (int q = 0; q < m; ++q) dT = dT * L.gamma;
+        const double p0 = dT * vel[0], p1 = dT * vel[1], p2 = dT * vel[2];
+        double A, B;
+        exp_coeffs(p0 * p0 + p1 * p1 + p2 * p2, A, B);
+        ab[m] = make_double2(A * dT, B * dT * dT);
+    }
+    __syncwarp();
+
+    const double t_p = L.t_p;
+    const float tpf = (float)t_p * 1.0000002f;          // >= t_p
+    const float tp2 = 2.0f * tpf, tp2sq3 = 3.0f * tpf * tpf;
+    const float m2tp = -2.0f * (float)t_p;
+    const int H = (n_t <= 16) ? 2 : 1;                  // hot constraints screened per rung
+    const int RPB = 32 / H;                             // rungs per screening block
+    const int KP = n_ps;                                // ladder candidates
+    const int NCH = 32 / KP;                            // constraint chunks of the full evaluation
+    const int ek = lane % KP, ech = lane / KP;
+    const bool e_act = ech < NCH;
+    unsigned e_mask = 0u;                               // lanes that share this lane's candidate
+    for (int c = 0; c < NCH; ++c) e_mask |= 1u << (ek + c * KP);
+    const unsigned kmask = (KP >= 32) ? FULL : ((1u << KP) - 1u);
+
+    unsigned long long st_pp32 = 0, st_lp32 = 0, st_ps = 0, st_ls = 0, st_acc = 0, st_fb = 0, st_vr = 0, st_pp = 0,
+                       st_lp = 0;
+    const bool stats = L.stats != nullptr;
+    bool hit = false;
+    bool moved = true;
+    int hot0 = 0, hot1 = 0;
+    float epsA = 0.f;
+    double rot_margin = CUDART_INF;
+    // cached across iterations while the pose does not move
+    float qf0 = 0.f, qf1 = 0.f, qf2 = 0.f, qcbl = CUDART_INF_F;   // screening row of (rung, hot) of this lane, block 0
+    bool q_valid = false;
+    int full_m = -1;                                    // rung whose rows sit in rowsL
+    float epsL = 0.f;
+    bool rdeadL = false;
+
+    for (int s = 1; s <= L.num_steps; ++s) {
+        // ================================================== set-up at the current pose (only after a move)
+        if (moved) {
+            float eps_l = 0.f;
+            uint32_t h1 = 0u, h2 = 0u;
+            double rm_l = CUDART_INF;
+            for (int i = lane; i < n; i += 32) {
+                const double *row = rows + i * ROW;
+                double u0, u1, u2, c;
+                affine_setup<RES>(R, t, row, u0, u1, u2, c);
+                float f0, f1, f2, fc, eps;
+                screen_row(u0, u1, u2, c, tp2, tp2sq3, f0, f1, f2, fc, eps);
+                rowsA[i] = make_float4(f0, f1, f2, fc);
+                eps_l = fmaxf(eps_l, eps);
+                const uint32_t hk = (fkey(fc - (float)row[RS::BETA + 1]) & ~0xfffu) | (uint32_t)i;   // tightest first
+                if (hk > h1) { h2 = h1; h1 = hk; } else if (hk > h2) h2 = hk;
+                if (RES == CLOSURE_POSE_REG_SPLIT) rm_l = dmin(rm_l, row[12] - sqrt(frob_sq(R, row)));
+            }
+            epsA = wmax_nonneg(eps_l);
+            const uint32_t g1 = __reduce_max_sync(FULL, h1);
+            const uint32_t g2 = __reduce_max_sync(FULL, h1 == g1 ? h2 : h1);
+            hot0 = (int)(g1 & 0xfffu);
+            hot1 = (g2 != 0u) ? (int)(g2 & 0xfffu) : hot0;
+            if (RES == CLOSURE_POSE_REG_SPLIT) rot_margin = wmin_f64(rm_l);
+            for (int m = lane; m < n_t; m += 32) {       // Exp(dT_m w) R* for every rung
+                const double2 c2 = ab[m];
+                double Rm[9];
+                rotate_left(R, vel[0], vel[1], vel[2], c2.x, c2.y, Rm);
+#pragma unroll
+                for (int e = 0; e < 9; ++e) RmS[m * 9 + e] = Rm[e];
+            }
+            q_valid = false;
+            full_m = -1;
+            if (stats) st_ps += n;
+            __syncwarp();
+        }
+
+        // ================================================== a2: perturbations of this lane
+        unsigned long long p0[NPK > 0 ? NPK : 1], p1[NPK > 0 ? NPK : 1], p2[NPK > 0 ? NPK : 1];
+        float o0 = 0.f, o1 = 0.f, o2 = 0.f;                  // the odd slot NQ-1
+        float dd[NQ];
+        {
+            int jv[NQ];
+            uint32_t x[NQ], y[NQ], z[NQ];
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) jv[q] = lane + 32 * q;
+            philox_batch<NQ>(rng, (uint32_t)s, jv, x, y, z);
+            float e0[NQ], e1[NQ], e2[NQ];
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) {
+                e0[q] = m2tp * pm1f(x[q]); e1[q] = m2tp * pm1f(y[q]); e2[q] = m2tp * pm1f(z[q]);
+                dd[q] = 0.25f * fmaf(e2[q], e2[q], fmaf(e1[q], e1[q], e0[q] * e0[q]));
+                pert[32 * q + lane] = make_float4(e0[q], e1[q], e2[q], -dd[q]);
+            }
+#pragma unroll
+            for (int k = 0; k < NPK; ++k) {
+                p0[k] = pk2(e0[2 * k], e0[2 * k + 1]);
+                p1[k] = pk2(e1[2 * k], e1[2 * k + 1]);
+                p2[k] = pk2(e2[2 * k], e2[2 * k + 1]);
+            }
+            if (ODD) { o0 = e0[NQ - 1]; o1 = e1[NQ - 1]; o2 = e2[NQ - 1]; }
+        }
+
+        // ================================================== a3: eq. (14) in fp32 with error bound
+        float dt[NQ];
+        float unc_l = 0.f;
+        {
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) dt[q] = CUDART_INF_F;
+            const float E0 = epsA + tp2sq3 * kMu19;          // bound on |a32 - a64| up to its own rounding
+            int i = 0;
+            for (int r = 0; r < n_runs; ++r) {
+                const int end = run_end[r];
+                const float bf = run_bf[r];
+                float mx[NQ];
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) mx[q] = -CUDART_INF_F;
+#pragma unroll 2
+                for (; i <= end; ++i) {
+                    const float4 f = rowsA[i];
+                    const unsigned long long F0 = pk2(f.x, f.x), F1 = pk2(f.y, f.y), F2 = pk2(f.z, f.z),
+                                             FC = pk2(f.w, f.w);
+#pragma unroll
+                    for (int k = 0; k < NPK; ++k) {
+                        const unsigned long long v = fma2(F0, p0[k], fma2(F1, p1[k], fma2(F2, p2[k], FC)));
+                        float lo, hi;
+                        upk2(v, lo, hi);
+                        mx[2 * k] = fmaxf(mx[2 * k], lo);
+                        mx[2 * k + 1] = fmaxf(mx[2 * k + 1], hi);
+                    }
+                    if (ODD) mx[NQ - 1] = fmaxf(mx[NQ - 1], fmaf(f.x, o0, fmaf(f.y, o1, fmaf(f.z, o2, f.w))));
+                }
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) {
+                    // a ~ max_i |u_i - d|^2 within E0 + 2^-22 a;  sq ~ sqrt(a) within 2^-21 relative
+                    const float a = fmaxf(mx[q] + dd[q], 1e-30f);
+                    const float rr = rsqrtf(a);
+                    const float sq = a * rr;
+                    const float du = 1.01f * fmaf(E0, rr, (bf + sq) * kMu19);
+                    unc_l = fmaxf(unc_l, du);
+                    dt[q] = fminf(dt[q], bf - sq);
+                }
+            }
+            if (stats) st_pp32 += (unsigned long long)n * n_p;
+        }
+
+        // ================================================== a4: top-N_P* with certified ranking
+        bool certified;
+        {
+            const float rmf = (float)rot_margin;            // +inf unless POSE_REG_SPLIT
+            uint32_t key[NQ];
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) {
+                const float v = (lane + 32 * q < n_p) ? fminf(dt[q], rmf) : -CUDART_INF_F;
+                key[q] = (fkey(v) & ~7u) | (uint32_t)q;
+            }
+            // local sort, descending (odd-even transposition network)
+#pragma unroll
+            for (int pass = 0; pass < NQ; ++pass)
+#pragma unroll
+                for (int a = (pass & 1); a + 1 < NQ; a += 2) {
+                    const uint32_t hi = max(key[a], key[a + 1]), lo = min(key[a], key[a + 1]);
+                    key[a] = hi; key[a + 1] = lo;
+                }
+            float unc = wmax_nonneg(unc_l);
+            if (RES == CLOSURE_POSE_REG_SPLIT) unc += 1.2e-7f * fabsf(rmf);
+            float myval = -CUDART_INF_F;
+            int myj = -1;
+            for (int r = 0; r <= n_ps; ++r) {               // extract the N_P* + 1 largest
+                const uint32_t g = __reduce_max_sync(FULL, key[0]);
+                const unsigned who = __ballot_sync(FULL, key[0] == g);
+                const int src = __ffs(who) - 1;
+                if (lane == r) { myval = fkey_inv(g); myj = src + 32 * (int)(g & 7u); }
+                if (lane == src) {
+#pragma unroll
+                    for (int q = 0; q + 1 < NQ; ++q) key[q] = key[q + 1];
+                    key[NQ - 1] = 0u;
+                }
+            }
+            const float prev = __shfl_up_sync(FULL, myval, 1);
+            bool ok = true;
+            if (lane < n_ps) ok = (myval > -CUDART_INF_F) && (myval < CUDART_INF_F);
+            if (lane >= 1 && lane <= n_ps) {
+                const bool none_left = (lane == n_ps) && (myval == -CUDART_INF_F);
+                const float need = fmaf(2.0f, unc, kMu19 * (fabsf(prev) + fabsf(myval)));
+                ok = ok && (none_left || (prev - myval > need));
+            }
+            if (L.exact_only & 4) ok = false;                // debug: every step takes the fp64 fallback
+            certified = __all_sync(FULL, ok);
+            if (certified && lane < n_ps) candj[lane] = myj;
+        }
+        if (!certified) {
+            // ---------------- fp64 fallback: the plain kernel's phase A, then (d desc, j asc) selection.
+            // Rare, so it is written for few registers: one perturbation at a time, values in shared memory.
+#pragma unroll 1
+            for (int q = 0; q < NQ; ++q) {
+                const int jv[1] = { lane + 32 * q };
+                double d[1];
+                exact_margins<RES, 1>(R, t, rows, n, rng, (uint32_t)s, t_p, rot_margin, jv, d);
+                dex[32 * q + lane] = (jv[0] < n_p) ? d[0] : -CUDART_INF;
+            }
+            unsigned taken = 0u;                             // slots of this lane already extracted
+#pragma unroll 1
+            for (int r = 0; r < n_ps; ++r) {
+                unsigned long long best = 0ull;
+                int bq = 0;
+#pragma unroll 1
+                for (int q = 0; q < NQ; ++q) {
+                    const unsigned long long kq = ((taken >> q) & 1u) || (lane + 32 * q >= n_p) ? 0ull : dkey(dex[32 * q + lane]);
+                    if (kq > best) { best = kq; bq = q; }
+                }
+                const uint32_t ghi = __reduce_max_sync(FULL, (uint32_t)(best >> 32));
+                const uint32_t glo = __reduce_max_sync(FULL, ((uint32_t)(best >> 32) == ghi) ? (uint32_t)best : 0u);
+                const unsigned long long g = ((unsigned long long)ghi << 32) | glo;
+                const int jm = (best == g && best != 0ull) ? lane + 32 * bq : 0x7fffffff;
+                const int jwin = __reduce_min_sync(FULL, jm);
+                if (jm == jwin) taken |= 1u << bq;
+                if (lane == 0) candj[r] = jwin;
+            }
+            if (stats) { ++st_fb; st_pp += (unsigned long long)n * n_p; }
+        }
+        __syncwarp();                                       // pert[], candj[] visible to all lanes
+
+        // ================================================== a5-a6: ladder, first feasible rung
+        int m0 = 0;
+        unsigned win = 0u;
+        for (int mb = 0; mb < n_t && m0 == 0; mb += RPB) {
+            // ---- screening of RPB rungs against the H tightest constraints: lane = (rung, constraint)
+            const int mq = mb + lane / H, hq = lane % H;
+            const bool q_act = (lane / H < RPB) && (mq < n_t);
+            float f0 = qf0, f1 = qf1, f2 = qf2, cbl = qcbl;
+            if (!(q_valid && mb == 0)) {
+                cbl = CUDART_INF_F; f0 = f1 = f2 = 0.f;
+                if (q_act) {
+                    double Rm[9];
+#pragma unroll
+                    for (int e = 0; e < 9; ++e) Rm[e] = RmS[mq * 9 + e];
+                    const double *row = rows + (hq == 0 ? hot0 : hot1) * ROW;
+                    double u0, u1, u2, c;
+                    affine_setup<RES>(Rm, t, row, u0, u1, u2, c);
+                    float fcb, eps;
+                    screen_row(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, f0, f1, f2, fcb, eps);
+                    cbl = fcb - eps;
+                    if (RES == CLOSURE_POSE_REG_SPLIT) {
+                        if (!(frob_sq(Rm, row) <= row[13])) cbl = CUDART_INF_F;   // rung dead for every candidate
+                    }
+                }
+                if (mb == 0) { qf0 = f0; qf1 = f1; qf2 = f2; qcbl = cbl; q_valid = true; }
+                if (stats) st_ls += (unsigned long long)min(RPB, n_t - mb) * H;
+            }
+            unsigned alive = 0u;
+            if (q_act) {
+                for (int k = 0; k < KP; ++k) {
+                    const float4 c4 = pert[candj[k]];
+                    const float v = fmaf(f0, c4.x, fmaf(f1, c4.y, fmaf(f2, c4.z, cbl)));
+                    if (!(v > c4.w)) alive |= 1u << k;       // not violated beyond the error bound
+                }
+            }
+            if (L.exact_only & 2) alive = q_act ? kmask : 0u;   // debug: the screening kills nothing
+            if (H == 2) alive &= __shfl_xor_sync(FULL, alive, 1);
+            unsigned qmask = __ballot_sync(FULL, q_act && hq == 0 && alive != 0u);
+            if (stats) st_lp32 += (unsigned long long)min(RPB, n_t - mb) * H * KP;
+
+            // ---- full evaluation of the surviving rungs, in order
+            while (qmask != 0u && m0 == 0) {
+                const int l0 = __ffs(qmask) - 1;
+                qmask &= qmask - 1u;
+                const int m1 = mb + l0 / H;
+                const unsigned cand_alive = __shfl_sync(FULL, alive, l0);
+                double Rm[9];
+#pragma unroll
+                for (int e = 0; e < 9; ++e) Rm[e] = RmS[m1 * 9 + e];
+                if (full_m != m1) {
+                    __syncwarp();                            // earlier readers of rowsL are done
+                    float eps_l = 0.f;
+                    bool rdead = false;
+                    for (int i = lane; i < n; i += 32) {
+                        const double *row = rows + i * ROW;
+                        double u0, u1, u2, c;
+                        affine_setup<RES>(Rm, t, row, u0, u1, u2, c);
+                        if (RES == CLOSURE_POSE_REG_SPLIT) {
+                            if (!(frob_sq(Rm, row) <= row[13])) rdead = true;     // exact: no perturbation involved
+                        }
+                        float g0, g1, g2, fcb, eps;
+                        screen_row(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
+                        rowsL[i] = make_float4(g0, g1, g2, fcb - eps);
+                        eps_l = fmaxf(eps_l, eps);
+                    }
+                    epsL = wmax_nonneg(eps_l);
+                    rdeadL = __any_sync(FULL, rdead);
+                    full_m = m1;
+                    if (stats) st_ls += n;
+                    __syncwarp();
+                }
+                if (stats) { ++st_vr; st_lp32 += (unsigned long long)n * KP; }
+                unsigned feas = 0u;
+                if (!rdeadL) {
+                    float M = -CUDART_INF_F;
+                    float4 c4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (e_act) {
+                        c4 = pert[candj[ek]];
+                        for (int i = ech; i < n; i += NCH) {
+                            const float4 f = rowsL[i];
+                            M = fmaxf(M, fmaf(f.x, c4.x, fmaf(f.y, c4.y, fmaf(f.z, c4.z, f.w))));
+                        }
+                        M = fkey_inv(__reduce_max_sync(e_mask, fkey(M)));
+                    }
+                    // M = max_i (v32_i - eps_i):  M > th  => some constraint violated for sure;
+                    // M + 2 eps_max <= th => every constraint satisfied for sure.
+                    const bool dead = M > c4.w;
+                    const bool sure = M <= c4.w - 2.0f * epsL;
+                    const bool mine = e_act && ech == 0;
+                    unsigned alive2 = __ballot_sync(FULL, mine && !dead) & cand_alive;
+                    unsigned undecided = __ballot_sync(FULL, mine && !dead && !sure) & cand_alive;
+                    if (L.exact_only & 2) { alive2 = cand_alive; undecided = cand_alive; }
+                    while (undecided != 0u) {                // rare: fp64 decides
+                        const int k = __ffs(undecided) - 1;
+                        undecided &= undecided - 1u;
+                        if (!exact_candidate_feasible<RES>(Rm, t, rows, n, rng, (uint32_t)s, candj[k], t_p, lane))
+                            alive2 &= ~(1u << k);
+                        if (stats) st_lp += n;
+                    }
+                    feas = alive2;
+                }
+                if (feas != 0u) { m0 = m1 + 1; win = feas; }
+            }
+        }
+
+        int j_win = 0;
+        if (m0) {
+            const int kw = __ffs(win) - 1;                    // lowest rank among the feasible (R-8)
+            j_win = candj[kw];
+#pragma unroll
+            for (int e = 0; e < 9; ++e) R[e] = RmS[(m0 - 1) * 9 + e];
+            double x, y, z;
+            rng.xi3((uint32_t)s, (uint32_t)j_win, 1u, x, y, z);
+            t[0] = __dadd_rn(t[0], __dmul_rn(t_p, x));
+            t[1] = __dadd_rn(t[1], __dmul_rn(t_p, y));
+            t[2] = __dadd_rn(t[2], __dmul_rn(t_p, z));
+            if (stats) ++st_acc;
+        }
+        moved = (m0 != 0);
+        if (m0 != 1) hit = true;                              // R-12 (R-11: nothing feasible -> unchanged)
+        if (L.out_trace != nullptr && lane == 0)
+            L.out_trace[((size_t)blockIdx.y * L.num_walkers + local) * L.num_steps + (s - 1)] = m0 | (j_win << 8);
+        __syncwarp();                                         // RmS / pert / candj readers done before the next step writes
+    }
+
+    // ---- a7: emit
+    if (lane == 0) {
+        const size_t o = (size_t)blockIdx.y * L.num_walkers + local;
+        double2 *dst = reinterpret_cast<double2 *>(L.out_samples + 12 * o);
+        dst[0] = make_double2(R[0], R[1]); dst[1] = make_double2(R[2], R[3]); dst[2] = make_double2(R[4], R[5]);
+        dst[3] = make_double2(R[6], R[7]); dst[4] = make_double2(R[8], t[0]); dst[5] = make_double2(t[1], t[2]);
+        L.out_flags[o] = hit ? 1 : 0;
+        if (stats) {
+            atomicAdd(L.stats + 0, st_pp); atomicAdd(L.stats + 1, st_lp); atomicAdd(L.stats + 2, st_ps);
+            atomicAdd(L.stats + 3, st_ls); atomicAdd(L.stats + 4, st_acc);
+            atomicAdd(L.stats + 5, (unsigned long long)L.num_steps);
+            atomicAdd(L.stats + 6, st_pp32); atomicAdd(L.stats + 7, st_lp32);
+            atomicAdd(L.stats + 8, st_fb); atomicAdd(L.stats + 9, st_vr);
+        }
+    }
+}
+
+template <int RES, int NQ>
+cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
+{
+    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ);
+    if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
+    cudaError_t e = cudaFuncSetAttribute(walker_coop_kernel<RES, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)lay.total);
+    if (e != cudaSuccess) return e;
+    const long long blocks = (L.num_walkers + kCoopWarps - 1) / kCoopWarps;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    dim3 grid((unsigned)blocks, (unsigned)n_instances, 1);
+    walker_coop_kernel<RES, NQ><<<grid, kCoopThreads, lay.total, stream>>>(L);
+    return cudaGetLastError();
+}
+
+template <int RES>
+cudaError_t launch_r(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
+{
+    if (L.n_p <= 32) return launch_q<RES, 1>(L, n_instances, max_rows_bytes, max_n, stream);
+    if (L.n_p <= 64) return launch_q<RES, 2>(L, n_instances, max_rows_bytes, max_n, stream);
+    if (L.n_p <= 160) return launch_q<RES, 5>(L, n_instances, max_rows_bytes, max_n, stream);
+    return launch_q<RES, 8>(L, n_instances, max_rows_bytes, max_n, stream);
+}
+
+}  // namespace
+
+bool coop_path_available(int residual_type, int mode, int n_p, int max_n)
+{
+    return mode == CLOSURE_MODE_ROT && residual_type != CLOSURE_REPROJ_2D3D && n_p <= 256 && max_n <= 4096;
+}
+
+cudaError_t launch_walkers_coop(int residual_type, const WalkLaunch &L, int n_instances, int max_rows_bytes,
+                                cudaStream_t stream)
+{
+    const int max_n = max_rows_bytes / (row_doubles(residual_type) * 8);
+    switch (residual_type) {
+    case CLOSURE_REG_3D3D: return launch_r<CLOSURE_REG_3D3D>(L, n_instances, max_rows_bytes, max_n, stream);
+    case CLOSURE_POSE_REG: return launch_r<CLOSURE_POSE_REG>(L, n_instances, max_rows_bytes, max_n, stream);
+    case CLOSURE_POSE_REG_SPLIT: return launch_r<CLOSURE_POSE_REG_SPLIT>(L, n_instances, max_rows_bytes, max_n, stream);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace closure

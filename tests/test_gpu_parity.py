@@ -161,3 +161,17 @@ def test_screened_kernel_falls_back_on_ties():
     plain = gpu_walk(sp, _small(sp.params, flags=1), I.make_init_poses(sp, 32), 512, 60, 5)
     for a, b in zip(fast, plain):
         assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("flags", [2, 4, 6, 8])
+@pytest.mark.parametrize("config,walkers,steps", [(2, 1024, 80), (4, 512, 80), (5, 512, 100)])
+def test_cooperative_kernel_forced_fp64_paths(config, walkers, steps, flags):
+    """Debug switches of the warp-cooperative kernel: 2 = every ladder candidate goes to the fp64 test,
+    4 = every iteration takes the fp64 top-k fallback, 8 = the one-walker-per-thread screened kernel.
+    All of them must reproduce the plain fp64 kernel bit for bit."""
+    inst = I.make_instance(config)
+    S0 = I.make_init_poses(inst, 128)
+    a = gpu_walk(inst, _small(inst.params, flags=flags), S0, walkers, steps, 99)
+    b = gpu_walk(inst, _small(inst.params, flags=1), S0, walkers, steps, 99)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
