@@ -197,7 +197,7 @@ __device__ __forceinline__ bool exact_candidate_feasible(const double (&Rm)[9], 
 }
 
 struct CoopSmem {
-    size_t run_end, run_bf, warp0, per_warp, rowsA, rowsL, pert, ab, RmS, dex, candj, total;
+    size_t run_end, run_bf, warp0, per_warp, rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, candj, candd, total;
 };
 
 __host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, int nq)
@@ -212,9 +212,12 @@ __host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, 
     s.rowsL = w; w += (size_t)n * 16;
     s.pert = w;  w += (size_t)nq * 32 * 16;
     s.ab = w;    w += (size_t)n_t * 16;
+    s.qrow = w;  w += (size_t)n_t * 32;
     s.RmS = w;   w += (size_t)((n_t * 72 + 15) & ~15);
     s.dex = w;   w += (size_t)nq * 32 * 8;
+    s.qL = w;    w += (size_t)((n_t * 4 + 15) & ~15);
     s.candj = w; w += 32 * 4;
+    s.candd = w; w += 32 * 4;
     s.per_warp = w;
     s.total = o + (size_t)kCoopWarps * w;
     return s;
@@ -272,9 +275,12 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     float4 *rowsL = reinterpret_cast<float4 *>(wp + lay.rowsL);
     float4 *pert = reinterpret_cast<float4 *>(wp + lay.pert);
     double2 *ab = reinterpret_cast<double2 *>(wp + lay.ab);
+    float4 *qrow = reinterpret_cast<float4 *>(wp + lay.qrow);     // [rung][2]: the two tightest rows of each rung
     double *RmS = reinterpret_cast<double *>(wp + lay.RmS);
     double *dex = reinterpret_cast<double *>(wp + lay.dex);      // fp64 fallback: exact d_j, [q][lane]
+    float *qL = reinterpret_cast<float *>(wp + lay.qL);           // [rung]: bound on the change of any residual norm
     int *candj = reinterpret_cast<int *>(wp + lay.candj);
+    float *candd = reinterpret_cast<float *>(wp + lay.candd);     // upper bounds of the candidates' eq. (14) values
 
     const unsigned long long w = (unsigned long long)(L.walker_begin + local);
     const unsigned long long seed = L.seed[blockIdx.y];
@@ -301,8 +307,8 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     const float tpf = (float)t_p * 1.0000002f;          // >= t_p
     const float tp2 = 2.0f * tpf, tp2sq3 = 3.0f * tpf * tpf;
     const float m2tp = -2.0f * (float)t_p;
-    const int H = (n_t <= 16) ? 2 : 1;                  // hot constraints screened per rung
-    const int RPB = 32 / H;                             // rungs per screening block
+    constexpr int H = 2;                                // constraints screened per rung
+    constexpr int RPB = 32 / H;                         // rungs per screening block
     const int KP = n_ps;                                // ladder candidates
     const int NCH = 32 / KP;                            // constraint chunks of the full evaluation
     const int ek = lane % KP, ech = lane / KP;
@@ -316,12 +322,9 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     const bool stats = L.stats != nullptr;
     bool hit = false;
     bool moved = true;
-    int hot0 = 0, hot1 = 0;
     float epsA = 0.f;
     double rot_margin = CUDART_INF;
     // cached across iterations while the pose does not move
-    float qf0 = 0.f, qf1 = 0.f, qf2 = 0.f, qcbl = CUDART_INF_F;   // screening row of (rung, hot) of this lane, block 0
-    bool q_valid = false;
     int full_m = -1;                                    // rung whose rows sit in rowsL
     float epsL = 0.f;
     bool rdeadL = false;
@@ -330,7 +333,6 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
         // ================================================== set-up at the current pose (only after a move)
         if (moved) {
             float eps_l = 0.f;
-            uint32_t h1 = 0u, h2 = 0u;
             double rm_l = CUDART_INF;
             for (int i = lane; i < n; i += 32) {
                 const double *row = rows + i * ROW;
@@ -340,15 +342,9 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
                 screen_row(u0, u1, u2, c, tp2, tp2sq3, f0, f1, f2, fc, eps);
                 rowsA[i] = make_float4(f0, f1, f2, fc);
                 eps_l = fmaxf(eps_l, eps);
-                const uint32_t hk = (fkey(fc - (float)row[RS::BETA + 1]) & ~0xfffu) | (uint32_t)i;   // tightest first
-                if (hk > h1) { h2 = h1; h1 = hk; } else if (hk > h2) h2 = hk;
                 if (RES == CLOSURE_POSE_REG_SPLIT) rm_l = dmin(rm_l, row[12] - sqrt(frob_sq(R, row)));
             }
             epsA = wmax_nonneg(eps_l);
-            const uint32_t g1 = __reduce_max_sync(FULL, h1);
-            const uint32_t g2 = __reduce_max_sync(FULL, h1 == g1 ? h2 : h1);
-            hot0 = (int)(g1 & 0xfffu);
-            hot1 = (g2 != 0u) ? (int)(g2 & 0xfffu) : hot0;
             if (RES == CLOSURE_POSE_REG_SPLIT) rot_margin = wmin_f64(rm_l);
             for (int m = lane; m < n_t; m += 32) {       // Exp(dT_m w) R* for every rung
                 const double2 c2 = ab[m];
@@ -357,9 +353,55 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
 #pragma unroll
                 for (int e = 0; e < 9; ++e) RmS[m * 9 + e] = Rm[e];
             }
-            q_valid = false;
             full_m = -1;
-            if (stats) st_ps += n;
+            __syncwarp();
+            // the two tightest constraints of every rung (largest c - beta^2 at the unperturbed
+            // translation): the rows the ladder screens each rung against while the pose stays here
+#pragma unroll 1
+            for (int m = 0; m < n_t; ++m) {
+                double Rm[9];
+#pragma unroll
+                for (int e = 0; e < 9; ++e) Rm[e] = RmS[m * 9 + e];
+                float4 b1 = make_float4(0.f, 0.f, 0.f, -CUDART_INF_F), b2 = b1;
+                bool rdead = false;
+                double dR[9], lip = 0.0;                     // max_i | ||g_i(R_m, .)|| - ||g_i(R*, .)|| | <= sqrt(lip)
+#pragma unroll
+                for (int e = 0; e < 9; ++e) dR[e] = Rm[e] - R[e];
+                if (RES != CLOSURE_REG_3D3D) {
+#pragma unroll
+                    for (int e = 0; e < 9; ++e) lip = fma(dR[e], dR[e], lip);      // ||R_m - R*||_F^2
+                }
+                for (int i = lane; i < n; i += 32) {
+                    const double *row = rows + i * ROW;
+                    double u0, u1, u2, c;
+                    affine_setup<RES>(Rm, t, row, u0, u1, u2, c);
+                    if (RES == CLOSURE_REG_3D3D) {           // ||(R_m - R*) a_i||^2
+                        const double q0 = dR[0] * row[0] + dR[1] * row[1] + dR[2] * row[2];
+                        const double q1 = dR[3] * row[0] + dR[4] * row[1] + dR[5] * row[2];
+                        const double q2 = dR[6] * row[0] + dR[7] * row[1] + dR[8] * row[2];
+                        lip = dmax(lip, q0 * q0 + q1 * q1 + q2 * q2);
+                    }
+                    if (RES == CLOSURE_POSE_REG_SPLIT) {
+                        if (!(frob_sq(Rm, row) <= row[13])) rdead = true;
+                    }
+                    float g0, g1, g2, fcb, eps;
+                    screen_row(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
+                    const float4 r4 = make_float4(g0, g1, g2, fcb - eps);
+                    if (r4.w > b1.w) { b2 = b1; b1 = r4; } else if (r4.w > b2.w) b2 = r4;
+                }
+                const uint32_t k1 = fkey(b1.w);
+                const uint32_t m1 = __reduce_max_sync(FULL, k1);
+                const int src1 = __ffs(__ballot_sync(FULL, k1 == m1)) - 1;
+                const uint32_t k2 = (lane == src1) ? fkey(b2.w) : k1;
+                const uint32_t m2 = __reduce_max_sync(FULL, k2);
+                const int src2 = __ffs(__ballot_sync(FULL, k2 == m2)) - 1;
+                if (__any_sync(FULL, rdead)) b1.w = CUDART_INF_F;          // rung dead for every candidate
+                if (lane == src1) qrow[2 * m] = b1;
+                if (lane == src2) qrow[2 * m + 1] = (lane == src1) ? b2 : b1;
+                const float lf = wmax_nonneg((float)sqrt(lip));
+                if (lane == 0) qL[m] = lf * 1.001f + 1e-30f;
+            }
+            if (stats) { st_ps += n; st_ls += (unsigned long long)n * n_t; }
             __syncwarp();
         }
 
@@ -475,7 +517,10 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
             }
             if (L.exact_only & 4) ok = false;                // debug: every step takes the fp64 fallback
             certified = __all_sync(FULL, ok);
-            if (certified && lane < n_ps) candj[lane] = myj;
+            if (certified && lane < n_ps) {
+                candj[lane] = myj;
+                candd[lane] = myval + fmaf(1.01f, unc, kMu19 * fabsf(myval));    // >= the fp64 value d_j
+            }
         }
         if (!certified) {
             // ---------------- fp64 fallback: the plain kernel's phase A, then (d desc, j asc) selection.
@@ -503,7 +548,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
                 const int jm = (best == g && best != 0ull) ? lane + 32 * bq : 0x7fffffff;
                 const int jwin = __reduce_min_sync(FULL, jm);
                 if (jm == jwin) taken |= 1u << bq;
-                if (lane == 0) candj[r] = jwin;
+                if (lane == 0) { candj[r] = jwin; candd[r] = CUDART_INF_F; }
             }
             if (stats) { ++st_fb; st_pp += (unsigned long long)n * n_p; }
         }
@@ -516,36 +561,21 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
             // ---- screening of RPB rungs against the H tightest constraints: lane = (rung, constraint)
             const int mq = mb + lane / H, hq = lane % H;
             const bool q_act = (lane / H < RPB) && (mq < n_t);
-            float f0 = qf0, f1 = qf1, f2 = qf2, cbl = qcbl;
-            if (!(q_valid && mb == 0)) {
-                cbl = CUDART_INF_F; f0 = f1 = f2 = 0.f;
-                if (q_act) {
-                    double Rm[9];
-#pragma unroll
-                    for (int e = 0; e < 9; ++e) Rm[e] = RmS[mq * 9 + e];
-                    const double *row = rows + (hq == 0 ? hot0 : hot1) * ROW;
-                    double u0, u1, u2, c;
-                    affine_setup<RES>(Rm, t, row, u0, u1, u2, c);
-                    float fcb, eps;
-                    screen_row(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, f0, f1, f2, fcb, eps);
-                    cbl = fcb - eps;
-                    if (RES == CLOSURE_POSE_REG_SPLIT) {
-                        if (!(frob_sq(Rm, row) <= row[13])) cbl = CUDART_INF_F;   // rung dead for every candidate
-                    }
-                }
-                if (mb == 0) { qf0 = f0; qf1 = f1; qf2 = f2; qcbl = cbl; q_valid = true; }
-                if (stats) st_ls += (unsigned long long)min(RPB, n_t - mb) * H;
-            }
+            const float4 qr = q_act ? qrow[2 * mq + hq] : make_float4(0.f, 0.f, 0.f, CUDART_INF_F);
+            const float f0 = qr.x, f1 = qr.y, f2 = qr.z, cbl = qr.w;
             unsigned alive = 0u;
             if (q_act) {
+                const float Lm = qL[mq];
                 for (int k = 0; k < KP; ++k) {
                     const float4 c4 = pert[candj[k]];
                     const float v = fmaf(f0, c4.x, fmaf(f1, c4.y, fmaf(f2, c4.z, cbl)));
-                    if (!(v > c4.w)) alive |= 1u << k;       // not violated beyond the error bound
+                    // dead for sure: a screened constraint is violated beyond the error bound, or the
+                    // candidate's margin at R* is more negative than the rotation to R_m can repair
+                    if (!(v > c4.w) && !(candd[k] + Lm < 0.f)) alive |= 1u << k;
                 }
             }
             if (L.exact_only & 2) alive = q_act ? kmask : 0u;   // debug: the screening kills nothing
-            if (H == 2) alive &= __shfl_xor_sync(FULL, alive, 1);
+            alive &= __shfl_xor_sync(FULL, alive, 1);
             unsigned qmask = __ballot_sync(FULL, q_act && hq == 0 && alive != 0u);
             if (stats) st_lp32 += (unsigned long long)min(RPB, n_t - mb) * H * KP;
 
