@@ -79,6 +79,13 @@ __device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigne
     return r;
 }
 
+__device__ __forceinline__ unsigned long long mul2(unsigned long long a, unsigned long long b)
+{
+    unsigned long long r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+
 // Philox4x32-10 for NJ counters that differ only in word 2 (= perturbation index): rolled rounds,
 // NJ independent dependency chains.
 template <int NJ>
@@ -197,7 +204,7 @@ __device__ __forceinline__ bool exact_candidate_feasible(const double (&Rm)[9], 
 }
 
 struct CoopSmem {
-    size_t run_end, run_bf, warp0, per_warp, rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, candj, candd, total;
+    size_t run_end, run_bf, warp0, per_warp, rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, cand4, candj, candd, total;
 };
 
 __host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, int nq)
@@ -216,6 +223,7 @@ __host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, 
     s.RmS = w;   w += (size_t)((n_t * 72 + 15) & ~15);
     s.dex = w;   w += (size_t)nq * 32 * 8;
     s.qL = w;    w += (size_t)((n_t * 4 + 15) & ~15);
+    s.cand4 = w; w += 32 * 16;
     s.candj = w; w += 32 * 4;
     s.candd = w; w += 32 * 4;
     s.per_warp = w;
@@ -279,6 +287,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     double *RmS = reinterpret_cast<double *>(wp + lay.RmS);
     double *dex = reinterpret_cast<double *>(wp + lay.dex);      // fp64 fallback: exact d_j, [q][lane]
     float *qL = reinterpret_cast<float *>(wp + lay.qL);           // [rung]: bound on the change of any residual norm
+    float4 *cand4 = reinterpret_cast<float4 *>(wp + lay.cand4);   // the kept perturbations (-2 d_j, -|d_j|^2), by rank
     int *candj = reinterpret_cast<int *>(wp + lay.candj);
     float *candd = reinterpret_cast<float *>(wp + lay.candd);     // upper bounds of the candidates' eq. (14) values
 
@@ -416,17 +425,25 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
             for (int q = 0; q < NQ; ++q) jv[q] = lane + 32 * q;
             philox_batch<NQ>(rng, (uint32_t)s, jv, x, y, z);
             float e0[NQ], e1[NQ], e2[NQ];
-#pragma unroll
-            for (int q = 0; q < NQ; ++q) {
-                e0[q] = m2tp * pm1f(x[q]); e1[q] = m2tp * pm1f(y[q]); e2[q] = m2tp * pm1f(z[q]);
-                dd[q] = 0.25f * fmaf(e2[q], e2[q], fmaf(e1[q], e1[q], e0[q] * e0[q]));
-                pert[32 * q + lane] = make_float4(e0[q], e1[q], e2[q], -dd[q]);
-            }
+            // packed slots are produced by packed instructions so that they live in aligned register pairs
+            // (same roundings as the scalar pm1f() * m2tp)
+            const unsigned long long C1 = pk2(4.656612873077392578125e-10f, 4.656612873077392578125e-10f);
+            const unsigned long long C2 = pk2(2.3283064365386962890625e-10f - 1.0f, 2.3283064365386962890625e-10f - 1.0f);
+            const unsigned long long M2 = pk2(m2tp, m2tp);
 #pragma unroll
             for (int k = 0; k < NPK; ++k) {
-                p0[k] = pk2(e0[2 * k], e0[2 * k + 1]);
-                p1[k] = pk2(e1[2 * k], e1[2 * k + 1]);
-                p2[k] = pk2(e2[2 * k], e2[2 * k + 1]);
+                p0[k] = mul2(M2, fma2(pk2((float)x[2 * k], (float)x[2 * k + 1]), C1, C2));
+                p1[k] = mul2(M2, fma2(pk2((float)y[2 * k], (float)y[2 * k + 1]), C1, C2));
+                p2[k] = mul2(M2, fma2(pk2((float)z[2 * k], (float)z[2 * k + 1]), C1, C2));
+                upk2(p0[k], e0[2 * k], e0[2 * k + 1]);
+                upk2(p1[k], e1[2 * k], e1[2 * k + 1]);
+                upk2(p2[k], e2[2 * k], e2[2 * k + 1]);
+            }
+            if (ODD) { e0[NQ - 1] = m2tp * pm1f(x[NQ - 1]); e1[NQ - 1] = m2tp * pm1f(y[NQ - 1]); e2[NQ - 1] = m2tp * pm1f(z[NQ - 1]); }
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) {
+                dd[q] = 0.25f * fmaf(e2[q], e2[q], fmaf(e1[q], e1[q], e0[q] * e0[q]));
+                pert[32 * q + lane] = make_float4(e0[q], e1[q], e2[q], -dd[q]);
             }
             if (ODD) { o0 = e0[NQ - 1]; o1 = e1[NQ - 1]; o2 = e2[NQ - 1]; }
         }
@@ -476,8 +493,9 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
 
         // ================================================== a4: top-N_P* with certified ranking
         bool certified;
+        const float rmf = (float)rot_margin;                // +inf unless POSE_REG_SPLIT
+        float unc, myval = -CUDART_INF_F;
         {
-            const float rmf = (float)rot_margin;            // +inf unless POSE_REG_SPLIT
             uint32_t key[NQ];
 #pragma unroll
             for (int q = 0; q < NQ; ++q) {
@@ -492,9 +510,8 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
                     const uint32_t hi = max(key[a], key[a + 1]), lo = min(key[a], key[a + 1]);
                     key[a] = hi; key[a + 1] = lo;
                 }
-            float unc = wmax_nonneg(unc_l);
+            unc = wmax_nonneg(unc_l);
             if (RES == CLOSURE_POSE_REG_SPLIT) unc += 1.2e-7f * fabsf(rmf);
-            float myval = -CUDART_INF_F;
             int myj = -1;
             for (int r = 0; r <= n_ps; ++r) {               // extract the N_P* + 1 largest
                 const uint32_t g = __reduce_max_sync(FULL, key[0]);
@@ -523,8 +540,47 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
             }
         }
         if (!certified) {
-            // ---------------- fp64 fallback: the plain kernel's phase A, then (d desc, j asc) selection.
-            // Rare, so it is written for few registers: one perturbation at a time, values in shared memory.
+            // ---------------- fp64 fallback (near-ties): the plain kernel's eq. (14), then (d desc, j asc).
+            // Only perturbations with d~_j >= T = (N_P*-th largest d~) - 2 unc can be among the exact
+            // top-N_P* (any other has N_P* exact values strictly above it); if they fit one per lane,
+            // only those are evaluated in fp64.
+            const float Tn = __shfl_sync(FULL, myval, n_ps - 1);
+            const float T = Tn - fmaf(2.02f, unc, 2.0f * kMu19 * fabsf(Tn));
+            int cnt = 33;
+            int *fbj = reinterpret_cast<int *>(dex);
+            if ((T > -CUDART_INF_F) && (T < CUDART_INF_F) && !(L.exact_only & 16)) {
+                cnt = 0;
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) {
+                    const bool in = (lane + 32 * q < n_p) && (fminf(dt[q], rmf) >= T);
+                    const unsigned b = __ballot_sync(FULL, in);
+                    if (in && cnt <= 32) {
+                        const int pos = cnt + __popc(b & ((1u << lane) - 1u));
+                        if (pos < 32) fbj[pos] = lane + 32 * q;
+                    }
+                    cnt += __popc(b);
+                }
+                __syncwarp();
+            }
+            if (cnt <= 32) {
+                const int jv[1] = { lane < cnt ? fbj[lane] : -1 };
+                double d[1];
+                exact_margins<RES, 1>(R, t, rows, n, rng, (uint32_t)s, t_p, rot_margin, jv, d);
+                unsigned long long key = (lane < cnt) ? dkey(d[0]) : 0ull;
+#pragma unroll 1
+                for (int r = 0; r < n_ps; ++r) {
+                    const uint32_t ghi = __reduce_max_sync(FULL, (uint32_t)(key >> 32));
+                    const uint32_t glo = __reduce_max_sync(FULL, ((uint32_t)(key >> 32) == ghi) ? (uint32_t)key : 0u);
+                    const unsigned long long g = ((unsigned long long)ghi << 32) | glo;
+                    const int jm = (key == g && key != 0ull) ? jv[0] : 0x7fffffff;
+                    const int jwin = __reduce_min_sync(FULL, jm);
+                    if (jm == jwin) key = 0ull;
+                    if (lane == 0) { candj[r] = jwin; candd[r] = CUDART_INF_F; }
+                }
+                if (stats) st_pp += (unsigned long long)n * cnt;
+            } else {
+            // every perturbation in fp64; written for few registers: one at a time, values in shared memory
+            __syncwarp();
 #pragma unroll 1
             for (int q = 0; q < NQ; ++q) {
                 const int jv[1] = { lane + 32 * q };
@@ -550,9 +606,13 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
                 if (jm == jwin) taken |= 1u << bq;
                 if (lane == 0) { candj[r] = jwin; candd[r] = CUDART_INF_F; }
             }
-            if (stats) { ++st_fb; st_pp += (unsigned long long)n * n_p; }
+            if (stats) st_pp += (unsigned long long)n * n_p;
+            }
+            if (stats) ++st_fb;
         }
         __syncwarp();                                       // pert[], candj[] visible to all lanes
+        if (lane < n_ps) cand4[lane] = pert[candj[lane]];
+        __syncwarp();
 
         // ================================================== a5-a6: ladder, first feasible rung
         int m0 = 0;
@@ -567,7 +627,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
             if (q_act) {
                 const float Lm = qL[mq];
                 for (int k = 0; k < KP; ++k) {
-                    const float4 c4 = pert[candj[k]];
+                    const float4 c4 = cand4[k];
                     const float v = fmaf(f0, c4.x, fmaf(f1, c4.y, fmaf(f2, c4.z, cbl)));
                     // dead for sure: a screened constraint is violated beyond the error bound, or the
                     // candidate's margin at R* is more negative than the rotation to R_m can repair
@@ -616,7 +676,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
                     float M = -CUDART_INF_F;
                     float4 c4 = make_float4(0.f, 0.f, 0.f, 0.f);
                     if (e_act) {
-                        c4 = pert[candj[ek]];
+                        c4 = cand4[ek];
                         for (int i = ech; i < n; i += NCH) {
                             const float4 f = rowsL[i];
                             M = fmaxf(M, fmaf(f.x, c4.x, fmaf(f.y, c4.y, fmaf(f.z, c4.z, f.w))));
