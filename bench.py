@@ -32,9 +32,10 @@ METRIC = "walker_steps_per_sec"
 UNIT = "walker-steps/s"
 WALK_SEED = 42
 
-# Algorithmic flops of the walker kernel's inner loops (FMA = 2):
-#   one (pose, constraint) pair  = 3 FMA + 1 compare/max                      = 7
-#   one per-constraint set-up    = R a (6 FMA + 3 MUL) + 6 ADD/SUB + |u|^2 (2 FMA + MUL) = 26 (+1 on the ladder)
+# Arithmetic of the walker kernel's inner loops (FMA = 2), multiplied by the executed
+# counts the kernel reports (closure_get_stats):
+#   one (pose, constraint) pair  = 3 FMA + 1 compare/max                      = 7   (fp32, or fp64 where it falls back)
+#   one per-constraint set-up    = R a (6 FMA + 3 MUL) + 6 ADD/SUB + |u|^2 (2 FMA + MUL) = 26 (+1 on the ladder), fp64
 FLOP_PAIR, FLOP_SETUP_A, FLOP_SETUP_L = 7.0, 26.0, 27.0
 
 
@@ -203,6 +204,7 @@ def run_cuda(args) -> None:
         torch.cuda.synchronize()
 
     peak64, _ = B.closure_alu_peak(64)
+    peak32, _ = B.closure_alu_peak(32)
     for w in range(args.warmup):
         step(WALK_SEED + 100 + w)
         flush.fill_(w)
@@ -236,10 +238,16 @@ def run_cuda(args) -> None:
         walk(WALK_SEED)
         st = handles[0].closure_get_stats()
         handles[0].closure_enable_stats(False)
-        flops = FLOP_PAIR * (st["perturb_pairs"] + st["ladder_pairs"]) + FLOP_SETUP_A * st["perturb_setups"] \
+        # the kernel decides in fp32 with certified error bounds and falls back to fp64:
+        # executed arithmetic per pipe, and the time the two CUDA-core pipes need for it at their measured peaks
+        flops64 = FLOP_PAIR * (st["perturb_pairs"] + st["ladder_pairs"]) + FLOP_SETUP_A * st["perturb_setups"] \
             + FLOP_SETUP_L * st["ladder_setups"]
+        flops32 = FLOP_PAIR * (st["perturb_pairs_f32"] + st["ladder_pairs_f32"])
+        flops = flops64 + flops32
         walk_s = statistics.mean(walk_ms) * 1e-3
         achieved = flops / walk_s / 1e12
+        t_min = flops64 / peak64 + flops32 / peak32
+        peak_mix = flops / t_min / 1e12
         nominal_pairs = (P.n_p + P.n_p_star * P.n_t) * inst.n
         n_cnt = int(count.item())
         comp_bytes = nb * W * 1 + n_cnt * 96 * 2
@@ -282,15 +290,23 @@ def run_cuda(args) -> None:
                        "params": _params_dict(P), "l2": "256 MiB buffer written between timed iterations",
                        "sharding": "walker ranges per rank, no collective"},
             "constraint_evals_per_sec_nominal": value * nominal_pairs,
-            "constraint_evals_per_sec_executed": (st["perturb_pairs"] + st["ladder_pairs"]) / walk_s * world,
+            "constraint_evals_per_sec_executed": (st["perturb_pairs"] + st["ladder_pairs"] + st["perturb_pairs_f32"]
+                                                  + st["ladder_pairs_f32"]) / walk_s * world,
             "latency_ms": {"walker_kernel": statistics.mean(walk_ms), "compaction_kernel": statistics.mean(comp_ms),
                            "host_megb": 1e3 * statistics.mean(megb_s), "e2e_per_instance": 1e3 * e2e_dt / (e2e_steps * nb)},
             "boundary_fraction": n_cnt / float(nb * W),
-            "roofline": {"bound": "alu", "kernel": "walker_kernel", "achieved": achieved, "peak": peak64 / 1e12,
-                         "unit": "TFLOP/s", "frac": achieved / (peak64 / 1e12), "traffic": None,
-                         "peak_source": "closure_alu_peak(64): DFMA chain measured in this run",
-                         "flops_per_launch": flops, "executed_pairs_per_walker_step":
-                             (st["perturb_pairs"] + st["ladder_pairs"]) / st["walker_steps"]},
+            "roofline": {"bound": "alu", "kernel": "walker_coop_kernel" if st["perturb_pairs_f32"] else "walker_kernel",
+                         "achieved": achieved, "peak": peak_mix, "unit": "TFLOP/s", "frac": achieved / peak_mix,
+                         "traffic": None,
+                         "peak_source": "executed flops / (fp64 flops / DFMA peak + fp32 flops / FFMA peak), both peaks "
+                                        "measured in this run by closure_alu_peak (register-resident FMA chains)",
+                         "fp32": {"flops_per_launch": flops32, "achieved": flops32 / walk_s / 1e12, "peak": peak32 / 1e12},
+                         "fp64": {"flops_per_launch": flops64, "achieved": flops64 / walk_s / 1e12, "peak": peak64 / 1e12},
+                         "flops_per_launch": flops,
+                         "executed_pairs_per_walker_step": (st["perturb_pairs"] + st["ladder_pairs"] + st["perturb_pairs_f32"]
+                                                            + st["ladder_pairs_f32"]) / st["walker_steps"],
+                         "fp64_fallback_steps": st["fallback_steps"] / st["walker_steps"],
+                         "accepted_steps": st["accepted_steps"] / st["walker_steps"]},
             "roofline_compaction": {"bound": "hbm", "kernel": "compact_kernel", "achieved": comp_bytes / comp_s / 1e9,
                                     "peak": hbm_peak, "unit": "GB/s", "frac": comp_bytes / comp_s / 1e9 / hbm_peak,
                                     "bytes_per_launch": comp_bytes, "peak_source": "MEASURED_PEAKS.json hbm_gbs"
