@@ -99,14 +99,20 @@ def _oracle_leg(inst, S0, walkers: int, steps: int, threads: int, seed: int) -> 
     return time.perf_counter() - t0
 
 
+def _sample_size(inst, S0, threads: int, target_s: float) -> int:
+    """Walkers for about target_s seconds of oracle time, from a short calibration leg."""
+    steps = max(1, min(inst.num_steps, 50))
+    dt = _oracle_leg(inst, S0, threads, steps, threads, WALK_SEED + 7)
+    rate = threads * steps / max(dt, 1e-6)                      # walker-steps/s
+    return int(min(inst.num_walkers, max(threads, round(target_s * rate / inst.num_steps))))
+
+
 def cpu_baseline(inst, S0) -> dict:
     """The oracle as it stands on the host cores, on a bounded sample of the same workload."""
     import oracle
     oracle.build()
     threads = os.cpu_count() or 1
-    P = inst.params
-    per_ws = 2.5e-8 * (P.n_p + P.n_p_star * P.n_t) * inst.n * 1.4        # rough CPU-seconds per walker-step
-    walkers = int(min(256, max(threads, round(20.0 / (per_ws * inst.num_steps)))))
+    walkers = _sample_size(inst, S0, threads, 15.0)
     dt = _oracle_leg(inst, S0, walkers, inst.num_steps, threads, WALK_SEED)
     return {"value": walkers * inst.num_steps / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
             "sample": f"{walkers} strided walkers x {inst.num_steps} iterations of the same instance, "
@@ -122,8 +128,7 @@ def run_reference(args) -> None:
     inst, S0 = _workload(args.config)
     threads = os.cpu_count() or 1
     P = inst.params
-    per_ws = 2.5e-8 * (P.n_p + P.n_p_star * P.n_t) * inst.n * 1.4
-    walkers = int(min(256, max(threads, round(20.0 / (per_ws * inst.num_steps)))))
+    walkers = _sample_size(inst, S0, threads, 60.0 / max(1, args.steps))
     for w in range(args.warmup):
         _oracle_leg(inst, S0, max(threads, walkers // 8), max(1, inst.num_steps // 8), threads, WALK_SEED + w)
     t0 = time.perf_counter()

@@ -67,8 +67,11 @@ typedef struct {
     double theta_p;  /* rotation perturbation scale (the paper's R_p): rotation vector uniform on
                         [-theta_p, theta_p]^3 (R-6) */
     int precision;   /* 64 (fp64, the parity path) or 32 (fp32 arithmetic, fp64 I/O) */
-    int flags;       /* bit 0 (CLOSURE_FLAG_EXACT_ONLY): run the plain fp64 kernel even where the fp32-screened
-                        kernel exists (same results bit for bit; for verification and timing) */
+    int flags;       /* bit 0 (CLOSURE_FLAG_EXACT_ONLY): run the plain fp64 one-walker-per-thread kernel even where
+                        the warp-cooperative fp32-certified kernel exists (same results bit for bit; for
+                        verification and timing).  Bits 1, 2, 4 force the cooperative kernel's fp64 fall-back
+                        paths (tests only): 2 = every ladder candidate is decided in fp64, 4 = every top-N_P*
+                        ranking is redone in fp64, 16 = ... on all N_P perturbations. */
 } closure_params;
 #define CLOSURE_FLAG_EXACT_ONLY 1
 

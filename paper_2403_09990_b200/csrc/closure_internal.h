@@ -50,7 +50,7 @@ struct WalkLaunch {
     unsigned char *out_flags;
     int *out_trace;                           // nullable
     unsigned long long *stats;                // nullable, kNumStats counters
-    int exact_only;                           // 1: plain fp64 kernel even where the screened kernel exists
+    int exact_only;                           // bit 0: plain fp64 kernel everywhere; bits 1, 2, 4: debug switches of walker_coop_kernel
 };
 
 int row_doubles(int residual_type);
@@ -58,11 +58,6 @@ int row_doubles(int residual_type);
 // walker_kernel.cu
 cudaError_t launch_walkers(int residual_type, int mode, bool stats, const WalkLaunch &L, int n_instances,
                            int max_rows_bytes, cudaStream_t stream, std::string *why);
-
-// walker_rot_kernel.cu: fp32-screened kernel for ROT mode on REG / POSE_REG / POSE_REG_SPLIT
-bool rot_fast_path_available(int residual_type, int mode);
-cudaError_t launch_walkers_rot_fast(int residual_type, bool stats, const WalkLaunch &L, dim3 grid,
-                                    int max_rows_bytes, cudaStream_t stream);
 
 // walker_coop_kernel.cu: warp-cooperative, fp32-certified kernel for ROT mode on REG / POSE_REG / POSE_REG_SPLIT
 bool coop_path_available(int residual_type, int mode, int n_p, int max_n);

@@ -163,11 +163,11 @@ def test_screened_kernel_falls_back_on_ties():
         assert np.array_equal(a, b)
 
 
-@pytest.mark.parametrize("flags", [2, 4, 6, 8, 20])
+@pytest.mark.parametrize("flags", [2, 4, 6, 20])
 @pytest.mark.parametrize("config,walkers,steps", [(2, 1024, 80), (4, 512, 80), (5, 512, 100)])
 def test_cooperative_kernel_forced_fp64_paths(config, walkers, steps, flags):
     """Debug switches of the warp-cooperative kernel: 2 = every ladder candidate goes to the fp64 test,
-    4 = every iteration takes the fp64 top-k fallback (16: on all N_P perturbations), 8 = the one-walker-per-thread screened kernel.
+    4 = every iteration takes the fp64 top-k fallback (16: on all N_P perturbations).
     All of them must reproduce the plain fp64 kernel bit for bit."""
     inst = I.make_instance(config)
     S0 = I.make_init_poses(inst, 128)
