@@ -204,7 +204,7 @@ __device__ __forceinline__ bool exact_candidate_feasible(const double (&Rm)[9], 
 }
 
 struct CoopSmem {
-    size_t run_end, run_bf, warp0, per_warp, rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, cand4, candj, candd, total;
+    size_t run_end, run_bf, warp0, per_warp, rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, cand4, candj, candd, pose, total;
 };
 
 __host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, int nq)
@@ -226,6 +226,7 @@ __host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, 
     s.cand4 = w; w += 32 * 16;
     s.candj = w; w += 32 * 4;
     s.candd = w; w += 32 * 4;
+    s.pose = w;  w += 16 * 8;
     s.per_warp = w;
     s.total = o + (size_t)kCoopWarps * w;
     return s;
@@ -290,6 +291,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     float4 *cand4 = reinterpret_cast<float4 *>(wp + lay.cand4);   // the kept perturbations (-2 d_j, -|d_j|^2), by rank
     int *candj = reinterpret_cast<int *>(wp + lay.candj);
     float *candd = reinterpret_cast<float *>(wp + lay.candd);     // upper bounds of the candidates' eq. (14) values
+    double *pose = reinterpret_cast<double *>(wp + lay.pose);     // R*(9) t*(3) omega(3): fp64, touched only on moves / fp64 paths
 
     const unsigned long long w = (unsigned long long)(L.walker_begin + local);
     const unsigned long long seed = L.seed[blockIdx.y];
@@ -300,15 +302,23 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     rng.k1 = (uint32_t)(seed >> 32);
 
     // ---- a1: walker init, replicated on the lanes (Alg. 2 l.8-9)
-    double R[9], t[3], vel[3];
-    init_walker<CLOSURE_MODE_ROT>(D, L, rng, w, R, t, vel);
-    for (int m = lane; m < n_t; m += 32) {             // ladder dT_m = gamma^(m-1) by repeated multiplication
-        double dT = 1.0;
-        for (int q = 0; q < m; ++q) dT = dT * L.gamma;
-        const double p0 = dT * vel[0], p1 = dT * vel[1], p2 = dT * vel[2];
-        double A, B;
-        exp_coeffs(p0 * p0 + p1 * p1 + p2 * p2, A, B);
-        ab[m] = make_double2(A * dT, B * dT * dT);
+    {
+        double R[9], t[3], vel[3];
+        init_walker<CLOSURE_MODE_ROT>(D, L, rng, w, R, t, vel);
+        for (int m = lane; m < n_t; m += 32) {         // ladder dT_m = gamma^(m-1) by repeated multiplication
+            double dT = 1.0;
+            for (int q = 0; q < m; ++q) dT = dT * L.gamma;
+            const double p0 = dT * vel[0], p1 = dT * vel[1], p2 = dT * vel[2];
+            double A, B;
+            exp_coeffs(p0 * p0 + p1 * p1 + p2 * p2, A, B);
+            ab[m] = make_double2(A * dT, B * dT * dT);
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int e = 0; e < 9; ++e) pose[e] = R[e];
+#pragma unroll
+            for (int e = 0; e < 3; ++e) { pose[9 + e] = t[e]; pose[12 + e] = vel[e]; }
+        }
     }
     __syncwarp();
 
@@ -316,15 +326,12 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     const float tpf = (float)t_p * 1.0000002f;          // >= t_p
     const float tp2 = 2.0f * tpf, tp2sq3 = 3.0f * tpf * tpf;
     const float m2tp = -2.0f * (float)t_p;
-    constexpr int H = 2;                                // constraints screened per rung
-    constexpr int RPB = 32 / H;                         // rungs per screening block
     const int KP = n_ps;                                // ladder candidates
     const int NCH = 32 / KP;                            // constraint chunks of the full evaluation
     const int ek = lane % KP, ech = lane / KP;
     const bool e_act = ech < NCH;
     unsigned e_mask = 0u;                               // lanes that share this lane's candidate
     for (int c = 0; c < NCH; ++c) e_mask |= 1u << (ek + c * KP);
-    const unsigned kmask = (KP >= 32) ? FULL : ((1u << KP) - 1u);
 
     unsigned long long st_pp32 = 0, st_lp32 = 0, st_ps = 0, st_ls = 0, st_acc = 0, st_fb = 0, st_vr = 0, st_pp = 0,
                        st_lp = 0;
@@ -341,6 +348,11 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     for (int s = 1; s <= L.num_steps; ++s) {
         // ================================================== set-up at the current pose (only after a move)
         if (moved) {
+            double R[9], t[3], vel[3];
+#pragma unroll
+            for (int e = 0; e < 9; ++e) R[e] = pose[e];
+#pragma unroll
+            for (int e = 0; e < 3; ++e) { t[e] = pose[9 + e]; vel[e] = pose[12 + e]; }
             float eps_l = 0.f;
             double rm_l = CUDART_INF;
             for (int i = lane; i < n; i += 32) {
@@ -411,6 +423,11 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
                 if (lane == 0) qL[m] = lf * 1.001f + 1e-30f;
             }
             if (stats) { st_ps += n; st_ls += (unsigned long long)n * n_t; }
+            __syncwarp();
+            if (lane == 0) {                                 // suffix maximum: qL[m] holds for every rung >= m
+                float sm = 0.f;
+                for (int m = n_t - 1; m >= 0; --m) { sm = fmaxf(sm, qL[m]); qL[m] = sm; }
+            }
             __syncwarp();
         }
 
@@ -544,6 +561,11 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
             // Only perturbations with d~_j >= T = (N_P*-th largest d~) - 2 unc can be among the exact
             // top-N_P* (any other has N_P* exact values strictly above it); if they fit one per lane,
             // only those are evaluated in fp64.
+            double R[9], t[3];
+#pragma unroll
+            for (int e = 0; e < 9; ++e) R[e] = pose[e];
+#pragma unroll
+            for (int e = 0; e < 3; ++e) t[e] = pose[9 + e];
             const float Tn = __shfl_sync(FULL, myval, n_ps - 1);
             const float T = Tn - fmaf(2.02f, unc, 2.0f * kMu19 * fabsf(Tn));
             int cnt = 33;
@@ -617,37 +639,52 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
         // ================================================== a5-a6: ladder, first feasible rung
         int m0 = 0;
         unsigned win = 0u;
-        for (int mb = 0; mb < n_t && m0 == 0; mb += RPB) {
-            // ---- screening of RPB rungs against the H tightest constraints: lane = (rung, constraint)
-            const int mq = mb + lane / H, hq = lane % H;
-            const bool q_act = (lane / H < RPB) && (mq < n_t);
-            const float4 qr = q_act ? qrow[2 * mq + hq] : make_float4(0.f, 0.f, 0.f, CUDART_INF_F);
-            const float f0 = qr.x, f1 = qr.y, f2 = qr.z, cbl = qr.w;
-            unsigned alive = 0u;
-            if (q_act) {
-                const float Lm = qL[mq];
-                for (int k = 0; k < KP; ++k) {
-                    const float4 c4 = cand4[k];
-                    const float v = fmaf(f0, c4.x, fmaf(f1, c4.y, fmaf(f2, c4.z, cbl)));
-                    // dead for sure: a screened constraint is violated beyond the error bound, or the
-                    // candidate's margin at R* is more negative than the rotation to R_m can repair
-                    if (!(v > c4.w) && !(candd[k] + Lm < 0.f)) alive |= 1u << k;
-                }
+        bool lip_stop = false;
+        const bool k_act = lane < KP;
+        const float4 kc4 = k_act ? cand4[lane] : make_float4(0.f, 0.f, 0.f, 0.f);
+        const float kcd = k_act ? candd[lane] : -CUDART_INF_F;
+        const float kcd_max = fkey_inv(__reduce_max_sync(FULL, fkey(kcd)));
+        for (int mb = 0; mb < n_t && m0 == 0 && !lip_stop; mb += 32) {
+            // ---- screening, lane = candidate: at which rungs of this block does it survive the two
+            // tightest rows and the Lipschitz bound?  qL[m] bounds the change of any residual norm for
+            // every rung >= m, so the block ends at the first rung no candidate can be repaired at.
+            int mend = min(n_t, mb + 32);
+            {
+                const bool dead_m = (mb + lane < mend) && (kcd_max + qL[min(mb + lane, n_t - 1)] < 0.f);
+                const unsigned lb = __ballot_sync(FULL, dead_m);
+                if (lb != 0u) { lip_stop = true; mend = mb + __ffs(lb) - 1; }
             }
-            if (L.exact_only & 2) alive = q_act ? kmask : 0u;   // debug: the screening kills nothing
-            alive &= __shfl_xor_sync(FULL, alive, 1);
-            unsigned qmask = __ballot_sync(FULL, q_act && hq == 0 && alive != 0u);
-            if (stats) st_lp32 += (unsigned long long)min(RPB, n_t - mb) * H * KP;
+            unsigned alive_r = 0u;
+#pragma unroll 4
+            for (int m = mb; m < mend; ++m) {
+                const float4 r0 = qrow[2 * m], r1 = qrow[2 * m + 1];
+                const float v0 = fmaf(r0.x, kc4.x, fmaf(r0.y, kc4.y, fmaf(r0.z, kc4.z, r0.w)));
+                const float v1 = fmaf(r1.x, kc4.x, fmaf(r1.y, kc4.y, fmaf(r1.z, kc4.z, r1.w)));
+                // dead for sure if a screened constraint is violated beyond the error bound, or if the
+                // candidate's margin at R* is more negative than the rotation to R_m can repair
+                if (!(v0 > kc4.w) && !(v1 > kc4.w) && !(kcd + qL[m] < 0.f)) alive_r |= 1u << (m - mb);
+            }
+            if (!k_act) alive_r = 0u;
+            const int m = mend;
+            if (L.exact_only & 2) {                          // debug: the screening kills nothing
+                lip_stop = false;
+                mend = min(n_t, mb + 32);
+                alive_r = k_act ? ((mend - mb >= 32) ? FULL : ((1u << (mend - mb)) - 1u)) : 0u;
+            }
+            unsigned qmask = __reduce_or_sync(FULL, alive_r);
+            if (stats) st_lp32 += (unsigned long long)(m - mb) * 2 * KP;
 
             // ---- full evaluation of the surviving rungs, in order
             while (qmask != 0u && m0 == 0) {
                 const int l0 = __ffs(qmask) - 1;
                 qmask &= qmask - 1u;
-                const int m1 = mb + l0 / H;
-                const unsigned cand_alive = __shfl_sync(FULL, alive, l0);
-                double Rm[9];
+                const int m1 = mb + l0;
+                const unsigned cand_alive = __ballot_sync(FULL, (alive_r >> l0) & 1u);
+                double Rm[9], t[3];
 #pragma unroll
                 for (int e = 0; e < 9; ++e) Rm[e] = RmS[m1 * 9 + e];
+#pragma unroll
+                for (int e = 0; e < 3; ++e) t[e] = pose[9 + e];
                 if (full_m != m1) {
                     __syncwarp();                            // earlier readers of rowsL are done
                     float eps_l = 0.f;
@@ -708,13 +745,15 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
         if (m0) {
             const int kw = __ffs(win) - 1;                    // lowest rank among the feasible (R-8)
             j_win = candj[kw];
-#pragma unroll
-            for (int e = 0; e < 9; ++e) R[e] = RmS[(m0 - 1) * 9 + e];
             double x, y, z;
             rng.xi3((uint32_t)s, (uint32_t)j_win, 1u, x, y, z);
-            t[0] = __dadd_rn(t[0], __dmul_rn(t_p, x));
-            t[1] = __dadd_rn(t[1], __dmul_rn(t_p, y));
-            t[2] = __dadd_rn(t[2], __dmul_rn(t_p, z));
+            const double t0 = __dadd_rn(pose[9], __dmul_rn(t_p, x));
+            const double t1 = __dadd_rn(pose[10], __dmul_rn(t_p, y));
+            const double t2 = __dadd_rn(pose[11], __dmul_rn(t_p, z));
+            const double re = (lane < 9) ? RmS[(m0 - 1) * 9 + lane] : 0.0;
+            __syncwarp();
+            if (lane < 9) pose[lane] = re;
+            if (lane == 9) { pose[9] = t0; pose[10] = t1; pose[11] = t2; }
             if (stats) ++st_acc;
         }
         moved = (m0 != 0);
@@ -728,8 +767,8 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     if (lane == 0) {
         const size_t o = (size_t)blockIdx.y * L.num_walkers + local;
         double2 *dst = reinterpret_cast<double2 *>(L.out_samples + 12 * o);
-        dst[0] = make_double2(R[0], R[1]); dst[1] = make_double2(R[2], R[3]); dst[2] = make_double2(R[4], R[5]);
-        dst[3] = make_double2(R[6], R[7]); dst[4] = make_double2(R[8], t[0]); dst[5] = make_double2(t[1], t[2]);
+#pragma unroll
+        for (int e = 0; e < 6; ++e) dst[e] = make_double2(pose[2 * e], pose[2 * e + 1]);
         L.out_flags[o] = hit ? 1 : 0;
         if (stats) {
             atomicAdd(L.stats + 0, st_pp); atomicAdd(L.stats + 1, st_lp); atomicAdd(L.stats + 2, st_ps);
