@@ -145,6 +145,27 @@ __device__ __forceinline__ void affine_setup(const double (&R)[9], const double 
     }
 }
 
+// Reprojection residual (eq. (2)) with the rotation part shared by all perturbations of a
+// pose: P = R Z_i once per constraint, then the squared residual at the camera-frame point P + s,
+// s = t* + d_j; +inf behind the camera (R-10).  Used by the plain kernel and by the fp64 paths of the
+// cooperative kernel, so both take bit-identical decisions.
+__device__ __forceinline__ void reproj_point(const double (&R)[9], const double *row, double &P0, double &P1, double &P2)
+{
+    const double Z0 = row[2], Z1 = row[3], Z2 = row[4];
+    P0 = fma(R[0], Z0, fma(R[1], Z1, R[2] * Z2));
+    P1 = fma(R[3], Z0, fma(R[4], Z1, R[5] * Z2));
+    P2 = fma(R[6], Z0, fma(R[7], Z1, R[8] * Z2));
+}
+__device__ __forceinline__ double reproj_sq(double P0, double P1, double P2, double s0, double s1, double s2,
+                                            const double *row, const double (&K)[4])
+{
+    const double p0 = P0 + s0, p1 = P1 + s1, p2 = P2 + s2;
+    if (!(p2 > 0.0)) return CUDART_INF;
+    const double g0 = row[0] - fma(K[0], p0 / p2, K[2]);
+    const double g1 = row[1] - fma(K[1], p1 / p2, K[3]);
+    return fma(g1, g1, g0 * g0);
+}
+
 // Direct evaluation of the squared residual at pose (R, t) (generic path).
 // part: POSE_REG_SPLIT only, 0 = rotation bound, 1 = translation bound.
 template <int RES>

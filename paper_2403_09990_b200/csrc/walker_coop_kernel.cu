@@ -25,100 +25,10 @@
 
 #include "closure_internal.h"
 #include "walker_common.cuh"
+#include "walker_coop_common.cuh"
 
 namespace closure {
 namespace {
-
-constexpr int kCoopWarps = 4;                 // walkers per CTA
-constexpr int kCoopThreads = 32 * kCoopWarps;
-constexpr unsigned FULL = 0xffffffffu;
-constexpr float kMu19 = 1.9073486328125e-06f;   // 2^-19
-
-// ---------------------------------------------------------------------------------- small helpers
-// order-preserving maps to unsigned keys
-__device__ __forceinline__ uint32_t fkey(float x)
-{
-    const uint32_t b = __float_as_uint(x);
-    return b ^ ((uint32_t)((int32_t)b >> 31) | 0x80000000u);
-}
-__device__ __forceinline__ float fkey_inv(uint32_t k)
-{
-    return __uint_as_float((k & 0x80000000u) ? (k ^ 0x80000000u) : ~k);
-}
-__device__ __forceinline__ unsigned long long dkey(double x)
-{
-    const unsigned long long b = (unsigned long long)__double_as_longlong(x);
-    return b ^ ((unsigned long long)((long long)b >> 63) | 0x8000000000000000ull);
-}
-__device__ __forceinline__ float wmax_nonneg(float v)      // v >= 0 (or NaN, which wins: callers then fall back)
-{
-    return __uint_as_float(__reduce_max_sync(FULL, __float_as_uint(v)));
-}
-__device__ __forceinline__ double wmin_f64(double v)
-{
-#pragma unroll
-    for (int o = 16; o >= 1; o >>= 1) v = dmin(v, __shfl_xor_sync(FULL, v, o));
-    return v;
-}
-
-// packed fp32 pairs (FFMA2 on sm_100a)
-__device__ __forceinline__ unsigned long long pk2(float lo, float hi)
-{
-    unsigned long long r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void upk2(unsigned long long v, float &lo, float &hi)
-{
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c)
-{
-    unsigned long long r;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
-    return r;
-}
-
-__device__ __forceinline__ unsigned long long mul2(unsigned long long a, unsigned long long b)
-{
-    unsigned long long r;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-    return r;
-}
-
-// Philox4x32-10 for NJ counters that differ only in word 2 (= perturbation index): rolled rounds,
-// NJ independent dependency chains.
-template <int NJ>
-__device__ __forceinline__ void philox_batch(const Rng &rng, uint32_t s, const int (&j)[NJ], uint32_t (&x)[NJ],
-                                             uint32_t (&y)[NJ], uint32_t (&z)[NJ])
-{
-    uint32_t c0[NJ], c1[NJ], c2[NJ], c3[NJ];
-#pragma unroll
-    for (int q = 0; q < NJ; ++q) { c0[q] = rng.w_lo; c1[q] = s; c2[q] = (uint32_t)j[q]; c3[q] = 1u | rng.w_hi8; }
-    uint32_t k0 = rng.k0, k1 = rng.k1;
-#pragma unroll 1
-    for (int r = 0; r < 10; ++r) {
-#pragma unroll
-        for (int q = 0; q < NJ; ++q) {
-            const uint32_t hi0 = __umulhi(0xD2511F53u, c0[q]), lo0 = 0xD2511F53u * c0[q];
-            const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2[q]), lo1 = 0xCD9E8D57u * c2[q];
-            c0[q] = hi1 ^ c1[q] ^ k0;
-            c1[q] = lo1;
-            c2[q] = hi0 ^ c3[q] ^ k1;
-            c3[q] = lo0;
-        }
-        k0 += 0x9E3779B9u;
-        k1 += 0xBB67AE85u;
-    }
-#pragma unroll
-    for (int q = 0; q < NJ; ++q) { x[q] = c0[q]; y[q] = c1[q]; z[q] = c2[q]; }
-}
-
-// fp32 image of pm1(): |pm1f(x) - pm1(x)| <= 2^-22.
-__device__ __forceinline__ float pm1f(uint32_t x)
-{
-    return fmaf((float)x, 4.656612873077392578125e-10f, 2.3283064365386962890625e-10f - 1.0f);
-}
 
 // fp32 image of one set-up row and the bound eps on |v32 - v64| for ANY perturbation with
 // |d_c| <= t_p, where v = c - 2 u.d is evaluated as three chained FMAs:
@@ -175,6 +85,25 @@ __device__ __forceinline__ void exact_margins(const double (&R)[9], const double
     }
 }
 
+// eq. (14) of one perturbation in the plain kernel's arithmetic (functor for topk_fp64)
+template <int RES>
+struct ExactMargin {
+    const double (&R)[9];
+    const double (&t)[3];
+    const double *rows;
+    int n;
+    const Rng &rng;
+    uint32_t s;
+    double t_p, rot_margin;
+    __device__ __forceinline__ double operator()(int j) const
+    {
+        const int jv[1] = { j };
+        double d[1];
+        exact_margins<RES, 1>(R, t, rows, n, rng, s, t_p, rot_margin, jv, d);
+        return d[0];
+    }
+};
+
 // fp64 in_purse of ladder candidate (Rm, t* + d_j), constraints dealt to the lanes; the arithmetic
 // of the plain kernel's ladder.  Warp-uniform result.
 template <int RES>
@@ -203,35 +132,6 @@ __device__ __forceinline__ bool exact_candidate_feasible(const double (&Rm)[9], 
     return __all_sync(FULL, ok);
 }
 
-struct CoopSmem {
-    size_t run_end, run_bf, warp0, per_warp, rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, cand4, candj, candd, pose, total;
-};
-
-__host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, int nq)
-{
-    CoopSmem s;
-    size_t o = 16 + (size_t)((rows_bytes + 15) & ~15);
-    s.run_end = o; o += (size_t)((n * 4 + 15) & ~15);
-    s.run_bf = o;  o += (size_t)((n * 4 + 15) & ~15);
-    s.warp0 = o;
-    size_t w = 0;
-    s.rowsA = w; w += (size_t)n * 16;
-    s.rowsL = w; w += (size_t)n * 16;
-    s.pert = w;  w += (size_t)nq * 32 * 16;
-    s.ab = w;    w += (size_t)n_t * 16;
-    s.qrow = w;  w += (size_t)n_t * 32;
-    s.RmS = w;   w += (size_t)((n_t * 72 + 15) & ~15);
-    s.dex = w;   w += (size_t)nq * 32 * 8;
-    s.qL = w;    w += (size_t)((n_t * 4 + 15) & ~15);
-    s.cand4 = w; w += 32 * 16;
-    s.candj = w; w += 32 * 4;
-    s.candd = w; w += 32 * 4;
-    s.pose = w;  w += 16 * 8;
-    s.per_warp = w;
-    s.total = o + (size_t)kCoopWarps * w;
-    return s;
-}
-
 // ---------------------------------------------------------------------------------- the kernel
 template <int RES, int NQ>
 __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __grid_constant__ WalkLaunch L)
@@ -251,7 +151,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
     double *rows = reinterpret_cast<double *>(smem_raw + 16);
     stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
-    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ);
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 1);
     int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
     float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
     if (warp == 0) {                                   // runs of equal bounds (rows are sorted by bound)
@@ -509,128 +409,22 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
         }
 
         // ================================================== a4: top-N_P* with certified ranking
-        bool certified;
         const float rmf = (float)rot_margin;                // +inf unless POSE_REG_SPLIT
-        float unc, myval = -CUDART_INF_F;
-        {
-            uint32_t key[NQ];
+        float dv[NQ];
 #pragma unroll
-            for (int q = 0; q < NQ; ++q) {
-                const float v = (lane + 32 * q < n_p) ? fminf(dt[q], rmf) : -CUDART_INF_F;
-                key[q] = (fkey(v) & ~7u) | (uint32_t)q;
-            }
-            // local sort, descending (odd-even transposition network)
-#pragma unroll
-            for (int pass = 0; pass < NQ; ++pass)
-#pragma unroll
-                for (int a = (pass & 1); a + 1 < NQ; a += 2) {
-                    const uint32_t hi = max(key[a], key[a + 1]), lo = min(key[a], key[a + 1]);
-                    key[a] = hi; key[a + 1] = lo;
-                }
-            unc = wmax_nonneg(unc_l);
-            if (RES == CLOSURE_POSE_REG_SPLIT) unc += 1.2e-7f * fabsf(rmf);
-            int myj = -1;
-            for (int r = 0; r <= n_ps; ++r) {               // extract the N_P* + 1 largest
-                const uint32_t g = __reduce_max_sync(FULL, key[0]);
-                const unsigned who = __ballot_sync(FULL, key[0] == g);
-                const int src = __ffs(who) - 1;
-                if (lane == r) { myval = fkey_inv(g); myj = src + 32 * (int)(g & 7u); }
-                if (lane == src) {
-#pragma unroll
-                    for (int q = 0; q + 1 < NQ; ++q) key[q] = key[q + 1];
-                    key[NQ - 1] = 0u;
-                }
-            }
-            const float prev = __shfl_up_sync(FULL, myval, 1);
-            bool ok = true;
-            if (lane < n_ps) ok = (myval > -CUDART_INF_F) && (myval < CUDART_INF_F);
-            if (lane >= 1 && lane <= n_ps) {
-                const bool none_left = (lane == n_ps) && (myval == -CUDART_INF_F);
-                const float need = fmaf(2.0f, unc, kMu19 * (fabsf(prev) + fabsf(myval)));
-                ok = ok && (none_left || (prev - myval > need));
-            }
-            if (L.exact_only & 4) ok = false;                // debug: every step takes the fp64 fallback
-            certified = __all_sync(FULL, ok);
-            if (certified && lane < n_ps) {
-                candj[lane] = myj;
-                candd[lane] = myval + fmaf(1.01f, unc, kMu19 * fabsf(myval));    // >= the fp64 value d_j
-            }
-        }
-        if (!certified) {
-            // ---------------- fp64 fallback (near-ties): the plain kernel's eq. (14), then (d desc, j asc).
-            // Only perturbations with d~_j >= T = (N_P*-th largest d~) - 2 unc can be among the exact
-            // top-N_P* (any other has N_P* exact values strictly above it); if they fit one per lane,
-            // only those are evaluated in fp64.
+        for (int q = 0; q < NQ; ++q) dv[q] = (lane + 32 * q < n_p) ? fminf(dt[q], rmf) : -CUDART_INF_F;
+        float unc = wmax_nonneg(unc_l), myval;
+        if (RES == CLOSURE_POSE_REG_SPLIT) unc += 1.2e-7f * fabsf(rmf);
+        // (exact_only & 4: debug, every step takes the fp64 fall-back; & 16: on all N_P perturbations)
+        if (!topk_certified<NQ>(dv, n_ps, unc, (L.exact_only & 4) != 0, lane, candj, candd, myval)) {
             double R[9], t[3];
 #pragma unroll
             for (int e = 0; e < 9; ++e) R[e] = pose[e];
 #pragma unroll
             for (int e = 0; e < 3; ++e) t[e] = pose[9 + e];
-            const float Tn = __shfl_sync(FULL, myval, n_ps - 1);
-            const float T = Tn - fmaf(2.02f, unc, 2.0f * kMu19 * fabsf(Tn));
-            int cnt = 33;
-            int *fbj = reinterpret_cast<int *>(dex);
-            if ((T > -CUDART_INF_F) && (T < CUDART_INF_F) && !(L.exact_only & 16)) {
-                cnt = 0;
-#pragma unroll
-                for (int q = 0; q < NQ; ++q) {
-                    const bool in = (lane + 32 * q < n_p) && (fminf(dt[q], rmf) >= T);
-                    const unsigned b = __ballot_sync(FULL, in);
-                    if (in && cnt <= 32) {
-                        const int pos = cnt + __popc(b & ((1u << lane) - 1u));
-                        if (pos < 32) fbj[pos] = lane + 32 * q;
-                    }
-                    cnt += __popc(b);
-                }
-                __syncwarp();
-            }
-            if (cnt <= 32) {
-                const int jv[1] = { lane < cnt ? fbj[lane] : -1 };
-                double d[1];
-                exact_margins<RES, 1>(R, t, rows, n, rng, (uint32_t)s, t_p, rot_margin, jv, d);
-                unsigned long long key = (lane < cnt) ? dkey(d[0]) : 0ull;
-#pragma unroll 1
-                for (int r = 0; r < n_ps; ++r) {
-                    const uint32_t ghi = __reduce_max_sync(FULL, (uint32_t)(key >> 32));
-                    const uint32_t glo = __reduce_max_sync(FULL, ((uint32_t)(key >> 32) == ghi) ? (uint32_t)key : 0u);
-                    const unsigned long long g = ((unsigned long long)ghi << 32) | glo;
-                    const int jm = (key == g && key != 0ull) ? jv[0] : 0x7fffffff;
-                    const int jwin = __reduce_min_sync(FULL, jm);
-                    if (jm == jwin) key = 0ull;
-                    if (lane == 0) { candj[r] = jwin; candd[r] = CUDART_INF_F; }
-                }
-                if (stats) st_pp += (unsigned long long)n * cnt;
-            } else {
-            // every perturbation in fp64; written for few registers: one at a time, values in shared memory
-            __syncwarp();
-#pragma unroll 1
-            for (int q = 0; q < NQ; ++q) {
-                const int jv[1] = { lane + 32 * q };
-                double d[1];
-                exact_margins<RES, 1>(R, t, rows, n, rng, (uint32_t)s, t_p, rot_margin, jv, d);
-                dex[32 * q + lane] = (jv[0] < n_p) ? d[0] : -CUDART_INF;
-            }
-            unsigned taken = 0u;                             // slots of this lane already extracted
-#pragma unroll 1
-            for (int r = 0; r < n_ps; ++r) {
-                unsigned long long best = 0ull;
-                int bq = 0;
-#pragma unroll 1
-                for (int q = 0; q < NQ; ++q) {
-                    const unsigned long long kq = ((taken >> q) & 1u) || (lane + 32 * q >= n_p) ? 0ull : dkey(dex[32 * q + lane]);
-                    if (kq > best) { best = kq; bq = q; }
-                }
-                const uint32_t ghi = __reduce_max_sync(FULL, (uint32_t)(best >> 32));
-                const uint32_t glo = __reduce_max_sync(FULL, ((uint32_t)(best >> 32) == ghi) ? (uint32_t)best : 0u);
-                const unsigned long long g = ((unsigned long long)ghi << 32) | glo;
-                const int jm = (best == g && best != 0ull) ? lane + 32 * bq : 0x7fffffff;
-                const int jwin = __reduce_min_sync(FULL, jm);
-                if (jm == jwin) taken |= 1u << bq;
-                if (lane == 0) { candj[r] = jwin; candd[r] = CUDART_INF_F; }
-            }
-            if (stats) st_pp += (unsigned long long)n * n_p;
-            }
-            if (stats) ++st_fb;
+            const ExactMargin<RES> exact{ R, t, rows, n, rng, (uint32_t)s, t_p, rot_margin };
+            const int cnt = topk_fp64<NQ>(dv, n_p, n_ps, unc, myval, (L.exact_only & 16) != 0, lane, dex, candj, candd, exact);
+            if (stats) { ++st_fb; st_pp += (unsigned long long)n * cnt; }
         }
         __syncwarp();                                       // pert[], candj[] visible to all lanes
         if (lane < n_ps) cand4[lane] = pert[candj[lane]];
@@ -783,7 +577,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
 template <int RES, int NQ>
 cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
 {
-    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ);
+    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 1);
     if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaFuncSetAttribute(walker_coop_kernel<RES, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)lay.total);
@@ -808,7 +602,7 @@ cudaError_t launch_r(const WalkLaunch &L, int n_instances, int max_rows_bytes, i
 
 bool coop_path_available(int residual_type, int mode, int n_p, int max_n)
 {
-    return mode == CLOSURE_MODE_ROT && residual_type != CLOSURE_REPROJ_2D3D && n_p <= 256 && max_n <= 4096;
+    return mode == CLOSURE_MODE_ROT && n_p <= 256 && max_n <= 4096;
 }
 
 cudaError_t launch_walkers_coop(int residual_type, const WalkLaunch &L, int n_instances, int max_rows_bytes,
@@ -816,6 +610,7 @@ cudaError_t launch_walkers_coop(int residual_type, const WalkLaunch &L, int n_in
 {
     const int max_n = max_rows_bytes / (row_doubles(residual_type) * 8);
     switch (residual_type) {
+    case CLOSURE_REPROJ_2D3D: return launch_walkers_coop_reproj(L, n_instances, max_rows_bytes, stream);
     case CLOSURE_REG_3D3D: return launch_r<CLOSURE_REG_3D3D>(L, n_instances, max_rows_bytes, max_n, stream);
     case CLOSURE_POSE_REG: return launch_r<CLOSURE_POSE_REG>(L, n_instances, max_rows_bytes, max_n, stream);
     case CLOSURE_POSE_REG_SPLIT: return launch_r<CLOSURE_POSE_REG_SPLIT>(L, n_instances, max_rows_bytes, max_n, stream);

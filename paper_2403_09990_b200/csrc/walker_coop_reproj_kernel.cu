@@ -1,0 +1,550 @@
+// Warp-cooperative walker kernel for the rotation-boundary sampler (Alg. 2) on the
+// 2D reprojection residual z_i - Pi(K(R Z_i + t)) (eq. (2)).  Same organisation as
+// walker_coop_kernel.cu (one warp per walker, set-ups once per accepted move, fp32 evaluation with
+// rigorous error bounds, fp64 only where a decision is not certain); what differs is the pair:
+//
+//   with p = R Z_i + t* + d and zeta = z_i - (cx, cy), for p_3 > 0
+//       ||z_i - Pi(K p)||  =  || (zeta_1 p_3 - fx p_1, zeta_2 p_3 - fy p_2) || / p_3  =:  ||q|| / p_3 ,
+//   and q, p_3 are AFFINE in the translation perturbation d:
+//       q_1 = A_1 + zeta_1 d_3 - fx d_1,   q_2 = A_2 + zeta_2 d_3 - fy d_2,   p_3 = P_3 + d_3 ,
+//   (A, P_3) depending on the pose only.  eq. (14) needs ||q||^2 / p_3^2 (one MUFU.RCP per pair, one
+//   rsqrt per run of equal bounds); in_purse is the cone test ||q||^2 - (beta p_3)^2 <= 0, no division.
+//
+// Error bounds (u = 2^-24; |d32 - d64| <= 6 u t_p per component, see walker_coop_kernel.cu):
+//   E_q1 = u (3 |A_1| + 9 t_p (|zeta_1| + fx)),  E_q2 alike,  E_p = u (2 |P_3| + 7 t_p),
+//   p_lo = P_3 - t_p > 0 (else nothing is certified),  rho_hi = (|A_1| + |A_2| + t_p (...)) / p_lo,
+//   |rho32 - rho64| <= (E_q1 + E_q2) / p_lo + rho_hi (E_p / p_lo + 2^-19)      (unc uses twice that)
+//   cone value g:  E_g = 2 (q1_hi E_q1 + q2_hi E_q2 + w_hi E_w) + 4 u (q1_hi^2 + q2_hi^2 + w_hi^2), x 1.5.
+// The fp64 reference of every decision is the plain kernel's arithmetic (reproj_point / reproj_sq in
+// walker_common.cuh); its own rounding (~1e-13 px) is far inside these bounds.
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include <stdint.h>
+
+#include "closure_internal.h"
+#include "walker_common.cuh"
+#include "walker_coop_common.cuh"
+
+namespace closure {
+namespace {
+
+constexpr int RES = CLOSURE_REPROJ_2D3D;
+constexpr int ROW = Res<RES>::ROW;
+constexpr int BETA = Res<RES>::BETA;
+constexpr double kU = 5.9604644775390625e-08;   // 2^-24
+
+// fp32 row of one constraint at the camera-frame point P (= R Z_i + t*): (A_1, A_2, P_3 or beta P_3, zeta_1),
+// (zeta_2, beta, -E_g, rho bound) and the error constants above.
+struct ReprojRow {
+    float4 a, b;
+    float unc;      // bound on |rho32 - rho64| for eq. (14) (phase A rows)
+    float g0;       // cone value at d = 0 minus E_g (ladder rows: tightness key)
+};
+
+template <bool LADDER>
+__device__ __forceinline__ ReprojRow reproj_row(double P0, double P1, double P2, const double *row, const double (&K)[4],
+                                                double t_p)
+{
+    const double z0 = row[0] - K[2], z1 = row[1] - K[3], beta = row[BETA];
+    const double A0 = z0 * P2 - K[0] * P0, A1 = z1 * P2 - K[1] * P1;
+    const double Eq0 = kU * (3.0 * fabs(A0) + 9.0 * t_p * (fabs(z0) + K[0]));
+    const double Eq1 = kU * (3.0 * fabs(A1) + 9.0 * t_p * (fabs(z1) + K[1]));
+    const double Ep = kU * (2.0 * fabs(P2) + 7.0 * t_p);       // phase A only: p_3 = P_3 + d_3
+    const double plo = P2 - 1.001 * t_p;
+    const double q0hi = fabs(A0) + t_p * (fabs(z0) + K[0]), q1hi = fabs(A1) + t_p * (fabs(z1) + K[1]);
+    ReprojRow r;
+    if (!LADDER) {
+        r.a = make_float4((float)A0, (float)A1, (float)P2, (float)z0);
+        r.b = make_float4((float)z1, (float)beta, 0.f, 0.f);
+        r.g0 = 0.f;
+        if (plo > 0.0) {
+            const double rho_hi = (q0hi + q1hi) / plo;
+            const double Erho = (Eq0 + Eq1) / plo + rho_hi * (Ep / plo + 1.9073486328125e-06);
+            r.unc = (float)(2.0 * Erho + 4.76837158203125e-07 * beta + 1e-12 * (rho_hi + beta)) * 1.0001f;
+        } else {
+            r.unc = CUDART_INF_F;
+        }
+    } else {
+        const double Bp = beta * P2;
+        const double whi = fabs(Bp) + beta * t_p;
+        const double Ew = kU * (2.0 * fabs(Bp) + 8.0 * beta * t_p);
+        const double ss = q0hi * q0hi + q1hi * q1hi + whi * whi;
+        double Eg = 1.5 * (2.0 * (q0hi * Eq0 + q1hi * Eq1 + whi * Ew) + 4.0 * kU * ss) + 1e-12 * ss;
+        float Egf = (float)Eg * 1.0001f;
+        if (!(plo > 0.0)) Egf = CUDART_INF_F;           // cheirality not certain: never certified, fp64 decides
+        r.a = make_float4((float)A0, (float)A1, (float)Bp, (float)z0);
+        r.b = make_float4((float)z1, (float)beta, -Egf, 0.f);
+        r.unc = Egf;
+        r.g0 = (float)(A0 * A0 + A1 * A1 - Bp * Bp) - Egf;
+    }
+    return r;
+}
+
+// eq. (14) of perturbation j in the plain kernel's arithmetic (functor for topk_fp64)
+struct ExactMarginReproj {
+    const double (&R)[9];
+    const double (&t)[3];
+    const double (&K)[4];
+    const double *rows;
+    int n;
+    const Rng &rng;
+    uint32_t s;
+    double t_p;
+    __device__ __forceinline__ double operator()(int j) const
+    {
+        double x, y, z;
+        rng.xi3(s, (uint32_t)j, 1u, x, y, z);
+        const double e0 = t_p * x, e1 = t_p * y, e2 = t_p * z;
+        double d = CUDART_INF;
+#pragma unroll 1
+        for (int i = 0; i < n; ++i) {
+            const double *row = rows + i * ROW;
+            double P0, P1, P2;
+            reproj_point(R, row, P0, P1, P2);
+            const double sq = reproj_sq(P0, P1, P2, t[0] + e0, t[1] + e1, t[2] + e2, row, K);
+            d = dmin(d, row[BETA] - sqrt(sq));
+        }
+        return d;
+    }
+};
+
+// fp64 in_purse of ladder candidate (Rm, t* + d_j), constraints dealt to the lanes (plain kernel's arithmetic)
+__device__ __forceinline__ bool exact_candidate_feasible_reproj(const double (&Rm)[9], const double (&t)[3],
+                                                                const double (&K)[4], const double *rows, int n,
+                                                                const Rng &rng, uint32_t s, int j, double t_p, int lane)
+{
+    double x, y, z;
+    rng.xi3(s, (uint32_t)j, 1u, x, y, z);
+    const double k0 = t_p * x, k1 = t_p * y, k2 = t_p * z;
+    bool ok = true;
+    for (int i = lane; i < n; i += 32) {
+        const double *row = rows + i * ROW;
+        double P0, P1, P2;
+        reproj_point(Rm, row, P0, P1, P2);
+        const double sq = reproj_sq(P0, P1, P2, t[0] + k0, t[1] + k1, t[2] + k2, row, K);
+        if (!(sq <= row[BETA + 1])) ok = false;
+    }
+    return __all_sync(FULL, ok);
+}
+
+// cone value of one (ladder row, candidate) pair minus its error bound
+__device__ __forceinline__ float cone_lo(const float4 &ra, const float4 &rb, const float4 &c, float nfx, float nfy)
+{
+    const float q0 = fmaf(ra.w, c.z, fmaf(nfx, c.x, ra.x));
+    const float q1 = fmaf(rb.x, c.z, fmaf(nfy, c.y, ra.y));
+    const float w = fmaf(rb.y, c.z, ra.z);
+    return fmaf(q0, q0, fmaf(q1, q1, fmaf(-w, w, rb.z)));
+}
+
+// ---------------------------------------------------------------------------------- the kernel
+template <int NQ>
+__global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(const __grid_constant__ WalkLaunch L)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ int n_runs_s;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const InstanceDesc *__restrict__ D = L.desc[blockIdx.y];
+    const int n = D->n;
+    const int rows_bytes = D->rows_bytes;
+    const int n_p = L.n_p, n_ps = L.n_p_star, n_t = L.n_t;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
+    double *rows = reinterpret_cast<double *>(smem_raw + 16);
+    stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 2);
+    int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
+    float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
+    if (warp == 0) {                                   // runs of equal bounds (rows are sorted by bound)
+        int cnt = 0;
+        for (int base = 0; base < n; base += 32) {
+            const int i = base + lane;
+            bool end = false;
+            double beta = 0.0;
+            if (i < n) {
+                beta = rows[i * ROW + BETA];
+                end = (i == n - 1) || (rows[(i + 1) * ROW + BETA] != beta);
+            }
+            const unsigned m = __ballot_sync(FULL, end);
+            if (end) {
+                const int r = cnt + __popc(m & ((1u << lane) - 1u));
+                run_end[r] = i;
+                run_bf[r] = (float)beta;
+            }
+            cnt += __popc(m);
+        }
+        if (lane == 0) n_runs_s = cnt;
+    }
+    __syncthreads();
+    const int n_runs = n_runs_s;
+
+    const long long local = (long long)blockIdx.x * kCoopWarps + warp;
+    if (local >= L.num_walkers) return;                // no block-wide barrier below this line
+    unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
+    float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);   // [n][2]
+    float4 *rowsL = reinterpret_cast<float4 *>(wp + lay.rowsL);   // [n][2]
+    float4 *pert = reinterpret_cast<float4 *>(wp + lay.pert);     // (d_j, 0)
+    double2 *ab = reinterpret_cast<double2 *>(wp + lay.ab);
+    float4 *qrow = reinterpret_cast<float4 *>(wp + lay.qrow);     // [rung][2 rows][2]
+    double *RmS = reinterpret_cast<double *>(wp + lay.RmS);
+    double *dex = reinterpret_cast<double *>(wp + lay.dex);
+    float *qL = reinterpret_cast<float *>(wp + lay.qL);
+    float4 *cand4 = reinterpret_cast<float4 *>(wp + lay.cand4);
+    int *candj = reinterpret_cast<int *>(wp + lay.candj);
+    float *candd = reinterpret_cast<float *>(wp + lay.candd);
+    double *pose = reinterpret_cast<double *>(wp + lay.pose);
+
+    const unsigned long long w = (unsigned long long)(L.walker_begin + local);
+    const unsigned long long seed = L.seed[blockIdx.y];
+    Rng rng;
+    rng.w_lo = (uint32_t)w;
+    rng.w_hi8 = (uint32_t)(w >> 32) << 8;
+    rng.k0 = (uint32_t)seed;
+    rng.k1 = (uint32_t)(seed >> 32);
+
+    // ---- a1: walker init, replicated on the lanes (Alg. 2 l.8-9)
+    {
+        double R[9], t[3], vel[3];
+        init_walker<CLOSURE_MODE_ROT>(D, L, rng, w, R, t, vel);
+        for (int m = lane; m < n_t; m += 32) {         // ladder dT_m = gamma^(m-1) by repeated multiplication
+            double dT = 1.0;
+            for (int q = 0; q < m; ++q) dT = dT * L.gamma;
+            const double p0 = dT * vel[0], p1 = dT * vel[1], p2 = dT * vel[2];
+            double A, B;
+            exp_coeffs(p0 * p0 + p1 * p1 + p2 * p2, A, B);
+            ab[m] = make_double2(A * dT, B * dT * dT);
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int e = 0; e < 9; ++e) pose[e] = R[e];
+#pragma unroll
+            for (int e = 0; e < 3; ++e) { pose[9 + e] = t[e]; pose[12 + e] = vel[e]; }
+        }
+    }
+    __syncwarp();
+
+    const double t_p = L.t_p;
+    const float tpfl = (float)t_p;
+    const float nfx = -(float)D->K[0], nfy = -(float)D->K[1];
+    const int KP = n_ps;                                // ladder candidates
+    const int NCH = 32 / KP;                            // constraint chunks of the full evaluation
+    const int ek = lane % KP, ech = lane / KP;
+    const bool e_act = ech < NCH;
+    unsigned e_mask = 0u;                               // lanes that share this lane's candidate
+    for (int c = 0; c < NCH; ++c) e_mask |= 1u << (ek + c * KP);
+
+    unsigned long long st_pp32 = 0, st_lp32 = 0, st_ps = 0, st_ls = 0, st_acc = 0, st_fb = 0, st_vr = 0, st_pp = 0,
+                       st_lp = 0;
+    const bool stats = L.stats != nullptr;
+    bool hit = false;
+    bool moved = true;
+    float uncA = CUDART_INF_F;
+    int full_m = -1;                                    // rung whose rows sit in rowsL
+    float epsL = 0.f;
+
+    for (int s = 1; s <= L.num_steps; ++s) {
+        // ================================================== set-up at the current pose (only after a move)
+        if (moved) {
+            double R[9], t[3], vel[3], K[4];
+#pragma unroll
+            for (int e = 0; e < 9; ++e) R[e] = pose[e];
+#pragma unroll
+            for (int e = 0; e < 3; ++e) { t[e] = pose[9 + e]; vel[e] = pose[12 + e]; }
+#pragma unroll
+            for (int e = 0; e < 4; ++e) K[e] = D->K[e];
+            float unc_l = 0.f;
+            for (int i = lane; i < n; i += 32) {
+                const double *row = rows + i * ROW;
+                double P0, P1, P2;
+                reproj_point(R, row, P0, P1, P2);
+                const ReprojRow r = reproj_row<false>(P0 + t[0], P1 + t[1], P2 + t[2], row, K, t_p);
+                rowsA[2 * i] = r.a;
+                rowsA[2 * i + 1] = r.b;
+                unc_l = fmaxf(unc_l, r.unc);
+            }
+            uncA = wmax_nonneg(unc_l);
+            for (int m = lane; m < n_t; m += 32) {       // Exp(dT_m w) R* for every rung
+                const double2 c2 = ab[m];
+                double Rm[9];
+                rotate_left(R, vel[0], vel[1], vel[2], c2.x, c2.y, Rm);
+#pragma unroll
+                for (int e = 0; e < 9; ++e) RmS[m * 9 + e] = Rm[e];
+            }
+            full_m = -1;
+            __syncwarp();
+            // per rung: the two tightest cone rows at d = 0 and the Lipschitz bound L_m on the change of
+            // any reprojection residual norm between R* and R_m, valid for every |d_c| <= t_p:
+            //   |d/dtau fx p_1/p_3| <= fx (|dP_1| + |p_1/p_3| |dP_3|) / p_3 along p(tau) = p + tau dP
+#pragma unroll 1
+            for (int m = 0; m < n_t; ++m) {
+                double Rm[9];
+#pragma unroll
+                for (int e = 0; e < 9; ++e) Rm[e] = RmS[m * 9 + e];
+                ReprojRow b1, b2;
+                b1.g0 = b2.g0 = -CUDART_INF_F;
+                b1.a = b1.b = b2.a = b2.b = make_float4(0.f, 0.f, 0.f, 0.f);
+                b1.b.z = b2.b.z = -CUDART_INF_F;            // a row that never kills
+                double lip = 0.0;
+                for (int i = lane; i < n; i += 32) {
+                    const double *row = rows + i * ROW;
+                    double P0, P1, P2, Q0, Q1, Q2;
+                    reproj_point(R, row, P0, P1, P2);
+                    reproj_point(Rm, row, Q0, Q1, Q2);
+                    const ReprojRow r = reproj_row<true>(Q0 + t[0], Q1 + t[1], Q2 + t[2], row, K, t_p);
+                    if (r.g0 > b1.g0) { b2 = b1; b1 = r; } else if (r.g0 > b2.g0) b2 = r;
+                    const double plo = dmin(P2, Q2) + t[2] - 1.001 * t_p;
+                    if (plo > 0.0) {
+                        const double x_hi = dmax(fabs(P0 + t[0]), fabs(Q0 + t[0])) + t_p;
+                        const double y_hi = dmax(fabs(P1 + t[1]), fabs(Q1 + t[1])) + t_p;
+                        const double d0 = fabs(Q0 - P0), d1 = fabs(Q1 - P1), d2 = fabs(Q2 - P2);
+                        const double lx = K[0] * (d0 + x_hi / plo * d2) / plo;
+                        const double ly = K[1] * (d1 + y_hi / plo * d2) / plo;
+                        lip = dmax(lip, lx + ly);
+                    } else {
+                        lip = CUDART_INF;
+                    }
+                }
+                const uint32_t k1 = fkey(b1.g0);
+                const uint32_t m1 = __reduce_max_sync(FULL, k1);
+                const int src1 = __ffs(__ballot_sync(FULL, k1 == m1)) - 1;
+                const uint32_t k2 = (lane == src1) ? fkey(b2.g0) : k1;
+                const uint32_t m2 = __reduce_max_sync(FULL, k2);
+                const int src2 = __ffs(__ballot_sync(FULL, k2 == m2)) - 1;
+                if (lane == src1) { qrow[4 * m] = b1.a; qrow[4 * m + 1] = b1.b; }
+                if (lane == src2) {
+                    qrow[4 * m + 2] = (lane == src1) ? b2.a : b1.a;
+                    qrow[4 * m + 3] = (lane == src1) ? b2.b : b1.b;
+                }
+                const float lf = wmax_nonneg((float)lip);
+                if (lane == 0) qL[m] = lf * 1.001f + 1e-30f;
+            }
+            if (stats) { st_ps += n; st_ls += (unsigned long long)n * n_t; }
+            __syncwarp();
+            if (lane == 0) {                                 // suffix maximum: qL[m] holds for every rung >= m
+                float sm = 0.f;
+                for (int m = n_t - 1; m >= 0; --m) { sm = fmaxf(sm, qL[m]); qL[m] = sm; }
+            }
+            __syncwarp();
+        }
+
+        // ================================================== a2: perturbations of this lane (d_j = t_p xi_j)
+        float d0[NQ], d1[NQ], d2[NQ];
+        {
+            int jv[NQ];
+            uint32_t x[NQ], y[NQ], z[NQ];
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) jv[q] = lane + 32 * q;
+            philox_batch<NQ>(rng, (uint32_t)s, jv, x, y, z);
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) {
+                d0[q] = tpfl * pm1f(x[q]); d1[q] = tpfl * pm1f(y[q]); d2[q] = tpfl * pm1f(z[q]);
+                pert[32 * q + lane] = make_float4(d0[q], d1[q], d2[q], 0.f);
+            }
+        }
+
+        // ================================================== a3: eq. (14) in fp32: max_i ||q||^2 / p_3^2 per run
+        float dv[NQ];
+        {
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) dv[q] = CUDART_INF_F;
+            int i = 0;
+            for (int r = 0; r < n_runs; ++r) {
+                const int end = run_end[r];
+                const float bf = run_bf[r];
+                float mx[NQ];
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) mx[q] = 0.f;
+                for (; i <= end; ++i) {
+                    const float4 ra = rowsA[2 * i], rb = rowsA[2 * i + 1];
+#pragma unroll
+                    for (int q = 0; q < NQ; ++q) {
+                        const float q0 = fmaf(ra.w, d2[q], fmaf(nfx, d0[q], ra.x));
+                        const float q1 = fmaf(rb.x, d2[q], fmaf(nfy, d1[q], ra.y));
+                        float wr;
+                        asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(wr) : "f"(ra.z + d2[q]));
+                        mx[q] = fmaxf(mx[q], fmaf(q0, q0, q1 * q1) * (wr * wr));
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) {
+                    const float a = fmaxf(mx[q], 1e-30f);
+                    dv[q] = fminf(dv[q], bf - a * rsqrtf(a));
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < NQ; ++q)
+                if (lane + 32 * q >= n_p) dv[q] = -CUDART_INF_F;
+            if (stats) st_pp32 += (unsigned long long)n * n_p;
+        }
+
+        // ================================================== a4: top-N_P* with certified ranking
+        float myval;
+        if (!topk_certified<NQ>(dv, n_ps, uncA, (L.exact_only & 4) != 0, lane, candj, candd, myval)) {
+            double R[9], t[3], K[4];
+#pragma unroll
+            for (int e = 0; e < 9; ++e) R[e] = pose[e];
+#pragma unroll
+            for (int e = 0; e < 3; ++e) t[e] = pose[9 + e];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) K[e] = D->K[e];
+            const ExactMarginReproj exact{ R, t, K, rows, n, rng, (uint32_t)s, t_p };
+            const int cnt = topk_fp64<NQ>(dv, n_p, n_ps, uncA, myval, (L.exact_only & 16) != 0, lane, dex, candj, candd, exact);
+            if (stats) { ++st_fb; st_pp += (unsigned long long)n * cnt; }
+        }
+        __syncwarp();                                       // pert[], candj[] visible to all lanes
+        if (lane < n_ps) cand4[lane] = pert[candj[lane]];
+        __syncwarp();
+
+        // ================================================== a5-a6: ladder, first feasible rung
+        int m0 = 0;
+        unsigned win = 0u;
+        bool lip_stop = false;
+        const bool k_act = lane < KP;
+        const float4 kc4 = k_act ? cand4[lane] : make_float4(0.f, 0.f, 0.f, 0.f);
+        const float kcd = k_act ? candd[lane] : -CUDART_INF_F;
+        const float kcd_max = fkey_inv(__reduce_max_sync(FULL, fkey(kcd)));
+        for (int mb = 0; mb < n_t && m0 == 0 && !lip_stop; mb += 32) {
+            // ---- screening, lane = candidate (see walker_coop_kernel.cu)
+            int mend = min(n_t, mb + 32);
+            {
+                const bool dead_m = (mb + lane < mend) && (kcd_max + qL[min(mb + lane, n_t - 1)] < 0.f);
+                const unsigned lb = __ballot_sync(FULL, dead_m);
+                if (lb != 0u) { lip_stop = true; mend = mb + __ffs(lb) - 1; }
+            }
+            unsigned alive_r = 0u;
+#pragma unroll 2
+            for (int m = mb; m < mend; ++m) {
+                const float v0 = cone_lo(qrow[4 * m], qrow[4 * m + 1], kc4, nfx, nfy);
+                const float v1 = cone_lo(qrow[4 * m + 2], qrow[4 * m + 3], kc4, nfx, nfy);
+                if (!(v0 > 0.f) && !(v1 > 0.f) && !(kcd + qL[m] < 0.f)) alive_r |= 1u << (m - mb);
+            }
+            if (!k_act) alive_r = 0u;
+            const int mscr = mend;
+            if (L.exact_only & 2) {                          // debug: the screening kills nothing
+                lip_stop = false;
+                mend = min(n_t, mb + 32);
+                alive_r = k_act ? ((mend - mb >= 32) ? FULL : ((1u << (mend - mb)) - 1u)) : 0u;
+            }
+            unsigned qmask = __reduce_or_sync(FULL, alive_r);
+            if (stats) st_lp32 += (unsigned long long)(mscr - mb) * 2 * KP;
+
+            // ---- full evaluation of the surviving rungs, in order
+            while (qmask != 0u && m0 == 0) {
+                const int l0 = __ffs(qmask) - 1;
+                qmask &= qmask - 1u;
+                const int m1 = mb + l0;
+                const unsigned cand_alive = __ballot_sync(FULL, (alive_r >> l0) & 1u);
+                double Rm[9], t[3], K[4];
+#pragma unroll
+                for (int e = 0; e < 9; ++e) Rm[e] = RmS[m1 * 9 + e];
+#pragma unroll
+                for (int e = 0; e < 3; ++e) t[e] = pose[9 + e];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) K[e] = D->K[e];
+                if (full_m != m1) {
+                    __syncwarp();                            // earlier readers of rowsL are done
+                    float eps_l = 0.f;
+                    for (int i = lane; i < n; i += 32) {
+                        const double *row = rows + i * ROW;
+                        double Q0, Q1, Q2;
+                        reproj_point(Rm, row, Q0, Q1, Q2);
+                        const ReprojRow r = reproj_row<true>(Q0 + t[0], Q1 + t[1], Q2 + t[2], row, K, t_p);
+                        rowsL[2 * i] = r.a;
+                        rowsL[2 * i + 1] = r.b;
+                        eps_l = fmaxf(eps_l, r.unc);
+                    }
+                    epsL = wmax_nonneg(eps_l);
+                    full_m = m1;
+                    if (stats) st_ls += n;
+                    __syncwarp();
+                }
+                if (stats) { ++st_vr; st_lp32 += (unsigned long long)n * KP; }
+                float M = -CUDART_INF_F;
+                if (e_act) {
+                    const float4 c4 = cand4[ek];
+                    for (int i = ech; i < n; i += NCH) M = fmaxf(M, cone_lo(rowsL[2 * i], rowsL[2 * i + 1], c4, nfx, nfy));
+                    M = fkey_inv(__reduce_max_sync(e_mask, fkey(M)));
+                }
+                // M = max_i (g32_i - E_g,i):  M > 0 => some constraint violated for sure;
+                // M + 2 max_i E_g,i <= 0 => every constraint satisfied (and in front of the camera) for sure.
+                const bool dead = M > 0.f;
+                const bool sure = M <= -2.0f * epsL;
+                const bool mine = e_act && ech == 0;
+                unsigned alive2 = __ballot_sync(FULL, mine && !dead) & cand_alive;
+                unsigned undecided = __ballot_sync(FULL, mine && !dead && !sure) & cand_alive;
+                if (L.exact_only & 2) { alive2 = cand_alive; undecided = cand_alive; }
+                while (undecided != 0u) {                    // rare: fp64 decides
+                    const int k = __ffs(undecided) - 1;
+                    undecided &= undecided - 1u;
+                    if (!exact_candidate_feasible_reproj(Rm, t, K, rows, n, rng, (uint32_t)s, candj[k], t_p, lane))
+                        alive2 &= ~(1u << k);
+                    if (stats) st_lp += n;
+                }
+                if (alive2 != 0u) { m0 = m1 + 1; win = alive2; }
+            }
+        }
+
+        int j_win = 0;
+        if (m0) {
+            const int kw = __ffs(win) - 1;                    // lowest rank among the feasible (R-8)
+            j_win = candj[kw];
+            double x, y, z;
+            rng.xi3((uint32_t)s, (uint32_t)j_win, 1u, x, y, z);
+            const double t0 = __dadd_rn(pose[9], __dmul_rn(t_p, x));
+            const double t1 = __dadd_rn(pose[10], __dmul_rn(t_p, y));
+            const double t2 = __dadd_rn(pose[11], __dmul_rn(t_p, z));
+            const double re = (lane < 9) ? RmS[(m0 - 1) * 9 + lane] : 0.0;
+            __syncwarp();
+            if (lane < 9) pose[lane] = re;
+            if (lane == 9) { pose[9] = t0; pose[10] = t1; pose[11] = t2; }
+            if (stats) ++st_acc;
+        }
+        moved = (m0 != 0);
+        if (m0 != 1) hit = true;                              // R-12 (R-11: nothing feasible -> unchanged)
+        if (L.out_trace != nullptr && lane == 0)
+            L.out_trace[((size_t)blockIdx.y * L.num_walkers + local) * L.num_steps + (s - 1)] = m0 | (j_win << 8);
+        __syncwarp();                                         // RmS / pert / candj readers done before the next step writes
+    }
+
+    // ---- a7: emit
+    if (lane == 0) {
+        const size_t o = (size_t)blockIdx.y * L.num_walkers + local;
+        double2 *dst = reinterpret_cast<double2 *>(L.out_samples + 12 * o);
+#pragma unroll
+        for (int e = 0; e < 6; ++e) dst[e] = make_double2(pose[2 * e], pose[2 * e + 1]);
+        L.out_flags[o] = hit ? 1 : 0;
+        if (stats) {
+            atomicAdd(L.stats + 0, st_pp); atomicAdd(L.stats + 1, st_lp); atomicAdd(L.stats + 2, st_ps);
+            atomicAdd(L.stats + 3, st_ls); atomicAdd(L.stats + 4, st_acc);
+            atomicAdd(L.stats + 5, (unsigned long long)L.num_steps);
+            atomicAdd(L.stats + 6, st_pp32); atomicAdd(L.stats + 7, st_lp32);
+            atomicAdd(L.stats + 8, st_fb); atomicAdd(L.stats + 9, st_vr);
+        }
+    }
+}
+
+template <int NQ>
+cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
+{
+    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 2);
+    if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
+    cudaError_t e = cudaFuncSetAttribute(walker_coop_reproj_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)lay.total);
+    if (e != cudaSuccess) return e;
+    const long long blocks = (L.num_walkers + kCoopWarps - 1) / kCoopWarps;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    dim3 grid((unsigned)blocks, (unsigned)n_instances, 1);
+    walker_coop_reproj_kernel<NQ><<<grid, kCoopThreads, lay.total, stream>>>(L);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_walkers_coop_reproj(const WalkLaunch &L, int n_instances, int max_rows_bytes, cudaStream_t stream)
+{
+    const int max_n = max_rows_bytes / (ROW * 8);
+    if (L.n_p <= 32) return launch_q<1>(L, n_instances, max_rows_bytes, max_n, stream);
+    if (L.n_p <= 64) return launch_q<2>(L, n_instances, max_rows_bytes, max_n, stream);
+    if (L.n_p <= 160) return launch_q<5>(L, n_instances, max_rows_bytes, max_n, stream);
+    return launch_q<8>(L, n_instances, max_rows_bytes, max_n, stream);
+}
+
+}  // namespace closure

@@ -122,20 +122,12 @@ __global__ void __launch_bounds__(kBlock, 2) walker_kernel(const __grid_constant
                     // REPROJ: P_i = R Z_i + t* once per constraint, then one projection per perturbation
                     for (int i = 0; i < n; ++i) {
                         const double *row = rows + i * ROW;
-                        const double Z0 = row[2], Z1 = row[3], Z2 = row[4];
-                        const double P0 = R[0] * Z0 + R[1] * Z1 + R[2] * Z2;
-                        const double P1 = R[3] * Z0 + R[4] * Z1 + R[5] * Z2;
-                        const double P2 = R[6] * Z0 + R[7] * Z1 + R[8] * Z2;
+                        double P0, P1, P2;
+                        reproj_point(R, row, P0, P1, P2);
                         const double beta = row[RS::BETA];
 #pragma unroll
                         for (int jj = 0; jj < kJT; ++jj) {
-                            const double p0 = P0 + (t[0] + e0[jj]), p1 = P1 + (t[1] + e1[jj]), p2 = P2 + (t[2] + e2[jj]);
-                            double sq = CUDART_INF;
-                            if (p2 > 0.0) {
-                                const double g0 = row[0] - (K[0] * (p0 / p2) + K[2]);
-                                const double g1 = row[1] - (K[1] * (p1 / p2) + K[3]);
-                                sq = g0 * g0 + g1 * g1;
-                            }
+                            const double sq = reproj_sq(P0, P1, P2, t[0] + e0[jj], t[1] + e1[jj], t[2] + e2[jj], row, K);
                             dmn[jj] = dmin(dmn[jj], beta - sqrt(sq));
                         }
                     }
@@ -194,21 +186,13 @@ __global__ void __launch_bounds__(kBlock, 2) walker_kernel(const __grid_constant
                             if (!(v <= kdd[k])) alive &= ~(1u << k);
                         }
                     } else {
-                        const double Z0 = row[2], Z1 = row[3], Z2 = row[4];
-                        const double P0 = Rm[0] * Z0 + Rm[1] * Z1 + Rm[2] * Z2;
-                        const double P1 = Rm[3] * Z0 + Rm[4] * Z1 + Rm[5] * Z2;
-                        const double P2 = Rm[6] * Z0 + Rm[7] * Z1 + Rm[8] * Z2;
+                        double P0, P1, P2;
+                        reproj_point(Rm, row, P0, P1, P2);
                         const double b2 = row[RS::BETA + 1];
 #pragma unroll
                         for (int k = 0; k < KCAP; ++k) {
-                            const double p0 = P0 + (t[0] + k0[k]), p1 = P1 + (t[1] + k1[k]), p2 = P2 + (t[2] + k2[k]);
-                            bool ok = false;
-                            if (p2 > 0.0) {
-                                const double g0 = row[0] - (K[0] * (p0 / p2) + K[2]);
-                                const double g1 = row[1] - (K[1] * (p1 / p2) + K[3]);
-                                ok = (g0 * g0 + g1 * g1) <= b2;
-                            }
-                            if (!ok) alive &= ~(1u << k);
+                            const double sq = reproj_sq(P0, P1, P2, t[0] + k0[k], t[1] + k1[k], t[2] + k2[k], row, K);
+                            if (!(sq <= b2)) alive &= ~(1u << k);
                         }
                     }
                     if (!__any_sync(FULL, alive != 0u)) { ++i; break; }

@@ -138,7 +138,7 @@ def test_samples_are_feasible_and_orthonormal():
         assert flag.mean() > 0.9
 
 
-@pytest.mark.parametrize("config,walkers,steps", [(2, 4096, 150), (1, 1024, 200), (4, 2048, 120), (5, 2048, 150)])
+@pytest.mark.parametrize("config,walkers,steps", [(2, 4096, 150), (1, 1024, 200), (4, 2048, 120), (5, 2048, 150), (3, 4096, 150)])
 def test_screened_kernel_is_bit_identical_to_exact_kernel(config, walkers, steps):
     """The fp32-screened kernel takes every decision on fp64 values: outputs and traces must equal the
     plain fp64 kernel's (CLOSURE_FLAG_EXACT_ONLY) bit for bit, on far more walkers than the oracle replays."""
@@ -164,7 +164,7 @@ def test_screened_kernel_falls_back_on_ties():
 
 
 @pytest.mark.parametrize("flags", [2, 4, 6, 20])
-@pytest.mark.parametrize("config,walkers,steps", [(2, 1024, 80), (4, 512, 80), (5, 512, 100)])
+@pytest.mark.parametrize("config,walkers,steps", [(2, 1024, 80), (4, 512, 80), (5, 512, 100), (3, 1024, 80)])
 def test_cooperative_kernel_forced_fp64_paths(config, walkers, steps, flags):
     """Debug switches of the warp-cooperative kernel: 2 = every ladder candidate goes to the fp64 test,
     4 = every iteration takes the fp64 top-k fallback (16: on all N_P perturbations).
