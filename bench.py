@@ -37,6 +37,8 @@ WALK_SEED = 42
 #   one (pose, constraint) pair  = 3 FMA + 1 compare/max                      = 7   (fp32, or fp64 where it falls back)
 #   one per-constraint set-up    = R a (6 FMA + 3 MUL) + 6 ADD/SUB + |u|^2 (2 FMA + MUL) = 26 (+1 on the ladder), fp64
 FLOP_PAIR, FLOP_SETUP_A, FLOP_SETUP_L = 7.0, 26.0, 27.0
+# reprojection residual: eq. (14) pair = 4 FMA + RCP + 3 MUL + max = 13; cone pair = 8 FMA + max = 17
+FLOP_PAIR_REPROJ_A, FLOP_PAIR_REPROJ_L = 13.0, 17.0
 
 
 def _params_dict(P) -> dict:
@@ -245,9 +247,10 @@ def run_cuda(args) -> None:
         handles[0].closure_enable_stats(False)
         # the kernel decides in fp32 with certified error bounds and falls back to fp64:
         # executed arithmetic per pipe, and the time the two CUDA-core pipes need for it at their measured peaks
-        flops64 = FLOP_PAIR * (st["perturb_pairs"] + st["ladder_pairs"]) + FLOP_SETUP_A * st["perturb_setups"] \
+        fpa, fpl = (FLOP_PAIR_REPROJ_A, FLOP_PAIR_REPROJ_L) if inst.residual_type == 1 else (FLOP_PAIR, FLOP_PAIR)
+        flops64 = fpa * st["perturb_pairs"] + fpl * st["ladder_pairs"] + FLOP_SETUP_A * st["perturb_setups"] \
             + FLOP_SETUP_L * st["ladder_setups"]
-        flops32 = FLOP_PAIR * (st["perturb_pairs_f32"] + st["ladder_pairs_f32"])
+        flops32 = fpa * st["perturb_pairs_f32"] + fpl * st["ladder_pairs_f32"]
         flops = flops64 + flops32
         walk_s = statistics.mean(walk_ms) * 1e-3
         achieved = flops / walk_s / 1e12
