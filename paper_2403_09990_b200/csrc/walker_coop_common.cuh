@@ -19,7 +19,7 @@ constexpr unsigned FULL = 0xffffffffu;
 constexpr float kMu19 = 1.9073486328125e-06f;   // 2^-19
 
 struct CoopSmem {
-    size_t run_end, run_bf, warp0, per_warp, rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, cand4, candj, candd, pose, total;
+    size_t run_end, run_bf, run_pend, pos, warp0, per_warp, rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, cand4, candj, candd, pose, total;
 };
 
 // Shared-memory layout; f4 = float4 words per fp32 constraint row (1: affine residuals, 2: reprojection)
@@ -29,9 +29,11 @@ __host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, 
     size_t o = 16 + (size_t)((rows_bytes + 15) & ~15);
     s.run_end = o; o += (size_t)((n * 4 + 15) & ~15);
     s.run_bf = o;  o += (size_t)((n * 4 + 15) & ~15);
+    s.run_pend = o; o += (size_t)((n * 4 + 15) & ~15);
+    s.pos = o;     o += (size_t)((n * 4 + 15) & ~15);
     s.warp0 = o;
     size_t w = 0;
-    s.rowsA = w; w += (size_t)n * 16 * f4;
+    s.rowsA = w; w += (size_t)n * 32;              // affine: pair-transposed, runs padded to even length
     s.rowsL = w; w += (size_t)n * 16 * f4;
     s.pert = w;  w += (size_t)nq * 32 * 16;
     s.ab = w;    w += (size_t)n_t * 16;

@@ -154,6 +154,8 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 1);
     int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
     float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
+    int *run_pend = reinterpret_cast<int *>(smem_raw + lay.run_pend);   // end of run r in rowsA, in PAIRS of rows
+    int *pos = reinterpret_cast<int *>(smem_raw + lay.pos);             // row of constraint i in rowsA (bit 30: write it twice)
     if (warp == 0) {                                   // runs of equal bounds (rows are sorted by bound)
         int cnt = 0;
         for (int base = 0; base < n; base += 32) {
@@ -172,7 +174,20 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
             }
             cnt += __popc(m);
         }
-        if (lane == 0) n_runs_s = cnt;
+        __syncwarp();
+        if (lane == 0) {
+            // rowsA holds the fp32 set-ups two constraints per entry; a run of odd length repeats its last
+            // constraint (a maximum does not see duplicates), so no pair straddles two bounds
+            n_runs_s = cnt;
+            int p = 0, start = 0;
+            for (int r = 0; r < cnt; ++r) {
+                const int end = run_end[r];
+                for (int i = start; i <= end; ++i) pos[i] = p++;
+                if (p & 1) { pos[end] |= 0x40000000; ++p; }
+                run_pend[r] = p >> 1;
+                start = end + 1;
+            }
+        }
     }
     __syncthreads();
     const int n_runs = n_runs_s;
@@ -261,7 +276,12 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
                 affine_setup<RES>(R, t, row, u0, u1, u2, c);
                 float f0, f1, f2, fc, eps;
                 screen_row(u0, u1, u2, c, tp2, tp2sq3, f0, f1, f2, fc, eps);
-                rowsA[i] = make_float4(f0, f1, f2, fc);
+                {
+                    const int pp = pos[i], p = pp & 0x3fffffff;
+                    float *A = reinterpret_cast<float *>(rowsA) + (p >> 1) * 8 + (p & 1);
+                    A[0] = f0; A[2] = f1; A[4] = f2; A[6] = fc;
+                    if (pp & 0x40000000) { A[1] = f0; A[3] = f1; A[5] = f2; A[7] = fc; }
+                }
                 eps_l = fmaxf(eps_l, eps);
                 if (RES == CLOSURE_POSE_REG_SPLIT) rm_l = dmin(rm_l, row[12] - sqrt(frob_sq(R, row)));
             }
@@ -372,27 +392,37 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
 #pragma unroll
             for (int q = 0; q < NQ; ++q) dt[q] = CUDART_INF_F;
             const float E0 = epsA + tp2sq3 * kMu19;          // bound on |a32 - a64| up to its own rounding
-            int i = 0;
+            int pp = 0;
             for (int r = 0; r < n_runs; ++r) {
-                const int end = run_end[r];
+                const int pend = run_pend[r];
                 const float bf = run_bf[r];
                 float mx[NQ];
 #pragma unroll
                 for (int q = 0; q < NQ; ++q) mx[q] = -CUDART_INF_F;
-#pragma unroll 2
-                for (; i <= end; ++i) {
-                    const float4 f = rowsA[i];
-                    const unsigned long long F0 = pk2(f.x, f.x), F1 = pk2(f.y, f.y), F2 = pk2(f.z, f.z),
-                                             FC = pk2(f.w, f.w);
+#pragma unroll(NQ <= 2 ? 4 : 2)
+                for (; pp < pend; ++pp) {
+                    // two constraints a, b per entry: X = (f0a f0b f1a f1b), Y = (f2a f2b fca fcb)
+                    const float4 X = rowsA[2 * pp], Y = rowsA[2 * pp + 1];
 #pragma unroll
                     for (int k = 0; k < NPK; ++k) {
-                        const unsigned long long v = fma2(F0, p0[k], fma2(F1, p1[k], fma2(F2, p2[k], FC)));
-                        float lo, hi;
-                        upk2(v, lo, hi);
-                        mx[2 * k] = fmaxf(mx[2 * k], lo);
-                        mx[2 * k + 1] = fmaxf(mx[2 * k + 1], hi);
+                        const unsigned long long va =
+                            fma2(pk2(X.x, X.x), p0[k], fma2(pk2(X.z, X.z), p1[k], fma2(pk2(Y.x, Y.x), p2[k], pk2(Y.z, Y.z))));
+                        const unsigned long long vb =
+                            fma2(pk2(X.y, X.y), p0[k], fma2(pk2(X.w, X.w), p1[k], fma2(pk2(Y.y, Y.y), p2[k], pk2(Y.w, Y.w))));
+                        float la, ha, lb, hb;
+                        upk2(va, la, ha);
+                        upk2(vb, lb, hb);
+                        mx[2 * k] = fmaxf(mx[2 * k], fmaxf(la, lb));
+                        mx[2 * k + 1] = fmaxf(mx[2 * k + 1], fmaxf(ha, hb));
                     }
-                    if (ODD) mx[NQ - 1] = fmaxf(mx[NQ - 1], fmaf(f.x, o0, fmaf(f.y, o1, fmaf(f.z, o2, f.w))));
+                    if (ODD) {                          // the odd slot takes both constraints in one packed chain
+                        const unsigned long long vo = fma2(pk2(X.x, X.y), pk2(o0, o0),
+                                                           fma2(pk2(X.z, X.w), pk2(o1, o1),
+                                                                fma2(pk2(Y.x, Y.y), pk2(o2, o2), pk2(Y.z, Y.w))));
+                        float lo, hi;
+                        upk2(vo, lo, hi);
+                        mx[NQ - 1] = fmaxf(mx[NQ - 1], fmaxf(lo, hi));
+                    }
                 }
 #pragma unroll
                 for (int q = 0; q < NQ; ++q) {
