@@ -176,6 +176,9 @@ def run_cuda(args) -> None:
     # sits on the data path.
     begin = rank * W
     handles = []
+    if args.precision == 32:
+        for it in insts:
+            it.params.precision = 32
     for it, s0 in zip(insts, S0s):
         h = B.Closure.closure_create(it)
         h.closure_set_init(s0)
@@ -288,10 +291,68 @@ def run_cuda(args) -> None:
         e2e_dt = time.perf_counter() - t0
         h2d = sum(it.measurements.nbytes + it.betas.nbytes + s0.nbytes + 256 for it, s0 in zip(insts, S0s))
 
+        fp32_report = None
+        if args.precision == 32:
+            # measured difference of the fp32 mode from the fp64 path: same instance, same seed, decision traces
+            import copy
+            Wc = min(W, 16384)
+            P64 = copy.copy(insts[0].params)
+            P64.precision = 64
+            h64 = B.Closure.closure_create(insts[0], P64)
+            h64.closure_set_init(S0s[0])
+            s32, f32_, t32 = handles[0].closure_sample(Wc, S, WALK_SEED, trace=True)
+            s64, f64_, t64 = h64.closure_sample(Wc, S, WALK_SEED, trace=True)
+            same = (t32 == t64).all(dim=1)
+            c32, n32 = handles[0].closure_compact(s32, f32_)
+            r32 = handles[0].closure_megb(c32, int(n32.item()))
+            c64, n64 = h64.closure_compact(s64, f64_)
+            r64 = h64.closure_megb(c64, int(n64.item()))
+            fp32_report = {"walkers_compared": Wc, "iterations": S,
+                           "walkers_with_identical_decisions": float(same.float().mean().item()),
+                           "max_abs_sample_difference_among_those": float((s32[same] - s64[same]).abs().max().item())
+                           if bool(same.any()) else None,
+                           "rot_radius_rel_diff": abs(r32["rot_radius"] - r64["rot_radius"]) / r64["rot_radius"],
+                           "trans_radius_rel_diff": abs(r32["trans_radius"] - r64["trans_radius"]) / r64["trans_radius"]}
+            h64.closure_destroy()
+            del s32, s64, t32, t64
+
+        # the compaction kernel alone at BASELINE config 5's size (4,194,304 walkers, every sample kept):
+        # the size at which it is HBM-bound rather than launch-bound
+        nbig = 4194304
+        big_s = torch.empty((nbig, 12), dtype=torch.float64, device=dev).fill_(1.0)
+        big_f = torch.ones((nbig,), dtype=torch.uint8, device=dev)
+        big_o = torch.empty_like(big_s)
+        big_ms = []
+        for k in range(7):
+            flush.fill_(k)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            handles[0].closure_compact(big_s, big_f, big_o, count, stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            if k >= 2:
+                big_ms.append(e0.elapsed_time(e1))
+        big_bytes = nbig * 1 + int(count.item()) * 96 * 2
+        big_gbs = big_bytes / (statistics.mean(big_ms) * 1e-3) / 1e9
+        del big_s, big_f, big_o
+
+        # per-instance latency at the paper's own scale (|S_0| N_W = 200 walks, N_I = 5):
+        # host buffers in, MEGB out, through closure_create + closure_set_init + closure_run
+        small_ms = []
+        for k in range(25):
+            t1 = time.perf_counter()
+            h = B.Closure.closure_create(insts[0])
+            h.closure_set_init(S0s[0])
+            h.closure_run(200, 5, WALK_SEED + k, stream)
+            h.closure_destroy()
+            small_ms.append(1e3 * (time.perf_counter() - t1))
+        small_ms = statistics.median(small_ms[5:])
+
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64" if args.precision == 64 else "f32 decisions, f64 poses", "data": "synthetic",
             "config": {"workload": inst.name, "residual": "3D registration" if inst.residual_type == 2 else
                        ("2D reprojection" if inst.residual_type == 1 else "pose regression"),
                        "N": inst.n, "walkers": W, "iterations": S, "instances": nb, "S0": 128,
@@ -301,7 +362,8 @@ def run_cuda(args) -> None:
             "constraint_evals_per_sec_executed": (st["perturb_pairs"] + st["ladder_pairs"] + st["perturb_pairs_f32"]
                                                   + st["ladder_pairs_f32"]) / walk_s * world,
             "latency_ms": {"walker_kernel": statistics.mean(walk_ms), "compaction_kernel": statistics.mean(comp_ms),
-                           "host_megb": 1e3 * statistics.mean(megb_s), "e2e_per_instance": 1e3 * e2e_dt / (e2e_steps * nb)},
+                           "host_megb": 1e3 * statistics.mean(megb_s), "e2e_per_instance": 1e3 * e2e_dt / (e2e_steps * nb),
+                           "e2e_200_walkers_x_5_iterations": small_ms},
             "boundary_fraction": n_cnt / float(nb * W),
             "roofline": {"bound": "alu", "kernel": "walker_coop_kernel" if st["perturb_pairs_f32"] else "walker_kernel",
                          "achieved": achieved, "peak": peak_mix, "unit": "TFLOP/s", "frac": achieved / peak_mix,
@@ -318,12 +380,17 @@ def run_cuda(args) -> None:
             "roofline_compaction": {"bound": "hbm", "kernel": "compact_kernel", "achieved": comp_bytes / comp_s / 1e9,
                                     "peak": hbm_peak, "unit": "GB/s", "frac": comp_bytes / comp_s / 1e9 / hbm_peak,
                                     "bytes_per_launch": comp_bytes, "peak_source": "MEASURED_PEAKS.json hbm_gbs"
-                                    if peaks else "fallback 6650"},
+                                    if peaks else "fallback 6650",
+                                    "at_4194304_walkers": {"achieved": big_gbs, "frac": big_gbs / hbm_peak,
+                                                           "bytes_per_launch": big_bytes,
+                                                           "ms": statistics.mean(big_ms)}},
             "e2e": {"value": e2e_steps * nb * W * S / e2e_dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h // e2e_steps},
             "gpu_launches": args.steps * (-(-nb // 96) + 1),     # walker launch(es) + compaction kernel per step
             "clocks": clk,
         }
+        if fp32_report is not None:
+            out["fp32_mode"] = fp32_report
         if not args.no_cpu_baseline and world == 1:
             out["cpu_baseline"] = cpu_baseline(inst, S0)
     for h in handles:
@@ -343,6 +410,9 @@ def main() -> None:
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config 1..5 (default 2 = configs[1])")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--precision", type=int, default=64, choices=[64, 32],
+                    help="64: every decision is the fp64 decision (default, the parity path); 32: fp32 mode, with its "
+                         "measured difference from the fp64 path in the output")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -66,7 +66,10 @@ typedef struct {
     double t_p;      /* translation perturbation scale: uniform on [-t_p, t_p]^3 (R-6) */
     double theta_p;  /* rotation perturbation scale (the paper's R_p): rotation vector uniform on
                         [-theta_p, theta_p]^3 (R-6) */
-    int precision;   /* 64 (fp64, the parity path) or 32 (fp32 arithmetic, fp64 I/O) */
+    int precision;   /* 64: every decision is the fp64 decision (the parity path).  32: rotation sampler only --
+                        decisions are taken on the fp32 values as they are (no certificate, no fp64 fall-back);
+                        poses stay fp64.  Differs from 64 only where an fp32 error bound straddles a
+                        threshold; bench.py --precision 32 reports the measured difference. */
     int flags;       /* bit 0 (CLOSURE_FLAG_EXACT_ONLY): run the plain fp64 one-walker-per-thread kernel even where
                         the warp-cooperative fp32-certified kernel exists (same results bit for bit; for
                         verification and timing).  Bits 1, 2, 4 force the cooperative kernel's fp64 fall-back

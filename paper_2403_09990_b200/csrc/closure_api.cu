@@ -85,7 +85,9 @@ int check_params(const closure_params *p, std::string *why)
     if (p->omega0 < 0.0 || p->v0 < 0.0 || p->t_p < 0.0 || p->theta_p < 0.0) { *why = "negative scale"; return CLOSURE_EINVAL; }
     if (p->precision != 64 && p->precision != 32) { *why = "precision must be 64 or 32"; return CLOSURE_EINVAL; }
     if (p->n_p_star > kMaxKStar) { *why = "n_p_star > 20 is not built"; return CLOSURE_EUNSUPPORTED; }
-    if (p->precision == 32) { *why = "fp32 mode is not built yet"; return CLOSURE_EUNSUPPORTED; }
+    if (p->precision == 32 && (p->mode != CLOSURE_MODE_ROT || p->n_p > 256)) {
+        *why = "fp32 mode exists for the rotation sampler with n_p <= 256 only"; return CLOSURE_EUNSUPPORTED;
+    }
     return CLOSURE_OK;
 }
 
@@ -149,7 +151,7 @@ void fill_launch(const closure_t *h, WalkLaunch &L)
     std::memset(&L, 0, sizeof(L));
     L.n_p = h->P.n_p; L.n_p_star = h->P.n_p_star; L.n_t = h->P.n_t;
     L.omega0 = h->P.omega0; L.v0 = h->P.v0; L.gamma = h->P.gamma; L.t_p = h->P.t_p; L.theta_p = h->P.theta_p;
-    L.exact_only = h->P.flags & 31;           // bit 0 documented; bits 1-2: debug switches of the screened kernel
+    L.exact_only = (h->P.flags & 31) | (h->P.precision == 32 ? 32 : 0);           // bit 0 documented; bits 1-2: debug switches of the screened kernel
 }
 
 bool same_params(const closure_params &a, const closure_params &b)

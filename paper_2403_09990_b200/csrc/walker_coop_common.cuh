@@ -145,7 +145,7 @@ __device__ __forceinline__ float pm1f(uint32_t x)
 // ranking is the same, strictly, so no tie-break is involved.  On success lane r < N_P* writes
 // candj[r] (index) and candd[r] (an upper bound of the fp64 value).  myval: lane r holds the r-th value.
 template <int NQ>
-__device__ __forceinline__ bool topk_certified(const float (&v)[NQ], int n_ps, float unc, bool force_fail, int lane,
+__device__ __forceinline__ bool topk_certified(const float (&v)[NQ], int n_ps, float unc, bool force_fail, bool trust, int lane,
                                                int *candj, float *candd, float &myval)
 {
     uint32_t key[NQ];
@@ -180,6 +180,7 @@ __device__ __forceinline__ bool topk_certified(const float (&v)[NQ], int n_ps, f
         const float need = fmaf(2.0f, unc, kMu19 * (fabsf(prev) + fabsf(myval)));
         ok = ok && (none_left || (prev - myval > need));
     }
+    if (trust) ok = true;                       // fp32 mode: the fp32 ranking is taken as it is
     if (force_fail) ok = false;
     const bool certified = __all_sync(FULL, ok);
     if (certified && lane < n_ps) {

@@ -377,7 +377,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
 
         // ================================================== a4: top-N_P* with certified ranking
         float myval;
-        if (!topk_certified<NQ>(dv, n_ps, uncA, (L.exact_only & 4) != 0, lane, candj, candd, myval)) {
+        if (!topk_certified<NQ>(dv, n_ps, uncA, (L.exact_only & 4) != 0, (L.exact_only & 32) != 0, lane, candj, candd, myval)) {
             double R[9], t[3], K[4];
 #pragma unroll
             for (int e = 0; e < 9; ++e) R[e] = pose[e];
@@ -471,6 +471,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
                 unsigned alive2 = __ballot_sync(FULL, mine && !dead) & cand_alive;
                 unsigned undecided = __ballot_sync(FULL, mine && !dead && !sure) & cand_alive;
                 if (L.exact_only & 2) { alive2 = cand_alive; undecided = cand_alive; }
+                if (L.exact_only & 32) undecided = 0u;       // fp32 mode: undecided counts as satisfied
                 while (undecided != 0u) {                    // rare: fp64 decides
                     const int k = __ffs(undecided) - 1;
                     undecided &= undecided - 1u;

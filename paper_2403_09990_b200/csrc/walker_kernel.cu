@@ -325,7 +325,11 @@ cudaError_t launch_walkers(int residual_type, int mode, bool stats, const WalkLa
         if (why) *why = "instance too large for shared-memory staging";
         return cudaErrorInvalidValue;
     }
-    if (!(L.exact_only & 1) &&
+    if ((L.exact_only & 32) && !coop_path_available(residual_type, mode, L.n_p, max_rows_bytes / (row_doubles(residual_type) * 8))) {
+        if (why) *why = "fp32 mode needs the cooperative kernel";
+        return cudaErrorInvalidValue;
+    }
+    if ((!(L.exact_only & 1) || (L.exact_only & 32)) &&
         coop_path_available(residual_type, mode, L.n_p, max_rows_bytes / (row_doubles(residual_type) * 8)))
         return launch_walkers_coop(residual_type, L, n_instances, max_rows_bytes, stream);
     switch (residual_type) {

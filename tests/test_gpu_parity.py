@@ -175,3 +175,31 @@ def test_cooperative_kernel_forced_fp64_paths(config, walkers, steps, flags):
     b = gpu_walk(inst, _small(inst.params, flags=1), S0, walkers, steps, 99)
     for x, y in zip(a, b):
         assert np.array_equal(x, y)
+
+
+@pytest.mark.parametrize("config", [1, 2, 3, 4, 5])
+def test_fp32_mode_measured_difference(config):
+    """precision = 32 takes the decisions on the fp32 values as they are (no certificate, no fp64 fall-back).
+    It may differ from the fp64 path only where an fp32 error bound straddles a threshold: most walkers
+    take identical decisions (then the fp64 poses are bit-identical), and every emitted pose is in S up to
+    the fp32 error."""
+    import oracle
+    inst = I.make_instance(config)
+    S0 = I.make_init_poses(inst, 128)
+    W, S = 2048, 100
+    f32 = gpu_walk(inst, _small(inst.params, precision=32), S0, W, S, 7)
+    f64 = gpu_walk(inst, inst.params, S0, W, S, 7)
+    same = (f32[2] == f64[2]).all(axis=1)
+    assert same.mean() > 0.9, f"only {same.mean():.3f} of the walkers take the fp64 decisions"
+    assert np.array_equal(f32[0][same], f64[0][same]) and np.array_equal(f32[1][same], f64[1][same])
+    scale = float(np.max(inst.betas))
+    worst = min(oracle.margin(inst, s[:9], s[9:]) for s in f32[0][::8])
+    assert worst >= -1e-5 * scale, f"fp32-mode sample violates a constraint by {-worst:.3e}"
+
+
+def test_fp32_mode_is_refused_where_it_does_not_exist():
+    from paper_2403_09990_b200 import binding as B
+    inst = I.make_instance(3)
+    with pytest.raises(B.ClosureError) as e:
+        B.Closure.closure_create(inst, _small(inst.params, precision=32, mode=I.MODE_TRANS, v0=0.05, theta_p=0.02))
+    assert e.value.status == B.EUNSUPPORTED
