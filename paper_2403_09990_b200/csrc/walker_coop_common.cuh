@@ -19,7 +19,7 @@ constexpr unsigned FULL = 0xffffffffu;
 constexpr float kMu19 = 1.9073486328125e-06f;   // 2^-19
 
 struct CoopSmem {
-    size_t run_end, run_bf, run_pend, pos, warp0, per_warp, rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, cand4, candj, candd, pose, total;
+    size_t run_end, run_bf, run_pend, pos, warp0, per_warp, rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, cand4, candj, candd, pose, stc, total;
 };
 
 // Shared-memory layout; f4 = float4 words per fp32 constraint row (1: affine residuals, 2: reprojection)
@@ -44,7 +44,8 @@ __host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, 
     s.cand4 = w; w += 32 * 16;
     s.candj = w; w += 32 * 4;
     s.candd = w; w += 32 * 4;
-    s.pose = w;  w += 16 * 8;
+    s.pose = w;  w += 18 * 8;
+    s.stc = w;   w += 16 * 8;
     s.per_warp = w;
     s.total = o + (size_t)kCoopWarps * w;
     return s;

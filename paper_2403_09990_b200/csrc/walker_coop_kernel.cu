@@ -132,6 +132,120 @@ __device__ __forceinline__ bool exact_candidate_feasible(const double (&Rm)[9], 
     return __all_sync(FULL, ok);
 }
 
+// ---------------------------------------------------------------------------------- set-up after a move
+// Everything that depends on the pose only (DESIGN.md 6.1b "state that only changes on an accepted
+// move"): fp32 set-up rows at R* (rowsA), Exp(dT_m w) R* for every rung (RmS), per rung the two
+// tightest rows (qrow) and the Lipschitz bound (qL).  fp64-heavy and rare, so it is kept out of line:
+// its registers do not count against the per-iteration code.  Results epsA, rot_margin -> pose[16], pose[15].
+template <int RES>
+__device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int warp, int lane, int rows_bytes, int n,
+                                                int n_t, int nq, double t_p, bool stats)
+{
+    using RS = Res<RES>;
+    constexpr int ROW = RS::ROW;
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, nq, 1);
+    const double *rows = reinterpret_cast<const double *>(smem_raw + 16);
+    const int *pos = reinterpret_cast<const int *>(smem_raw + lay.pos);
+    unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
+    float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);
+    const double2 *ab = reinterpret_cast<const double2 *>(wp + lay.ab);
+    float4 *qrow = reinterpret_cast<float4 *>(wp + lay.qrow);
+    double *RmS = reinterpret_cast<double *>(wp + lay.RmS);
+    float *qL = reinterpret_cast<float *>(wp + lay.qL);
+    double *pose = reinterpret_cast<double *>(wp + lay.pose);
+    unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
+    const float tpf = (float)t_p * 1.0000002f;          // >= t_p
+    const float tp2 = 2.0f * tpf, tp2sq3 = 3.0f * tpf * tpf;
+    double R[9], t[3], vel[3];
+#pragma unroll
+    for (int e = 0; e < 9; ++e) R[e] = pose[e];
+#pragma unroll
+    for (int e = 0; e < 3; ++e) { t[e] = pose[9 + e]; vel[e] = pose[12 + e]; }
+    float eps_l = 0.f;
+    double rm_l = CUDART_INF;
+    for (int i = lane; i < n; i += 32) {
+        const double *row = rows + i * ROW;
+        double u0, u1, u2, c;
+        affine_setup<RES>(R, t, row, u0, u1, u2, c);
+        float f0, f1, f2, fc, eps;
+        screen_row(u0, u1, u2, c, tp2, tp2sq3, f0, f1, f2, fc, eps);
+        {
+            const int pp = pos[i], p = pp & 0x3fffffff;
+            float *A = reinterpret_cast<float *>(rowsA) + (p >> 1) * 8 + (p & 1);
+            A[0] = f0; A[2] = f1; A[4] = f2; A[6] = fc;
+            if (pp & 0x40000000) { A[1] = f0; A[3] = f1; A[5] = f2; A[7] = fc; }
+        }
+        eps_l = fmaxf(eps_l, eps);
+        if (RES == CLOSURE_POSE_REG_SPLIT) rm_l = dmin(rm_l, row[12] - sqrt(frob_sq(R, row)));
+    }
+    const float epsA = wmax_nonneg(eps_l);
+    double rot_margin = CUDART_INF;
+    if (RES == CLOSURE_POSE_REG_SPLIT) rot_margin = wmin_f64(rm_l);
+    for (int m = lane; m < n_t; m += 32) {       // Exp(dT_m w) R* for every rung
+        const double2 c2 = ab[m];
+        double Rm[9];
+        rotate_left(R, vel[0], vel[1], vel[2], c2.x, c2.y, Rm);
+#pragma unroll
+        for (int e = 0; e < 9; ++e) RmS[m * 9 + e] = Rm[e];
+    }
+    __syncwarp();
+    // the two tightest constraints of every rung (largest c - beta^2 at the unperturbed
+    // translation): the rows the ladder screens each rung against while the pose stays here
+#pragma unroll 1
+    for (int m = 0; m < n_t; ++m) {
+        double Rm[9];
+#pragma unroll
+        for (int e = 0; e < 9; ++e) Rm[e] = RmS[m * 9 + e];
+        float4 b1 = make_float4(0.f, 0.f, 0.f, -CUDART_INF_F), b2 = b1;
+        bool rdead = false;
+        double dR[9], lip = 0.0;                     // max_i | ||g_i(R_m, .)|| - ||g_i(R*, .)|| | <= sqrt(lip)
+#pragma unroll
+        for (int e = 0; e < 9; ++e) dR[e] = Rm[e] - R[e];
+        if (RES != CLOSURE_REG_3D3D) {
+#pragma unroll
+            for (int e = 0; e < 9; ++e) lip = fma(dR[e], dR[e], lip);      // ||R_m - R*||_F^2
+        }
+        for (int i = lane; i < n; i += 32) {
+            const double *row = rows + i * ROW;
+            double u0, u1, u2, c;
+            affine_setup<RES>(Rm, t, row, u0, u1, u2, c);
+            if (RES == CLOSURE_REG_3D3D) {           // ||(R_m - R*) a_i||^2
+                const double q0 = dR[0] * row[0] + dR[1] * row[1] + dR[2] * row[2];
+                const double q1 = dR[3] * row[0] + dR[4] * row[1] + dR[5] * row[2];
+                const double q2 = dR[6] * row[0] + dR[7] * row[1] + dR[8] * row[2];
+                lip = dmax(lip, q0 * q0 + q1 * q1 + q2 * q2);
+            }
+            if (RES == CLOSURE_POSE_REG_SPLIT) {
+                if (!(frob_sq(Rm, row) <= row[13])) rdead = true;
+            }
+            float g0, g1, g2, fcb, eps;
+            screen_row(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
+            const float4 r4 = make_float4(g0, g1, g2, fcb - eps);
+            if (r4.w > b1.w) { b2 = b1; b1 = r4; } else if (r4.w > b2.w) b2 = r4;
+        }
+        const uint32_t k1 = fkey(b1.w);
+        const uint32_t m1 = __reduce_max_sync(FULL, k1);
+        const int src1 = __ffs(__ballot_sync(FULL, k1 == m1)) - 1;
+        const uint32_t k2 = (lane == src1) ? fkey(b2.w) : k1;
+        const uint32_t m2 = __reduce_max_sync(FULL, k2);
+        const int src2 = __ffs(__ballot_sync(FULL, k2 == m2)) - 1;
+        if (__any_sync(FULL, rdead)) b1.w = CUDART_INF_F;          // rung dead for every candidate
+        if (lane == src1) qrow[2 * m] = b1;
+        if (lane == src2) qrow[2 * m + 1] = (lane == src1) ? b2 : b1;
+        const float lf = wmax_nonneg((float)sqrt(lip));
+        if (lane == 0) qL[m] = lf * 1.001f + 1e-30f;
+    }
+    if (stats) { stc[2] += n; stc[3] += (unsigned long long)n * n_t; }
+    __syncwarp();
+    if (lane == 0) {                                 // suffix maximum: qL[m] holds for every rung >= m
+        float sm = 0.f;
+        for (int m = n_t - 1; m >= 0; --m) { sm = fmaxf(sm, qL[m]); qL[m] = sm; }
+    }
+    __syncwarp();
+    if (lane == 0) { pose[15] = rot_margin; pose[16] = (double)epsA; }
+    __syncwarp();
+}
+
 // ---------------------------------------------------------------------------------- the kernel
 template <int RES, int NQ>
 __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __grid_constant__ WalkLaunch L)
@@ -248,9 +362,12 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     unsigned e_mask = 0u;                               // lanes that share this lane's candidate
     for (int c = 0; c < NCH; ++c) e_mask |= 1u << (ek + c * KP);
 
-    unsigned long long st_pp32 = 0, st_lp32 = 0, st_ps = 0, st_ls = 0, st_acc = 0, st_fb = 0, st_vr = 0, st_pp = 0,
-                       st_lp = 0;
-    const bool stats = L.stats != nullptr;
+    // executed-work counters (closure_get_stats): in shared memory, touched by lane 0 and only when asked for
+    unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
+    const bool stats = (L.stats != nullptr) && lane == 0;
+    if (stats) {
+        for (int k = 0; k < 10; ++k) stc[k] = 0ull;
+    }
     bool hit = false;
     bool moved = true;
     float epsA = 0.f;
@@ -263,92 +380,10 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     for (int s = 1; s <= L.num_steps; ++s) {
         // ================================================== set-up at the current pose (only after a move)
         if (moved) {
-            double R[9], t[3], vel[3];
-#pragma unroll
-            for (int e = 0; e < 9; ++e) R[e] = pose[e];
-#pragma unroll
-            for (int e = 0; e < 3; ++e) { t[e] = pose[9 + e]; vel[e] = pose[12 + e]; }
-            float eps_l = 0.f;
-            double rm_l = CUDART_INF;
-            for (int i = lane; i < n; i += 32) {
-                const double *row = rows + i * ROW;
-                double u0, u1, u2, c;
-                affine_setup<RES>(R, t, row, u0, u1, u2, c);
-                float f0, f1, f2, fc, eps;
-                screen_row(u0, u1, u2, c, tp2, tp2sq3, f0, f1, f2, fc, eps);
-                {
-                    const int pp = pos[i], p = pp & 0x3fffffff;
-                    float *A = reinterpret_cast<float *>(rowsA) + (p >> 1) * 8 + (p & 1);
-                    A[0] = f0; A[2] = f1; A[4] = f2; A[6] = fc;
-                    if (pp & 0x40000000) { A[1] = f0; A[3] = f1; A[5] = f2; A[7] = fc; }
-                }
-                eps_l = fmaxf(eps_l, eps);
-                if (RES == CLOSURE_POSE_REG_SPLIT) rm_l = dmin(rm_l, row[12] - sqrt(frob_sq(R, row)));
-            }
-            epsA = wmax_nonneg(eps_l);
-            if (RES == CLOSURE_POSE_REG_SPLIT) rot_margin = wmin_f64(rm_l);
-            for (int m = lane; m < n_t; m += 32) {       // Exp(dT_m w) R* for every rung
-                const double2 c2 = ab[m];
-                double Rm[9];
-                rotate_left(R, vel[0], vel[1], vel[2], c2.x, c2.y, Rm);
-#pragma unroll
-                for (int e = 0; e < 9; ++e) RmS[m * 9 + e] = Rm[e];
-            }
+            coop_setup_on_move<RES>(smem_raw, warp, lane, rows_bytes, n, n_t, NQ, t_p, stats);
+            epsA = (float)pose[16];
+            rot_margin = pose[15];
             full_m = -1;
-            __syncwarp();
-            // the two tightest constraints of every rung (largest c - beta^2 at the unperturbed
-            // translation): the rows the ladder screens each rung against while the pose stays here
-#pragma unroll 1
-            for (int m = 0; m < n_t; ++m) {
-                double Rm[9];
-#pragma unroll
-                for (int e = 0; e < 9; ++e) Rm[e] = RmS[m * 9 + e];
-                float4 b1 = make_float4(0.f, 0.f, 0.f, -CUDART_INF_F), b2 = b1;
-                bool rdead = false;
-                double dR[9], lip = 0.0;                     // max_i | ||g_i(R_m, .)|| - ||g_i(R*, .)|| | <= sqrt(lip)
-#pragma unroll
-                for (int e = 0; e < 9; ++e) dR[e] = Rm[e] - R[e];
-                if (RES != CLOSURE_REG_3D3D) {
-#pragma unroll
-                    for (int e = 0; e < 9; ++e) lip = fma(dR[e], dR[e], lip);      // ||R_m - R*||_F^2
-                }
-                for (int i = lane; i < n; i += 32) {
-                    const double *row = rows + i * ROW;
-                    double u0, u1, u2, c;
-                    affine_setup<RES>(Rm, t, row, u0, u1, u2, c);
-                    if (RES == CLOSURE_REG_3D3D) {           // ||(R_m - R*) a_i||^2
-                        const double q0 = dR[0] * row[0] + dR[1] * row[1] + dR[2] * row[2];
-                        const double q1 = dR[3] * row[0] + dR[4] * row[1] + dR[5] * row[2];
-                        const double q2 = dR[6] * row[0] + dR[7] * row[1] + dR[8] * row[2];
-                        lip = dmax(lip, q0 * q0 + q1 * q1 + q2 * q2);
-                    }
-                    if (RES == CLOSURE_POSE_REG_SPLIT) {
-                        if (!(frob_sq(Rm, row) <= row[13])) rdead = true;
-                    }
-                    float g0, g1, g2, fcb, eps;
-                    screen_row(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
-                    const float4 r4 = make_float4(g0, g1, g2, fcb - eps);
-                    if (r4.w > b1.w) { b2 = b1; b1 = r4; } else if (r4.w > b2.w) b2 = r4;
-                }
-                const uint32_t k1 = fkey(b1.w);
-                const uint32_t m1 = __reduce_max_sync(FULL, k1);
-                const int src1 = __ffs(__ballot_sync(FULL, k1 == m1)) - 1;
-                const uint32_t k2 = (lane == src1) ? fkey(b2.w) : k1;
-                const uint32_t m2 = __reduce_max_sync(FULL, k2);
-                const int src2 = __ffs(__ballot_sync(FULL, k2 == m2)) - 1;
-                if (__any_sync(FULL, rdead)) b1.w = CUDART_INF_F;          // rung dead for every candidate
-                if (lane == src1) qrow[2 * m] = b1;
-                if (lane == src2) qrow[2 * m + 1] = (lane == src1) ? b2 : b1;
-                const float lf = wmax_nonneg((float)sqrt(lip));
-                if (lane == 0) qL[m] = lf * 1.001f + 1e-30f;
-            }
-            if (stats) { st_ps += n; st_ls += (unsigned long long)n * n_t; }
-            __syncwarp();
-            if (lane == 0) {                                 // suffix maximum: qL[m] holds for every rung >= m
-                float sm = 0.f;
-                for (int m = n_t - 1; m >= 0; --m) { sm = fmaxf(sm, qL[m]); qL[m] = sm; }
-            }
-            __syncwarp();
         }
 
         // ================================================== a2: perturbations of this lane
@@ -435,7 +470,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
                     dt[q] = fminf(dt[q], bf - sq);
                 }
             }
-            if (stats) st_pp32 += (unsigned long long)n * n_p;
+            if (stats) stc[6] += (unsigned long long)n * n_p;
         }
 
         // ================================================== a4: top-N_P* with certified ranking
@@ -454,7 +489,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
             for (int e = 0; e < 3; ++e) t[e] = pose[9 + e];
             const ExactMargin<RES> exact{ R, t, rows, n, rng, (uint32_t)s, t_p, rot_margin };
             const int cnt = topk_fp64<NQ>(dv, n_p, n_ps, unc, myval, (L.exact_only & 16) != 0, lane, dex, candj, candd, exact);
-            if (stats) { ++st_fb; st_pp += (unsigned long long)n * cnt; }
+            if (stats) { stc[8] += 1; stc[0] += (unsigned long long)n * cnt; }
         }
         __syncwarp();                                       // pert[], candj[] visible to all lanes
         if (lane < n_ps) cand4[lane] = pert[candj[lane]];
@@ -496,7 +531,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
                 alive_r = k_act ? ((mend - mb >= 32) ? FULL : ((1u << (mend - mb)) - 1u)) : 0u;
             }
             unsigned qmask = __reduce_or_sync(FULL, alive_r);
-            if (stats) st_lp32 += (unsigned long long)(m - mb) * 2 * KP;
+            if (stats) stc[7] += (unsigned long long)(m - mb) * 2 * KP;
 
             // ---- full evaluation of the surviving rungs, in order
             while (qmask != 0u && m0 == 0) {
@@ -528,10 +563,10 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
                     epsL = wmax_nonneg(eps_l);
                     rdeadL = __any_sync(FULL, rdead);
                     full_m = m1;
-                    if (stats) st_ls += n;
+                    if (stats) stc[3] += n;
                     __syncwarp();
                 }
-                if (stats) { ++st_vr; st_lp32 += (unsigned long long)n * KP; }
+                if (stats) { stc[9] += 1; stc[7] += (unsigned long long)n * KP; }
                 unsigned feas = 0u;
                 if (!rdeadL) {
                     float M = -CUDART_INF_F;
@@ -558,7 +593,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
                         undecided &= undecided - 1u;
                         if (!exact_candidate_feasible<RES>(Rm, t, rows, n, rng, (uint32_t)s, candj[k], t_p, lane))
                             alive2 &= ~(1u << k);
-                        if (stats) st_lp += n;
+                        if (stats) stc[1] += n;
                     }
                     feas = alive2;
                 }
@@ -579,7 +614,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
             __syncwarp();
             if (lane < 9) pose[lane] = re;
             if (lane == 9) { pose[9] = t0; pose[10] = t1; pose[11] = t2; }
-            if (stats) ++st_acc;
+            if (stats) stc[4] += 1;
         }
         moved = (m0 != 0);
         if (m0 != 1) hit = true;                              // R-12 (R-11: nothing feasible -> unchanged)
@@ -596,11 +631,8 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
         for (int e = 0; e < 6; ++e) dst[e] = make_double2(pose[2 * e], pose[2 * e + 1]);
         L.out_flags[o] = hit ? 1 : 0;
         if (stats) {
-            atomicAdd(L.stats + 0, st_pp); atomicAdd(L.stats + 1, st_lp); atomicAdd(L.stats + 2, st_ps);
-            atomicAdd(L.stats + 3, st_ls); atomicAdd(L.stats + 4, st_acc);
-            atomicAdd(L.stats + 5, (unsigned long long)L.num_steps);
-            atomicAdd(L.stats + 6, st_pp32); atomicAdd(L.stats + 7, st_lp32);
-            atomicAdd(L.stats + 8, st_fb); atomicAdd(L.stats + 9, st_vr);
+            stc[5] = (unsigned long long)L.num_steps;
+            for (int k = 0; k < 10; ++k) atomicAdd(L.stats + k, stc[k]);
         }
     }
 }

@@ -231,9 +231,12 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
     unsigned e_mask = 0u;                               // lanes that share this lane's candidate
     for (int c = 0; c < NCH; ++c) e_mask |= 1u << (ek + c * KP);
 
-    unsigned long long st_pp32 = 0, st_lp32 = 0, st_ps = 0, st_ls = 0, st_acc = 0, st_fb = 0, st_vr = 0, st_pp = 0,
-                       st_lp = 0;
-    const bool stats = L.stats != nullptr;
+    // executed-work counters (closure_get_stats): in shared memory, touched by lane 0 and only when asked for
+    unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
+    const bool stats = (L.stats != nullptr) && lane == 0;
+    if (stats) {
+        for (int k = 0; k < 10; ++k) stc[k] = 0ull;
+    }
     bool hit = false;
     bool moved = true;
     float uncA = CUDART_INF_F;
@@ -316,7 +319,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
                 const float lf = wmax_nonneg((float)lip);
                 if (lane == 0) qL[m] = lf * 1.001f + 1e-30f;
             }
-            if (stats) { st_ps += n; st_ls += (unsigned long long)n * n_t; }
+            if (stats) { stc[2] += n; stc[3] += (unsigned long long)n * n_t; }
             __syncwarp();
             if (lane == 0) {                                 // suffix maximum: qL[m] holds for every rung >= m
                 float sm = 0.f;
@@ -372,7 +375,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
 #pragma unroll
             for (int q = 0; q < NQ; ++q)
                 if (lane + 32 * q >= n_p) dv[q] = -CUDART_INF_F;
-            if (stats) st_pp32 += (unsigned long long)n * n_p;
+            if (stats) stc[6] += (unsigned long long)n * n_p;
         }
 
         // ================================================== a4: top-N_P* with certified ranking
@@ -387,7 +390,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
             for (int e = 0; e < 4; ++e) K[e] = D->K[e];
             const ExactMarginReproj exact{ R, t, K, rows, n, rng, (uint32_t)s, t_p };
             const int cnt = topk_fp64<NQ>(dv, n_p, n_ps, uncA, myval, (L.exact_only & 16) != 0, lane, dex, candj, candd, exact);
-            if (stats) { ++st_fb; st_pp += (unsigned long long)n * cnt; }
+            if (stats) { stc[8] += 1; stc[0] += (unsigned long long)n * cnt; }
         }
         __syncwarp();                                       // pert[], candj[] visible to all lanes
         if (lane < n_ps) cand4[lane] = pert[candj[lane]];
@@ -424,7 +427,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
                 alive_r = k_act ? ((mend - mb >= 32) ? FULL : ((1u << (mend - mb)) - 1u)) : 0u;
             }
             unsigned qmask = __reduce_or_sync(FULL, alive_r);
-            if (stats) st_lp32 += (unsigned long long)(mscr - mb) * 2 * KP;
+            if (stats) stc[7] += (unsigned long long)(mscr - mb) * 2 * KP;
 
             // ---- full evaluation of the surviving rungs, in order
             while (qmask != 0u && m0 == 0) {
@@ -453,10 +456,10 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
                     }
                     epsL = wmax_nonneg(eps_l);
                     full_m = m1;
-                    if (stats) st_ls += n;
+                    if (stats) stc[3] += n;
                     __syncwarp();
                 }
-                if (stats) { ++st_vr; st_lp32 += (unsigned long long)n * KP; }
+                if (stats) { stc[9] += 1; stc[7] += (unsigned long long)n * KP; }
                 float M = -CUDART_INF_F;
                 if (e_act) {
                     const float4 c4 = cand4[ek];
@@ -477,7 +480,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
                     undecided &= undecided - 1u;
                     if (!exact_candidate_feasible_reproj(Rm, t, K, rows, n, rng, (uint32_t)s, candj[k], t_p, lane))
                         alive2 &= ~(1u << k);
-                    if (stats) st_lp += n;
+                    if (stats) stc[1] += n;
                 }
                 if (alive2 != 0u) { m0 = m1 + 1; win = alive2; }
             }
@@ -496,7 +499,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
             __syncwarp();
             if (lane < 9) pose[lane] = re;
             if (lane == 9) { pose[9] = t0; pose[10] = t1; pose[11] = t2; }
-            if (stats) ++st_acc;
+            if (stats) stc[4] += 1;
         }
         moved = (m0 != 0);
         if (m0 != 1) hit = true;                              // R-12 (R-11: nothing feasible -> unchanged)
@@ -513,11 +516,8 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
         for (int e = 0; e < 6; ++e) dst[e] = make_double2(pose[2 * e], pose[2 * e + 1]);
         L.out_flags[o] = hit ? 1 : 0;
         if (stats) {
-            atomicAdd(L.stats + 0, st_pp); atomicAdd(L.stats + 1, st_lp); atomicAdd(L.stats + 2, st_ps);
-            atomicAdd(L.stats + 3, st_ls); atomicAdd(L.stats + 4, st_acc);
-            atomicAdd(L.stats + 5, (unsigned long long)L.num_steps);
-            atomicAdd(L.stats + 6, st_pp32); atomicAdd(L.stats + 7, st_lp32);
-            atomicAdd(L.stats + 8, st_fb); atomicAdd(L.stats + 9, st_vr);
+            stc[5] = (unsigned long long)L.num_steps;
+            for (int k = 0; k < 10; ++k) atomicAdd(L.stats + k, stc[k]);
         }
     }
 }
