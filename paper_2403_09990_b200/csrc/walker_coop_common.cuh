@@ -160,19 +160,21 @@ __device__ __forceinline__ bool topk_certified(const float (&v)[NQ], int n_ps, f
             const uint32_t hi = max(key[a], key[a + 1]), lo = min(key[a], key[a + 1]);
             key[a] = hi; key[a + 1] = lo;
         }
-    myval = -CUDART_INF_F;
-    int myj = -1;
+    uint32_t myg = fkey(-CUDART_INF_F);
+    int mysrc = 0;
     for (int r = 0; r <= n_ps; ++r) {               // extract the N_P* + 1 largest
         const uint32_t g = __reduce_max_sync(FULL, key[0]);
         const unsigned who = __ballot_sync(FULL, key[0] == g);
         const int src = __ffs(who) - 1;
-        if (lane == r) { myval = fkey_inv(g); myj = src + 32 * (int)(g & 7u); }
+        if (lane == r) { myg = g; mysrc = src; }
         if (lane == src) {
 #pragma unroll
             for (int q = 0; q + 1 < NQ; ++q) key[q] = key[q + 1];
             key[NQ - 1] = 0u;
         }
     }
+    myval = fkey_inv(myg);
+    const int myj = mysrc + 32 * (int)(myg & 7u);
     const float prev = __shfl_up_sync(FULL, myval, 1);
     bool ok = true;
     if (lane < n_ps) ok = (myval > -CUDART_INF_F) && (myval < CUDART_INF_F);

@@ -332,6 +332,8 @@ cudaError_t launch_walkers(int residual_type, int mode, bool stats, const WalkLa
     if ((!(L.exact_only & 1) || (L.exact_only & 32)) &&
         coop_path_available(residual_type, mode, L.n_p, max_rows_bytes / (row_doubles(residual_type) * 8)))
         return launch_walkers_coop(residual_type, L, n_instances, max_rows_bytes, stream);
+    if (!(L.exact_only & 1) && mode == CLOSURE_MODE_TRANS && L.n_p <= 256)
+        return launch_walkers_coop_trans(residual_type, L, n_instances, max_rows_bytes, stream);
     switch (residual_type) {
     case CLOSURE_REG_3D3D: return launch_r<CLOSURE_REG_3D3D>(mode, stats, L, grid, smem, stream);
     case CLOSURE_REPROJ_2D3D: return launch_r<CLOSURE_REPROJ_2D3D>(mode, stats, L, grid, smem, stream);

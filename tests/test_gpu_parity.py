@@ -203,3 +203,26 @@ def test_fp32_mode_is_refused_where_it_does_not_exist():
     with pytest.raises(B.ClosureError) as e:
         B.Closure.closure_create(inst, _small(inst.params, precision=32, mode=I.MODE_TRANS, v0=0.05, theta_p=0.02))
     assert e.value.status == B.EUNSUPPORTED
+
+
+@pytest.mark.parametrize("kind", ["reproj", "reg", "posereg", "split"])
+def test_cooperative_translation_sampler_is_bit_identical_to_plain_kernel(kind):
+    """Alg. A8 on the warp-cooperative fp64 kernel against the one-walker-per-thread kernel
+    (CLOSURE_FLAG_EXACT_ONLY): same fp64 functions, so samples, flags and traces must be identical."""
+    if kind == "reproj":
+        inst = I.make_instance(3)
+        P = _small(inst.params, mode=I.MODE_TRANS, v0=0.05, theta_p=0.02)
+    elif kind == "reg":
+        inst = I.make_instance(2)
+        P = _small(inst.params, mode=I.MODE_TRANS, v0=0.1, theta_p=0.02, n_p=70, n_p_star=7)
+    else:
+        inst = I.make_instance(4)
+        if kind == "split":
+            inst = I.to_split(inst)
+        P = _small(inst.params, mode=I.MODE_TRANS, v0=0.02, theta_p=0.02, n_p=33, n_p_star=20, n_t=12)
+    S0 = I.make_init_poses(inst, 64)
+    a = gpu_walk(inst, P, S0, 1500, 60, 17)
+    b = gpu_walk(inst, _small(P, flags=1), S0, 1500, 60, 17)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+    assert (a[2] & 0xff).max() >= 1          # some moves were accepted
