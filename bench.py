@@ -128,6 +128,8 @@ def run_reference(args) -> None:
     import oracle
     oracle.build()
     inst, S0 = _workload(args.config)
+    if args.mode == "trans":
+        inst.params.mode = I.MODE_TRANS
     threads = os.cpu_count() or 1
     P = inst.params
     walkers = _sample_size(inst, S0, threads, 60.0 / max(1, args.steps))
@@ -179,6 +181,11 @@ def run_cuda(args) -> None:
     if args.precision == 32:
         for it in insts:
             it.params.precision = 32
+    if args.mode == "trans":
+        if not (P.v0 > 0.0 and P.theta_p > 0.0):
+            raise SystemExit("--mode trans needs v0 > 0 and theta_p > 0 (BASELINE config 3)")
+        for it in insts:
+            it.params.mode = I.MODE_TRANS
     for it, s0 in zip(insts, S0s):
         h = B.Closure.closure_create(it)
         h.closure_set_init(s0)
@@ -251,8 +258,14 @@ def run_cuda(args) -> None:
         # the kernel decides in fp32 with certified error bounds and falls back to fp64:
         # executed arithmetic per pipe, and the time the two CUDA-core pipes need for it at their measured peaks
         fpa, fpl = (FLOP_PAIR_REPROJ_A, FLOP_PAIR_REPROJ_L) if inst.residual_type == 1 else (FLOP_PAIR, FLOP_PAIR)
-        flops64 = fpa * st["perturb_pairs"] + fpl * st["ladder_pairs"] + FLOP_SETUP_A * st["perturb_setups"] \
-            + FLOP_SETUP_L * st["ladder_setups"]
+        fsa, fsl = FLOP_SETUP_A, FLOP_SETUP_L
+        if args.mode == "trans":
+            # Alg. A8: every perturbation has its own rotation, a pair is one direct residual evaluation
+            # (REG 26, REPROJ 31 + reciprocal, POSE_REG 36 flop); no shared set-up
+            fpa = fpl = {1: 31.0, 2: 26.0}.get(inst.residual_type, 36.0)
+            fsa = fsl = 0.0
+        flops64 = fpa * st["perturb_pairs"] + fpl * st["ladder_pairs"] + fsa * st["perturb_setups"] \
+            + fsl * st["ladder_setups"]
         flops32 = fpa * st["perturb_pairs_f32"] + fpl * st["ladder_pairs_f32"]
         flops = flops64 + flops32
         walk_s = statistics.mean(walk_ms) * 1e-3
@@ -365,7 +378,8 @@ def run_cuda(args) -> None:
                            "host_megb": 1e3 * statistics.mean(megb_s), "e2e_per_instance": 1e3 * e2e_dt / (e2e_steps * nb),
                            "e2e_200_walkers_x_5_iterations": small_ms},
             "boundary_fraction": n_cnt / float(nb * W),
-            "roofline": {"bound": "alu", "kernel": "walker_coop_kernel" if st["perturb_pairs_f32"] else "walker_kernel",
+            "roofline": {"bound": "alu", "kernel": "walker_coop_trans_kernel" if args.mode == "trans" else
+                         ("walker_coop_reproj_kernel" if inst.residual_type == 1 else "walker_coop_kernel"),
                          "achieved": achieved, "peak": peak_mix, "unit": "TFLOP/s", "frac": achieved / peak_mix,
                          "traffic": None,
                          "peak_source": "executed flops / (fp64 flops / DFMA peak + fp32 flops / FFMA peak), both peaks "
@@ -410,6 +424,9 @@ def main() -> None:
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config 1..5 (default 2 = configs[1])")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mode", default="rot", choices=["rot", "trans"],
+                    help="rot: Alg. 2, the rotation-boundary sampler (default); trans: Alg. A8, the translation-boundary "
+                         "sampler (config 3 carries the paper's v0 and theta_p; other configs have v0 = 0)")
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32],
                     help="64: every decision is the fp64 decision (default, the parity path); 32: fp32 mode, with its "
                          "measured difference from the fp64 path in the output")
