@@ -400,41 +400,40 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
         int m0 = 0;
         unsigned win = 0u;
         bool lip_stop = false;
-        const bool k_act = lane < KP;
-        const float4 kc4 = k_act ? cand4[lane] : make_float4(0.f, 0.f, 0.f, 0.f);
-        const float kcd = k_act ? candd[lane] : -CUDART_INF_F;
-        const float kcd_max = fkey_inv(__reduce_max_sync(FULL, fkey(kcd)));
-        for (int mb = 0; mb < n_t && m0 == 0 && !lip_stop; mb += 32) {
-            // ---- screening, lane = candidate (see walker_coop_kernel.cu)
-            int mend = min(n_t, mb + 32);
-            {
-                const bool dead_m = (mb + lane < mend) && (kcd_max + qL[min(mb + lane, n_t - 1)] < 0.f);
-                const unsigned lb = __ballot_sync(FULL, dead_m);
-                if (lb != 0u) { lip_stop = true; mend = mb + __ffs(lb) - 1; }
+        const int khalf = (KP + 1) >> 1;
+        for (int mb = 0; mb < n_t && m0 == 0 && !lip_stop; mb += 16) {
+            // ---- screening of 16 rungs, lane = (rung, half of the candidates) (see walker_coop_kernel.cu)
+            const int mq = mb + (lane & 15), hq = lane >> 4;
+            const bool q_act = mq < n_t;
+            unsigned alive = 0u;
+            if (q_act) {
+                const float4 r0a = qrow[4 * mq], r0b = qrow[4 * mq + 1], r1a = qrow[4 * mq + 2], r1b = qrow[4 * mq + 3];
+                const float Lm = qL[mq];
+                const int k1 = min(KP, (hq + 1) * khalf);
+                for (int k = hq * khalf; k < k1; ++k) {
+                    const float4 c4 = cand4[k];
+                    const float v0 = cone_lo(r0a, r0b, c4, nfx, nfy);
+                    const float v1 = cone_lo(r1a, r1b, c4, nfx, nfy);
+                    if (!(v0 > 0.f) && !(v1 > 0.f) && !(candd[k] + Lm < 0.f)) alive |= 1u << k;
+                }
             }
-            unsigned alive_r = 0u;
-#pragma unroll 2
-            for (int m = mb; m < mend; ++m) {
-                const float v0 = cone_lo(qrow[4 * m], qrow[4 * m + 1], kc4, nfx, nfy);
-                const float v1 = cone_lo(qrow[4 * m + 2], qrow[4 * m + 3], kc4, nfx, nfy);
-                if (!(v0 > 0.f) && !(v1 > 0.f) && !(kcd + qL[m] < 0.f)) alive_r |= 1u << (m - mb);
+            alive |= __shfl_xor_sync(FULL, alive, 16);
+            if (L.exact_only & 2) alive = q_act ? ((KP >= 32) ? FULL : ((1u << KP) - 1u)) : 0u;   // debug: nothing is screened out
+            if (mb + 16 < n_t && !(L.exact_only & 2)) {
+                // no candidate can be repaired at the last rung of this block => none at any later rung
+                float cdm = candd[0];
+                for (int k = 1; k < KP; ++k) cdm = fmaxf(cdm, candd[k]);
+                if (cdm + qL[mb + 15] < 0.f) lip_stop = true;
             }
-            if (!k_act) alive_r = 0u;
-            const int mscr = mend;
-            if (L.exact_only & 2) {                          // debug: the screening kills nothing
-                lip_stop = false;
-                mend = min(n_t, mb + 32);
-                alive_r = k_act ? ((mend - mb >= 32) ? FULL : ((1u << (mend - mb)) - 1u)) : 0u;
-            }
-            unsigned qmask = __reduce_or_sync(FULL, alive_r);
-            if (stats) stc[7] += (unsigned long long)(mscr - mb) * 2 * KP;
+            unsigned qmask = __ballot_sync(FULL, lane < 16 && alive != 0u);
+            if (stats) stc[7] += (unsigned long long)(min(n_t, mb + 16) - mb) * 2 * KP;
 
             // ---- full evaluation of the surviving rungs, in order
             while (qmask != 0u && m0 == 0) {
                 const int l0 = __ffs(qmask) - 1;
                 qmask &= qmask - 1u;
                 const int m1 = mb + l0;
-                const unsigned cand_alive = __ballot_sync(FULL, (alive_r >> l0) & 1u);
+                const unsigned cand_alive = __shfl_sync(FULL, alive, l0);
                 double Rm[9], t[3], K[4];
 #pragma unroll
                 for (int e = 0; e < 9; ++e) Rm[e] = RmS[m1 * 9 + e];
