@@ -102,3 +102,31 @@ def test_c5_batch_of_64_instances_full_size():
     finally:
         for h in hs:
             h.closure_destroy()
+
+
+@pytest.mark.parametrize("config,walkers,steps", [(1, 65536, 200), (2, 65536, 400), (3, 65536, 400), (4, 65536, 400),
+                                                  (5, 65536, 400)])
+def test_certified_kernels_equal_plain_fp64_kernel_at_scale(config, walkers, steps):
+    """The certificates of the cooperative kernels under load: ~2.6e7 walker-iterations per config, every sample
+    and flag bit-identical to the one-walker-per-thread fp64 kernel (CLOSURE_FLAG_EXACT_ONLY).  One wrong
+    certificate anywhere (a ranking accepted although fp64 ranks differently, a candidate classified against
+    fp64) sends that walker down another path and shows up here."""
+    import copy
+    import torch
+    inst = I.make_instance(config)
+    S0 = I.make_init_poses(inst, 128)
+    out = []
+    for flags in (0, 1):
+        P = copy.copy(inst.params)
+        P.flags = flags
+        h = B.Closure.closure_create(inst, P)
+        try:
+            h.closure_set_init(S0)
+            smp, flag = h.closure_sample(walkers, steps, 2024 + config)
+            torch.cuda.synchronize()
+            out.append((smp.cpu().numpy(), flag.cpu().numpy()))
+        finally:
+            h.closure_destroy()
+    assert np.array_equal(out[0][1], out[1][1])
+    diff = np.nonzero((out[0][0] != out[1][0]).any(axis=1))[0]
+    assert diff.size == 0, f"{diff.size} walkers differ from the fp64 kernel, first {diff[:5]}"
