@@ -77,6 +77,7 @@ typedef struct {
                         ranking is redone in fp64, 16 = ... on all N_P perturbations. */
 } closure_params;
 #define CLOSURE_FLAG_EXACT_ONLY 1
+#define CLOSURE_FLAG_HOST_MEGB 8    /* closure_megb: copy the cloud to the host and run the miniball there, whatever its size */
 
 typedef struct closure_s closure_t;   /* opaque; owns device copies of the instance and of S_0 */
 
@@ -145,14 +146,17 @@ typedef struct {
     long long rot_support[5]; /* indices (into the given samples) of the rotation ball's support set */
     long long trans_support[4];
     int n_rot_support, n_trans_support;
-    double host_seconds;      /* wall time of the host miniball part (reported separately) */
+    double host_seconds;      /* wall time of Step III inside closure_megb, device passes and copies included
+                                 (reported separately) */
     double reserved;
 } closure_megb_result;
 
 /* Step III (Alg. 1 l.6-7): minimum enclosing ball of {t} in R^3 and of the
  * sign-aligned unit quaternions {q(R)} in R^4 (R-15, R-16) by Gaertner's miniball.
  *   samples  DEVICE, count x 12 (e.g. closure_compact's output)
- * Synchronises `cuda_stream`, copies the samples to the host and solves there.
+ * Synchronises `cuda_stream`.  The support basis is solved on the host; for count >= 4096 the cloud stays on
+ * the device (one embedding pass, one max-reduction launch per miniball pivot, 16 bytes back per pivot),
+ * smaller clouds -- or every cloud with CLOSURE_FLAG_HOST_MEGB -- are copied to the host.  Same result either way.
  * Errors: CLOSURE_EINVAL (count <= 0), CLOSURE_ENOINIT (R_bar needed for the sign), CLOSURE_ECUDA. */
 int closure_megb(closure_t *h, const double *samples, long long count, closure_megb_result *out,
                  void *cuda_stream);

@@ -7,6 +7,7 @@
 #include <chrono>
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <numeric>
 #include <string>
@@ -42,6 +43,11 @@ struct closure_s {
 };
 
 namespace {
+
+constexpr long long kDeviceMegbMin = 4096;
+constexpr int kMaxDevices = 64;
+std::mutex g_megb_mutex;
+DeviceMegb *g_megb[kMaxDevices] = { nullptr };   // device-side Step III state, one per device, kept for the process   // below this the D2H of the cloud is cheaper than the pivot launches
 
 int fail(closure_t *h, int code, const std::string &msg)
 {
@@ -126,11 +132,48 @@ bool host_in_purse(const closure_t *h, const double *pose)
     return true;
 }
 
+// closure_run's device buffers.  A destroyed handle parks them in a one-slot cache per device instead of
+// freeing them (cudaFree of tens of MB costs up to ~100 ms now and then), so a create / run / destroy loop
+// allocates once.
+struct RunBuffers {
+    double *samples = nullptr, *compact = nullptr;
+    unsigned char *flags = nullptr;
+    long long *count = nullptr;
+    long long capacity = 0;
+};
+RunBuffers g_run_cache[kMaxDevices];
+
+void cuda_free_run(RunBuffers &b)
+{
+    cudaFree(b.samples); cudaFree(b.compact); cudaFree(b.flags); cudaFree(b.count);
+    b = RunBuffers();
+}
+
 void free_run_buffers(closure_t *h)
 {
-    cudaFree(h->d_samples); cudaFree(h->d_compact); cudaFree(h->d_flags); cudaFree(h->d_count);
+    RunBuffers mine;
+    mine.samples = h->d_samples; mine.compact = h->d_compact; mine.flags = h->d_flags; mine.count = h->d_count;
+    mine.capacity = h->run_capacity;
     h->d_samples = h->d_compact = nullptr; h->d_flags = nullptr; h->d_count = nullptr;
     h->run_capacity = 0;
+    if (mine.capacity == 0) return;
+    int dev = -1;
+    std::lock_guard<std::mutex> lock(g_megb_mutex);
+    if (cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < kMaxDevices && g_run_cache[dev].capacity < mine.capacity)
+        std::swap(g_run_cache[dev], mine);
+    if (mine.capacity) cuda_free_run(mine);
+}
+
+bool take_cached_run_buffers(closure_t *h, long long need)
+{
+    int dev = -1;
+    std::lock_guard<std::mutex> lock(g_megb_mutex);
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices || g_run_cache[dev].capacity < need) return false;
+    RunBuffers &c = g_run_cache[dev];
+    h->d_samples = c.samples; h->d_compact = c.compact; h->d_flags = c.flags; h->d_count = c.count;
+    h->run_capacity = c.capacity;
+    c = RunBuffers();
+    return true;
 }
 
 int ensure_scratch(closure_t *h, long long n)
@@ -425,32 +468,48 @@ int closure_megb(closure_t *h, const double *samples, long long count, closure_m
     if (!out || !samples || count <= 0) return fail(h, CLOSURE_EINVAL, "closure_megb needs count > 0 samples");
     if (!h->has_init) return fail(h, CLOSURE_ENOINIT, "R_bar (closure_set_init) is needed to align quaternion signs");
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-    std::vector<double> host;
-    try {
-        host.resize((size_t)count * 12);
-    } catch (const std::bad_alloc &) {
-        return fail(h, CLOSURE_ENOMEM, "host buffer for samples");
-    }
-    cudaError_t e = cudaMemcpyAsync(host.data(), samples, host.size() * sizeof(double), cudaMemcpyDeviceToHost, stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
-    if (e != cudaSuccess) return cuda_fail(h, e, "copy of samples to the host");
-
-    const auto t0 = std::chrono::steady_clock::now();
-    std::vector<double> tp((size_t)count * 3), qp((size_t)count * 4);
     double qbar[4];
     rotation_to_quat(h->h_desc.Rbar, qbar);
-    for (long long i = 0; i < count; ++i) {
-        const double *s = host.data() + (size_t)i * 12;
-        std::memcpy(tp.data() + (size_t)i * 3, s + 9, 3 * sizeof(double));
-        double q[4];
-        rotation_to_quat(s, q);
-        const double dot = q[0] * qbar[0] + q[1] * qbar[1] + q[2] * qbar[2] + q[3] * qbar[3];
-        const double sg = dot < 0.0 ? -1.0 : 1.0;                   // R-15
-        for (int k = 0; k < 4; ++k) qp[(size_t)i * 4 + k] = sg * q[k];
-    }
     Ball bt, bq;
-    if (!miniball(tp.data(), count, 3, &bt) || !miniball(qp.data(), count, 4, &bq))
-        return fail(h, CLOSURE_EINVAL, "miniball failed");
+    const auto t0 = std::chrono::steady_clock::now();
+    if (count >= kDeviceMegbMin && !(h->P.flags & CLOSURE_FLAG_HOST_MEGB)) {
+        // the cloud stays on the device: one embedding pass, then one max-reduction per miniball pivot
+        // (its buffers are shared by all handles of the process on this device and grow on demand)
+        std::lock_guard<std::mutex> lock(g_megb_mutex);
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e == cudaSuccess && (dev < 0 || dev >= kMaxDevices)) e = cudaErrorInvalidDevice;
+        if (e == cudaSuccess && !g_megb[dev]) g_megb[dev] = device_megb_create(&e);
+        if (e == cudaSuccess) e = device_megb_prepare(g_megb[dev], samples, count, qbar, stream);
+        if (e != cudaSuccess) return cuda_fail(h, e, "device MEGB set-up");
+        DeviceMegb *dm = g_megb[dev];
+        const bool ok = miniball_source(device_megb_trans(dm), count, 3, &bt) &&
+                        miniball_source(device_megb_quats(dm), count, 4, &bq);
+        if (device_megb_status(dm) != cudaSuccess) return cuda_fail(h, device_megb_status(dm), "device MEGB pivot");
+        if (!ok) return fail(h, CLOSURE_EINVAL, "miniball failed");
+    } else {
+        std::vector<double> host;
+        try {
+            host.resize((size_t)count * 12);
+        } catch (const std::bad_alloc &) {
+            return fail(h, CLOSURE_ENOMEM, "host buffer for samples");
+        }
+        cudaError_t e = cudaMemcpyAsync(host.data(), samples, host.size() * sizeof(double), cudaMemcpyDeviceToHost, stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+        if (e != cudaSuccess) return cuda_fail(h, e, "copy of samples to the host");
+        std::vector<double> tp((size_t)count * 3), qp((size_t)count * 4);
+        for (long long i = 0; i < count; ++i) {
+            const double *s = host.data() + (size_t)i * 12;
+            std::memcpy(tp.data() + (size_t)i * 3, s + 9, 3 * sizeof(double));
+            double q[4];
+            rotation_to_quat(s, q);
+            const double dot = q[0] * qbar[0] + q[1] * qbar[1] + q[2] * qbar[2] + q[3] * qbar[3];
+            const double sg = dot < 0.0 ? -1.0 : 1.0;                   // R-15
+            for (int k = 0; k < 4; ++k) qp[(size_t)i * 4 + k] = sg * q[k];
+        }
+        if (!miniball(tp.data(), count, 3, &bt) || !miniball(qp.data(), count, 4, &bq))
+            return fail(h, CLOSURE_EINVAL, "miniball failed");
+    }
     std::memset(out, 0, sizeof(*out));
     const double hn = std::sqrt(bq.center[0] * bq.center[0] + bq.center[1] * bq.center[1] +
                                 bq.center[2] * bq.center[2] + bq.center[3] * bq.center[3]);
@@ -478,12 +537,21 @@ int closure_run(closure_t *h, long long num_walkers, int num_steps, unsigned lon
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     if (num_walkers > h->run_capacity) {
         free_run_buffers(h);
-        cudaError_t e = cudaMalloc(&h->d_samples, (size_t)num_walkers * 96);
-        if (e == cudaSuccess) e = cudaMalloc(&h->d_compact, (size_t)num_walkers * 96);
-        if (e == cudaSuccess) e = cudaMalloc(&h->d_flags, (size_t)num_walkers);
-        if (e == cudaSuccess) e = cudaMalloc(&h->d_count, sizeof(long long));
-        if (e != cudaSuccess) { free_run_buffers(h); return cuda_fail(h, e, "cudaMalloc(run buffers)"); }
-        h->run_capacity = num_walkers;
+        if (!take_cached_run_buffers(h, num_walkers)) {
+            cudaError_t e = cudaMalloc(&h->d_samples, (size_t)num_walkers * 96);
+            if (e == cudaSuccess) e = cudaMalloc(&h->d_compact, (size_t)num_walkers * 96);
+            if (e == cudaSuccess) e = cudaMalloc(&h->d_flags, (size_t)num_walkers);
+            if (e == cudaSuccess) e = cudaMalloc(&h->d_count, sizeof(long long));
+            h->run_capacity = num_walkers;
+            if (e != cudaSuccess) {
+                RunBuffers b;
+                b.samples = h->d_samples; b.compact = h->d_compact; b.flags = h->d_flags; b.count = h->d_count;
+                cuda_free_run(b);
+                h->d_samples = h->d_compact = nullptr; h->d_flags = nullptr; h->d_count = nullptr;
+                h->run_capacity = 0;
+                return cuda_fail(h, e, "cudaMalloc(run buffers)");
+            }
+        }
     }
     int rc = closure_sample(h, num_walkers, num_steps, seed, h->d_samples, h->d_flags, cuda_stream);
     if (rc != CLOSURE_OK) return rc;

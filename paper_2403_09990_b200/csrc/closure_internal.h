@@ -88,6 +88,25 @@ struct Ball {
 };
 // Gaertner-style exact smallest enclosing ball of n points in R^d (d <= 4), points row-major.
 bool miniball(const double *pts, long long n, int d, Ball *out);
+// The same solver over an abstract cloud: the pivot step ("the point farthest from the centre") is the
+// only pass over all points; everything else touches single points by index.
+struct PointSource {
+    virtual ~PointSource() {}
+    virtual bool farthest(const double *center, long long *index, double *sq_dist) = 0;   // lowest index among ties
+    virtual const double *point(long long i) = 0;                                           // valid until the next call
+};
+bool miniball_source(PointSource *src, long long n, int d, Ball *out);
+
+// megb_kernels.cu: Step III with the cloud kept on the device.  Quaternion
+// embedding + sign alignment in one pass, then the miniball pivot as a max-reduction per iteration.
+struct DeviceMegb;
+DeviceMegb *device_megb_create(cudaError_t *err);
+cudaError_t device_megb_prepare(DeviceMegb *m, const double *d_samples, long long count, const double qbar[4],
+                                cudaStream_t stream);
+PointSource *device_megb_quats(DeviceMegb *m);     // cloud of aligned unit quaternions in R^4
+PointSource *device_megb_trans(DeviceMegb *m);     // cloud of translations in R^3
+cudaError_t device_megb_status(DeviceMegb *m);
+void device_megb_destroy(DeviceMegb *m);
 void rotation_to_quat(const double R[9], double q[4]);
 void quat_to_rotation(const double q[4], double R[9]);
 bool project_so3(const double M[9], double R[9]);   // nearest rotation to M (polar factor)

@@ -82,8 +82,34 @@ private:
     long long idx_[kD + 1];
 };
 
+// Host cloud: the points as they are; the pivot is a plain scan.
+class HostCloud : public PointSource {
+public:
+    HostCloud(const double *p, long long n, int d) : pts_(p), n_(n), d_(d) {}
+    bool farthest(const double *center, long long *index, double *sq_dist) override
+    {
+        long long far = -1;
+        double far_d2 = -1.0;
+        for (long long i = 0; i < n_; ++i) {
+            const double *p = pts_ + (size_t)i * d_;
+            double s = 0.0;
+            for (int a = 0; a < d_; ++a) s += (p[a] - center[a]) * (p[a] - center[a]);
+            if (s > far_d2) { far_d2 = s; far = i; }
+        }
+        *index = far;
+        *sq_dist = far_d2;
+        return true;
+    }
+    const double *point(long long i) override { return pts_ + (size_t)i * d_; }
+
+private:
+    const double *pts_;
+    long long n_;
+    int d_;
+};
+
 struct Solver {
-    const double *pts;
+    PointSource *src;
     int d;
     Basis basis;
     std::list<long long> cand;          // support candidates, most recently violating first
@@ -92,7 +118,7 @@ struct Solver {
     long long support[kD + 1];
     int n_support;
 
-    Solver(const double *p, int dim) : pts(p), d(dim), basis(dim), r2(-1.0), n_support(0) {}
+    Solver(PointSource *p, int dim) : src(p), d(dim), basis(dim), r2(-1.0), n_support(0) {}
 
     void snapshot()
     {
@@ -104,7 +130,7 @@ struct Solver {
 
     double excess(long long i) const
     {
-        const double *p = pts + (size_t)i * d;
+        const double *p = src->point(i);
         double s = 0.0;
         for (int a = 0; a < d; ++a) s += (p[a] - center[a]) * (p[a] - center[a]);
         return s - r2;
@@ -119,7 +145,7 @@ struct Solver {
         for (auto it = cand.begin(); it != end;) {
             auto cur = it++;
             if (excess(*cur) > 1e-15 * std::max(r2, 0.0)) {
-                if (basis.push(pts + (size_t)(*cur) * d, *cur)) {
+                if (basis.push(src->point(*cur), *cur)) {
                     move_to_front(cur);
                     basis.pop();
                     cand.splice(cand.begin(), cand, cur);
@@ -131,28 +157,27 @@ struct Solver {
 
 }  // namespace
 
-bool miniball(const double *pts, long long n, int d, Ball *out)
+bool miniball_source(PointSource *src, long long n, int d, Ball *out)
 {
-    if (n <= 0 || d <= 0 || d > kD) return false;
-    Solver S(pts, d);
-    std::memcpy(S.center, pts, sizeof(double) * d);
+    if (n <= 0 || d <= 0 || d > kD || !src) return false;
+    Solver S(src, d);
+    const double *p0 = src->point(0);
+    if (!p0) return false;
+    std::memcpy(S.center, p0, sizeof(double) * d);
     S.r2 = -1.0;                      // no ball yet: the first pivot always makes progress
     S.n_support = 1;
     S.support[0] = 0;
     for (int iter = 0; iter < 10000; ++iter) {
-        // pivot: the point farthest from the current centre
+        // pivot: the point farthest from the current centre (the only pass over the whole cloud)
         long long far = -1;
         double far_d2 = -1.0;
-        for (long long i = 0; i < n; ++i) {
-            const double *p = pts + (size_t)i * d;
-            double s = 0.0;
-            for (int a = 0; a < d; ++a) s += (p[a] - S.center[a]) * (p[a] - S.center[a]);
-            if (s > far_d2) { far_d2 = s; far = i; }
-        }
+        if (!src->farthest(S.center, &far, &far_d2) || far < 0) return false;
         if (far_d2 - S.r2 <= 1e-14 * far_d2) break;           // everything inside: optimal
         const double old_r2 = S.r2;
+        const double *pf = src->point(far);
+        if (!pf) return false;
         S.basis.reset();
-        S.basis.push(pts + (size_t)far * d, far);
+        S.basis.push(pf, far);
         S.move_to_front(S.cand.end());
         S.basis.reset();
         S.cand.remove(far);
@@ -166,6 +191,13 @@ bool miniball(const double *pts, long long n, int d, Ball *out)
     for (int k = 0; k < S.n_support; ++k) out->support[k] = S.support[k];
     std::sort(out->support, out->support + out->n_support);
     return true;
+}
+
+bool miniball(const double *pts, long long n, int d, Ball *out)
+{
+    if (!pts || n <= 0 || d <= 0 || d > kD) return false;
+    HostCloud cloud(pts, n, d);
+    return miniball_source(&cloud, n, d, out);
 }
 
 // Unit quaternion (w, x, y, z) of a rotation matrix: take the largest of the four squared

@@ -187,3 +187,36 @@ def test_alu_peak_is_plausible():
     f64, _ = B.closure_alu_peak(64)
     f32, _ = B.closure_alu_peak(32)
     assert 1e13 < f64 < 6e13 and 3e13 < f32 < 1.6e14
+
+
+@pytest.mark.parametrize("config,walkers", [(1, 6000), (3, 20000), (4, 70000)])
+def test_device_side_megb_equals_host_side_and_oracle(config, walkers):
+    """closure_megb keeps clouds of >= 4096 samples on the device (embedding pass + one max-reduction per
+    miniball pivot); CLOSURE_FLAG_HOST_MEGB = 8 forces the host path.  Same pivots, same support sets, radii
+    equal to the last bit or two; both within 1e-9 of the oracle's Welzl solver."""
+    import copy
+    inst = I.make_instance(config)
+    S0 = I.make_init_poses(inst, 64)
+    res = {}
+    for name, flags in (("device", 0), ("host", 8)):
+        P = copy.copy(inst.params)
+        P.flags = flags
+        h = B.Closure.closure_create(inst, P)
+        try:
+            h.closure_set_init(S0)
+            smp, flag = h.closure_sample(walkers, 40, 5)
+            comp, cnt = h.closure_compact(smp, flag)
+            count = int(cnt.item())
+            assert count >= 4096
+            res[name] = h.closure_megb(comp, count)
+            host = comp.cpu().numpy()[:count]
+        finally:
+            h.closure_destroy()
+    d, hst = res["device"], res["host"]
+    assert set(d["rot_support"]) == set(hst["rot_support"]) and set(d["trans_support"]) == set(hst["trans_support"])
+    assert abs(d["rot_radius"] - hst["rot_radius"]) <= 1e-13 * hst["rot_radius"]
+    assert abs(d["trans_radius"] - hst["trans_radius"]) <= 1e-13 * hst["trans_radius"]
+    ref = oracle.megb(host, oracle.mean_pose(S0)[0])
+    assert abs(d["rot_radius"] - ref["rot_radius"]) <= 1e-9 * ref["rot_radius"]
+    assert abs(d["trans_radius"] - ref["trans_radius"]) <= 1e-9 * ref["trans_radius"]
+    assert np.allclose(d["R"], ref["R"], atol=1e-9) and np.allclose(d["t"], ref["t"], atol=1e-9)
