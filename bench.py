@@ -375,7 +375,7 @@ def run_cuda(args) -> None:
             "constraint_evals_per_sec_executed": (st["perturb_pairs"] + st["ladder_pairs"] + st["perturb_pairs_f32"]
                                                   + st["ladder_pairs_f32"]) / walk_s * world,
             "latency_ms": {"walker_kernel": statistics.mean(walk_ms), "compaction_kernel": statistics.mean(comp_ms),
-                           "host_megb": 1e3 * statistics.mean(megb_s), "e2e_per_instance": 1e3 * e2e_dt / (e2e_steps * nb),
+                           "megb": 1e3 * statistics.mean(megb_s), "e2e_per_instance": 1e3 * e2e_dt / (e2e_steps * nb),
                            "e2e_200_walkers_x_5_iterations": small_ms},
             "boundary_fraction": n_cnt / float(nb * W),
             "roofline": {"bound": "alu", "kernel": "walker_coop_trans_kernel" if args.mode == "trans" else

@@ -329,11 +329,21 @@ cudaError_t launch_walkers(int residual_type, int mode, bool stats, const WalkLa
         if (why) *why = "fp32 mode needs the cooperative kernel";
         return cudaErrorInvalidValue;
     }
+    // the cooperative kernels report cudaErrorInvalidConfiguration when their per-warp shared memory does not
+    // fit (very large N x N_T): the one-walker-per-thread kernel below then takes the launch
     if ((!(L.exact_only & 1) || (L.exact_only & 32)) &&
-        coop_path_available(residual_type, mode, L.n_p, max_rows_bytes / (row_doubles(residual_type) * 8)))
-        return launch_walkers_coop(residual_type, L, n_instances, max_rows_bytes, stream);
-    if (!(L.exact_only & 1) && mode == CLOSURE_MODE_TRANS && L.n_p <= 256)
-        return launch_walkers_coop_trans(residual_type, L, n_instances, max_rows_bytes, stream);
+        coop_path_available(residual_type, mode, L.n_p, max_rows_bytes / (row_doubles(residual_type) * 8))) {
+        const cudaError_t e = launch_walkers_coop(residual_type, L, n_instances, max_rows_bytes, stream);
+        if (e != cudaErrorInvalidConfiguration) return e;
+        if (L.exact_only & 32) {
+            if (why) *why = "instance too large for the fp32-mode kernel";
+            return cudaErrorInvalidValue;
+        }
+    }
+    if (!(L.exact_only & 1) && mode == CLOSURE_MODE_TRANS && L.n_p <= 256) {
+        const cudaError_t e = launch_walkers_coop_trans(residual_type, L, n_instances, max_rows_bytes, stream);
+        if (e != cudaErrorInvalidConfiguration) return e;
+    }
     switch (residual_type) {
     case CLOSURE_REG_3D3D: return launch_r<CLOSURE_REG_3D3D>(mode, stats, L, grid, smem, stream);
     case CLOSURE_REPROJ_2D3D: return launch_r<CLOSURE_REPROJ_2D3D>(mode, stats, L, grid, smem, stream);

@@ -72,9 +72,10 @@ def test_parameter_edges(n_p, n_p_star, n_t):
     assert_parity(inst, P, I.make_init_poses(inst, 16), 130, 25, 5)
 
 
-@pytest.mark.parametrize("n,distinct", [(1, False), (2, True), (7, True), (33, True), (200, False)])
+@pytest.mark.parametrize("n,distinct", [(1, False), (2, True), (7, True), (33, True), (200, False), (1500, False)])
 def test_constraint_count_edges(n, distinct):
-    """N = 1, odd N, every beta different (one sqrt per constraint), the maximum config size."""
+    """N = 1, odd N, every beta different (one sqrt per constraint), the maximum config size, and an N whose
+    per-warp tables do not fit the cooperative kernel (the one-walker-per-thread kernel takes over)."""
     inst = I.make_custom_reg(n, 100 + n, distinct_betas=distinct)
     P = _small(inst.params, n_p=30, n_p_star=4, n_t=8, t_p=0.05)
     assert_parity(inst, P, I.make_init_poses(inst, 8), 96, 20, 9)
