@@ -104,6 +104,26 @@ int closure_set_params(closure_t *h, const closure_params *p);
  * mean_out (host, 12 doubles, may be NULL) receives [R_bar, t_bar]. */
 int closure_set_init(closure_t *h, const double *poses, int n0, double *mean_out);
 
+/* Step I for Ex.2 and Ex.3: independent trials on the device.
+ *   CLOSURE_REG_3D3D               RANSAG trial: 3 distinct random correspondences, Arun's least-squares rigid
+ *                                  fit, kept iff the pose satisfies the PURSE
+ *   CLOSURE_POSE_REG / _SPLIT      a random convex combination of the hypotheses (rotation = proj_SO(3) of the
+ *                                  weighted sum), kept iff it satisfies the PURSE
+ *   CLOSURE_REPROJ_2D3D            CLOSURE_EUNSUPPORTED (needs a P3P solver)
+ * Trial k = trial_begin + q draws from Philox4x32-10 keyed by (seed; k) (R-21, R-22), so any trial can
+ * be replayed alone.  ASYNC.
+ *   out_poses  DEVICE, num_trials x 12 doubles: the candidate (R row-major, t), zeros where rejected
+ *   out_ok     DEVICE, num_trials bytes: 1 iff the candidate is inside the PURSE
+ * closure_compact(out_poses, out_ok) yields S_0 in trial order. */
+int closure_init_sample(closure_t *h, long long trial_begin, long long num_trials, unsigned long long seed,
+                        double *out_poses, unsigned char *out_ok, void *cuda_stream);
+
+/* Step I end to end: num_trials trials (closure_init_sample from trial 0), compaction, and closure_set_init with
+ * the first max_poses accepted poses.  Synchronises the stream.  *n0_out (may be NULL) = |S_0|.
+ * CLOSURE_EINIT if no trial produced a pose inside the PURSE. */
+int closure_init_from_trials(closure_t *h, long long num_trials, unsigned long long seed, int max_poses, int *n0_out,
+                             void *cuda_stream);
+
 /* Step II.  ASYNC.  Runs walkers w = walker_begin .. walker_begin + num_walkers - 1, each for
  * exactly num_steps iterations of Alg. 2 (ROT) / Alg. A8 (TRANS) from S_0[w mod n0]
  * (the paper's repeat(S_0, N_W)), with Philox4x32-10 randomness keyed by

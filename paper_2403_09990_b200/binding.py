@@ -21,7 +21,7 @@ OK, EINVAL, EINIT, ENOINIT, ECUDA, ENOMEM, EUNSUPPORTED = 0, -1, -2, -3, -4, -5,
 EXPORTS = [
     "closure_default_params", "closure_create", "closure_set_params", "closure_set_init",
     "closure_sample_range", "closure_sample", "closure_sample_batch", "closure_compact", "closure_megb",
-    "closure_run", "closure_enable_stats", "closure_get_stats", "closure_alu_peak", "closure_miniball_host",
+    "closure_init_sample", "closure_init_from_trials", "closure_run", "closure_enable_stats", "closure_get_stats", "closure_alu_peak", "closure_miniball_host",
     "closure_last_error", "closure_strerror", "closure_abi_version", "closure_destroy",
 ]
 
@@ -83,6 +83,8 @@ def load_library():
     L.closure_enable_stats.argtypes = [c_void_p, c_int]
     L.closure_get_stats.argtypes = [c_void_p, POINTER(Stats)]
     L.closure_alu_peak.argtypes = [c_int, POINTER(c_double), POINTER(c_double), c_void_p]
+    L.closure_init_sample.argtypes = [c_void_p, c_longlong, c_longlong, c_ulonglong, c_void_p, c_void_p, c_void_p]
+    L.closure_init_from_trials.argtypes = [c_void_p, c_longlong, c_ulonglong, c_int, POINTER(c_int), c_void_p]
     L.closure_miniball_host.argtypes = [POINTER(c_double), c_longlong, c_int, POINTER(c_double),
                                         POINTER(c_double), POINTER(c_longlong), POINTER(c_int)]
     L.closure_last_error.argtypes = [c_void_p]
@@ -202,6 +204,27 @@ class Closure:
         self._check(load_library().closure_set_init(self._h, _dp(S0), S0.shape[0], _dp(mean)))
         self.mean_pose = (mean[:9].reshape(3, 3).copy(), mean[9:].copy())
         return mean
+
+    def closure_init_sample(self, num_trials: int, seed: int, out_poses=None, out_ok=None, stream=None, *,
+                            trial_begin: int = 0):
+        """Step I trials -> (poses (T,12) f64 cuda tensor, ok (T,) u8 cuda tensor)."""
+        import torch
+        dev = torch.device("cuda")
+        if out_poses is None:
+            out_poses = torch.empty((num_trials, 12), dtype=torch.float64, device=dev)
+        if out_ok is None:
+            out_ok = torch.empty((num_trials,), dtype=torch.uint8, device=dev)
+        self._check(load_library().closure_init_sample(
+            self._h, trial_begin, num_trials, seed, c_void_p(out_poses.data_ptr()), c_void_p(out_ok.data_ptr()),
+            _stream_ptr(stream)))
+        return out_poses, out_ok
+
+    def closure_init_from_trials(self, num_trials: int, seed: int, max_poses: int = 128, stream=None) -> int:
+        """Step I end to end (trials, compaction, closure_set_init) -> |S_0|."""
+        n0 = c_int(0)
+        self._check(load_library().closure_init_from_trials(self._h, num_trials, seed, max_poses, byref(n0),
+                                                            _stream_ptr(stream)))
+        return int(n0.value)
 
     def closure_sample(self, num_walkers: int, num_steps: int, seed: int, out_samples=None,
                        out_on_boundary=None, stream=None, *, walker_begin: int = 0, trace: bool = False):

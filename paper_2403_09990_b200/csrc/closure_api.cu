@@ -26,6 +26,7 @@ struct closure_s {
     double K[4] = { 0, 0, 0, 0 };
     InstanceDesc h_desc{};
     double *d_rows = nullptr;
+    int *d_perm = nullptr;
     InstanceDesc *d_desc = nullptr;
     double *d_S0 = nullptr;
     bool has_init = false;
@@ -306,20 +307,32 @@ int closure_create(int residual_type, const double *measurements, int n, const d
         }
     }
     const size_t bytes = rows.size() * sizeof(double);     // row is 8 or 16 doubles: multiple of 16 B
+    std::vector<int> perm(n);
+    for (int k = 0; k < n; ++k) perm[order[k]] = k;
     cudaError_t e = cudaMalloc(&h->d_rows, bytes);
     if (e == cudaSuccess) e = cudaMemcpy(h->d_rows, rows.data(), bytes, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&h->d_perm, sizeof(int) * (size_t)n);
+    if (e == cudaSuccess) e = cudaMemcpy(h->d_perm, perm.data(), sizeof(int) * (size_t)n, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc(&h->d_desc, sizeof(InstanceDesc));
     if (e == cudaSuccess) e = cudaMalloc(&h->d_stats, kNumStats * sizeof(unsigned long long));
     if (e != cudaSuccess) {
         // no handle is returned: the failure text can only be seen through the status code
-        cudaFree(h->d_rows); cudaFree(h->d_desc); cudaFree(h->d_stats);
+        cudaFree(h->d_rows); cudaFree(h->d_perm); cudaFree(h->d_desc); cudaFree(h->d_stats);
         delete h;
         return CLOSURE_ECUDA;
     }
     h->h_desc.rows = h->d_rows;
+    h->h_desc.perm = h->d_perm;
     h->h_desc.n = n;
     h->h_desc.rows_bytes = (int)bytes;
     std::memcpy(h->h_desc.K, h->K, sizeof(h->K));
+    // the descriptor is complete for Step I now; closure_set_init adds S_0, R_bar, t_bar
+    e = cudaMemcpy(h->d_desc, &h->h_desc, sizeof(InstanceDesc), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        cudaFree(h->d_rows); cudaFree(h->d_perm); cudaFree(h->d_desc); cudaFree(h->d_stats);
+        delete h;
+        return CLOSURE_ECUDA;
+    }
     *out = h;
     return CLOSURE_OK;
 }
@@ -359,6 +372,58 @@ int closure_set_init(closure_t *h, const double *poses, int n0, double *mean_out
         std::memcpy(mean_out + 9, tb, sizeof(tb));
     }
     return CLOSURE_OK;
+}
+
+int closure_init_sample(closure_t *h, long long trial_begin, long long num_trials, unsigned long long seed,
+                        double *out_poses, unsigned char *out_ok, void *cuda_stream)
+{
+    if (!h) return CLOSURE_EINVAL;
+    if (trial_begin < 0 || num_trials < 0) return fail(h, CLOSURE_EINVAL, "negative size");
+    if (h->type == CLOSURE_REPROJ_2D3D)
+        return fail(h, CLOSURE_EUNSUPPORTED, "Step I for the reprojection residual needs a P3P solver (not built)");
+    if (h->type == CLOSURE_REG_3D3D && h->n < 3) return fail(h, CLOSURE_EINVAL, "RANSAG needs at least 3 correspondences");
+    if (num_trials == 0) return CLOSURE_OK;
+    if (!out_poses || !out_ok) return fail(h, CLOSURE_EINVAL, "output buffer is NULL");
+    if (reinterpret_cast<uintptr_t>(out_poses) & 15u) return fail(h, CLOSURE_EINVAL, "pose buffer must be 16-byte aligned");
+    cudaError_t e = launch_step1(h->type, h->d_desc, h->h_desc.rows_bytes, trial_begin, num_trials, seed, out_poses,
+                                 out_ok, static_cast<cudaStream_t>(cuda_stream));
+    if (e != cudaSuccess) return cuda_fail(h, e, "Step I kernel launch");
+    return CLOSURE_OK;
+}
+
+int closure_init_from_trials(closure_t *h, long long num_trials, unsigned long long seed, int max_poses, int *n0_out,
+                             void *cuda_stream)
+{
+    if (!h) return CLOSURE_EINVAL;
+    if (num_trials <= 0 || max_poses <= 0) return fail(h, CLOSURE_EINVAL, "need num_trials > 0 and max_poses > 0");
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    double *d_poses = nullptr, *d_kept = nullptr;
+    unsigned char *d_ok = nullptr;
+    long long *d_cnt = nullptr;
+    cudaError_t e = cudaMalloc(&d_poses, (size_t)num_trials * 96);
+    if (e == cudaSuccess) e = cudaMalloc(&d_kept, (size_t)num_trials * 96);
+    if (e == cudaSuccess) e = cudaMalloc(&d_ok, (size_t)num_trials);
+    if (e == cudaSuccess) e = cudaMalloc(&d_cnt, sizeof(long long));
+    int rc = e == cudaSuccess ? CLOSURE_OK : cuda_fail(h, e, "cudaMalloc(Step I buffers)");
+    if (rc == CLOSURE_OK) rc = closure_init_sample(h, 0, num_trials, seed, d_poses, d_ok, cuda_stream);
+    if (rc == CLOSURE_OK) rc = closure_compact(h, d_poses, d_ok, num_trials, d_kept, d_cnt, cuda_stream);   // trial order kept
+    long long cnt = 0;
+    std::vector<double> host;
+    if (rc == CLOSURE_OK) {
+        e = cudaMemcpyAsync(&cnt, d_cnt, sizeof(cnt), cudaMemcpyDeviceToHost, stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+        if (e == cudaSuccess && cnt > 0) {
+            const long long take = std::min<long long>(cnt, max_poses);
+            host.resize((size_t)take * 12);
+            e = cudaMemcpy(host.data(), d_kept, host.size() * sizeof(double), cudaMemcpyDeviceToHost);
+        }
+        if (e != cudaSuccess) rc = cuda_fail(h, e, "Step I trials");
+    }
+    cudaFree(d_poses); cudaFree(d_kept); cudaFree(d_ok); cudaFree(d_cnt);
+    if (rc != CLOSURE_OK) return rc;
+    if (n0_out) *n0_out = (int)(host.size() / 12);
+    if (host.empty()) return fail(h, CLOSURE_EINIT, "no Step I trial produced a pose inside the PURSE");
+    return closure_set_init(h, host.data(), (int)(host.size() / 12), nullptr);
 }
 
 int closure_sample_range(closure_t *h, long long walker_begin, long long num_walkers, int num_steps,
@@ -613,7 +678,8 @@ int closure_miniball_host(const double *points, long long n, int d, double *cent
 void closure_destroy(closure_t *h)
 {
     if (!h) return;
-    cudaFree(h->d_rows); cudaFree(h->d_desc); cudaFree(h->d_S0); cudaFree(h->d_scratch); cudaFree(h->d_stats);
+    cudaFree(h->d_rows); cudaFree(h->d_perm); cudaFree(h->d_desc); cudaFree(h->d_S0); cudaFree(h->d_scratch);
+    cudaFree(h->d_stats);
     free_run_buffers(h);
     delete h;
 }

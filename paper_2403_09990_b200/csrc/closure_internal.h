@@ -27,6 +27,7 @@ struct InstanceDesc {
     const double *S0;       // device, n0 x 12
     int n0;
     int pad_;
+    const int *perm;        // device, n: row of the caller's constraint i in the sorted table (Step I draws by i)
     double Rbar[9];
     double tbar[3];
     double K[4];            // fx fy cx cy
@@ -70,6 +71,11 @@ cudaError_t launch_walkers_coop_reproj(const WalkLaunch &L, int n_instances, int
 // walker_coop_trans_kernel.cu: warp-cooperative fp64 kernel for TRANS mode (Alg. A8), all residuals
 cudaError_t launch_walkers_coop_trans(int residual_type, const WalkLaunch &L, int n_instances, int max_rows_bytes,
                                       cudaStream_t stream);
+
+// step1_kernel.cu: Step I trials (RANSAG with Arun's method for Ex.2, convex combinations for Ex.3)
+cudaError_t launch_step1(int residual_type, const InstanceDesc *d_desc, int rows_bytes, long long trial_begin,
+                         long long num_trials, unsigned long long seed, double *out_poses, unsigned char *out_ok,
+                         cudaStream_t stream);
 
 // compact_kernel.cu
 size_t compact_scratch_bytes(long long n);
