@@ -222,6 +222,7 @@ def run_cuda(args) -> None:
 
     peak64, _ = B.closure_alu_peak(64)
     peak32, _ = B.closure_alu_peak(32)
+    peak_philox, _ = B.closure_alu_peak(4)          # Philox4x32-10 calls per second
     for w in range(args.warmup):
         step(WALK_SEED + 100 + w)
         flush.fill_(w)
@@ -272,6 +273,9 @@ def run_cuda(args) -> None:
         achieved = flops / walk_s / 1e12
         t_min = flops64 / peak64 + flops32 / peak32
         peak_mix = flops / t_min / 1e12
+        # the integer work a flop count does not see: one Philox4x32-10 call per perturbation and iteration
+        philox_calls = float(st["walker_steps"]) * (P.n_p + 1)
+        t_min_rng = t_min + philox_calls / peak_philox
         nominal_pairs = (P.n_p + P.n_p_star * P.n_t) * inst.n
         n_cnt = int(count.item())
         comp_bytes = nb * W * 1 + n_cnt * 96 * 2
@@ -414,6 +418,9 @@ def run_cuda(args) -> None:
                          "fp32": {"flops_per_launch": flops32, "achieved": flops32 / walk_s / 1e12, "peak": peak32 / 1e12},
                          "fp64": {"flops_per_launch": flops64, "achieved": flops64 / walk_s / 1e12, "peak": peak64 / 1e12},
                          "flops_per_launch": flops,
+                         "philox": {"calls_per_launch": philox_calls, "peak_calls_per_s": peak_philox,
+                                    "note": "Philox4x32-10 calls at the rate of a kernel that does nothing else"},
+                         "frac_incl_philox": t_min_rng / walk_s,
                          "executed_pairs_per_walker_step": (st["perturb_pairs"] + st["ladder_pairs"] + st["perturb_pairs_f32"]
                                                             + st["ladder_pairs_f32"]) / st["walker_steps"],
                          "fp64_fallback_steps": st["fallback_steps"] / st["walker_steps"],

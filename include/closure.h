@@ -207,7 +207,8 @@ int closure_get_stats(closure_t *h, closure_stats *out);
 
 /* Measured CUDA-core peak of this device: a register-resident FMA chain, fp64 (precision = 64)
  * or fp32 (32).  Returns FLOP/s (FMA = 2) in *flops_per_s and the kernel time in *seconds.
- * Synchronous.  Used as the roofline denominator for the walker kernel. */
+ * precision = 4 measures the integer side instead: Philox4x32-10 calls per second (in *flops_per_s).
+ * Synchronous.  Used as the roofline denominators for the walker kernel. */
 int closure_alu_peak(int precision, double *flops_per_s, double *seconds, void *cuda_stream);
 
 /* The host solver of Step III on its own: exact smallest enclosing ball of n points in R^d

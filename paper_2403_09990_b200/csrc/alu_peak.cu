@@ -69,12 +69,73 @@ cudaError_t run(double *flops_per_s, double *seconds, cudaStream_t stream)
     return cudaSuccess;
 }
 
+// Philox4x32-10 calls per second: 4 independent counters per thread, nothing else (the integer work of an
+// iteration that a flop count does not see: 150 calls per walker-step at the paper's N_P).
+constexpr int kPhiloxIters = 512;
+
+__global__ void __launch_bounds__(256) philox_rate_kernel(unsigned int *sink, unsigned int k0, unsigned int k1)
+{
+    unsigned int acc = 0;
+    for (int it = 0; it < kPhiloxIters; ++it) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            unsigned int c0 = threadIdx.x + blockIdx.x * 256u, c1 = it, c2 = q, c3 = 1u, a0 = k0, a1 = k1;
+#pragma unroll
+            for (int r = 0; r < 10; ++r) {
+                const unsigned int hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+                const unsigned int hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+                c0 = hi1 ^ c1 ^ a0; c1 = lo1; c2 = hi0 ^ c3 ^ a1; c3 = lo0;
+                a0 += 0x9E3779B9u; a1 += 0xBB67AE85u;
+            }
+            acc ^= c0 ^ c1 ^ c2;
+        }
+    }
+    if (acc == 0x12345678u) sink[0] = acc;       // practically never true; keeps the calls live
+}
+
+cudaError_t run_philox(double *calls_per_s, double *seconds, cudaStream_t stream)
+{
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    unsigned int *sink = nullptr;
+    e = cudaMalloc(&sink, sizeof(unsigned int));
+    if (e != cudaSuccess) return e;
+    cudaEvent_t t0, t1;
+    cudaEventCreate(&t0);
+    cudaEventCreate(&t1);
+    const int blocks = sms * 16;
+    float best_ms = 1e30f;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(t0, stream);
+        philox_rate_kernel<<<blocks, 256, 0, stream>>>(sink, 1u + rep, 2u);
+        cudaEventRecord(t1, stream);
+        e = cudaEventSynchronize(t1);
+        if (e != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, t0, t1);
+        if (rep >= 2 && ms < best_ms) best_ms = ms;
+    }
+    cudaEventDestroy(t0);
+    cudaEventDestroy(t1);
+    cudaFree(sink);
+    if (e != cudaSuccess) return e;
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    *seconds = best_ms * 1e-3;
+    *calls_per_s = (double)blocks * 256.0 * kPhiloxIters * 4.0 / (best_ms * 1e-3);
+    return cudaSuccess;
+}
+
 }  // namespace
 
 cudaError_t measure_alu_peak(int precision, double *flops_per_s, double *seconds, cudaStream_t stream)
 {
     if (precision == 64) return run<double>(flops_per_s, seconds, stream);
     if (precision == 32) return run<float>(flops_per_s, seconds, stream);
+    if (precision == 4) return run_philox(flops_per_s, seconds, stream);
     return cudaErrorInvalidValue;
 }
 

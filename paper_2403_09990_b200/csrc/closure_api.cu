@@ -657,7 +657,7 @@ int closure_get_stats(closure_t *h, closure_stats *out)
 
 int closure_alu_peak(int precision, double *flops_per_s, double *seconds, void *cuda_stream)
 {
-    if (!flops_per_s || !seconds || (precision != 64 && precision != 32)) return CLOSURE_EINVAL;
+    if (!flops_per_s || !seconds || (precision != 64 && precision != 32 && precision != 4)) return CLOSURE_EINVAL;
     cudaError_t e = measure_alu_peak(precision, flops_per_s, seconds, static_cast<cudaStream_t>(cuda_stream));
     return e == cudaSuccess ? CLOSURE_OK : CLOSURE_ECUDA;
 }

@@ -187,6 +187,8 @@ def test_alu_peak_is_plausible():
     f64, _ = B.closure_alu_peak(64)
     f32, _ = B.closure_alu_peak(32)
     assert 1e13 < f64 < 6e13 and 3e13 < f32 < 1.6e14
+    ph, _ = B.closure_alu_peak(4)                     # Philox4x32-10 calls per second
+    assert 1e11 < ph < 5e12
 
 
 @pytest.mark.parametrize("config,walkers", [(1, 6000), (3, 20000), (4, 70000)])
