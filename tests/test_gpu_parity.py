@@ -64,9 +64,11 @@ def test_split_pose_regression_rot_mode():
 
 
 @pytest.mark.parametrize("n_p,n_p_star,n_t", [(1, 1, 1), (7, 1, 3), (37, 3, 5), (150, 10, 15), (23, 15, 4),
-                                              (64, 20, 6), (10, 10, 2)])
+                                              (64, 20, 6), (10, 10, 2), (40, 4, 33), (33, 2, 64), (200, 10, 8),
+                                              (256, 20, 17), (300, 5, 6)])
 def test_parameter_edges(n_p, n_p_star, n_t):
-    """Ragged perturbation tiles, every top-k capacity, degenerate N_P = N_P* = N_T = 1."""
+    """Ragged perturbation tiles, every top-k capacity, degenerate N_P = N_P* = N_T = 1, ladders longer than one
+    screening block (N_T > 16), every NQ of the cooperative kernel, and N_P > 256 (plain kernel)."""
     inst = I.make_instance(1)
     P = _small(inst.params, n_p=n_p, n_p_star=n_p_star, n_t=n_t)
     assert_parity(inst, P, I.make_init_poses(inst, 16), 130, 25, 5)
