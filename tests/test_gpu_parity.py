@@ -229,3 +229,12 @@ def test_cooperative_translation_sampler_is_bit_identical_to_plain_kernel(kind):
     for x, y in zip(a, b):
         assert np.array_equal(x, y)
     assert (a[2] & 0xff).max() >= 1          # some moves were accepted
+
+
+@pytest.mark.parametrize("config", [3, 4])
+@pytest.mark.parametrize("n_p,n_p_star,n_t", [(33, 2, 40), (200, 10, 8), (64, 20, 6), (5, 5, 1)])
+def test_parameter_edges_other_residuals(config, n_p, n_p_star, n_t):
+    """The same edges on the reprojection kernel and on the stacked pose-regression residual."""
+    inst = I.make_instance(config)
+    P = _small(inst.params, n_p=n_p, n_p_star=n_p_star, n_t=n_t)
+    assert_parity(inst, P, I.make_init_poses(inst, 16), 100, 25, 5)
