@@ -39,6 +39,10 @@ WALK_SEED = 42
 FLOP_PAIR, FLOP_SETUP_A, FLOP_SETUP_L = 7.0, 26.0, 27.0
 # reprojection residual: eq. (14) pair = 4 FMA + RCP + 3 MUL + max = 13; cone pair = 8 FMA + max = 17
 FLOP_PAIR_REPROJ_A, FLOP_PAIR_REPROJ_L = 13.0, 17.0
+# DRAM traffic of the walker kernel per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
+# `ncu --set full` captures of this very command line: profiles/r1_v4_walker_coop_ncu.md (C2, default arguments)
+# and profiles/r1_v4_reproj_megb_ncu.md (--config 3).  Other workloads have no capture: null.
+NCU_TRAFFIC_BYTES = {("C2_reg_n50", "rot", 64): 471296 + 1280, ("C3_reproj_n8", "rot", 64): 549376 + 776448}
 
 
 def _params_dict(P) -> dict:
@@ -412,7 +416,7 @@ def run_cuda(args) -> None:
             "roofline": {"bound": "alu", "kernel": "walker_coop_trans_kernel" if args.mode == "trans" else
                          ("walker_coop_reproj_kernel" if inst.residual_type == 1 else "walker_coop_kernel"),
                          "achieved": achieved, "peak": peak_mix, "unit": "TFLOP/s", "frac": achieved / peak_mix,
-                         "traffic": None,
+                         "traffic": NCU_TRAFFIC_BYTES.get((inst.name, args.mode, args.precision)),
                          "peak_source": "executed flops / (fp64 flops / DFMA peak + fp32 flops / FFMA peak), both peaks "
                                         "measured in this run by closure_alu_peak (register-resident FMA chains)",
                          "fp32": {"flops_per_launch": flops32, "achieved": flops32 / walk_s / 1e12, "peak": peak32 / 1e12},
