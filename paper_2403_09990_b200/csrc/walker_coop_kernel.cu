@@ -10,15 +10,16 @@
 //          `unc`; the top-N_P* are extracted with warp reductions and the ranking is accepted only
 //          if consecutive values (and the N_P*-th against the next) are more than 2 unc apart.
 //          Otherwise the step falls back to the fp64 evaluation of the plain kernel.
-//   a5-a6  every rung m = 1..N_T is screened first against the two tightest constraints (lane =
-//          (rung, constraint)); rungs with a surviving candidate are then evaluated in full, lane =
+//   a5-a6  every rung m = 1..N_T is screened first (lane = (rung, half of the candidates)) against the
+//          rung's two tightest constraints and against a Lipschitz bound on what the rotation to R_m
+//          can repair; rungs with a surviving candidate are then evaluated in full, lane =
 //          (candidate, constraint chunk), in fp32 with a three-way outcome per candidate: violated
 //          for sure / satisfied for sure / undecided -> fp64.
 //
 // Every accept/reject decision is therefore the decision the fp64 arithmetic of walker_kernel.cu
-// takes (DESIGN.md 6.1 "Certified fp32 evaluation"); the pose itself is only ever updated in fp64.
-// Unlike the one-walker-per-thread kernels all lanes of a warp follow the same walker: no
-// divergence between walkers, the set-up is not repeated per register tile, ~100 registers.
+// takes (DESIGN.md 6.1b "Certified fp32 evaluation"); the pose itself is only ever updated in fp64.
+// Unlike the one-walker-per-thread kernel all lanes of a warp follow the same walker: no divergence
+// between walkers, the set-up is not repeated per register tile, 128 registers (16 warps per SM).
 #include <cuda_runtime.h>
 #include <math_constants.h>
 #include <stdint.h>
