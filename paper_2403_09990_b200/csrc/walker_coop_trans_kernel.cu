@@ -9,10 +9,20 @@
 //          order (m, k) Alg. A8 visits them, 32 at a time, each lane running in_purse on its
 //          candidate with an exit at the first violated constraint; the first feasible one wins.
 //
-// Every residual is evaluated by the same fp64 functions as in the one-walker-per-thread kernel
-// (margin_direct / in_purse_direct in walker_common.cuh), so the two kernels agree bit for bit;
-// unlike the rotation sampler nothing is shared between the perturbations of a pose (each has its
-// own rotation), so there is no cheap fp32 image to certify and this kernel stays in fp64.
+// Every fp64 residual is evaluated by the same functions as in the one-walker-per-thread kernel
+// (margin_direct / in_purse_direct in walker_common.cuh), so the two kernels agree bit for bit.
+//
+// Reprojection residual (Ex.1, the one example the paper runs this sampler on): eq. (14) of the N_P
+// poses is evaluated in fp32 with a certificate, as in walker_coop_reproj_kernel.cu.  With
+// P_i = R* Z_i set up once per move, a pair is p = E_j P_i + t*, q = (zeta_1 p_3 - fx p_1,
+// zeta_2 p_3 - fy p_2), rho = ||q|| / p_3, where E_j = Exp(theta_p xi_j) comes from the series of
+// sin(th)/th and (1 - cos th)/th^2 (|theta_p xi| <= 0.7).  Error bounds, u = 2^-24, th_max = sqrt(3) theta_p:
+//   |E32 - E64| <= e_E = 2 u (1 + 13 th_max + 25 th_max^2) per entry,
+//   E_p = (e_E + 4 u) |P_i|_1 + 4 u |t_r|,   E_q1 = |zeta_1| E_p + fx E_p + 3 u (|zeta_1| p3_hi + fx p1_hi),
+//   p_lo = t_3 - |P_i| - E_p > 0 (else nothing is certified),   rho_hi = (sum of the |.| terms of q) / p_lo,
+//   |rho32 - rho64| <= (E_q1 + E_q2) / p_lo + rho_hi (E_p / p_lo + 2^-19)          (unc = twice that).
+// The ranking is accepted only if consecutive values differ by more than 2 unc; otherwise the candidates
+// that can still be in the top N_P* are re-evaluated in fp64 (topk_fp64).  The ladder stays in fp64.
 #include <cuda_runtime.h>
 #include <math_constants.h>
 #include <stdint.h>
@@ -24,14 +34,18 @@
 namespace closure {
 namespace {
 
+constexpr double kU = 5.9604644775390625e-08;   // 2^-24
+
 struct TransSmem {
-    size_t warp0, per_warp, pose, dex, Rc, candj, candd, stc, total;
+    size_t run_end, run_bf, warp0, per_warp, pose, dex, Rc, candj, candd, stc, rowsA, total;
 };
 
-__host__ __device__ inline TransSmem trans_layout(int rows_bytes, int nq)
+__host__ __device__ inline TransSmem trans_layout(int rows_bytes, int nq, int n_fast)
 {
     TransSmem s;
-    const size_t o = 16 + (size_t)((rows_bytes + 15) & ~15);
+    size_t o = 16 + (size_t)((rows_bytes + 15) & ~15);
+    s.run_end = o; o += (size_t)((n_fast * 4 + 15) & ~15);     // runs of equal bounds (reprojection only)
+    s.run_bf = o;  o += (size_t)((n_fast * 4 + 15) & ~15);
     s.warp0 = o;
     size_t w = 0;
     s.pose = w;  w += 16 * 8;                    // R*(9) t*(3) v(3)
@@ -40,6 +54,7 @@ __host__ __device__ inline TransSmem trans_layout(int rows_bytes, int nq)
     s.candj = w; w += 32 * 4;
     s.candd = w; w += 32 * 4;
     s.stc = w;   w += 16 * 8;
+    s.rowsA = w; w += (size_t)n_fast * 32;       // reprojection only: fp32 rows (R* Z_i, zeta) of the certified eq. (14)
     s.per_warp = w;
     s.total = o + (size_t)kCoopWarps * w;
     return s;
@@ -78,10 +93,37 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
     const double *rows = reinterpret_cast<const double *>(smem_raw + 16);
     stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
+    const TransSmem lay = trans_layout(rows_bytes, NQ, RES == CLOSURE_REPROJ_2D3D ? n : 0);
+    __shared__ int n_runs_s;
+    int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
+    float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
+    if (RES == CLOSURE_REPROJ_2D3D) {                  // runs of equal bounds (rows are sorted by bound)
+        if (warp == 0) {
+            int cnt = 0;
+            for (int base = 0; base < n; base += 32) {
+                const int i = base + lane;
+                bool end = false;
+                double beta = 0.0;
+                if (i < n) {
+                    beta = rows[i * Res<RES>::ROW + Res<RES>::BETA];
+                    end = (i == n - 1) || (rows[(i + 1) * Res<RES>::ROW + Res<RES>::BETA] != beta);
+                }
+                const unsigned m = __ballot_sync(FULL, end);
+                if (end) {
+                    const int r = cnt + __popc(m & ((1u << lane) - 1u));
+                    run_end[r] = i;
+                    run_bf[r] = (float)beta;
+                }
+                cnt += __popc(m);
+            }
+            if (lane == 0) n_runs_s = cnt;
+        }
+        __syncthreads();
+    }
+    const int n_runs = (RES == CLOSURE_REPROJ_2D3D) ? n_runs_s : 0;
 
     const long long local = (long long)blockIdx.x * kCoopWarps + warp;
     if (local >= L.num_walkers) return;                // no block-wide barrier below this line
-    const TransSmem lay = trans_layout(rows_bytes, NQ);
     unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
     double *pose = reinterpret_cast<double *>(wp + lay.pose);
     double *dex = reinterpret_cast<double *>(wp + lay.dex);
@@ -110,12 +152,117 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
         for (int k = 0; k < 10; ++k) stc[k] = 0ull;
     }
     bool hit = false;
+    // Reprojection residual: eq. (14) of the N_P poses in certified fp32 (see the header); needs the series of
+    // Exp to hold (|theta_p xi| <= 0.7).  exact_only & 4 keeps the fp64 ranking (tests).
+    constexpr bool FAST = (RES == CLOSURE_REPROJ_2D3D);
+    const bool fast = FAST && (1.7320508075688772 * L.theta_p <= 0.7);
+    float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);
+    const float thpf = (float)L.theta_p;
+    const float nfx = -(float)K[0], nfy = -(float)K[1];
+    float uncA = CUDART_INF_F, t0f = 0.f, t1f = 0.f, t2f = 0.f;
+    bool moved = true;
     const int KP = n_ps;
     const int items = KP * n_t;                          // ladder candidates, in Alg. A8's order (m, k)
 
     for (int s = 1; s <= L.num_steps; ++s) {
-        // ================================================== a2-a4: perturb, eq. (14), top-N_P* (fp64)
-        {
+        // ================================================== a2-a4: perturb, eq. (14), top-N_P*
+        bool ranked = false;
+        if (fast) {
+            if (moved) {
+                // pose-only part of the pairs: P_i = R* Z_i and the bound unc on |rho32 - rho64| (header)
+                const double th = 1.7320508075688772 * L.theta_p;
+                const double eE = 2.0 * kU * (1.0 + 13.0 * th + 25.0 * th * th);
+                float unc_l = 0.f;
+                for (int i = lane; i < n; i += 32) {
+                    const double *row = rows + i * Res<RES>::ROW;
+                    double P0, P1, P2;
+                    reproj_point(R, row, P0, P1, P2);
+                    const double z0 = fabs(row[0] - K[2]), z1 = fabs(row[1] - K[3]), beta = row[Res<RES>::BETA];
+                    const double Pn = sqrt(P0 * P0 + P1 * P1 + P2 * P2), P1n = fabs(P0) + fabs(P1) + fabs(P2);
+                    const double p0hi = Pn + fabs(t[0]), p1hi = Pn + fabs(t[1]), p2hi = Pn + fabs(t[2]);
+                    const double Ep0 = (eE + 4.0 * kU) * P1n + 4.0 * kU * fabs(t[0]) + 1e-13;
+                    const double Ep1 = (eE + 4.0 * kU) * P1n + 4.0 * kU * fabs(t[1]) + 1e-13;
+                    const double Ep2 = (eE + 4.0 * kU) * P1n + 4.0 * kU * fabs(t[2]) + 1e-13;
+                    const double plo = t[2] - Pn - Ep2;
+                    const double Eq0 = z0 * Ep2 + K[0] * Ep0 + 3.0 * kU * (z0 * p2hi + K[0] * p0hi);
+                    const double Eq1 = z1 * Ep2 + K[1] * Ep1 + 3.0 * kU * (z1 * p2hi + K[1] * p1hi);
+                    float unc_i = CUDART_INF_F;
+                    if (plo > 0.0) {
+                        const double rho_hi = (z0 * p2hi + K[0] * p0hi + z1 * p2hi + K[1] * p1hi) / plo;
+                        const double Erho = (Eq0 + Eq1) / plo + rho_hi * (Ep2 / plo + 1.9073486328125e-06);
+                        unc_i = (float)(2.0 * Erho + 4.76837158203125e-07 * beta + 1e-12 * (rho_hi + beta)) * 1.0001f;
+                    }
+                    unc_l = fmaxf(unc_l, unc_i);
+                    rowsA[2 * i] = make_float4((float)P0, (float)P1, (float)P2, (float)(row[0] - K[2]));
+                    rowsA[2 * i + 1] = make_float4((float)(row[1] - K[3]), 0.f, 0.f, 0.f);
+                }
+                uncA = wmax_nonneg(unc_l);
+                t0f = (float)t[0]; t1f = (float)t[1]; t2f = (float)t[2];
+                __syncwarp();
+            }
+            float dv[NQ];
+            {
+                int jv[NQ];
+                uint32_t x[NQ], y[NQ], z[NQ];
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) jv[q] = lane + 32 * q;
+                philox_batch<NQ>(rng, (uint32_t)s, jv, x, y, z);
+                float E[NQ][9], mx[NQ];
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) {
+                    // Exp(phi) = I + A [phi]x + B [phi]x^2 with the series of A = sin(th)/th, B = (1 - cos th)/th^2
+                    const float f0 = thpf * pm1f(x[q]), f1 = thpf * pm1f(y[q]), f2 = thpf * pm1f(z[q]);
+                    const float s0 = f0 * f0, s1 = f1 * f1, s2 = f2 * f2;
+                    const float th2 = s0 + s1 + s2;
+                    const float A = fmaf(th2, fmaf(th2, fmaf(th2, fmaf(th2, 2.7557319e-06f, -1.9841270e-04f), 8.3333333e-03f), -1.6666667e-01f), 1.0f);
+                    const float B = fmaf(th2, fmaf(th2, fmaf(th2, fmaf(th2, 2.7557319e-07f, -2.4801587e-05f), 1.3888889e-03f), -4.1666667e-02f), 0.5f);
+                    const float a0 = A * f0, a1 = A * f1, a2 = A * f2;
+                    E[q][0] = fmaf(-B, s1 + s2, 1.0f); E[q][1] = fmaf(B, f0 * f1, -a2); E[q][2] = fmaf(B, f0 * f2, a1);
+                    E[q][3] = fmaf(B, f0 * f1, a2);    E[q][4] = fmaf(-B, s0 + s2, 1.0f); E[q][5] = fmaf(B, f1 * f2, -a0);
+                    E[q][6] = fmaf(B, f0 * f2, -a1);   E[q][7] = fmaf(B, f1 * f2, a0);   E[q][8] = fmaf(-B, s0 + s1, 1.0f);
+                    dv[q] = CUDART_INF_F;
+                }
+                int i = 0;
+                for (int r = 0; r < n_runs; ++r) {
+                    const int end = run_end[r];
+                    const float bf = run_bf[r];
+#pragma unroll
+                    for (int q = 0; q < NQ; ++q) mx[q] = 0.f;
+                    for (; i <= end; ++i) {
+                        const float4 ra = rowsA[2 * i], rb = rowsA[2 * i + 1];
+#pragma unroll
+                        for (int q = 0; q < NQ; ++q) {
+                            const float p0 = fmaf(E[q][0], ra.x, fmaf(E[q][1], ra.y, fmaf(E[q][2], ra.z, t0f)));
+                            const float p1 = fmaf(E[q][3], ra.x, fmaf(E[q][4], ra.y, fmaf(E[q][5], ra.z, t1f)));
+                            const float p2 = fmaf(E[q][6], ra.x, fmaf(E[q][7], ra.y, fmaf(E[q][8], ra.z, t2f)));
+                            const float q0 = fmaf(ra.w, p2, nfx * p0);
+                            const float q1 = fmaf(rb.x, p2, nfy * p1);
+                            float wr;
+                            asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(wr) : "f"(p2));
+                            mx[q] = fmaxf(mx[q], fmaf(q0, q0, q1 * q1) * (wr * wr));
+                        }
+                    }
+#pragma unroll
+                    for (int q = 0; q < NQ; ++q) {
+                        const float a = fmaxf(mx[q], 1e-30f);
+                        dv[q] = fminf(dv[q], bf - a * rsqrtf(a));
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < NQ; ++q)
+                    if (lane + 32 * q >= n_p) dv[q] = -CUDART_INF_F;
+                if (stats) stc[6] += (unsigned long long)n * n_p;
+            }
+            float myval;
+            ranked = topk_certified<NQ>(dv, n_ps, uncA, (L.exact_only & 4) != 0, false, lane, candj, candd, myval);
+            if (!ranked) {
+                const ExactMarginTrans<RES> exact{ R, t, K, rows, n, rng, (uint32_t)s, L.theta_p };
+                const int cnt = topk_fp64<NQ>(dv, n_p, n_ps, uncA, myval, (L.exact_only & 16) != 0, lane, dex, candj, candd, exact);
+                if (stats) { stc[8] += 1; stc[0] += (unsigned long long)n * cnt; stc[2] += (unsigned long long)n * cnt; }
+                ranked = true;
+            }
+        }
+        if (!ranked) {
             const ExactMarginTrans<RES> exact{ R, t, K, rows, n, rng, (uint32_t)s, L.theta_p };
             float dummy[NQ];
 #pragma unroll
@@ -174,6 +321,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
             for (int e = 0; e < 9; ++e) R[e] = Rc[k * 9 + e];
             if (stats) stc[4] += 1;
         }
+        moved = (m0 != 0);
         if (m0 != 1) hit = true;                              // R-12 (R-11: nothing feasible -> unchanged)
         if (L.out_trace != nullptr && lane == 0)
             L.out_trace[((size_t)blockIdx.y * L.num_walkers + local) * L.num_steps + (s - 1)] = m0 | (j_win << 8);
@@ -197,7 +345,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
 template <int RES, int NQ>
 cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, cudaStream_t stream)
 {
-    const TransSmem lay = trans_layout(max_rows_bytes, NQ);
+    const TransSmem lay = trans_layout(max_rows_bytes, NQ, RES == CLOSURE_REPROJ_2D3D ? max_rows_bytes / (Res<RES>::ROW * 8) : 0);
     if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaFuncSetAttribute(walker_coop_trans_kernel<RES, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)lay.total);
