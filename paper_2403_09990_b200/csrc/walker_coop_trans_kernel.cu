@@ -14,12 +14,15 @@
 //
 // Reprojection residual (Ex.1, the one example the paper runs this sampler on): eq. (14) of the N_P
 // poses is evaluated in fp32 with a certificate, as in walker_coop_reproj_kernel.cu.  With
-// P_i = R* Z_i set up once per move, a pair is p = E_j P_i + t*, q = (zeta_1 p_3 - fx p_1,
-// zeta_2 p_3 - fy p_2), rho = ||q|| / p_3, where E_j = Exp(theta_p xi_j) comes from the series of
-// sin(th)/th and (1 - cos th)/th^2 (|theta_p xi| <= 0.7).  Error bounds, u = 2^-24, th_max = sqrt(3) theta_p:
-//   |E32 - E64| <= e_E = 2 u (1 + 13 th_max + 25 th_max^2) per entry,
-//   E_p = (e_E + 4 u) |P_i|_1 + 4 u |t_r|,   E_q1 = |zeta_1| E_p + fx E_p + 3 u (|zeta_1| p3_hi + fx p1_hi),
-//   p_lo = t_3 - |P_i| - E_p > 0 (else nothing is certified),   rho_hi = (sum of the |.| terms of q) / p_lo,
+// P_i = R* Z_i, b_i = P_i + t* and A = (zeta_1 b_3 - fx b_1, zeta_2 b_3 - fy b_2) set up in fp64 once per move,
+// a pair is g = D_j P_i, q = A + (zeta_1 g_3 - fx g_1, zeta_2 g_3 - fy g_2), p_3 = b_3 + g_3, rho = ||q|| / p_3,
+// where D_j = Exp(theta_p xi_j) - I comes from the series of sin(th)/th and (1 - cos th)/th^2
+// (|theta_p xi| <= 0.7): only the small rotation part is computed in fp32.  Error bounds, u = 2^-24,
+// th_max = sqrt(3) theta_p, |g| <= th_max |P_i|:
+//   |D32 - D64| <= e_D = 2 u (13.5 th_max + 13 th_max^2) per entry (phi from pm1f: 6 u theta_p; series 5 u),
+//   E_g = (e_D + 4 u th_max) |P_i|_1 + 3 u |g|_hi,   E_q1 = (|zeta_1| + fx)(E_g + 4 u |g|_hi) + 3 u |A_1|,
+//   E_p = E_g + 2 u (|b_3| + |g|_hi),   p_lo = b_3 - |g|_hi - E_p > 0 (else nothing is certified),
+//   rho_hi = (|A_1| + |A_2| + (|zeta_1| + fx + |zeta_2| + fy) |g|_hi) / p_lo,
 //   |rho32 - rho64| <= (E_q1 + E_q2) / p_lo + rho_hi (E_p / p_lo + 2^-19)          (unc = twice that).
 // The ranking is accepted only if consecutive values differ by more than 2 unc; otherwise the candidates
 // that can still be in the top N_P* are re-evaluated in fp64 (topk_fp64).  The ladder stays in fp64.
@@ -159,7 +162,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
     float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);
     const float thpf = (float)L.theta_p;
     const float nfx = -(float)K[0], nfy = -(float)K[1];
-    float uncA = CUDART_INF_F, t0f = 0.f, t1f = 0.f, t2f = 0.f;
+    float uncA = CUDART_INF_F;
     bool moved = true;
     const int KP = n_ps;
     const int items = KP * n_t;                          // ladder candidates, in Alg. A8's order (m, k)
@@ -170,34 +173,38 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
         if (fast) {
             if (moved) {
                 // pose-only part of the pairs: P_i = R* Z_i and the bound unc on |rho32 - rho64| (header)
+                // With D_j = E_j - I (entries O(theta)):  p = (P_i + t*) + D_j P_i,
+                //   q_1 = A_1 + zeta_1 (D P)_3 - fx (D P)_1,   A_1 = zeta_1 (P + t)_3 - fx (P + t)_1  (fp64, then rounded),
+                // so that only the small rotation part is computed in fp32.
                 const double th = 1.7320508075688772 * L.theta_p;
-                const double eE = 2.0 * kU * (1.0 + 13.0 * th + 25.0 * th * th);
+                const double eD = 2.0 * kU * (13.5 * th + 13.0 * th * th);          // |D32 - D64| per entry
                 float unc_l = 0.f;
                 for (int i = lane; i < n; i += 32) {
                     const double *row = rows + i * Res<RES>::ROW;
                     double P0, P1, P2;
                     reproj_point(R, row, P0, P1, P2);
-                    const double z0 = fabs(row[0] - K[2]), z1 = fabs(row[1] - K[3]), beta = row[Res<RES>::BETA];
+                    const double zs0 = row[0] - K[2], zs1 = row[1] - K[3], beta = row[Res<RES>::BETA];
+                    const double z0 = fabs(zs0), z1 = fabs(zs1);
+                    const double b0 = P0 + t[0], b1 = P1 + t[1], b2 = P2 + t[2];
+                    const double A0 = zs0 * b2 - K[0] * b0, A1 = zs1 * b2 - K[1] * b1;
                     const double Pn = sqrt(P0 * P0 + P1 * P1 + P2 * P2), P1n = fabs(P0) + fabs(P1) + fabs(P2);
-                    const double p0hi = Pn + fabs(t[0]), p1hi = Pn + fabs(t[1]), p2hi = Pn + fabs(t[2]);
-                    const double Ep0 = (eE + 4.0 * kU) * P1n + 4.0 * kU * fabs(t[0]) + 1e-13;
-                    const double Ep1 = (eE + 4.0 * kU) * P1n + 4.0 * kU * fabs(t[1]) + 1e-13;
-                    const double Ep2 = (eE + 4.0 * kU) * P1n + 4.0 * kU * fabs(t[2]) + 1e-13;
-                    const double plo = t[2] - Pn - Ep2;
-                    const double Eq0 = z0 * Ep2 + K[0] * Ep0 + 3.0 * kU * (z0 * p2hi + K[0] * p0hi);
-                    const double Eq1 = z1 * Ep2 + K[1] * Ep1 + 3.0 * kU * (z1 * p2hi + K[1] * p1hi);
+                    const double dhi = th * Pn * 1.01;                              // |D P| <= 2 sin(th/2) |P| <= th |P|
+                    const double Ed = (eD + 4.0 * kU * th) * P1n + 3.0 * kU * dhi + 1e-13;   // error of each (D P)_r
+                    const double Ep2 = Ed + 2.0 * kU * (fabs(b2) + dhi);           // p_3 = b_3 + (D P)_3
+                    const double plo = b2 - dhi - Ep2;
+                    const double Eq0 = (z0 + K[0]) * Ed + 3.0 * kU * fabs(A0) + 4.0 * kU * (z0 + K[0]) * dhi;
+                    const double Eq1 = (z1 + K[1]) * Ed + 3.0 * kU * fabs(A1) + 4.0 * kU * (z1 + K[1]) * dhi;
                     float unc_i = CUDART_INF_F;
                     if (plo > 0.0) {
-                        const double rho_hi = (z0 * p2hi + K[0] * p0hi + z1 * p2hi + K[1] * p1hi) / plo;
+                        const double rho_hi = (fabs(A0) + fabs(A1) + (z0 + K[0] + z1 + K[1]) * dhi) / plo;
                         const double Erho = (Eq0 + Eq1) / plo + rho_hi * (Ep2 / plo + 1.9073486328125e-06);
                         unc_i = (float)(2.0 * Erho + 4.76837158203125e-07 * beta + 1e-12 * (rho_hi + beta)) * 1.0001f;
                     }
                     unc_l = fmaxf(unc_l, unc_i);
-                    rowsA[2 * i] = make_float4((float)P0, (float)P1, (float)P2, (float)(row[0] - K[2]));
-                    rowsA[2 * i + 1] = make_float4((float)(row[1] - K[3]), 0.f, 0.f, 0.f);
+                    rowsA[2 * i] = make_float4((float)P0, (float)P1, (float)P2, (float)zs0);
+                    rowsA[2 * i + 1] = make_float4((float)zs1, (float)A0, (float)A1, (float)b2);
                 }
                 uncA = wmax_nonneg(unc_l);
-                t0f = (float)t[0]; t1f = (float)t[1]; t2f = (float)t[2];
                 __syncwarp();
             }
             float dv[NQ];
@@ -217,9 +224,10 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
                     const float A = fmaf(th2, fmaf(th2, fmaf(th2, fmaf(th2, 2.7557319e-06f, -1.9841270e-04f), 8.3333333e-03f), -1.6666667e-01f), 1.0f);
                     const float B = fmaf(th2, fmaf(th2, fmaf(th2, fmaf(th2, 2.7557319e-07f, -2.4801587e-05f), 1.3888889e-03f), -4.1666667e-02f), 0.5f);
                     const float a0 = A * f0, a1 = A * f1, a2 = A * f2;
-                    E[q][0] = fmaf(-B, s1 + s2, 1.0f); E[q][1] = fmaf(B, f0 * f1, -a2); E[q][2] = fmaf(B, f0 * f2, a1);
-                    E[q][3] = fmaf(B, f0 * f1, a2);    E[q][4] = fmaf(-B, s0 + s2, 1.0f); E[q][5] = fmaf(B, f1 * f2, -a0);
-                    E[q][6] = fmaf(B, f0 * f2, -a1);   E[q][7] = fmaf(B, f1 * f2, a0);   E[q][8] = fmaf(-B, s0 + s1, 1.0f);
+                    // D = E - I
+                    E[q][0] = -B * (s1 + s2);        E[q][1] = fmaf(B, f0 * f1, -a2); E[q][2] = fmaf(B, f0 * f2, a1);
+                    E[q][3] = fmaf(B, f0 * f1, a2);  E[q][4] = -B * (s0 + s2);        E[q][5] = fmaf(B, f1 * f2, -a0);
+                    E[q][6] = fmaf(B, f0 * f2, -a1); E[q][7] = fmaf(B, f1 * f2, a0);  E[q][8] = -B * (s0 + s1);
                     dv[q] = CUDART_INF_F;
                 }
                 int i = 0;
@@ -232,11 +240,12 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
                         const float4 ra = rowsA[2 * i], rb = rowsA[2 * i + 1];
 #pragma unroll
                         for (int q = 0; q < NQ; ++q) {
-                            const float p0 = fmaf(E[q][0], ra.x, fmaf(E[q][1], ra.y, fmaf(E[q][2], ra.z, t0f)));
-                            const float p1 = fmaf(E[q][3], ra.x, fmaf(E[q][4], ra.y, fmaf(E[q][5], ra.z, t1f)));
-                            const float p2 = fmaf(E[q][6], ra.x, fmaf(E[q][7], ra.y, fmaf(E[q][8], ra.z, t2f)));
-                            const float q0 = fmaf(ra.w, p2, nfx * p0);
-                            const float q1 = fmaf(rb.x, p2, nfy * p1);
+                            const float g0 = fmaf(E[q][0], ra.x, fmaf(E[q][1], ra.y, E[q][2] * ra.z));   // D P
+                            const float g1 = fmaf(E[q][3], ra.x, fmaf(E[q][4], ra.y, E[q][5] * ra.z));
+                            const float g2 = fmaf(E[q][6], ra.x, fmaf(E[q][7], ra.y, E[q][8] * ra.z));
+                            const float q0 = fmaf(ra.w, g2, fmaf(nfx, g0, rb.y));
+                            const float q1 = fmaf(rb.x, g2, fmaf(nfy, g1, rb.z));
+                            const float p2 = rb.w + g2;
                             float wr;
                             asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(wr) : "f"(p2));
                             mx[q] = fmaxf(mx[q], fmaf(q0, q0, q1 * q1) * (wr * wr));
