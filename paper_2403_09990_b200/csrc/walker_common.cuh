@@ -53,13 +53,15 @@ __device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : 
 __device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
 
 // ---------------------------------------------------------------------------------- small math
+// Every multiply-add below is written as an explicit fma(): several kernels share these helpers and must
+// round identically (the tests compare them bit for bit), which implicit contraction does not guarantee.
 __device__ __forceinline__ void mat3_mul(const double (&A)[9], const double (&B)[9], double (&C)[9])
 {
 #pragma unroll
     for (int r = 0; r < 3; ++r)
 #pragma unroll
         for (int c = 0; c < 3; ++c)
-            C[3 * r + c] = A[3 * r] * B[c] + A[3 * r + 1] * B[3 + c] + A[3 * r + 2] * B[6 + c];
+            C[3 * r + c] = fma(A[3 * r + 2], B[6 + c], fma(A[3 * r + 1], B[3 + c], A[3 * r] * B[c]));
 }
 
 // Rodrigues coefficients of Exp(phi): Exp = I + A [phi]x + B [phi]x^2 (series below 1e-4).
@@ -82,12 +84,12 @@ __device__ __forceinline__ void exp_coeffs(double th2, double &A, double &B)
 __device__ __forceinline__ void exp_so3(double p0, double p1, double p2, double (&E)[9])
 {
     double A, B;
-    exp_coeffs(p0 * p0 + p1 * p1 + p2 * p2, A, B);
+    exp_coeffs(fma(p2, p2, fma(p1, p1, p0 * p0)), A, B);
     const double K[9] = { 0.0, -p2, p1, p2, 0.0, -p0, -p1, p0, 0.0 };
     double K2[9];
     mat3_mul(K, K, K2);
 #pragma unroll
-    for (int e = 0; e < 9; ++e) E[e] = ((e % 4 == 0) ? 1.0 : 0.0) + A * K[e] + B * K2[e];
+    for (int e = 0; e < 9; ++e) E[e] = fma(B, K2[e], fma(A, K[e], (e % 4 == 0) ? 1.0 : 0.0));
 }
 
 // Rm = R + a (w x R) + b (w x (w x R)), cross products taken column by column:
@@ -98,11 +100,11 @@ __device__ __forceinline__ void rotate_left(const double (&R)[9], double w0, dou
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const double x = R[c], y = R[3 + c], z = R[6 + c];
-        const double p0 = w1 * z - w2 * y, p1 = w2 * x - w0 * z, p2 = w0 * y - w1 * x;       // w x col
-        const double q0 = w1 * p2 - w2 * p1, q1 = w2 * p0 - w0 * p2, q2 = w0 * p1 - w1 * p0; // w x (w x col)
-        Rm[c] = x + a * p0 + b * q0;
-        Rm[3 + c] = y + a * p1 + b * q1;
-        Rm[6 + c] = z + a * p2 + b * q2;
+        const double p0 = fma(w1, z, -(w2 * y)), p1 = fma(w2, x, -(w0 * z)), p2 = fma(w0, y, -(w1 * x));       // w x col
+        const double q0 = fma(w1, p2, -(w2 * p1)), q1 = fma(w2, p0, -(w0 * p2)), q2 = fma(w0, p1, -(w1 * p0)); // w x (w x col)
+        Rm[c] = fma(b, q0, fma(a, p0, x));
+        Rm[3 + c] = fma(b, q1, fma(a, p1, y));
+        Rm[6 + c] = fma(b, q2, fma(a, p2, z));
     }
 }
 
@@ -174,19 +176,15 @@ __device__ __forceinline__ double direct_sq(const double (&R)[9], const double (
 {
     if (RES == CLOSURE_REG_3D3D) {
         const double a0 = row[0], a1 = row[1], a2 = row[2];
-        const double g0 = row[3] - ((R[0] * a0 + R[1] * a1 + R[2] * a2) + t[0]);
-        const double g1 = row[4] - ((R[3] * a0 + R[4] * a1 + R[5] * a2) + t[1]);
-        const double g2 = row[5] - ((R[6] * a0 + R[7] * a1 + R[8] * a2) + t[2]);
-        return g0 * g0 + g1 * g1 + g2 * g2;
+        const double g0 = row[3] - (fma(R[0], a0, fma(R[1], a1, R[2] * a2)) + t[0]);
+        const double g1 = row[4] - (fma(R[3], a0, fma(R[4], a1, R[5] * a2)) + t[1]);
+        const double g2 = row[5] - (fma(R[6], a0, fma(R[7], a1, R[8] * a2)) + t[2]);
+        return fma(g2, g2, fma(g1, g1, g0 * g0));
     } else if (RES == CLOSURE_REPROJ_2D3D) {
         const double Z0 = row[2], Z1 = row[3], Z2 = row[4];
-        const double p0 = (R[0] * Z0 + R[1] * Z1 + R[2] * Z2) + t[0];
-        const double p1 = (R[3] * Z0 + R[4] * Z1 + R[5] * Z2) + t[1];
-        const double p2 = (R[6] * Z0 + R[7] * Z1 + R[8] * Z2) + t[2];
-        if (!(p2 > 0.0)) return CUDART_INF;                       // cheirality (R-10)
-        const double g0 = row[0] - (K[0] * (p0 / p2) + K[2]);
-        const double g1 = row[1] - (K[1] * (p1 / p2) + K[3]);
-        return g0 * g0 + g1 * g1;
+        double P0, P1, P2;
+        reproj_point(R, row, P0, P1, P2);
+        return reproj_sq(P0, P1, P2, t[0], t[1], t[2], row, K);      // cheirality (R-10) inside
     } else {
         double s = 0.0;
         if (RES == CLOSURE_POSE_REG || part == 0) s = frob_sq(R, row);
@@ -320,7 +318,7 @@ __device__ __forceinline__ void init_walker(const InstanceDesc *__restrict__ D, 
     philox4x32_10(rng.w_lo, 0u, 0u, 0u | rng.w_hi8, rng.k0, rng.k1, o);
     const double z = pm1(o[0]);
     const double phi = CUDART_PI * (pm1(o[1]) + 1.0);
-    const double s = sqrt(1.0 - z * z);
+    const double s = sqrt(fma(-z, z, 1.0));
     double sp, cp;
     sincos(phi, &sp, &cp);
     const double r0 = s * cp, r1 = s * sp, r2 = z;                    // random unit vector (R-4)
@@ -332,9 +330,9 @@ __device__ __forceinline__ void init_walker(const InstanceDesc *__restrict__ D, 
         for (int r = 0; r < 3; ++r)                                   // M = R_0 Rbar^T (R-2)
 #pragma unroll
             for (int c = 0; c < 3; ++c)
-                M[3 * r + c] = R[3 * r] * Rb[3 * c] + R[3 * r + 1] * Rb[3 * c + 1] + R[3 * r + 2] * Rb[3 * c + 2];
+                M[3 * r + c] = fma(R[3 * r + 2], Rb[3 * c + 2], fma(R[3 * r + 1], Rb[3 * c + 1], R[3 * r] * Rb[3 * c]));
         const double v0 = M[7] - M[5], v1 = M[2] - M[6], v2 = M[3] - M[1];
-        const double nv = sqrt(v0 * v0 + v1 * v1 + v2 * v2);
+        const double nv = sqrt(fma(v2, v2, fma(v1, v1, v0 * v0)));
         const double theta = atan2(nv, (M[0] + M[4] + M[8]) - 1.0);
         double u0 = 0.0, u1 = 0.0, u2 = 0.0;
         if (nv > 0.0 && !(theta < 1e-12)) { u0 = v0 / nv; u1 = v1 / nv; u2 = v2 / nv; }   // R-3
@@ -343,7 +341,7 @@ __device__ __forceinline__ void init_walker(const InstanceDesc *__restrict__ D, 
         vel[2] = L.omega0 * (u2 + r2);
     } else {
         const double d0 = t[0] - D->tbar[0], d1 = t[1] - D->tbar[1], d2 = t[2] - D->tbar[2];
-        const double nd = sqrt(d0 * d0 + d1 * d1 + d2 * d2);
+        const double nd = sqrt(fma(d2, d2, fma(d1, d1, d0 * d0)));
         const bool far = !(nd < 1e-12);
         vel[0] = L.v0 * ((far ? d0 / nd : 0.0) + r0);
         vel[1] = L.v0 * ((far ? d1 / nd : 0.0) + r1);
@@ -360,7 +358,7 @@ __device__ __forceinline__ void fill_ladder(const WalkLaunch &L, const double (&
     for (int m = 0; m < L.n_t; ++m) {
         const double p0 = dT * vel[0], p1 = dT * vel[1], p2 = dT * vel[2];
         double A, B;
-        exp_coeffs(p0 * p0 + p1 * p1 + p2 * p2, A, B);
+        exp_coeffs(fma(p2, p2, fma(p1, p1, p0 * p0)), A, B);
         ladder[m * kBlock + threadIdx.x] = make_double2(A * dT, B * dT * dT);
         dT = dT * L.gamma;
     }

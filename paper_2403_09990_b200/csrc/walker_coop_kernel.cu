@@ -340,7 +340,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
             for (int q = 0; q < m; ++q) dT = dT * L.gamma;
             const double p0 = dT * vel[0], p1 = dT * vel[1], p2 = dT * vel[2];
             double A, B;
-            exp_coeffs(p0 * p0 + p1 * p1 + p2 * p2, A, B);
+            exp_coeffs(fma(p2, p2, fma(p1, p1, p0 * p0)), A, B);
             ab[m] = make_double2(A * dT, B * dT * dT);
         }
         if (lane == 0) {
@@ -581,7 +581,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
                     // M = max_i (v32_i - eps_i):  M > th  => some constraint violated for sure;
                     // M + 2 eps_max <= th => every constraint satisfied for sure.
                     const bool dead = M > c4.w;
-                    const bool sure = M <= c4.w - 2.0f * epsL;
+                    const bool sure = (epsL < CUDART_INF_F) && (M <= c4.w - 2.0f * epsL);
                     const bool mine = e_act && ech == 0;
                     unsigned alive2 = __ballot_sync(FULL, mine && !dead) & cand_alive;
                     unsigned undecided = __ballot_sync(FULL, mine && !dead && !sure) & cand_alive;

@@ -209,7 +209,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
             for (int q = 0; q < m; ++q) dT = dT * L.gamma;
             const double p0 = dT * vel[0], p1 = dT * vel[1], p2 = dT * vel[2];
             double A, B;
-            exp_coeffs(p0 * p0 + p1 * p1 + p2 * p2, A, B);
+            exp_coeffs(fma(p2, p2, fma(p1, p1, p0 * p0)), A, B);
             ab[m] = make_double2(A * dT, B * dT * dT);
         }
         if (lane == 0) {
@@ -468,7 +468,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
                 // M = max_i (g32_i - E_g,i):  M > 0 => some constraint violated for sure;
                 // M + 2 max_i E_g,i <= 0 => every constraint satisfied (and in front of the camera) for sure.
                 const bool dead = M > 0.f;
-                const bool sure = M <= -2.0f * epsL;
+                const bool sure = (epsL < CUDART_INF_F) && (M <= -2.0f * epsL);   // (an infinite bound certifies nothing)
                 const bool mine = e_act && ech == 0;
                 unsigned alive2 = __ballot_sync(FULL, mine && !dead) & cand_alive;
                 unsigned undecided = __ballot_sync(FULL, mine && !dead && !sure) & cand_alive;

@@ -25,7 +25,13 @@
 //   rho_hi = (|A_1| + |A_2| + (|zeta_1| + fx + |zeta_2| + fy) |g|_hi) / p_lo,
 //   |rho32 - rho64| <= (E_q1 + E_q2) / p_lo + rho_hi (E_p / p_lo + 2^-19)          (unc = twice that).
 // The ranking is accepted only if consecutive values differ by more than 2 unc; otherwise the candidates
-// that can still be in the top N_P* are re-evaluated in fp64 (topk_fp64).  The ladder stays in fp64.
+// that can still be in the top N_P* are re-evaluated in fp64 (topk_fp64).
+// The ladder candidate (k, m) has the cone value g(s) = (q_1 + s c_1)^2 + (q_2 + s c_2)^2 - (w + s c_w)^2 at s = dT_m,
+// q, w = beta p_3 of candidate k as above, c = (zeta_1 v_3 - fx v_1, zeta_2 v_3 - fy v_2), c_w = beta v_3:
+//   |g32 - g| <= 2 W (E_q + E_w) + 8 u W^2 + 4097 E_q^2 + E_w^2 + (2^-12 + 4 u) |g|,   W = beta p3_hi + |c_w|,
+// (2 Q E_q <= 2^-12 |g| + 2^12 E_q^2 + 2 W E_q with Q^2 = g + W^2), so with tau = 1.5 x the absolute part
+// g32 > tau means violated, g32 < -tau with beta p_3 > E_w satisfied,
+// and anything else goes to the fp64 in_purse of the plain kernel.
 #include <cuda_runtime.h>
 #include <math_constants.h>
 #include <stdint.h>
@@ -40,8 +46,10 @@ namespace {
 constexpr double kU = 5.9604644775390625e-08;   // 2^-24
 
 struct TransSmem {
-    size_t run_end, run_bf, warp0, per_warp, pose, dex, Rc, candj, candd, stc, rowsA, total;
+    size_t run_end, run_bf, warp0, per_warp, pose, dex, Rc, candj, candd, stc, rowsA, crow, betaf, Dc, krow, sT, total;
 };
+
+constexpr int kKrowMax = 512;                  // (candidate, constraint) rows of the certified ladder
 
 __host__ __device__ inline TransSmem trans_layout(int rows_bytes, int nq, int n_fast)
 {
@@ -58,6 +66,11 @@ __host__ __device__ inline TransSmem trans_layout(int rows_bytes, int nq, int n_
     s.candd = w; w += 32 * 4;
     s.stc = w;   w += 16 * 8;
     s.rowsA = w; w += (size_t)n_fast * 32;       // reprojection only: fp32 rows (R* Z_i, zeta) of the certified eq. (14)
+    s.crow = w;  w += (size_t)n_fast * 16;       // per constraint: shift of the cone row per unit step along v, -tau
+    s.betaf = w; w += (size_t)((n_fast * 4 + 15) & ~15);
+    s.Dc = w;    w += (n_fast ? 32 * 12 * 4 : 0);               // D = Exp - I of the kept perturbations (fp32)
+    s.krow = w;  w += (n_fast ? (size_t)kKrowMax * 16 : 0);     // cone rows of (candidate, constraint) at step 0
+    s.sT = w;    w += (n_fast ? 64 * 4 : 0);                    // ladder steps dT_m in fp32
     s.per_warp = w;
     s.total = o + (size_t)kCoopWarps * w;
     return s;
@@ -162,7 +175,21 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
     float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);
     const float thpf = (float)L.theta_p;
     const float nfx = -(float)K[0], nfy = -(float)K[1];
-    float uncA = CUDART_INF_F;
+    float4 *crow = reinterpret_cast<float4 *>(wp + lay.crow);
+    float *betaf = reinterpret_cast<float *>(wp + lay.betaf);
+    float *Dc = reinterpret_cast<float *>(wp + lay.Dc);
+    float4 *krow = reinterpret_cast<float4 *>(wp + lay.krow);
+    float *sT = reinterpret_cast<float *>(wp + lay.sT);
+    // the ladder is certified too when its (candidate, constraint) rows fit; exact_only & 2: every candidate to fp64
+    const bool fast_ladder = fast && (n_ps * n <= kKrowMax);
+    if (fast) {
+        for (int m = lane; m < n_t; m += 32) {
+            double dT = 1.0;
+            for (int q = 0; q < m; ++q) dT = dT * L.gamma;
+            sT[m] = (float)dT;
+        }
+    }
+    float uncA = CUDART_INF_F, tauMax = CUDART_INF_F, ewMax = CUDART_INF_F;
     bool moved = true;
     const int KP = n_ps;
     const int items = KP * n_t;                          // ladder candidates, in Alg. A8's order (m, k)
@@ -178,7 +205,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
                 // so that only the small rotation part is computed in fp32.
                 const double th = 1.7320508075688772 * L.theta_p;
                 const double eD = 2.0 * kU * (13.5 * th + 13.0 * th * th);          // |D32 - D64| per entry
-                float unc_l = 0.f;
+                float unc_l = 0.f, tau_l = 0.f, ew_l = 0.f;
                 for (int i = lane; i < n; i += 32) {
                     const double *row = rows + i * Res<RES>::ROW;
                     double P0, P1, P2;
@@ -203,7 +230,24 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
                     unc_l = fmaxf(unc_l, unc_i);
                     rowsA[2 * i] = make_float4((float)P0, (float)P1, (float)P2, (float)zs0);
                     rowsA[2 * i + 1] = make_float4((float)zs1, (float)A0, (float)A1, (float)b2);
+                    // ladder: cone value g(s) = (q_1 + s c_1)^2 + (q_2 + s c_2)^2 - (w + s c_w)^2, s = dT_m in [0, 1],
+                    // with c = (zeta_1 v_3 - fx v_1, zeta_2 v_3 - fy v_2), w = beta p_3, c_w = beta v_3.  |g32 - g| <=
+                    // a + b |g| with the a below (header), so g32 > tau => violated, g32 < -tau => satisfied.
+                    const double c0 = zs0 * vel[2] - K[0] * vel[0], c1 = zs1 * vel[2] - K[1] * vel[1], cw = beta * vel[2];
+                    const double q0khi = fabs(A0) + (z0 + K[0]) * dhi, q1khi = fabs(A1) + (z1 + K[1]) * dhi;
+                    const double p2hi = fabs(b2) + dhi;
+                    const double EqL = (Eq0 + 3.0 * kU * fabs(c0) + kU * q0khi) + (Eq1 + 3.0 * kU * fabs(c1) + kU * q1khi);
+                    const double EwL = beta * Ep2 + 3.0 * kU * beta * p2hi + 3.0 * kU * fabs(cw);
+                    const double Whi = beta * p2hi + fabs(cw);
+                    const double a = 2.0 * Whi * (EqL + EwL) + 8.0 * kU * Whi * Whi + 4097.0 * EqL * EqL + EwL * EwL;
+                    float tau = (float)(1.5 * a + 1e-12 * Whi * Whi) * 1.0001f;
+                    ew_l = fmaxf(ew_l, (float)EwL * 1.0001f);
+                    crow[i] = make_float4((float)c0, (float)c1, (float)cw, -tau);
+                    betaf[i] = (float)beta;
+                    tau_l = fmaxf(tau_l, tau);
                 }
+                tauMax = wmax_nonneg(tau_l);
+                ewMax = wmax_nonneg(ew_l);
                 uncA = wmax_nonneg(unc_l);
                 __syncwarp();
             }
@@ -280,6 +324,83 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
             if (stats) { stc[0] += (unsigned long long)n * n_p; stc[2] += (unsigned long long)n * n_p; }
         }
         __syncwarp();
+        int win = -1;
+        double Rw[9];                                        // rotation of the winning candidate
+        if (fast_ladder) {
+            // ================================================== a5-a6, certified fp32 ladder (reprojection)
+            if (lane < KP) {                                 // D = Exp(theta_p xi) - I of the kept perturbations, as in a2
+                uint32_t o[4];
+                philox4x32_10(rng.w_lo, (uint32_t)s, (uint32_t)candj[lane], 1u | rng.w_hi8, rng.k0, rng.k1, o);
+                const float f0 = thpf * pm1f(o[0]), f1 = thpf * pm1f(o[1]), f2 = thpf * pm1f(o[2]);
+                const float s0 = f0 * f0, s1 = f1 * f1, s2 = f2 * f2;
+                const float th2 = s0 + s1 + s2;
+                const float A = fmaf(th2, fmaf(th2, fmaf(th2, fmaf(th2, 2.7557319e-06f, -1.9841270e-04f), 8.3333333e-03f), -1.6666667e-01f), 1.0f);
+                const float B = fmaf(th2, fmaf(th2, fmaf(th2, fmaf(th2, 2.7557319e-07f, -2.4801587e-05f), 1.3888889e-03f), -4.1666667e-02f), 0.5f);
+                const float a0 = A * f0, a1 = A * f1, a2 = A * f2;
+                float *d = Dc + 12 * lane;
+                d[0] = -B * (s1 + s2);        d[1] = fmaf(B, f0 * f1, -a2); d[2] = fmaf(B, f0 * f2, a1);
+                d[3] = fmaf(B, f0 * f1, a2);  d[4] = -B * (s0 + s2);        d[5] = fmaf(B, f1 * f2, -a0);
+                d[6] = fmaf(B, f0 * f2, -a1); d[7] = fmaf(B, f1 * f2, a0);  d[8] = -B * (s0 + s1);
+            }
+            __syncwarp();
+            for (int pi = lane; pi < KP * n; pi += 32) {    // cone rows of (candidate k, constraint i) at step 0
+                const int k = pi / n, i = pi - k * n;
+                const float4 ra = rowsA[2 * i], rb = rowsA[2 * i + 1];
+                const float *d = Dc + 12 * k;
+                const float g0 = fmaf(d[0], ra.x, fmaf(d[1], ra.y, d[2] * ra.z));
+                const float g1 = fmaf(d[3], ra.x, fmaf(d[4], ra.y, d[5] * ra.z));
+                const float g2 = fmaf(d[6], ra.x, fmaf(d[7], ra.y, d[8] * ra.z));
+                krow[i * KP + k] = make_float4(fmaf(ra.w, g2, fmaf(nfx, g0, rb.y)), fmaf(rb.x, g2, fmaf(nfy, g1, rb.z)),
+                                       betaf[i] * (rb.w + g2), 0.f);
+            }
+            __syncwarp();
+            for (int base = 0; base < items && win < 0; base += 32) {
+                const int it = base + lane;
+                bool dead = true, sure = false;
+                if (it < items) {
+                    const int m = it / KP, k = it - m * KP;
+                    const float sm = sT[m];
+                    float M = -CUDART_INF_F, Wmin = CUDART_INF_F;
+                    for (int i = 0; i < n; ++i) {
+                        const float4 kr = krow[i * KP + k], cr = crow[i];          // [i][k]: lanes of a round differ in k
+                        const float q0 = fmaf(sm, cr.x, kr.x), q1 = fmaf(sm, cr.y, kr.y), w = fmaf(sm, cr.z, kr.z);
+                        M = fmaxf(M, fmaf(q0, q0, fmaf(q1, q1, fmaf(-w, w, cr.w))));
+                        Wmin = fminf(Wmin, w);
+                    }
+                    // g32 - tau > 0: violated for sure (behind the camera counts as violated either way, R-10);
+                    // satisfied for sure needs every g32 + tau <= 0 and beta p_3 > 0 beyond its error
+                    dead = M > 0.f;
+                    sure = (tauMax < CUDART_INF_F) && (M <= -2.0f * tauMax) && (Wmin > ewMax);
+                    if (L.exact_only & 2) { dead = false; sure = false; }
+                }
+                if (stats) stc[7] += (unsigned long long)n * min(32, items - base);
+                unsigned alive = __ballot_sync(FULL, !dead);
+                const unsigned sures = __ballot_sync(FULL, sure);
+                while (alive != 0u && win < 0) {             // in Alg. A8's order; undecided ones go to fp64
+                    const int l = __ffs(alive) - 1;
+                    alive &= alive - 1u;
+                    const int itl = base + l;
+                    const int m = itl / KP, k = itl - m * KP;
+                    double x, y, z, E[9];
+                    rng.xi3((uint32_t)s, (uint32_t)candj[k], 1u, x, y, z);
+                    exp_so3(L.theta_p * x, L.theta_p * y, L.theta_p * z, E);
+                    mat3_mul(E, R, Rw);
+                    bool ok = (sures >> l) & 1u;
+                    if (!ok) {
+                        double dT = 1.0;
+                        for (int q = 0; q < m; ++q) dT = dT * L.gamma;
+                        double tm[3];
+                        tm[0] = __dadd_rn(t[0], __dmul_rn(dT, vel[0]));
+                        tm[1] = __dadd_rn(t[1], __dmul_rn(dT, vel[1]));
+                        tm[2] = __dadd_rn(t[2], __dmul_rn(dT, vel[2]));
+                        unsigned long long pairs = 0;
+                        ok = in_purse_direct<RES>(Rw, tm, rows, n, K, pairs);
+                        if (stats) { stc[1] += pairs; stc[3] += pairs; stc[9] += 1; }
+                    }
+                    if (ok) win = itl;
+                }
+            }
+        } else {
         if (lane < KP) {                                 // rotations of the kept perturbations
             double x, y, z, E[9], Rj[9];
             rng.xi3((uint32_t)s, (uint32_t)candj[lane], 1u, x, y, z);
@@ -291,7 +412,6 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
         __syncwarp();
 
         // ================================================== a5-a6: ladder, first feasible candidate in (m, k) order
-        int win = -1;
         for (int base = 0; base < items && win < 0; base += 32) {
             const int it = base + lane;
             bool ok = false;
@@ -315,6 +435,12 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
             const unsigned fm = __ballot_sync(FULL, ok);
             if (fm != 0u) win = base + __ffs(fm) - 1;
         }
+        if (win >= 0) {
+            const int k = win % KP;
+#pragma unroll
+            for (int e = 0; e < 9; ++e) Rw[e] = Rc[k * 9 + e];
+        }
+        }
 
         int m0 = 0, j_win = 0;
         if (win >= 0) {
@@ -327,7 +453,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
             t[1] = __dadd_rn(t[1], __dmul_rn(dT, vel[1]));
             t[2] = __dadd_rn(t[2], __dmul_rn(dT, vel[2]));
 #pragma unroll
-            for (int e = 0; e < 9; ++e) R[e] = Rc[k * 9 + e];
+            for (int e = 0; e < 9; ++e) R[e] = Rw[e];
             if (stats) stc[4] += 1;
         }
         moved = (m0 != 0);

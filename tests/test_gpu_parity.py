@@ -240,11 +240,13 @@ def test_parameter_edges_other_residuals(config, n_p, n_p_star, n_t):
     assert_parity(inst, P, I.make_init_poses(inst, 16), 100, 25, 5)
 
 
-@pytest.mark.parametrize("flags,theta_p,v0", [(0, 0.2, 2.0), (0, 0.05, 0.02), (4, 0.2, 0.05), (20, 0.05, 0.02), (0, 0.5, 0.02)])
+@pytest.mark.parametrize("flags,theta_p,v0", [(0, 0.2, 2.0), (0, 0.05, 0.02), (4, 0.2, 0.05), (20, 0.05, 0.02), (0, 0.5, 0.02),
+                                              (2, 0.05, 0.02), (0, 0.02, 0.005), (0, 0.2, 0.3)])
 def test_certified_translation_sampler_on_reprojection(flags, theta_p, v0):
     """Alg. A8 on the reprojection residual: eq. (14) runs in certified fp32 (series of Exp, error bound unc,
     fp64 re-ranking of near-ties).  Bit-identical to the plain fp64 kernel at the paper's theta_p = 0.2 and v0 = 2,
-    at small steps where walkers keep moving, with the fp64 ranking forced (4, 20), and beyond the range of the
+    at small steps where walkers keep moving, with the fp64 ranking forced (4, 20) or every ladder candidate sent
+    to fp64 (2), and beyond the range of the
     series (theta_p = 0.5: the fp64 evaluation takes over)."""
     inst = I.make_instance(3)
     P = _small(inst.params, mode=I.MODE_TRANS, v0=v0, theta_p=theta_p, flags=flags)
