@@ -77,6 +77,9 @@ typedef struct {
                         ranking is redone in fp64, 16 = ... on all N_P perturbations. */
 } closure_params;
 #define CLOSURE_FLAG_EXACT_ONLY 1
+#define CLOSURE_FLAG_PCA_VELOCITY 64 /* translation sampler: rescale the centre velocity by the relative spread of S_0's
+                                        translations along their principal axes, v <- sqrtm(Cov) / sqrt(lambda_max) v
+                                        (PAPER.md:324, 1074-1076); read by closure_set_init */
 #define CLOSURE_FLAG_HOST_MEGB 8    /* closure_megb: copy the cloud to the host and run the miniball there, whatever its size */
 
 typedef struct closure_s closure_t;   /* opaque; owns device copies of the instance and of S_0 */

@@ -30,7 +30,7 @@ _lib = None
 class _Params(ctypes.Structure):
     _fields_ = [("mode", c_int), ("n_p", c_int), ("n_p_star", c_int), ("n_t", c_int),
                 ("omega0", c_double), ("v0", c_double), ("gamma", c_double),
-                ("t_p", c_double), ("theta_p", c_double)]
+                ("t_p", c_double), ("theta_p", c_double), ("vel_scale", c_double * 9)]
 
 
 def build(force: bool = False) -> str:
@@ -135,6 +135,22 @@ def mean_pose(S0) -> tuple[np.ndarray, np.ndarray]:
     return U @ D @ Vt, S0[:, 9:].mean(axis=0)
 
 
+def pca_velocity_scale(S0) -> np.ndarray:
+    """S = sqrtm(Cov(S_t0)) / sqrt(lambda_max): the centre velocity is rescaled by the relative spread of the
+    initial translations along their principal axes ("rescale the center velocity based
+    on the expansion of S_t0 on 3 PCA weights"; R-23).  Identity for fewer than two poses or no spread."""
+    t = _f64(S0).reshape(-1, 12)[:, 9:]
+    if t.shape[0] < 2:
+        return np.eye(3)
+    d = t - t.mean(axis=0)
+    C = d.T @ d / t.shape[0]
+    lam, U = np.linalg.eigh(C)
+    lam = np.clip(lam, 0.0, None)
+    if not lam.max() > 0.0:
+        return np.eye(3)
+    return (U * np.sqrt(lam / lam.max())) @ U.T
+
+
 # ------------------------------------------------------------------ the walk
 
 def walk(inst, params, S0, walker_ids, n_steps: int, seed: int, *, trace: bool = False,
@@ -149,9 +165,11 @@ def walk(inst, params, S0, walker_ids, n_steps: int, seed: int, *, trace: bool =
     Rbar = _f64(Rbar, 9); tbar = _f64(tbar, 3)
     ids = np.ascontiguousarray(np.asarray(walker_ids, dtype=np.int64)).reshape(-1)
     W = ids.shape[0]
+    # flag 64 = CLOSURE_FLAG_PCA_VELOCITY: the PCA normalisation of the centre velocity (R-23)
+    scale = pca_velocity_scale(S0) if (int(getattr(params, "flags", 0)) & 64) else np.eye(3)
     P = _Params(int(params.mode), int(params.n_p), int(params.n_p_star), int(params.n_t),
                 float(params.omega0), float(params.v0), float(params.gamma),
-                float(params.t_p), float(params.theta_p))
+                float(params.t_p), float(params.theta_p), (c_double * 9)(*scale.reshape(9)))
     samples = np.zeros((W, 12))
     flags = np.zeros(W, dtype=np.uint8)
     tr = np.zeros((W, n_steps), dtype=np.int32) if trace else None

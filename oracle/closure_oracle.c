@@ -225,6 +225,7 @@ typedef struct {
     int mode;                 /* ORA_MODE_ROT: Alg. 2; ORA_MODE_TRANS: Alg. A8 */
     int n_p, n_p_star, n_t;   /* N_P, N_P*, N_T */
     double omega0, v0, gamma, t_p, theta_p;
+    double vel_scale[9];      /* PCA normalisation of the centre velocity (R-23); I if off */
 } ora_params;
 
 /* random unit vector from two uniforms (R-4): z = xi0, phi = pi (xi1 + 1). */
@@ -294,10 +295,15 @@ static void walk_one(int type, int n, const double *meas, const double *beta, co
     } else {
         double dvec[3] = { t[0] - tbar[0], t[1] - tbar[1], t[2] - tbar[2] };
         double nd = sqrt(dvec[0] * dvec[0] + dvec[1] * dvec[1] + dvec[2] * dvec[2]);
+        double v_raw[3];
         for (int r = 0; r < 3; ++r) {
             double dir = nd < 1e-12 ? 0.0 : dvec[r] / nd;   /* R-3 */
-            v[r] = P->v0 * (dir + rnd[r]);
+            v_raw[r] = P->v0 * (dir + rnd[r]);
         }
+        /* "additional normalization to the translation velocity according to the PCA analysis of S_0"
+         * (App. E): v <- S v, S = sqrtm(Cov(S_t0)) / sqrt(lambda_max) (R-23) */
+        for (int r = 0; r < 3; ++r)
+            v[r] = P->vel_scale[3 * r] * v_raw[0] + P->vel_scale[3 * r + 1] * v_raw[1] + P->vel_scale[3 * r + 2] * v_raw[2];
     }
 
     int hit = 0;

@@ -364,6 +364,11 @@ int closure_set_init(closure_t *h, const double *poses, int n0, double *mean_out
     h->h_desc.n0 = n0;
     std::memcpy(h->h_desc.Rbar, Rb, sizeof(Rb));
     std::memcpy(h->h_desc.tbar, tb, sizeof(tb));
+    if (h->P.flags & CLOSURE_FLAG_PCA_VELOCITY) {
+        pca_velocity_scale(poses, n0, h->h_desc.vscale);
+    } else {
+        for (int e = 0; e < 9; ++e) h->h_desc.vscale[e] = (e % 4 == 0) ? 1.0 : 0.0;
+    }
     e = cudaMemcpy(h->d_desc, &h->h_desc, sizeof(InstanceDesc), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return cuda_fail(h, e, "upload of instance descriptor");
     h->has_init = true;

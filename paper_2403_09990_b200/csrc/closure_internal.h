@@ -31,6 +31,7 @@ struct InstanceDesc {
     double Rbar[9];
     double tbar[3];
     double K[4];            // fx fy cx cy
+    double vscale[9];       // TRANS: v <- vscale v (PCA normalisation of the centre velocity, R-23); identity if off
 };
 
 constexpr int kMaxBatch = 96;
@@ -116,5 +117,7 @@ void device_megb_destroy(DeviceMegb *m);
 void rotation_to_quat(const double R[9], double q[4]);
 void quat_to_rotation(const double q[4], double R[9]);
 bool project_so3(const double M[9], double R[9]);   // nearest rotation to M (polar factor)
+// sqrtm(Cov(t_j)) / sqrt(lambda_max) of the translations of n0 poses (n0 x 12); identity if there is no spread
+void pca_velocity_scale(const double *poses, int n0, double S[9]);
 
 }  // namespace closure

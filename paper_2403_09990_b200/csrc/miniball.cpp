@@ -261,4 +261,55 @@ bool project_so3(const double M[9], double R[9])
     return true;
 }
 
+// PCA normalisation of the centre velocity (R-23): S = sqrtm(C) / sqrt(lambda_max),
+// C the covariance of the initial translations, by cyclic Jacobi rotations on the symmetric 3x3.
+void pca_velocity_scale(const double *poses, int n0, double S[9])
+{
+    for (int e = 0; e < 9; ++e) S[e] = (e % 4 == 0) ? 1.0 : 0.0;
+    if (n0 < 2) return;
+    double mean[3] = { 0, 0, 0 }, C[3][3] = { { 0 } };
+    for (int s = 0; s < n0; ++s)
+        for (int r = 0; r < 3; ++r) mean[r] += poses[(size_t)s * 12 + 9 + r];
+    for (int r = 0; r < 3; ++r) mean[r] /= (double)n0;
+    for (int s = 0; s < n0; ++s)
+        for (int r = 0; r < 3; ++r)
+            for (int c = 0; c < 3; ++c)
+                C[r][c] += (poses[(size_t)s * 12 + 9 + r] - mean[r]) * (poses[(size_t)s * 12 + 9 + c] - mean[c]);
+    for (int r = 0; r < 3; ++r)
+        for (int c = 0; c < 3; ++c) C[r][c] /= (double)n0;
+    double U[3][3] = { { 1, 0, 0 }, { 0, 1, 0 }, { 0, 0, 1 } };
+    for (int sweep = 0; sweep < 50; ++sweep) {
+        const double off = std::fabs(C[0][1]) + std::fabs(C[0][2]) + std::fabs(C[1][2]);
+        if (!(off > 1e-300) || off <= 1e-17 * (std::fabs(C[0][0]) + std::fabs(C[1][1]) + std::fabs(C[2][2]))) break;
+        for (int p = 0; p < 2; ++p)
+            for (int q = p + 1; q < 3; ++q) {
+                if (C[p][q] == 0.0) continue;
+                const double theta = (C[q][q] - C[p][p]) / (2.0 * C[p][q]);
+                const double tt = (theta >= 0.0 ? 1.0 : -1.0) / (std::fabs(theta) + std::sqrt(theta * theta + 1.0));
+                const double c = 1.0 / std::sqrt(tt * tt + 1.0), sn = tt * c;
+                for (int k = 0; k < 3; ++k) {                      // C <- C G
+                    const double ckp = C[k][p], ckq = C[k][q];
+                    C[k][p] = c * ckp - sn * ckq; C[k][q] = sn * ckp + c * ckq;
+                }
+                for (int k = 0; k < 3; ++k) {                      // C <- G^T C
+                    const double cpk = C[p][k], cqk = C[q][k];
+                    C[p][k] = c * cpk - sn * cqk; C[q][k] = sn * cpk + c * cqk;
+                }
+                for (int k = 0; k < 3; ++k) {                      // U <- U G
+                    const double ukp = U[k][p], ukq = U[k][q];
+                    U[k][p] = c * ukp - sn * ukq; U[k][q] = sn * ukp + c * ukq;
+                }
+            }
+    }
+    double lam[3] = { std::max(C[0][0], 0.0), std::max(C[1][1], 0.0), std::max(C[2][2], 0.0) };
+    const double lmax = std::max(lam[0], std::max(lam[1], lam[2]));
+    if (!(lmax > 0.0)) return;
+    for (int r = 0; r < 3; ++r)
+        for (int c = 0; c < 3; ++c) {
+            double v = 0.0;
+            for (int k = 0; k < 3; ++k) v += U[r][k] * std::sqrt(lam[k] / lmax) * U[c][k];
+            S[3 * r + c] = v;
+        }
+}
+
 }  // namespace closure

@@ -343,9 +343,13 @@ __device__ __forceinline__ void init_walker(const InstanceDesc *__restrict__ D, 
         const double d0 = t[0] - D->tbar[0], d1 = t[1] - D->tbar[1], d2 = t[2] - D->tbar[2];
         const double nd = sqrt(fma(d2, d2, fma(d1, d1, d0 * d0)));
         const bool far = !(nd < 1e-12);
-        vel[0] = L.v0 * ((far ? d0 / nd : 0.0) + r0);
-        vel[1] = L.v0 * ((far ? d1 / nd : 0.0) + r1);
-        vel[2] = L.v0 * ((far ? d2 / nd : 0.0) + r2);
+        const double w0 = L.v0 * ((far ? d0 / nd : 0.0) + r0);
+        const double w1 = L.v0 * ((far ? d1 / nd : 0.0) + r1);
+        const double w2 = L.v0 * ((far ? d2 / nd : 0.0) + r2);
+        // PCA normalisation (R-23): identity unless CLOSURE_FLAG_PCA_VELOCITY was set
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+            vel[r] = fma(D->vscale[3 * r + 2], w2, fma(D->vscale[3 * r + 1], w1, D->vscale[3 * r] * w0));
     }
 }
 

@@ -255,3 +255,20 @@ def test_certified_translation_sampler_on_reprojection(flags, theta_p, v0):
     b = gpu_walk(inst, _small(P, flags=1), S0, 4096, 100, 23)
     for x, y in zip(a, b):
         assert np.array_equal(x, y)
+
+
+@pytest.mark.parametrize("config,flags", [(3, 64), (3, 65), (1, 64)])
+def test_pca_normalised_centre_velocity(config, flags):
+    """CLOSURE_FLAG_PCA_VELOCITY (R-23): closure_set_init rescales the centre velocity by
+    sqrtm(Cov(S_t0)) / sqrt(lambda_max) (host Jacobi) -- against the oracle (numpy eigh), on the cooperative and on
+    the plain kernel, with an anisotropic S_0."""
+    inst = I.make_instance(config)
+    S0 = I.make_init_poses(inst, 64)
+    S0[:, 10] = inst.t_gt[1] + (S0[:, 10] - inst.t_gt[1]) * 0.1                  # squeeze the cloud along y
+    P = _small(inst.params, mode=I.MODE_TRANS, v0=0.05 if config == 3 else 0.1, theta_p=0.02, n_p=40, n_p_star=5,
+               n_t=10, flags=flags)
+    assert_parity(inst, P, S0, 200, 40, 7)
+    # the flag changes the walk
+    a = gpu_walk(inst, P, S0, 64, 10, 7)
+    b = gpu_walk(inst, _small(P, flags=flags & 1), S0, 64, 10, 7)
+    assert not np.array_equal(a[0], b[0])

@@ -324,3 +324,44 @@ def test_sampled_extent_agrees_with_dense_grid():
         assert res["trans_radius"] <= d_grid + h_t
     assert g["rot_radius"] >= 0.85 * D_grid               # each sampler on the set it targets
     assert gt["trans_radius"] >= 0.85 * d_grid
+
+
+# ------------------------------------------------------------------ PCA normalisation of the centre velocity (R-23)
+def test_pca_velocity_scale_closed_forms():
+    """S = sqrtm(Cov) / sqrt(lambda_max): exact on a cloud with a known covariance."""
+    from scipy.spatial.transform import Rotation
+    Q = Rotation.from_rotvec([0.3, -0.7, 0.2]).as_matrix()
+    sig = np.array([3.0, 1.0, 0.1])
+    # +-sigma_k along each principal axis: covariance Q diag(sigma^2) Q^T / 3 exactly
+    pts = np.concatenate([+sig[k] * Q[:, k][None, :] for k in range(3)] + [-sig[k] * Q[:, k][None, :] for k in range(3)])
+    S0 = np.zeros((6, 12)); S0[:, :9] = np.eye(3).reshape(9); S0[:, 9:] = pts + np.array([5.0, -2.0, 1.0])
+    S = oracle.pca_velocity_scale(S0)
+    assert np.allclose(S, Q @ np.diag(sig / sig.max()) @ Q.T, atol=1e-13)
+    assert np.allclose(S, S.T) and np.allclose(S @ Q[:, 0], Q[:, 0])            # longest axis kept, others shrunk
+    iso = S0.copy(); iso[:, 9:] = np.concatenate([np.eye(3), -np.eye(3)])
+    assert np.allclose(oracle.pca_velocity_scale(iso), np.eye(3), atol=1e-14)   # no anisotropy, no rescaling
+    assert np.array_equal(oracle.pca_velocity_scale(S0[:1]), np.eye(3))        # a single pose has no spread
+
+
+def test_pca_velocity_changes_only_the_direction_of_travel():
+    """Rotation frozen (theta_p = 0): the walker moves along its velocity; with the flag the displacement is
+    parallel to S times the unflagged displacement direction, and an isotropic S_0 changes nothing."""
+    import copy
+    inst = I.make_instance(1)
+    S0 = I.make_init_poses(inst, 32)
+    S0[:, 9] = inst.t_gt[0] + (S0[:, 9] - inst.t_gt[0]) * 0.05                  # squeeze the cloud along x
+    P = copy.copy(inst.params); P.mode = I.MODE_TRANS; P.theta_p = 0.0; P.v0 = 0.02; P.n_p = 4; P.n_p_star = 1; P.n_t = 12
+    Pf = copy.copy(P); Pf.flags = 64
+    ids = np.arange(40)
+    a, _ = oracle.walk(inst, P, S0, ids, 1, 3)
+    b, _ = oracle.walk(inst, Pf, S0, ids, 1, 3)
+    S = oracle.pca_velocity_scale(S0)
+    assert S[0, 0] < 0.5                                                         # x is the thin direction
+    moved = 0
+    for w in ids:
+        t0 = S0[w % 32, 9:]
+        da, db = a[w, 9:] - t0, b[w, 9:] - t0
+        if np.linalg.norm(da) > 1e-6 and np.linalg.norm(db) > 1e-6:
+            moved += 1
+            assert np.linalg.norm(np.cross(S @ da, db)) <= 1e-9 * np.linalg.norm(S @ da) * np.linalg.norm(db)
+    assert moved > 10
