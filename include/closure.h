@@ -200,10 +200,10 @@ typedef struct {
     unsigned long long ladder_setups;   /* per-(rung, constraint) set-ups, a5 */
     unsigned long long accepted_steps;  /* iterations that moved the walker */
     unsigned long long walker_steps;    /* walkers x iterations */
-    unsigned long long perturb_pairs_f32; /* pairs evaluated in fp32 by the screening pass, a3 */
-    unsigned long long ladder_pairs_f32;  /* pairs evaluated in fp32 by the lenient ladder pass, a5 */
-    unsigned long long fallback_steps;  /* iterations whose candidate list could not be proven complete */
-    unsigned long long verified_rungs;  /* ladder rungs re-run in fp64 */
+    unsigned long long perturb_pairs_f32; /* pairs evaluated in certified fp32, a3 */
+    unsigned long long ladder_pairs_f32;  /* pairs evaluated in certified fp32 (rung screening + full rungs), a5 */
+    unsigned long long fallback_steps;  /* iterations whose fp32 ranking was not certified (fp64 re-ranking) */
+    unsigned long long verified_rungs;  /* ladder rungs evaluated in full (ROT) / candidates sent to fp64 (TRANS) */
 } closure_stats;
 int closure_enable_stats(closure_t *h, int on);
 int closure_get_stats(closure_t *h, closure_stats *out);
