@@ -161,20 +161,24 @@ __device__ __forceinline__ bool topk_certified(const float (&v)[NQ], int n_ps, f
             key[a] = hi; key[a + 1] = lo;
         }
     uint32_t myg = fkey(-CUDART_INF_F);
-    int mysrc = 0;
+    unsigned mywho = 1u;
     for (int r = 0; r <= n_ps; ++r) {               // extract the N_P* + 1 largest
+        // every lane whose head equals the maximum pops it: the next reduction waits for one compare only.
+        // Two lanes popping together (equal keys) is a tie: detected below, never certified, and the values
+        // reported from then on are not larger than the true ones, which keeps the fall-back's threshold valid.
         const uint32_t g = __reduce_max_sync(FULL, key[0]);
-        const unsigned who = __ballot_sync(FULL, key[0] == g);
-        const int src = __ffs(who) - 1;
-        if (lane == r) { myg = g; mysrc = src; }
-        if (lane == src) {
+        const bool pop = key[0] == g;
+        const unsigned who = __ballot_sync(FULL, pop);
+        if (lane == r) { myg = g; mywho = who; }
+        if (pop) {
 #pragma unroll
             for (int q = 0; q + 1 < NQ; ++q) key[q] = key[q + 1];
             key[NQ - 1] = 0u;
         }
     }
     myval = fkey_inv(myg);
-    const int myj = mysrc + 32 * (int)(myg & 7u);
+    const int myj = (__ffs(mywho) - 1) + 32 * (int)(myg & 7u);
+    const bool tie = (lane <= n_ps) && ((mywho & (mywho - 1u)) != 0u) && (myval > -CUDART_INF_F);   // empty slots all look alike
     const float prev = __shfl_up_sync(FULL, myval, 1);
     bool ok = true;
     if (lane < n_ps) ok = (myval > -CUDART_INF_F) && (myval < CUDART_INF_F);
@@ -183,6 +187,7 @@ __device__ __forceinline__ bool topk_certified(const float (&v)[NQ], int n_ps, f
         const float need = fmaf(2.0f, unc, kMu19 * (fabsf(prev) + fabsf(myval)));
         ok = ok && (none_left || (prev - myval > need));
     }
+    if (tie) ok = false;
     if (trust) ok = true;                       // fp32 mode: the fp32 ranking is taken as it is
     if (force_fail) ok = false;
     const bool certified = __all_sync(FULL, ok);
