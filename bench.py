@@ -312,11 +312,11 @@ def run_cuda(args) -> None:
         e2e_dt = time.perf_counter() - t0
         h2d = sum(it.measurements.nbytes + it.betas.nbytes + s0.nbytes + 256 for it, s0 in zip(insts, S0s))
 
-        # Step I on the device (SURVEY.md 8(f) NEXT-2; not part of the timed step): trials -> compaction -> S_0 for
+        # Step I on the device (SURVEY.md 8(f) NEXT-2 / NEXT-3; not part of the timed step): trials -> compaction -> S_0 for
         # 1,000 trials end to end, and the trial kernel alone at the 100,000 trials of the paper's pure-RANSAG
-        # comparison.  Ex.1 needs a P3P solver (not built).
+        # comparison.  Ex.1: P3P trials; Ex.2: Arun; Ex.3: convex combinations.
         step1 = None
-        if inst.residual_type != 1:
+        if True:
             hs1 = B.Closure.closure_create(insts[0])
             t_s1 = []
             for k in range(12):

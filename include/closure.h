@@ -107,13 +107,18 @@ int closure_set_params(closure_t *h, const closure_params *p);
  * mean_out (host, 12 doubles, may be NULL) receives [R_bar, t_bar]. */
 int closure_set_init(closure_t *h, const double *poses, int n0, double *mean_out);
 
-/* Step I for Ex.2 and Ex.3: independent trials on the device.
+/* Step I: independent trials on the device.
  *   CLOSURE_REG_3D3D               RANSAG trial: 3 distinct random correspondences, Arun's least-squares rigid
  *                                  fit, kept iff the pose satisfies the PURSE
  *   CLOSURE_POSE_REG / _SPLIT      a random convex combination of the hypotheses (rotation = proj_SO(3) of the
  *                                  weighted sum), kept iff it satisfies the PURSE
- *   CLOSURE_REPROJ_2D3D            CLOSURE_EUNSUPPORTED (needs a P3P solver)
- * Trial k = trial_begin + q draws from Philox4x32-10 keyed by (seed; k) (R-21, R-22), so any trial can
+ *   CLOSURE_REPROJ_2D3D            RANSAG trial: 3 distinct random constraints, a random 2D point inside each
+ *                                  (uniform in the disc of radius beta_i around z_i), the perspective-3-point
+ *                                  problem for the three rays; its (up to four) poses are tried in ascending
+ *                                  order of the first depth and the first one that satisfies the PURSE is kept
+ *                                  (R-24)
+ * CLOSURE_EINVAL if a RANSAG residual has fewer than 3 constraints.
+ * Trial k = trial_begin + q draws from Philox4x32-10 keyed by (seed; k) (R-21, R-22, R-24), so any trial can
  * be replayed alone.  ASYNC.
  *   out_poses  DEVICE, num_trials x 12 doubles: the candidate (R row-major, t), zeros where rejected
  *   out_ok     DEVICE, num_trials bytes: 1 iff the candidate is inside the PURSE

@@ -93,14 +93,77 @@ def test_init_from_trials_feeds_the_walk():
         h.closure_destroy()
 
 
-def test_step1_errors():
-    h = B.Closure.closure_create(I.make_instance(3))
+def _compare_p3p(inst, T, seed, begin=0):
+    """Ex.1 (R-24).  The oracle takes the roots of the quartic from numpy's companion-matrix
+    eigenvalues, the kernel isolates them by bisection; both polish the depths by Newton on the distance
+    equations, so well-conditioned trials agree to ~1e-12.  A trial the oracle flags as ill-conditioned (nearly
+    double root, nearly singular Jacobian: the SET of solutions is not stable under rounding) is not compared;
+    an accept decision may differ only where some candidate's oracle margin is below 1e-9."""
+    g_poses, g_ok = _gpu_trials(inst, T, seed, begin)
+    o_poses, o_ok = step1.init_sample(inst, T, seed, trial_begin=begin)
+    skipped = near = 0
+    for q in range(T):
+        sols, ill, _ = step1.p3p_trial(inst, seed, begin + q)
+        if ill:
+            skipped += 1
+            continue
+        if g_ok[q] != o_ok[q]:
+            ms = [abs(oracle.margin(inst, R.reshape(9), t)) for _, R, t in sols]
+            assert ms and min(ms) < 1e-9, f"trial {begin + q}: accept decision differs, oracle margins {ms}"
+            near += 1
+            continue
+        if o_ok[q]:
+            err = np.abs(g_poses[q] - o_poses[q])
+            assert np.all(err <= 1e-9 * np.abs(o_poses[q]) + 1e-11), f"trial {begin + q}: pose differs by {err.max():.2e}"
+        else:
+            assert np.all(g_poses[q] == 0.0)
+    assert skipped <= max(2, T // 50), f"{skipped} of {T} trials ill-conditioned"
+    assert near <= max(1, T // 200)
+    return g_ok
+
+
+def test_p3p_trials_match_oracle():
+    inst = I.make_instance(3)
+    ok = _compare_p3p(inst, 3000, 11)
+    assert ok.mean() > 0.02                                       # ~5 % of the trials land inside the PURSE
+    for T in (1, 127, 129):
+        _compare_p3p(inst, T, 2)
+    _compare_p3p(inst, 64, 9, begin=(1 << 32) + 7)               # high counter word
+    full = _gpu_trials(inst, 400, 9)
+    part = _gpu_trials(inst, 100, 9, begin=150)
+    assert np.array_equal(full[0][150:250], part[0]) and np.array_equal(full[1][150:250], part[1])
+
+
+def test_p3p_candidates_reproject_onto_the_sampled_pixels_and_feed_the_walk():
+    """Property at any size: an accepted pose maps the three selected 3D points onto the three sampled pixels
+    (each within its own ellipse), and satisfies every constraint of the instance."""
+    import torch
+    inst = I.make_instance(3)
+    T, seed = 20000, 5
+    poses, ok = _gpu_trials(inst, T, seed)
+    meas, K = np.asarray(inst.measurements), np.asarray(inst.intrinsics).reshape(4)
+    acc = np.nonzero(ok)[0]
+    assert acc.size > 400
+    for q in acc[:300]:
+        R, t = poses[q, :9].reshape(3, 3), poses[q, 9:]
+        assert oracle.margin(inst, poses[q, :9], t) >= -1e-9
+        _, _, (idx, ys) = step1.p3p_trial(inst, seed, int(q))
+        for i, y in zip(idx, ys):
+            pc = R @ meas[i, 2:5] + t
+            px = np.array([K[0] * pc[0] / pc[2] + K[2], K[1] * pc[1] / pc[2] + K[3]])
+            assert np.abs(px - np.array(y)).max() < 1e-7
+    h = B.Closure.closure_create(inst)
     try:
-        with pytest.raises(B.ClosureError) as e:
-            h.closure_init_sample(10, 1)
-        assert e.value.status == B.EUNSUPPORTED
+        n0 = h.closure_init_from_trials(4000, 21, max_poses=100)
+        assert n0 == 100
+        res = h.closure_run(4096, 60, 3)
+        assert res["count"] > 3500 and res["rot_radius"] > 0 and res["trans_radius"] > 0
+        torch.cuda.synchronize()
     finally:
         h.closure_destroy()
+
+
+def test_step1_errors():
     h = B.Closure.closure_create(I.make_custom_reg(2, 5))
     try:
         with pytest.raises(B.ClosureError) as e:

@@ -1,5 +1,6 @@
-"""Pins of the Step I oracle (oracle/step1.py): Arun's method, the RANSAG triplets and the convex-combination
-sampler, against closed forms, a library routine and brute-force perturbation -- not against itself."""
+"""Pins of the Step I oracle (oracle/step1.py): Arun's method, the RANSAG triplets, the convex-combination
+sampler and the P3P solver, against closed forms, a library routine, brute-force perturbation and a brute-force
+scan of the P3P distance equations -- not against itself."""
 import numpy as np
 import pytest
 from scipy.spatial.transform import Rotation
@@ -89,7 +90,7 @@ def test_convex_weights_and_pose():
     assert np.allclose(R.reshape(9), meas[3, :9], atol=1e-12) and np.allclose(t, meas[3, 9:12])
 
 
-@pytest.mark.parametrize("config", [1, 2, 4, 5])
+@pytest.mark.parametrize("config", [1, 2, 3, 4, 5])
 def test_init_sample_yields_poses_inside_the_purse(config):
     inst = I.make_instance(config)
     poses, ok = step1.init_sample(inst, 300, 11)
@@ -105,10 +106,136 @@ def test_init_sample_yields_poses_inside_the_purse(config):
     assert np.abs(poses[ok == 1][:, 9:] - inst.t_gt).max() < 0.5
 
 
-def test_split_form_and_unsupported_residual():
+def test_split_form():
     sp = I.to_split(I.make_instance(4))
     poses, ok = step1.init_sample(sp, 100, 3)
     for q in np.nonzero(ok)[0]:
         assert oracle.in_purse(sp, poses[q, :9], poses[q, 9:])
-    with pytest.raises(ValueError):
-        step1.init_sample(I.make_instance(3), 4, 1)
+
+
+# ---------------------------------------------------------------------------------------------- P3P (Ex.1, R-24)
+
+def _p3p_problem(rng, depth=(3.0, 8.0), size=1.0):
+    R = _rand_rot(rng)
+    t = np.array([rng.uniform(-1, 1), rng.uniform(-1, 1), rng.uniform(*depth)])
+    X = rng.uniform(-size, size, (3, 3))
+    b = X @ R.T + t
+    return R, t, X, b / np.linalg.norm(b, axis=1)[:, None]
+
+
+def test_p3p_recovers_the_generating_pose_and_every_solution_is_exact():
+    """Exact data: the generating pose is one of the solutions; every solution is a rotation, has positive depths
+    and maps X_l onto the ray f_l at depth d_l ("the perspective-3-point (P3P) minimal solver")."""
+    rng = np.random.default_rng(0)
+    multi = 0
+    for it in range(300):
+        R, t, X, f = _p3p_problem(rng)
+        sols, ill = step1.p3p(f, X)
+        if ill:
+            continue
+        assert 1 <= len(sols) <= 4
+        multi += len(sols) > 1
+        assert min(np.abs(Rs - R).max() + np.abs(ts - t).max() for _, Rs, ts in sols) < 1e-8
+        assert all(a[0][0] <= b[0][0] for a, b in zip(sols, sols[1:]))           # ascending d_1
+        for d, Rs, ts in sols:
+            assert np.all(d > 0)
+            assert np.allclose(Rs @ Rs.T, np.eye(3), atol=1e-10) and np.linalg.det(Rs) > 0
+            assert np.abs(X @ Rs.T + ts - d[:, None] * f).max() < 1e-8
+    assert multi > 50                                            # the two- and four-solution cases are exercised
+
+
+def _p3p_brute_force_d1(f, X, d_max, grid=40001):
+    """Every d_1 in (0, d_max) that solves the three law-of-cosines equations, found without any elimination:
+    for a trial d_1, (1) and (2) are quadratics in d_2 and d_3 (two branches each); the residual of (3) along each
+    of the four branch pairs changes sign at a solution."""
+    c12, c13, c23 = f[0] @ f[1], f[0] @ f[2], f[1] @ f[2]
+    a12, a13, a23 = ((X[0] - X[1]) ** 2).sum(), ((X[0] - X[2]) ** 2).sum(), ((X[1] - X[2]) ** 2).sum()
+
+    def resid(d1, s2, s3):
+        with np.errstate(invalid="ignore"):
+            d2 = c12 * d1 + s2 * np.sqrt(a12 - (1 - c12 * c12) * d1 * d1)
+            d3 = c13 * d1 + s3 * np.sqrt(a13 - (1 - c13 * c13) * d1 * d1)
+            h = d2 * d2 + d3 * d3 - 2 * c23 * d2 * d3 - a23
+        return np.where((d2 > 0) & (d3 > 0), h, np.nan)
+    found = []
+    g = np.linspace(0.0, d_max, grid)[1:]
+    for s2 in (-1.0, 1.0):
+        for s3 in (-1.0, 1.0):
+            h = resid(g, s2, s3)
+            for i in np.nonzero(np.isfinite(h[:-1]) & np.isfinite(h[1:]) & (np.sign(h[:-1]) != np.sign(h[1:])))[0]:
+                lo, hi = g[i], g[i + 1]
+                for _ in range(60):
+                    mid = 0.5 * (lo + hi)
+                    if np.sign(resid(np.array([mid]), s2, s3)[0]) == np.sign(resid(np.array([lo]), s2, s3)[0]):
+                        lo = mid
+                    else:
+                        hi = mid
+                found.append(0.5 * (lo + hi))
+    return sorted(found)
+
+
+def test_p3p_is_complete_against_a_brute_force_scan_of_the_distance_equations():
+    rng = np.random.default_rng(3)
+    checked = 0
+    for it in range(40):
+        R, t, X, f = _p3p_problem(rng, depth=(2.0, 5.0))
+        sols, ill = step1.p3p(f, X)
+        if ill:
+            continue
+        mine = [d[0] for d, _, _ in sols]
+        brute = _p3p_brute_force_d1(f, X, 20.0)
+        for d1 in brute:                                          # nothing the scan finds is missing
+            assert min(abs(d1 - m) for m in mine) < 1e-6, (it, brute, mine)
+        for m in mine:                                            # and nothing spurious (up to branch end points)
+            near_end = any(abs(m * m * (1 - c * c) - a) < 1e-3 * a for c, a in
+                           ((f[0] @ f[1], ((X[0] - X[1]) ** 2).sum()), (f[0] @ f[2], ((X[0] - X[2]) ** 2).sum())))
+            assert near_end or min(abs(m - d1) for d1 in brute) < 1e-6, (it, brute, mine)
+        checked += 1
+    assert checked >= 30
+
+
+def test_p3p_quartic_on_the_danger_cylinder():
+    """Equilateral triangle of side a seen from height h on its axis: d_1 = d_2 = d_3 = sqrt(h^2 + a^2/3), i.e.
+    u = v = 1, and the camera centre lies on the cylinder through the three points (axis normal to their plane),
+    where the P3P solution is a double one: G(1) = G'(1) = 0, and the oracle flags the trial."""
+    P = np.polynomial.polynomial
+    a, h = 1.0, 4.0
+    X = np.array([[a / np.sqrt(3), 0, 0], [-a / (2 * np.sqrt(3)), a / 2, 0], [-a / (2 * np.sqrt(3)), -a / 2, 0]])
+    b = X + np.array([0, 0, h])
+    f = b / np.linalg.norm(b, axis=1)[:, None]
+    G, p, q, _, (a12, a13, a23) = step1.p3p_quartic(f, X)
+    scale = np.abs(G).sum()
+    assert abs(P.polyval(1.0, G)) < 1e-12 * scale and abs(P.polyval(1.0, P.polyder(G))) < 1e-12 * scale
+    assert abs(P.polyval(1.0, p)) < 1e-12 and abs(P.polyval(1.0, q)) < 1e-12      # u = p/q is 0/0 there: flagged
+    assert abs(np.sqrt(a13 / (2.0 - 2.0 * f[0] @ f[2])) - np.sqrt(h * h + a * a / 3)) < 1e-12     # d_1 from eq. (2)
+    assert step1.p3p(f, X)[1] is True
+    # off the axis the same triangle is a regular case again
+    b = X + np.array([0.3, -0.2, h])
+    f = b / np.linalg.norm(b, axis=1)[:, None]
+    sols, ill = step1.p3p(f, X)
+    assert not ill and any(np.abs(R - np.eye(3)).max() < 1e-9 and np.abs(t - [0.3, -0.2, h]).max() < 1e-9 for _, R, t in sols)
+
+
+def test_disc_points_and_p3p_trials_on_config_3():
+    inst = I.make_instance(3)
+    meas, betas, K = np.asarray(inst.measurements), np.asarray(inst.betas).reshape(-1), np.asarray(inst.intrinsics).reshape(4)
+    pts = np.array([step1.disc_point(7, k, l) for k in range(1500) for l in range(3)])
+    r2 = (pts ** 2).sum(axis=1)
+    assert r2.max() <= 1.0
+    assert abs(r2.mean() - 0.5) < 0.02                            # uniform in the disc: E r^2 = 1/2
+    assert np.abs(pts.mean(axis=0)).max() < 0.03
+    assert abs((r2 < 0.25).mean() - 0.25) < 0.02                  # P(r < 1/2) = 1/4
+    assert step1.disc_point(7, 3, 1) == step1.disc_point(7, 3, 1) != step1.disc_point(7, 3, 2)
+    n_sol = 0
+    for k in range(200):
+        sols, ill, (idx, ys) = step1.p3p_trial(inst, 7, k)
+        assert len(set(idx)) == 3
+        for i, y in zip(idx, ys):                                 # "a 2D point in each constraint"
+            assert np.hypot(y[0] - meas[i, 0], y[1] - meas[i, 1]) <= betas[i] * (1 + 1e-12)
+        for d, R, t in sols:                                      # the pose projects Z_l exactly onto y_l
+            n_sol += 1
+            for i, y in zip(idx, ys):
+                pc = R @ meas[i, 2:5] + t
+                px = np.array([K[0] * pc[0] / pc[2] + K[2], K[1] * pc[1] / pc[2] + K[3]])
+                assert pc[2] > 0 and np.abs(px - np.array(y)).max() < 1e-7
+    assert n_sol > 200
