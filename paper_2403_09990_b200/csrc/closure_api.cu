@@ -25,6 +25,7 @@ struct closure_s {
     std::vector<double> betas;
     double K[4] = { 0, 0, 0, 0 };
     InstanceDesc h_desc{};
+    int n_pairs = 0;                 // pair-entries of the cooperative kernel's fp32 table: sum over runs of equal bound of ceil(len / 2)
     double *d_rows = nullptr;
     int *d_perm = nullptr;
     InstanceDesc *d_desc = nullptr;
@@ -195,6 +196,7 @@ void fill_launch(const closure_t *h, WalkLaunch &L)
     std::memset(&L, 0, sizeof(L));
     L.n_p = h->P.n_p; L.n_p_star = h->P.n_p_star; L.n_t = h->P.n_t;
     L.omega0 = h->P.omega0; L.v0 = h->P.v0; L.gamma = h->P.gamma; L.t_p = h->P.t_p; L.theta_p = h->P.theta_p;
+    L.pairs_cap = h->n_pairs;
     L.exact_only = (h->P.flags & 31) | (h->P.precision == 32 ? 32 : 0);           // bit 0 documented; bits 1-2: debug switches of the screened kernel
 }
 
@@ -305,6 +307,10 @@ int closure_create(int residual_type, const double *measurements, int n, const d
             r[12] = betas[2 * i]; r[13] = betas[2 * i] * betas[2 * i];
             r[14] = betas[2 * i + 1]; r[15] = betas[2 * i + 1] * betas[2 * i + 1];
         }
+    }
+    for (int k = 0, len = 0; k < n; ++k) {                 // runs of equal bound in sorted order
+        ++len;
+        if (k == n - 1 || key(order[k + 1]) != key(order[k])) { h->n_pairs += (len + 1) / 2; len = 0; }
     }
     const size_t bytes = rows.size() * sizeof(double);     // row is 8 or 16 doubles: multiple of 16 B
     std::vector<int> perm(n);
@@ -497,6 +503,7 @@ int closure_sample_batch(closure_t *const *handles, int n_instances, long long w
             L.desc[b] = handles[b0 + b]->d_desc;
             L.seed[b] = seeds[b0 + b];
             max_bytes = std::max(max_bytes, handles[b0 + b]->h_desc.rows_bytes);
+            L.pairs_cap = std::max(L.pairs_cap, handles[b0 + b]->n_pairs);
         }
         L.walker_begin = 0;
         L.num_walkers = walkers_per_instance;

@@ -52,6 +52,7 @@ struct WalkLaunch {
     unsigned char *out_flags;
     int *out_trace;                           // nullable
     unsigned long long *stats;                // nullable, kNumStats counters
+    int pairs_cap;                            // affine cooperative kernel: 32-byte entries of rowsA (max over the batch)
     int exact_only;                           // bit 0: plain fp64 kernel everywhere; bits 1, 2, 4: debug switches of walker_coop_kernel
 };
 

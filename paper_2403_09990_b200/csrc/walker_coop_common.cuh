@@ -22,8 +22,9 @@ struct CoopSmem {
     size_t run_end, run_bf, run_pend, pos, warp0, per_warp, rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, cand4, candj, candd, pose, stc, total;
 };
 
-// Shared-memory layout; f4 = float4 words per fp32 constraint row (1: affine residuals, 2: reprojection)
-__host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, int nq, int f4)
+// Shared-memory layout; f4 = float4 words per fp32 constraint row (1: affine residuals, 2: reprojection);
+// pairs = 32-byte entries of rowsA (affine: pair-entries, runs padded to even length; otherwise n)
+__host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, int nq, int f4, int pairs)
 {
     CoopSmem s;
     size_t o = 16 + (size_t)((rows_bytes + 15) & ~15);
@@ -33,7 +34,7 @@ __host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, 
     s.pos = o;     o += (size_t)((n * 4 + 15) & ~15);
     s.warp0 = o;
     size_t w = 0;
-    s.rowsA = w; w += (size_t)n * 32;              // affine: pair-transposed, runs padded to even length
+    s.rowsA = w; w += (size_t)pairs * 32;          // affine: pair-transposed, runs padded to even length
     s.rowsL = w; w += (size_t)n * 16 * f4;
     s.pert = w;  w += (size_t)nq * 32 * 16;
     s.ab = w;    w += (size_t)n_t * 16;

@@ -140,11 +140,11 @@ __device__ __forceinline__ bool exact_candidate_feasible(const double (&Rm)[9], 
 // its registers do not count against the per-iteration code.  Results epsA, rot_margin -> pose[16], pose[15].
 template <int RES>
 __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int warp, int lane, int rows_bytes, int n,
-                                                int n_t, int nq, double t_p, bool stats)
+                                                int n_t, int nq, int pairs, double t_p, bool stats)
 {
     using RS = Res<RES>;
     constexpr int ROW = RS::ROW;
-    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, nq, 1);
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, nq, 1, pairs);
     const double *rows = reinterpret_cast<const double *>(smem_raw + 16);
     const int *pos = reinterpret_cast<const int *>(smem_raw + lay.pos);
     unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
@@ -247,6 +247,47 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
     __syncwarp();
 }
 
+// ---------------------------------------------------------------------------------- eq. (14), constraint-major
+// For N_P <= 32 (one perturbation per lane) the perturbation-major loop below leaves lanes idle and issues two
+// shared-memory loads for three FFMA2.  Here the roles are swapped for one run of equal bounds: every lane keeps
+// up to PE pair-entries of the run in registers, the perturbations are broadcast from pert[] one by one, and
+// the maximum over the constraints is a warp reduction; lane j keeps the result of perturbation j.  Same
+// products, same chain order, and a maximum does not depend on the order: bit-identical to the other loop.
+template <int PE>
+__device__ __forceinline__ uint32_t eq14_constraint_major(const float4 *rowsA, const float4 *pert, int p0, int pend,
+                                                          int n_p, int lane)
+{
+    unsigned long long A0[PE], A1[PE], A2[PE], A3[PE];       // (f0a f0b) (f1a f1b) (f2a f2b) (fca fcb)
+#pragma unroll
+    for (int k = 0; k < PE; ++k) {
+        const int e = p0 + lane + 32 * k;
+        if (e < pend) {
+            const float4 X = rowsA[2 * e], Y = rowsA[2 * e + 1];
+            A0[k] = pk2(X.x, X.y); A1[k] = pk2(X.z, X.w); A2[k] = pk2(Y.x, Y.y); A3[k] = pk2(Y.z, Y.w);
+        } else {
+            A0[k] = A1[k] = A2[k] = pk2(0.f, 0.f);
+            A3[k] = pk2(-CUDART_INF_F, -CUDART_INF_F);
+        }
+    }
+    uint32_t mine = fkey(-CUDART_INF_F);
+#pragma unroll 4
+    for (int j = 0; j < n_p; ++j) {
+        const float4 pj = pert[j];
+        float m = -CUDART_INF_F;
+#pragma unroll
+        for (int k = 0; k < PE; ++k) {
+            const unsigned long long vo =
+                fma2(A0[k], pk2(pj.x, pj.x), fma2(A1[k], pk2(pj.y, pj.y), fma2(A2[k], pk2(pj.z, pj.z), A3[k])));
+            float lo, hi;
+            upk2(vo, lo, hi);
+            m = fmaxf(m, fmaxf(lo, hi));
+        }
+        const uint32_t g = __reduce_max_sync(FULL, fkey(m));
+        if (lane == j) mine = g;
+    }
+    return mine;
+}
+
 // ---------------------------------------------------------------------------------- the kernel
 template <int RES, int NQ>
 __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __grid_constant__ WalkLaunch L)
@@ -257,7 +298,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     constexpr bool ODD = (NQ & 1) != 0;    // plus one scalar slot
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ int n_runs_s;
+    __shared__ int n_runs_s, cmajor_s;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const InstanceDesc *__restrict__ D = L.desc[blockIdx.y];
     const int n = D->n;
@@ -266,7 +307,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
     double *rows = reinterpret_cast<double *>(smem_raw + 16);
     stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
-    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 1);
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 1, L.pairs_cap);
     int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
     float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
     int *run_pend = reinterpret_cast<int *>(smem_raw + lay.run_pend);   // end of run r in rowsA, in PAIRS of rows
@@ -294,18 +335,24 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
             // rowsA holds the fp32 set-ups two constraints per entry; a run of odd length repeats its last
             // constraint (a maximum does not see duplicates), so no pair straddles two bounds
             n_runs_s = cnt;
-            int p = 0, start = 0;
+            int p = 0, start = 0, longest = 0;
             for (int r = 0; r < cnt; ++r) {
                 const int end = run_end[r];
+                const int p_begin = p >> 1;
                 for (int i = start; i <= end; ++i) pos[i] = p++;
                 if (p & 1) { pos[end] |= 0x40000000; ++p; }
                 run_pend[r] = p >> 1;
+                longest = max(longest, (p >> 1) - p_begin);
                 start = end + 1;
             }
+            // constraint-major eq. (14): one perturbation per lane, enough pair-entries to fill the lanes,
+            // every run fits the registers of one pass (4 pair-entries per lane)
+            cmajor_s = (NQ == 1 && (p >> 1) >= 64 && longest <= 128) ? 1 : 0;
         }
     }
     __syncthreads();
     const int n_runs = n_runs_s;
+    const bool cmajor = NQ == 1 && cmajor_s != 0;
 
     const long long local = (long long)blockIdx.x * kCoopWarps + warp;
     if (local >= L.num_walkers) return;                // no block-wide barrier below this line
@@ -381,7 +428,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
     for (int s = 1; s <= L.num_steps; ++s) {
         // ================================================== set-up at the current pose (only after a move)
         if (moved) {
-            coop_setup_on_move<RES>(smem_raw, warp, lane, rows_bytes, n, n_t, NQ, t_p, stats);
+            coop_setup_on_move<RES>(smem_raw, warp, lane, rows_bytes, n, n_t, NQ, L.pairs_cap, t_p, stats);
             epsA = (float)pose[16];
             rot_margin = pose[15];
             full_m = -1;
@@ -435,6 +482,18 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
                 float mx[NQ];
 #pragma unroll
                 for (int q = 0; q < NQ; ++q) mx[q] = -CUDART_INF_F;
+                if (NQ == 1 && cmajor) {
+                    __syncwarp();                        // pert[] of this iteration is complete
+                    const int len = pend - pp;
+                    uint32_t key;
+                    if (len <= 32) key = eq14_constraint_major<1>(rowsA, pert, pp, pend, n_p, lane);
+                    else if (len <= 64) key = eq14_constraint_major<2>(rowsA, pert, pp, pend, n_p, lane);
+                    else if (len <= 96) key = eq14_constraint_major<3>(rowsA, pert, pp, pend, n_p, lane);
+                    else key = eq14_constraint_major<4>(rowsA, pert, pp, pend, n_p, lane);
+                    // lanes without a perturbation: any finite value (their d is masked below; -inf would blow up unc)
+                    mx[0] = lane < n_p ? fkey_inv(key) : 1.0f;
+                    pp = pend;
+                }
 #pragma unroll(NQ <= 2 ? 4 : 2)
                 for (; pp < pend; ++pp) {
                     // two constraints a, b per entry: X = (f0a f0b f1a f1b), Y = (f2a f2b fca fcb)
@@ -639,7 +698,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
 template <int RES, int NQ>
 cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
 {
-    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 1);
+    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 1, L.pairs_cap);
     if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaFuncSetAttribute(walker_coop_kernel<RES, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)lay.total);

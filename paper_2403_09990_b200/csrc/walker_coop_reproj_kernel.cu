@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
     double *rows = reinterpret_cast<double *>(smem_raw + 16);
     stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
-    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 2);
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 2, n);
     int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
     float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
     if (warp == 0) {                                   // runs of equal bounds (rows are sorted by bound)
@@ -524,7 +524,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(con
 template <int NQ>
 cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
 {
-    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 2);
+    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 2, max_n);
     if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaFuncSetAttribute(walker_coop_reproj_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)lay.total);
