@@ -9,6 +9,7 @@ import copy
 import numpy as np
 import pytest
 
+from paper_2403_09990_b200 import binding as B
 from paper_2403_09990_b200 import instances as I
 from tests.gpu_common import assert_parity, gpu_walk
 
@@ -81,6 +82,51 @@ def test_constraint_count_edges(n, distinct):
     inst = I.make_custom_reg(n, 100 + n, distinct_betas=distinct)
     P = _small(inst.params, n_p=30, n_p_star=4, n_t=8, t_p=0.05)
     assert_parity(inst, P, I.make_init_poses(inst, 8), 96, 20, 9)
+
+
+def _three_bounds(n, seed, counts):
+    inst = I.make_custom_reg(n, seed)
+    scale = np.concatenate([np.full(c, f) for c, f in zip(counts, (1.0, 1.25, 1.6))])
+    inst.betas = inst.betas * np.random.default_rng(seed).permutation(scale)
+    return inst
+
+
+@pytest.mark.parametrize("n,counts,n_p", [(200, (51, 67, 82), 24), (200, None, 20), (300, (1, 290, 9), 32), (130, (129, 1, 0), 9)])
+def test_constraint_major_loop_with_several_runs(n, counts, n_p):
+    """N_P <= 32 with a long table: the constraint-major eq. (14) loop, on runs of odd length, a run longer than 128
+    pair-entries (the perturbation-major loop takes over), runs of one constraint, and every bound different."""
+    inst = _three_bounds(n, 300 + n, counts) if counts else I.make_custom_reg(n, 300 + n, distinct_betas=True)
+    P = _small(inst.params, n_p=n_p, n_p_star=3, n_t=6, t_p=0.05)
+    S0 = I.make_init_poses(inst, 8)
+    assert_parity(inst, P, S0, 64, 16, 11)
+    fast = gpu_walk(inst, P, S0, 2048, 60, 77)
+    plain = gpu_walk(inst, _small(P, flags=1), S0, 2048, 60, 77)
+    for a, b in zip(fast, plain):
+        assert np.array_equal(a, b)
+
+
+def test_batch_members_with_different_tables():
+    """closure_sample_batch over instances whose fp32 tables differ in size and run structure: the launch sizes
+    shared memory for the largest, every member equals its own single-instance launch bit for bit."""
+    import torch
+    insts = [I.make_custom_reg(200, 41), _three_bounds(120, 42, (31, 40, 49)), I.make_custom_reg(9, 43, distinct_betas=True)]
+    P = _small(insts[0].params, n_p=20, n_p_star=2, n_t=5, t_p=0.05)
+    hs, single = [], []
+    try:
+        for it in insts:
+            h = B.Closure.closure_create(it, P)
+            h.closure_set_init(I.make_init_poses(it, 8))
+            hs.append(h)
+        smp, flag = B.closure_sample_batch(hs, 512, 40, [5, 6, 7])
+        torch.cuda.synchronize()
+        for b, h in enumerate(hs):
+            s1, f1 = h.closure_sample(512, 40, 5 + b)
+            torch.cuda.synchronize()
+            assert np.array_equal(s1.cpu().numpy(), smp[b].cpu().numpy())
+            assert np.array_equal(f1.cpu().numpy(), flag[b].cpu().numpy())
+    finally:
+        for h in hs:
+            h.closure_destroy()
 
 
 @pytest.mark.parametrize("walkers", [1, 31, 127, 128, 129])
