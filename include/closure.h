@@ -101,6 +101,15 @@ int closure_create(int residual_type, const double *measurements, int n, const d
 /* Replace the walk parameters of an existing handle (same validation as closure_create). */
 int closure_set_params(closure_t *h, const closure_params *p);
 
+/* Body pivot of update_rotation (Alg. 2 l.20, which the paper never defines; R-1).
+ * With pivot c (host, 3 doubles, in the frame of the source points a_i / Z_i) a rotation step keeps the image of
+ * the body point c fixed:  R' = Exp(dT w) R,  t' = t + (R - R') c  -- the "object movement" reading of
+ * PAPER.md:328, 336.  The default c = 0 is rotation about the origin of the source frame (t untouched).
+ * Rotation sampler (CLOSURE_MODE_ROT) and residuals with source points (REG_3D3D, REPROJ_2D3D) only:
+ * CLOSURE_EUNSUPPORTED otherwise for a non-zero pivot.  Invalidates S_0: call closure_set_init (or
+ * closure_init_from_trials) again.  Inputs and outputs of every call stay in the caller's (R, t). */
+int closure_set_pivot(closure_t *h, const double *pivot);
+
 /* Give the initial pose set S_0 (output of Step I).  poses: host, n0 x 12.  Computes
  * R_bar = proj_SO(3)(sum R_j) and t_bar = mean t_j on the host (Alg. 2 l.3-4),
  * checks every pose against the PURSE (CLOSURE_EINIT if one is outside) and uploads.

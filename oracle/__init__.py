@@ -30,7 +30,7 @@ _lib = None
 class _Params(ctypes.Structure):
     _fields_ = [("mode", c_int), ("n_p", c_int), ("n_p_star", c_int), ("n_t", c_int),
                 ("omega0", c_double), ("v0", c_double), ("gamma", c_double),
-                ("t_p", c_double), ("theta_p", c_double), ("vel_scale", c_double * 9)]
+                ("t_p", c_double), ("theta_p", c_double), ("vel_scale", c_double * 9), ("pivot", c_double * 3)]
 
 
 def build(force: bool = False) -> str:
@@ -169,7 +169,8 @@ def walk(inst, params, S0, walker_ids, n_steps: int, seed: int, *, trace: bool =
     scale = pca_velocity_scale(S0) if (int(getattr(params, "flags", 0)) & 64) else np.eye(3)
     P = _Params(int(params.mode), int(params.n_p), int(params.n_p_star), int(params.n_t),
                 float(params.omega0), float(params.v0), float(params.gamma),
-                float(params.t_p), float(params.theta_p), (c_double * 9)(*scale.reshape(9)))
+                float(params.t_p), float(params.theta_p), (c_double * 9)(*scale.reshape(9)),
+                (c_double * 3)(*[float(x) for x in getattr(params, "pivot", (0.0, 0.0, 0.0))]))
     samples = np.zeros((W, 12))
     flags = np.zeros(W, dtype=np.uint8)
     tr = np.zeros((W, n_steps), dtype=np.int32) if trace else None

@@ -226,6 +226,7 @@ typedef struct {
     int n_p, n_p_star, n_t;   /* N_P, N_P*, N_T */
     double omega0, v0, gamma, t_p, theta_p;
     double vel_scale[9];      /* PCA normalisation of the centre velocity (R-23); I if off */
+    double pivot[3];          /* body pivot c of update_rotation (R-1 alternative); 0: rotation about the origin */
 } ora_params;
 
 /* random unit vector from two uniforms (R-4): z = xi0, phi = pi (xi1 + 1). */
@@ -355,6 +356,15 @@ static void walk_one(int type, int n, const double *meas, const double *beta, co
                     ora_exp_so3(phi, E);
                     mat3_mul(E, Rp, Rc);
                     memcpy(tc, tp, 3 * sizeof(double));
+                    if (P->pivot[0] != 0.0 || P->pivot[1] != 0.0 || P->pivot[2] != 0.0) {
+                        /* rotate about the body point c ("object movement"): the image
+                         * R c + t of c stays where it is, t' = t + (R - R') c  (R-1, alternative reading) */
+                        for (int r = 0; r < 3; ++r) {
+                            double before = Rp[3 * r] * P->pivot[0] + Rp[3 * r + 1] * P->pivot[1] + Rp[3 * r + 2] * P->pivot[2];
+                            double after = Rc[3 * r] * P->pivot[0] + Rc[3 * r + 1] * P->pivot[1] + Rc[3 * r + 2] * P->pivot[2];
+                            tc[r] = tp[r] + (before - after);
+                        }
+                    }
                 } else {                                    /* update_translation: t + dT v (R-7) */
                     memcpy(Rc, Rp, 9 * sizeof(double));
                     for (int r = 0; r < 3; ++r) tc[r] = tp[r] + dT * v[r];

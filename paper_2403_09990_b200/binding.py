@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libclosure_b200.so")
 OK, EINVAL, EINIT, ENOINIT, ECUDA, ENOMEM, EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = [
-    "closure_default_params", "closure_create", "closure_set_params", "closure_set_init",
+    "closure_default_params", "closure_create", "closure_set_params", "closure_set_pivot", "closure_set_init",
     "closure_sample_range", "closure_sample", "closure_sample_batch", "closure_compact", "closure_megb",
     "closure_init_sample", "closure_init_from_trials", "closure_run", "closure_enable_stats", "closure_get_stats", "closure_alu_peak", "closure_miniball_host",
     "closure_last_error", "closure_strerror", "closure_abi_version", "closure_destroy",
@@ -70,6 +70,7 @@ def load_library():
     L.closure_create.argtypes = [c_int, POINTER(c_double), c_int, POINTER(c_double), POINTER(c_double),
                                  POINTER(ClosureParams), POINTER(c_void_p)]
     L.closure_set_params.argtypes = [c_void_p, POINTER(ClosureParams)]
+    L.closure_set_pivot.argtypes = [c_void_p, POINTER(c_double)]
     L.closure_set_init.argtypes = [c_void_p, POINTER(c_double), c_int, POINTER(c_double)]
     L.closure_sample_range.argtypes = [c_void_p, c_longlong, c_longlong, c_int, c_ulonglong, c_void_p,
                                        c_void_p, c_void_p, c_void_p]
@@ -197,6 +198,10 @@ class Closure:
         P = params if isinstance(params, ClosureParams) else make_params(params)
         self._check(load_library().closure_set_params(self._h, byref(P)))
         self.params = P
+
+    def closure_set_pivot(self, pivot):
+        c = np.ascontiguousarray(pivot, dtype=np.float64).reshape(3)
+        self._check(load_library().closure_set_pivot(self._h, _dp(c)))
 
     def closure_set_init(self, poses) -> np.ndarray:
         S0 = np.ascontiguousarray(poses, dtype=np.float64).reshape(-1, 12)

@@ -25,6 +25,9 @@ struct closure_s {
     std::vector<double> betas;
     double K[4] = { 0, 0, 0, 0 };
     InstanceDesc h_desc{};
+    std::vector<int> order;          // sorted row k holds the caller's constraint order[k]
+    double pivot[3] = { 0, 0, 0 };   // body pivot of update_rotation (closure_set_pivot, R-1); zero: rotation about the origin
+    bool has_pivot = false;
     int n_pairs = 0;                 // pair-entries of the cooperative kernel's fp32 table: sum over runs of equal bound of ceil(len / 2)
     double *d_rows = nullptr;
     int *d_perm = nullptr;
@@ -191,6 +194,37 @@ int ensure_scratch(closure_t *h, long long n)
     return CLOSURE_OK;
 }
 
+// Device rows, sorted by the translation-side bound: [measurement, beta, beta^2, ...].  With a body pivot c
+// (closure_set_pivot) the source points are stored as a - c (Z - c): the kernels then walk (R, tau = t + R c),
+// for which "rotate about c" is the plain left multiplication (R-1).
+void pack_rows(const closure_t *h, std::vector<double> &rows)
+{
+    const int type = h->type, n = h->n, row = row_doubles(type), cols = meas_cols(type);
+    rows.assign((size_t)n * row, 0.0);
+    const double *betas = h->betas.data();
+    for (int k = 0; k < n; ++k) {
+        const int i = h->order[k];
+        const double *m = h->meas.data() + (size_t)i * cols;
+        double *r = rows.data() + (size_t)k * row;
+        if (type == CLOSURE_REG_3D3D) {
+            std::memcpy(r, m, 6 * sizeof(double));
+            for (int c = 0; c < 3; ++c) r[c] = m[c] - h->pivot[c];
+            r[6] = betas[i]; r[7] = betas[i] * betas[i];
+        } else if (type == CLOSURE_REPROJ_2D3D) {
+            std::memcpy(r, m, 5 * sizeof(double));
+            for (int c = 0; c < 3; ++c) r[2 + c] = m[2 + c] - h->pivot[c];
+            r[5] = betas[i]; r[6] = betas[i] * betas[i];
+        } else if (type == CLOSURE_POSE_REG) {
+            std::memcpy(r, m, 12 * sizeof(double));
+            r[12] = betas[i]; r[13] = betas[i] * betas[i];
+        } else {
+            std::memcpy(r, m, 12 * sizeof(double));
+            r[12] = betas[2 * i]; r[13] = betas[2 * i] * betas[2 * i];
+            r[14] = betas[2 * i + 1]; r[15] = betas[2 * i + 1] * betas[2 * i + 1];
+        }
+    }
+}
+
 void fill_launch(const closure_t *h, WalkLaunch &L)
 {
     std::memset(&L, 0, sizeof(L));
@@ -251,6 +285,8 @@ int closure_set_params(closure_t *h, const closure_params *p)
     std::string why;
     const int rc = check_params(p, &why);
     if (rc != CLOSURE_OK) return fail(h, rc, why);
+    if (h->has_pivot && p->mode != CLOSURE_MODE_ROT)
+        return fail(h, CLOSURE_EUNSUPPORTED, "a body pivot is set: Alg. A8 has no update_rotation (clear it with closure_set_pivot first)");
     h->P = *p;
     return CLOSURE_OK;
 }
@@ -283,31 +319,13 @@ int closure_create(int residual_type, const double *measurements, int n, const d
     if (residual_type == CLOSURE_REPROJ_2D3D) std::memcpy(h->K, intrinsics, sizeof(h->K));
 
     // pack rows, sorted by the translation-side bound (stable)
-    const int row = row_doubles(residual_type);
     auto key = [&](int i) { return residual_type == CLOSURE_POSE_REG_SPLIT ? betas[2 * i + 1] : betas[i]; };
     std::vector<int> order(n);
     std::iota(order.begin(), order.end(), 0);
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return key(a) < key(b); });
-    std::vector<double> rows((size_t)n * row, 0.0);
-    for (int k = 0; k < n; ++k) {
-        const int i = order[k];
-        const double *m = measurements + (size_t)i * cols;
-        double *r = rows.data() + (size_t)k * row;
-        if (residual_type == CLOSURE_REG_3D3D) {
-            std::memcpy(r, m, 6 * sizeof(double));
-            r[6] = betas[i]; r[7] = betas[i] * betas[i];
-        } else if (residual_type == CLOSURE_REPROJ_2D3D) {
-            std::memcpy(r, m, 5 * sizeof(double));
-            r[5] = betas[i]; r[6] = betas[i] * betas[i];
-        } else if (residual_type == CLOSURE_POSE_REG) {
-            std::memcpy(r, m, 12 * sizeof(double));
-            r[12] = betas[i]; r[13] = betas[i] * betas[i];
-        } else {
-            std::memcpy(r, m, 12 * sizeof(double));
-            r[12] = betas[2 * i]; r[13] = betas[2 * i] * betas[2 * i];
-            r[14] = betas[2 * i + 1]; r[15] = betas[2 * i + 1] * betas[2 * i + 1];
-        }
-    }
+    h->order = order;
+    std::vector<double> rows;
+    pack_rows(h, rows);
     for (int k = 0, len = 0; k < n; ++k) {                 // runs of equal bound in sorted order
         ++len;
         if (k == n - 1 || key(order[k + 1]) != key(order[k])) { h->n_pairs += (len + 1) / 2; len = 0; }
@@ -343,6 +361,25 @@ int closure_create(int residual_type, const double *measurements, int n, const d
     return CLOSURE_OK;
 }
 
+int closure_set_pivot(closure_t *h, const double *pivot)
+{
+    if (!h) return CLOSURE_EINVAL;
+    if (!pivot || !all_finite(pivot, 3)) return fail(h, CLOSURE_EINVAL, "pivot is NULL or not finite");
+    const bool nonzero = pivot[0] != 0.0 || pivot[1] != 0.0 || pivot[2] != 0.0;
+    if (nonzero && h->type != CLOSURE_REG_3D3D && h->type != CLOSURE_REPROJ_2D3D)
+        return fail(h, CLOSURE_EUNSUPPORTED, "a body pivot needs source points (Ex.1 / Ex.2)");
+    if (nonzero && h->P.mode != CLOSURE_MODE_ROT)
+        return fail(h, CLOSURE_EUNSUPPORTED, "Alg. A8 has no update_rotation: a body pivot applies to the rotation sampler only");
+    std::memcpy(h->pivot, pivot, sizeof(h->pivot));
+    h->has_pivot = nonzero;
+    h->has_init = false;                                 // S_0 is stored relative to the pivot: give it again
+    std::vector<double> rows;
+    pack_rows(h, rows);
+    cudaError_t e = cudaMemcpy(h->d_rows, rows.data(), rows.size() * sizeof(double), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return cuda_fail(h, e, "upload of constraint rows");
+    return CLOSURE_OK;
+}
+
 int closure_set_init(closure_t *h, const double *poses, int n0, double *mean_out)
 {
     if (!h) return CLOSURE_EINVAL;
@@ -364,7 +401,19 @@ int closure_set_init(closure_t *h, const double *poses, int n0, double *mean_out
     h->d_S0 = nullptr;
     h->has_init = false;
     cudaError_t e = cudaMalloc(&h->d_S0, (size_t)n0 * 12 * sizeof(double));
-    if (e == cudaSuccess) e = cudaMemcpy(h->d_S0, poses, (size_t)n0 * 12 * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        if (h->has_pivot) {                              // the kernels walk (R, tau = t + R c)
+            std::vector<double> tau(poses, poses + (size_t)n0 * 12);
+            for (int s = 0; s < n0; ++s) {
+                double *q = tau.data() + (size_t)s * 12;
+                for (int r = 0; r < 3; ++r)
+                    q[9 + r] = q[9 + r] + (q[3 * r] * h->pivot[0] + q[3 * r + 1] * h->pivot[1] + q[3 * r + 2] * h->pivot[2]);
+            }
+            e = cudaMemcpy(h->d_S0, tau.data(), (size_t)n0 * 12 * sizeof(double), cudaMemcpyHostToDevice);
+        } else {
+            e = cudaMemcpy(h->d_S0, poses, (size_t)n0 * 12 * sizeof(double), cudaMemcpyHostToDevice);
+        }
+    }
     if (e != cudaSuccess) return cuda_fail(h, e, "upload of S_0");
     h->h_desc.S0 = h->d_S0;
     h->h_desc.n0 = n0;
@@ -396,6 +445,7 @@ int closure_init_sample(closure_t *h, long long trial_begin, long long num_trial
     if (reinterpret_cast<uintptr_t>(out_poses) & 15u) return fail(h, CLOSURE_EINVAL, "pose buffer must be 16-byte aligned");
     cudaError_t e = launch_step1(h->type, h->d_desc, h->h_desc.rows_bytes, trial_begin, num_trials, seed, out_poses,
                                  out_ok, static_cast<cudaStream_t>(cuda_stream));
+    if (e == cudaSuccess && h->has_pivot) e = launch_pivot_back(out_poses, num_trials, h->pivot, static_cast<cudaStream_t>(cuda_stream));
     if (e != cudaSuccess) return cuda_fail(h, e, "Step I kernel launch");
     return CLOSURE_OK;
 }
@@ -462,6 +512,7 @@ int closure_sample_range(closure_t *h, long long walker_begin, long long num_wal
     }
     std::string why;
     cudaError_t e = launch_walkers(h->type, h->P.mode, h->stats_on, L, 1, h->h_desc.rows_bytes, stream, &why);
+    if (e == cudaSuccess && h->has_pivot) e = launch_pivot_back(out_samples, num_walkers, h->pivot, stream);   // t = tau - R c
     h->last_stream = stream;
     if (e != cudaSuccess) return cuda_fail(h, e, why.empty() ? "walker kernel launch" : why.c_str());
     return CLOSURE_OK;
@@ -514,6 +565,10 @@ int closure_sample_batch(closure_t *const *handles, int n_instances, long long w
         L.stats = h0->stats_on ? h0->d_stats : nullptr;
         std::string why;
         cudaError_t e = launch_walkers(h0->type, h0->P.mode, h0->stats_on, L, nb, max_bytes, stream, &why);
+        for (int b = 0; b < nb && e == cudaSuccess; ++b)
+            if (handles[b0 + b]->has_pivot)
+                e = launch_pivot_back(L.out_samples + (size_t)b * walkers_per_instance * 12, walkers_per_instance,
+                                      handles[b0 + b]->pivot, stream);
         if (e != cudaSuccess) return cuda_fail(h0, e, why.empty() ? "walker kernel launch" : why.c_str());
     }
     h0->last_stream = stream;

@@ -74,6 +74,9 @@ cudaError_t launch_walkers_coop_reproj(const WalkLaunch &L, int n_instances, int
 cudaError_t launch_walkers_coop_trans(int residual_type, const WalkLaunch &L, int n_instances, int max_rows_bytes,
                                       cudaStream_t stream);
 
+// compact_kernel.cu: t <- t - R c on n poses (back from the pivot-relative translation, closure_set_pivot)
+cudaError_t launch_pivot_back(double *poses, long long n, const double *pivot, cudaStream_t stream);
+
 // step1_kernel.cu: Step I trials (RANSAG with Arun's method for Ex.2, convex combinations for Ex.3)
 cudaError_t launch_step1(int residual_type, const InstanceDesc *d_desc, int rows_bytes, long long trial_begin,
                          long long num_trials, unsigned long long seed, double *out_poses, unsigned char *out_ok,

@@ -148,6 +148,27 @@ size_t compact_scratch_bytes(long long n)
     return (size_t)(tiles + 1) * sizeof(unsigned long long);
 }
 
+// t <- t - R c on n poses [R row-major (9), t (3)]: the walk with a body pivot c (closure_set_pivot, R-1)
+// runs on (R, tau = t + R c); this turns its output back into the caller's translation.  One pose per thread.
+__global__ void pivot_back_kernel(double *__restrict__ poses, long long n, double c0, double c1, double c2)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double *q = poses + 12 * i;
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+        q[9 + r] = q[9 + r] - (q[3 * r] * c0 + q[3 * r + 1] * c1 + q[3 * r + 2] * c2);
+}
+
+cudaError_t launch_pivot_back(double *poses, long long n, const double *pivot, cudaStream_t stream)
+{
+    if (n <= 0) return cudaSuccess;
+    const long long blocks = (n + 255) / 256;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
+    pivot_back_kernel<<<(unsigned)blocks, 256, 0, stream>>>(poses, n, pivot[0], pivot[1], pivot[2]);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_compact(const double *samples, const unsigned char *flags, long long n, double *out,
                            long long *out_count, void *scratch, cudaStream_t stream)
 {

@@ -41,6 +41,7 @@ class WalkParams:
     t_p: float = 0.1
     theta_p: float = 0.0    # the paper's R_p
     flags: int = 0          # include/closure.h CLOSURE_FLAG_* (1 = plain fp64 kernel only)
+    pivot: tuple = (0.0, 0.0, 0.0)   # body pivot of update_rotation (closure_set_pivot; R-1)
 
 
 @dataclass

@@ -13,6 +13,8 @@ def gpu_walk(inst, P, S0, num_walkers, steps, seed, *, walker_begin=0, trace=Tru
     import torch
     h = B.Closure.closure_create(inst, P)
     try:
+        if any(getattr(P, "pivot", (0.0, 0.0, 0.0))):
+            h.closure_set_pivot(P.pivot)
         h.closure_set_init(S0)
         out = h.closure_sample(num_walkers, steps, seed, walker_begin=walker_begin, trace=trace)
         torch.cuda.synchronize()

@@ -318,3 +318,79 @@ def test_pca_normalised_centre_velocity(config, flags):
     a = gpu_walk(inst, P, S0, 64, 10, 7)
     b = gpu_walk(inst, _small(P, flags=flags & 1), S0, 64, 10, 7)
     assert not np.array_equal(a[0], b[0])
+
+
+@pytest.mark.parametrize("config,flags", [(2, 0), (2, 1), (3, 0), (1, 0)])
+def test_body_pivot_of_update_rotation(config, flags):
+    """closure_set_pivot (R-1): the oracle applies t' = t + (R - R')c at every rotation step, the CUDA
+    path walks the problem re-centred at c and maps the output back; inputs and outputs stay in (R, t)."""
+    inst = I.make_instance(config)
+    P = _small(inst.params, pivot=(0.3, -0.2, 0.45), flags=flags)
+    S0 = I.make_init_poses(inst, 32)
+    assert_parity(inst, P, S0, 192, 30, 17)
+    plain = gpu_walk(inst, _small(P, pivot=(0.0, 0.0, 0.0)), S0, 192, 30, 17)
+    piv = gpu_walk(inst, P, S0, 192, 30, 17)
+    assert np.abs(plain[0] - piv[0]).max() > 1e-4                       # a different walk, not a no-op
+
+
+def test_body_pivot_api_edges():
+    import torch
+    inst = I.make_instance(2)
+    S0 = I.make_init_poses(inst, 16)
+    h = B.Closure.closure_create(inst)
+    try:
+        h.closure_set_init(S0)
+        ref = [o.cpu().numpy() for o in h.closure_sample(256, 20, 3)]
+        h.closure_set_pivot((0.5, 0.1, -0.3))
+        with pytest.raises(B.ClosureError) as e:                        # S_0 has to be given again
+            h.closure_sample(16, 2, 3)
+        assert e.value.status == B.ENOINIT
+        poses, ok = h.closure_init_sample(500, 4)                       # Step I does not depend on the pivot
+        h.closure_set_pivot((0.0, 0.0, 0.0))
+        poses0, ok0 = h.closure_init_sample(500, 4)
+        torch.cuda.synchronize()
+        assert np.array_equal(ok.cpu().numpy(), ok0.cpu().numpy())
+        assert np.abs(poses.cpu().numpy() - poses0.cpu().numpy()).max() < 1e-12
+        h.closure_set_init(S0)                                          # pivot cleared: the default walk again
+        again = [o.cpu().numpy() for o in h.closure_sample(256, 20, 3)]
+        assert np.array_equal(ref[0], again[0]) and np.array_equal(ref[1], again[1])
+        h.closure_set_pivot((0.5, 0.1, -0.3))
+        Pt = _small(inst.params, mode=I.MODE_TRANS, v0=0.05, theta_p=0.05)
+        with pytest.raises(B.ClosureError) as e:                        # Alg. A8 has no update_rotation
+            h.closure_set_params(Pt)
+        assert e.value.status == B.EUNSUPPORTED
+        with pytest.raises(B.ClosureError) as e:
+            h.closure_set_pivot((np.nan, 0.0, 0.0))
+        assert e.value.status == B.EINVAL
+    finally:
+        h.closure_destroy()
+    h = B.Closure.closure_create(I.make_instance(4))
+    try:
+        h.closure_set_pivot((0.0, 0.0, 0.0))
+        with pytest.raises(B.ClosureError) as e:                        # no source points in Ex.3
+            h.closure_set_pivot((0.1, 0.0, 0.0))
+        assert e.value.status == B.EUNSUPPORTED
+    finally:
+        h.closure_destroy()
+    # batch members with different pivots; closure_run end to end
+    insts = [I.make_instance(1), I.make_instance(1, 1)]
+    P = _small(insts[0].params, n_p=20, n_p_star=2, n_t=5)
+    hs = []
+    try:
+        for b, it in enumerate(insts):
+            hb = B.Closure.closure_create(it, P)
+            if b == 1:
+                hb.closure_set_pivot((0.2, 0.2, -0.1))
+            hb.closure_set_init(I.make_init_poses(it, 8))
+            hs.append(hb)
+        smp, flag = B.closure_sample_batch(hs, 300, 25, [8, 9])
+        torch.cuda.synchronize()
+        for b, hb in enumerate(hs):
+            s1, f1 = hb.closure_sample(300, 25, 8 + b)
+            torch.cuda.synchronize()
+            assert np.array_equal(s1.cpu().numpy(), smp[b].cpu().numpy())
+        res = hs[1].closure_run(1024, 30, 5)
+        assert res["count"] > 900 and res["trans_radius"] > 0
+    finally:
+        for hb in hs:
+            hb.closure_destroy()

@@ -365,3 +365,67 @@ def test_pca_velocity_changes_only_the_direction_of_travel():
             moved += 1
             assert np.linalg.norm(np.cross(S @ da, db)) <= 1e-9 * np.linalg.norm(S @ da) * np.linalg.norm(db)
     assert moved > 10
+
+
+# ----------------------------------------------------------------------------- body pivot of update_rotation (R-1)
+
+def _shifted(inst, c):
+    """The same problem with source points a - c: pose (R, tau = t + R c) there is pose (R, t) here."""
+    out = copy.copy(inst)
+    meas = np.array(inst.measurements, dtype=np.float64, copy=True)
+    lo = 0 if inst.residual_type == I.REG_3D3D else 2
+    meas[:, lo:lo + 3] -= c
+    out.measurements = meas
+    return out
+
+
+@pytest.mark.parametrize("config", [1, 3])
+def test_body_pivot_keeps_the_pivot_point_fixed_and_equals_the_recentred_problem(config):
+    """update_rotation about a body point c ("object movement"; R-1): (a) pivot 0 is the
+    default walk bit for bit; (b) an accepted step leaves the image of c where the perturbed pose had it,
+    R' c + t' = R* c + t_j; (c) the walk equals the pivot-free walk of the problem re-centred at c
+    (source points a - c, translations tau = t + R c), mapped back by t = tau - R c."""
+    inst = I.make_instance(config)
+    S0 = I.make_init_poses(inst, 16)
+    P = copy.copy(inst.params); P.n_p = 12; P.n_p_star = 3; P.n_t = 8
+    c = np.array([0.3, -0.2, 0.45])
+    Pc = copy.copy(P); Pc.pivot = tuple(c)
+    P0 = copy.copy(P); P0.pivot = (0.0, 0.0, 0.0)
+    ids = np.arange(48)
+    base = oracle.walk(inst, P, S0, ids, 6, 5, trace=True)
+    zero = oracle.walk(inst, P0, S0, ids, 6, 5, trace=True)
+    assert np.array_equal(base[0], zero[0]) and np.array_equal(base[2], zero[2])            # (a)
+
+    one, _, tr, _ = oracle.walk(inst, Pc, S0, ids, 1, 5, trace=True)                         # (b)
+    moved = 0
+    for w in ids:
+        m0, j0 = int(tr[w, 0]) & 0xFF, int(tr[w, 0]) >> 8
+        R0, t0 = S0[w % 16, :9].reshape(3, 3), S0[w % 16, 9:]
+        R1, t1 = one[w, :9].reshape(3, 3), one[w, 9:]
+        if m0 == 0:
+            assert np.array_equal(one[w], S0[w % 16])
+            continue
+        x = oracle.philox4x32_10([w, 1, j0, 1], [5, 0])
+        tj = t0 + P.t_p * np.array([oracle.u32_to_pm1(int(x[r])) for r in range(3)])
+        assert np.abs((R1 @ c + t1) - (R0 @ c + tj)).max() < 1e-12
+        assert np.abs(R1 - R0).max() > 1e-6                                                  # it did rotate
+        moved += 1
+    assert moved > 20
+
+    sh = _shifted(inst, c)                                                                   # (c)
+    S0s = S0.copy()
+    S0s[:, 9:] += S0[:, :9].reshape(-1, 3, 3) @ c
+    a_smp, a_flag, a_tr, a_sl = oracle.walk(inst, Pc, S0, ids, 6, 5, trace=True)
+    b_smp, b_flag, b_tr, b_sl = oracle.walk(sh, P0, S0s, ids, 6, 5, trace=True)
+    same = 0
+    for w in ids:
+        if not np.array_equal(a_tr[w], b_tr[w]):
+            first = int(np.argmax(a_tr[w] != b_tr[w]))
+            assert min(a_sl[w, first], b_sl[w, first]) < 1e-9                               # a near-tie only
+            continue
+        back = b_smp[w].copy()
+        back[9:] -= b_smp[w, :9].reshape(3, 3) @ c
+        assert np.abs(back - a_smp[w]).max() < 1e-11 and a_flag[w] == b_flag[w]
+        same += 1
+    assert same >= 46
+    assert np.abs(a_smp - base[0]).max() > 1e-3                                              # and it is a different walk
