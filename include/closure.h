@@ -47,8 +47,15 @@ extern "C" {
  *   CLOSURE_POSE_REG        [R_i(9 row-major) t_i(3)]   g = [vec(R)-vec(R_i); t-t_i], ONE bound per hypothesis
  *   CLOSURE_POSE_REG_SPLIT  same rows; TWO bounds per hypothesis, betas[2i] on ||vec(R)-vec(R_i)||,
  *                           betas[2i+1] on ||t-t_i||  (PURSEreg; R-13)
- * Lambda_i = I throughout (R-14). */
-enum { CLOSURE_REPROJ_2D3D = 1, CLOSURE_REG_3D3D = 2, CLOSURE_POSE_REG = 3, CLOSURE_POSE_REG_SPLIT = 4 };
+ *   CLOSURE_REPROJ_2D3D_ELL [z(2) Z(3) Lambda(4: 2x2 row-major)]    the same g, bounded in the ellipse norm
+ *   CLOSURE_REG_3D3D_ELL    [a(3) b(3) Lambda(9: 3x3 row-major)]    ||g||_Lambda = sqrt(g^T Lambda_i g) <= beta_i
+ * Lambda_i = I for the first four (R-14).  The _ELL types carry the positive definite Lambda_i of eq. (6)
+ * (the ellipses / ellipsoids of PAPER.md:179-191): symmetric, positive definite
+ * (CLOSURE_EINVAL otherwise).  They run on the one-walker-per-thread fp64 kernel (rotation sampler) and the
+ * warp-cooperative fp64 kernel (translation sampler); there is no fp32-certified kernel and no fp32 mode for them.
+ * Step I: REG_3D3D_ELL as REG_3D3D; REPROJ_2D3D_ELL is not built (CLOSURE_EUNSUPPORTED). */
+enum { CLOSURE_REPROJ_2D3D = 1, CLOSURE_REG_3D3D = 2, CLOSURE_POSE_REG = 3, CLOSURE_POSE_REG_SPLIT = 4,
+       CLOSURE_REG_3D3D_ELL = 5, CLOSURE_REPROJ_2D3D_ELL = 6 };
 
 /* which boundary is sampled: CLOSURE_MODE_ROT = Alg. 2 (fixed angular velocity, translation
  * perturbations); CLOSURE_MODE_TRANS = Alg. A8 (fixed centre velocity, rotation perturbations). */
@@ -91,7 +98,7 @@ int closure_default_params(int residual_type, closure_params *p);
 /* Describe a PURSE  S = { (R,t) : ||g(x, y_i)|| <= beta_i } and upload it.
  *   measurements  host, n rows in the layout of `residual_type`
  *   betas         host, n bounds (2n for CLOSURE_POSE_REG_SPLIT), each finite and > 0
- *   intrinsics    host, {fx, fy, cx, cy}; required for CLOSURE_REPROJ_2D3D, ignored (may be NULL) else
+ *   intrinsics    host, {fx, fy, cx, cy}; required for CLOSURE_REPROJ_2D3D(_ELL), ignored (may be NULL) else
  *   p             walk parameters (copied)
  *   out           receives the handle; destroy with closure_destroy
  * Synchronous (small H2D copy).  Errors: CLOSURE_EINVAL, CLOSURE_ECUDA, CLOSURE_ENOMEM. */

@@ -33,6 +33,8 @@
 #define ORA_REG_3D3D 2
 #define ORA_POSE_REG 3
 #define ORA_POSE_REG_SPLIT 4
+#define ORA_REG_3D3D_ELL 5      /* eq. (6) with a general Lambda_i: ellipsoids */
+#define ORA_REPROJ_2D3D_ELL 6   /* eq. (6) with a general Lambda_i: ellipses */
 #define ORA_MODE_ROT 0
 #define ORA_MODE_TRANS 1
 
@@ -135,6 +137,8 @@ static int row_len(int type)
     switch (type) {
     case ORA_REPROJ_2D3D: return 5;      /* [z(2) Z(3)] */
     case ORA_REG_3D3D: return 6;         /* [a(3) b(3)] */
+    case ORA_REG_3D3D_ELL: return 15;    /* [a(3) b(3) Lambda(9 row-major)] */
+    case ORA_REPROJ_2D3D_ELL: return 9;  /* [z(2) Z(3) Lambda(4 row-major)] */
     default: return 12;                  /* [R_i(9 row-major) t_i(3)] */
     }
 }
@@ -145,7 +149,8 @@ static int row_len(int type)
  *   Ex.2 eq.(3) PAPER.md:33.
  *   Ex.3 eq.(4) PAPER.md:39 (stacked, one bound) or PURSEreg PAPER.md:173 (split: constraint
  *        2i bounds ||vec(R)-vec(R_i)||, constraint 2i+1 bounds ||t-t_i||) (R-13).
- * Lambda_i = I (R-14). */
+ * Lambda_i = I (R-14), except the _ELL types: ||g||_Lambda^2 = g^T Lambda_i g, eq. (6) PAPER.md:58,
+ * written out as the double sum over the entries of Lambda_i. */
 double ora_residual_sq(int type, int c, const double *meas, const double *K, const double R[9], const double t[3])
 {
     double sq = 0.0;
@@ -157,6 +162,23 @@ double ora_residual_sq(int type, int c, const double *meas, const double *K, con
             double g = b[r] - (Ra[r] + t[r]);
             sq = sq + g * g;
         }
+    } else if (type == ORA_REG_3D3D_ELL) {
+        const double *a = meas + 15 * c, *b = a + 3, *Lam = a + 6;
+        double Ra[3], g[3];
+        mat3_vec(R, a, Ra);
+        for (int r = 0; r < 3; ++r) g[r] = b[r] - (Ra[r] + t[r]);
+        for (int r = 0; r < 3; ++r)
+            for (int q = 0; q < 3; ++q) sq = sq + g[r] * Lam[3 * r + q] * g[q];
+    } else if (type == ORA_REPROJ_2D3D_ELL) {
+        const double *z = meas + 9 * c, *Z = z + 2, *Lam = z + 5;
+        double p[3], g[2];
+        mat3_vec(R, Z, p);
+        for (int r = 0; r < 3; ++r) p[r] = p[r] + t[r];
+        if (!(p[2] > 0.0)) return INFINITY;
+        g[0] = z[0] - (K[0] * (p[0] / p[2]) + K[2]);
+        g[1] = z[1] - (K[1] * (p[1] / p[2]) + K[3]);
+        for (int r = 0; r < 2; ++r)
+            for (int q = 0; q < 2; ++q) sq = sq + g[r] * Lam[2 * r + q] * g[q];
     } else if (type == ORA_REPROJ_2D3D) {
         const double *z = meas + 5 * c, *Z = z + 2;
         double p[3];

@@ -44,7 +44,7 @@ import numpy as np
 import oracle
 
 TAG_TRIPLET, TAG_WEIGHTS, TAG_DISC = 2, 3, 4
-REPROJ_2D3D, REG_3D3D, POSE_REG, POSE_REG_SPLIT = 1, 2, 3, 4
+REPROJ_2D3D, REG_3D3D, POSE_REG, POSE_REG_SPLIT, REG_3D3D_ELL, REPROJ_2D3D_ELL = 1, 2, 3, 4, 5, 6
 
 
 def trial_words(seed: int, k: int, c: int, tag: int, a: int = 0) -> np.ndarray:
@@ -258,7 +258,7 @@ def init_sample(inst, num_trials: int, seed: int, trial_begin: int = 0):
     ok = np.zeros(num_trials, dtype=np.uint8)
     for q in range(num_trials):
         k = trial_begin + q
-        if ty == REG_3D3D:
+        if ty in (REG_3D3D, REG_3D3D_ELL):               # the ellipsoid norm changes the PURSE test only
             if n < 3:
                 raise ValueError("RANSAG needs at least 3 correspondences")
             idx = list(triplet(seed, k, n))
@@ -274,7 +274,7 @@ def init_sample(inst, num_trials: int, seed: int, trial_begin: int = 0):
                     cand = (Rc, tc)
                     break
         else:
-            raise ValueError("unknown residual type")
+            raise ValueError("Step I is not built for this residual type")
         if cand is None:
             continue
         R, t = cand

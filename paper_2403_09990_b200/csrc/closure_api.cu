@@ -77,6 +77,8 @@ int meas_cols(int type)
     switch (type) {
     case CLOSURE_REPROJ_2D3D: return 5;
     case CLOSURE_REG_3D3D: return 6;
+    case CLOSURE_REG_3D3D_ELL: return 15;
+    case CLOSURE_REPROJ_2D3D_ELL: return 9;
     case CLOSURE_POSE_REG:
     case CLOSURE_POSE_REG_SPLIT: return 12;
     default: return 0;
@@ -108,20 +110,27 @@ bool host_in_purse(const closure_t *h, const double *pose)
     const double *R = pose, *t = pose + 9;
     for (int i = 0; i < h->n; ++i) {
         const double *m = h->meas.data() + (size_t)i * meas_cols(h->type);
-        if (h->type == CLOSURE_REG_3D3D) {
-            double sq = 0.0;
-            for (int r = 0; r < 3; ++r) {
-                const double g = m[3 + r] - ((R[3 * r] * m[0] + R[3 * r + 1] * m[1] + R[3 * r + 2] * m[2]) + t[r]);
-                sq += g * g;
+        if (h->type == CLOSURE_REG_3D3D || h->type == CLOSURE_REG_3D3D_ELL) {
+            double g[3], sq = 0.0;
+            for (int r = 0; r < 3; ++r)
+                g[r] = m[3 + r] - ((R[3 * r] * m[0] + R[3 * r + 1] * m[1] + R[3 * r + 2] * m[2]) + t[r]);
+            if (h->type == CLOSURE_REG_3D3D) {
+                for (int r = 0; r < 3; ++r) sq += g[r] * g[r];
+            } else {                                       // g^T Lambda g (eq. (6))
+                for (int r = 0; r < 3; ++r)
+                    for (int c = 0; c < 3; ++c) sq += g[r] * m[6 + 3 * r + c] * g[c];
             }
             if (!(sq <= h->betas[i] * h->betas[i])) return false;
-        } else if (h->type == CLOSURE_REPROJ_2D3D) {
+        } else if (h->type == CLOSURE_REPROJ_2D3D || h->type == CLOSURE_REPROJ_2D3D_ELL) {
             double p[3];
             for (int r = 0; r < 3; ++r) p[r] = (R[3 * r] * m[2] + R[3 * r + 1] * m[3] + R[3 * r + 2] * m[4]) + t[r];
             if (!(p[2] > 0.0)) return false;
             const double g0 = m[0] - (h->K[0] * (p[0] / p[2]) + h->K[2]);
             const double g1 = m[1] - (h->K[1] * (p[1] / p[2]) + h->K[3]);
-            if (!(g0 * g0 + g1 * g1 <= h->betas[i] * h->betas[i])) return false;
+            const double sq = h->type == CLOSURE_REPROJ_2D3D
+                                  ? g0 * g0 + g1 * g1
+                                  : g0 * (m[5] * g0 + m[6] * g1) + g1 * (m[7] * g0 + m[8] * g1);
+            if (!(sq <= h->betas[i] * h->betas[i])) return false;
         } else {
             double sr = 0.0, st = 0.0;
             for (int e = 0; e < 9; ++e) sr += (R[e] - m[e]) * (R[e] - m[e]);
@@ -214,6 +223,16 @@ void pack_rows(const closure_t *h, std::vector<double> &rows)
             std::memcpy(r, m, 5 * sizeof(double));
             for (int c = 0; c < 3; ++c) r[2 + c] = m[2 + c] - h->pivot[c];
             r[5] = betas[i]; r[6] = betas[i] * betas[i];
+        } else if (type == CLOSURE_REG_3D3D_ELL) {         // [a - c, b, beta, beta^2, L00 L01 L02 L11 L12 L22]
+            std::memcpy(r, m, 6 * sizeof(double));
+            for (int c = 0; c < 3; ++c) r[c] = m[c] - h->pivot[c];
+            r[6] = betas[i]; r[7] = betas[i] * betas[i];
+            r[8] = m[6]; r[9] = m[7]; r[10] = m[8]; r[11] = m[10]; r[12] = m[11]; r[13] = m[14];
+        } else if (type == CLOSURE_REPROJ_2D3D_ELL) {      // [z, Z - c, beta, beta^2, L00 L01 L11]
+            std::memcpy(r, m, 5 * sizeof(double));
+            for (int c = 0; c < 3; ++c) r[2 + c] = m[2 + c] - h->pivot[c];
+            r[5] = betas[i]; r[6] = betas[i] * betas[i];
+            r[7] = m[5]; r[8] = m[6]; r[9] = m[8];
         } else if (type == CLOSURE_POSE_REG) {
             std::memcpy(r, m, 12 * sizeof(double));
             r[12] = betas[i]; r[13] = betas[i] * betas[i];
@@ -270,11 +289,11 @@ int closure_default_params(int residual_type, closure_params *p)
     p->n_p = 150; p->n_p_star = 10; p->n_t = 15;
     p->gamma = 0.5;
     p->precision = 64;
-    if (residual_type == CLOSURE_REPROJ_2D3D) {       // PAPER.md:374 (t_p rescaled to metres at ~1 m depth)
+    if (residual_type == CLOSURE_REPROJ_2D3D || residual_type == CLOSURE_REPROJ_2D3D_ELL) {   // PAPER.md:374 (t_p rescaled to metres at ~1 m depth)
         p->omega0 = 1.0; p->v0 = 2.0; p->theta_p = 0.2; p->t_p = 0.01;
     } else {
         p->omega0 = 0.5; p->v0 = 0.0; p->theta_p = 0.0; p->t_p = 0.1;
-        if (residual_type != CLOSURE_REG_3D3D) p->n_t = 10;
+        if (residual_type != CLOSURE_REG_3D3D && residual_type != CLOSURE_REG_3D3D_ELL) p->n_t = 10;
     }
     return CLOSURE_OK;
 }
@@ -305,9 +324,26 @@ int closure_create(int residual_type, const double *measurements, int n, const d
     if (!all_finite(measurements, (size_t)n * cols) || !all_finite(betas, nb)) return CLOSURE_EINVAL;
     for (int i = 0; i < nb; ++i)
         if (!(betas[i] > 0.0)) return CLOSURE_EINVAL;
-    if (residual_type == CLOSURE_REPROJ_2D3D) {
+    if (residual_type == CLOSURE_REPROJ_2D3D || residual_type == CLOSURE_REPROJ_2D3D_ELL) {
         if (!intrinsics || !all_finite(intrinsics, 4) || !(intrinsics[0] > 0.0) || !(intrinsics[1] > 0.0))
             return CLOSURE_EINVAL;
+    }
+    if (residual_type == CLOSURE_REG_3D3D_ELL || residual_type == CLOSURE_REPROJ_2D3D_ELL) {
+        // Lambda_i symmetric positive definite (eq. (6)): leading principal minors > 0
+        for (int i = 0; i < n; ++i) {
+            const double *m = measurements + (size_t)i * cols;
+            if (residual_type == CLOSURE_REPROJ_2D3D_ELL) {
+                const double *A = m + 5;
+                if (A[1] != A[2] || !(A[0] > 0.0) || !(A[0] * A[3] - A[1] * A[2] > 0.0)) return CLOSURE_EINVAL;
+            } else {
+                const double *A = m + 6;
+                if (A[1] != A[3] || A[2] != A[6] || A[5] != A[7]) return CLOSURE_EINVAL;
+                const double d2 = A[0] * A[4] - A[1] * A[3];
+                const double d3 = A[0] * (A[4] * A[8] - A[5] * A[7]) - A[1] * (A[3] * A[8] - A[5] * A[6]) +
+                                  A[2] * (A[3] * A[7] - A[4] * A[6]);
+                if (!(A[0] > 0.0) || !(d2 > 0.0) || !(d3 > 0.0)) return CLOSURE_EINVAL;
+            }
+        }
     }
     closure_t *h = new (std::nothrow) closure_s;
     if (!h) return CLOSURE_ENOMEM;
@@ -316,7 +352,7 @@ int closure_create(int residual_type, const double *measurements, int n, const d
     h->P = *p;
     h->meas.assign(measurements, measurements + (size_t)n * cols);
     h->betas.assign(betas, betas + nb);
-    if (residual_type == CLOSURE_REPROJ_2D3D) std::memcpy(h->K, intrinsics, sizeof(h->K));
+    if (residual_type == CLOSURE_REPROJ_2D3D || residual_type == CLOSURE_REPROJ_2D3D_ELL) std::memcpy(h->K, intrinsics, sizeof(h->K));
 
     // pack rows, sorted by the translation-side bound (stable)
     auto key = [&](int i) { return residual_type == CLOSURE_POSE_REG_SPLIT ? betas[2 * i + 1] : betas[i]; };
@@ -366,7 +402,7 @@ int closure_set_pivot(closure_t *h, const double *pivot)
     if (!h) return CLOSURE_EINVAL;
     if (!pivot || !all_finite(pivot, 3)) return fail(h, CLOSURE_EINVAL, "pivot is NULL or not finite");
     const bool nonzero = pivot[0] != 0.0 || pivot[1] != 0.0 || pivot[2] != 0.0;
-    if (nonzero && h->type != CLOSURE_REG_3D3D && h->type != CLOSURE_REPROJ_2D3D)
+    if (nonzero && (h->type == CLOSURE_POSE_REG || h->type == CLOSURE_POSE_REG_SPLIT))
         return fail(h, CLOSURE_EUNSUPPORTED, "a body pivot needs source points (Ex.1 / Ex.2)");
     if (nonzero && h->P.mode != CLOSURE_MODE_ROT)
         return fail(h, CLOSURE_EUNSUPPORTED, "Alg. A8 has no update_rotation: a body pivot applies to the rotation sampler only");
@@ -439,7 +475,9 @@ int closure_init_sample(closure_t *h, long long trial_begin, long long num_trial
 {
     if (!h) return CLOSURE_EINVAL;
     if (trial_begin < 0 || num_trials < 0) return fail(h, CLOSURE_EINVAL, "negative size");
-    if ((h->type == CLOSURE_REG_3D3D || h->type == CLOSURE_REPROJ_2D3D) && h->n < 3) return fail(h, CLOSURE_EINVAL, "RANSAG needs at least 3 correspondences");
+    if (h->type == CLOSURE_REPROJ_2D3D_ELL)
+        return fail(h, CLOSURE_EUNSUPPORTED, "Step I for the ellipse-norm reprojection residual is not built");
+    if ((h->type == CLOSURE_REG_3D3D || h->type == CLOSURE_REG_3D3D_ELL || h->type == CLOSURE_REPROJ_2D3D) && h->n < 3) return fail(h, CLOSURE_EINVAL, "RANSAG needs at least 3 correspondences");
     if (num_trials == 0) return CLOSURE_OK;
     if (!out_poses || !out_ok) return fail(h, CLOSURE_EINVAL, "output buffer is NULL");
     if (reinterpret_cast<uintptr_t>(out_poses) & 15u) return fail(h, CLOSURE_EINVAL, "pose buffer must be 16-byte aligned");

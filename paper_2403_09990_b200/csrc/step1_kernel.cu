@@ -276,7 +276,7 @@ __global__ void __launch_bounds__(kStep1Block) step1_kernel(const InstanceDesc *
     double R[9], t[3];
     bool have = false;
     bool ok = false;
-    if (RES == CLOSURE_REG_3D3D || RES == CLOSURE_REPROJ_2D3D) {
+    if (RES == CLOSURE_REG_3D3D || RES == CLOSURE_REG_3D3D_ELL || RES == CLOSURE_REPROJ_2D3D) {
         uint32_t x[4];
         philox4x32_10(k_lo, 0u, 0u, 2u | k_hi8, s0, s1, x);
         int i1 = (int)(x[0] % (uint32_t)n);
@@ -287,7 +287,7 @@ __global__ void __launch_bounds__(kStep1Block) step1_kernel(const InstanceDesc *
         if (i3 >= lo) ++i3;
         if (i3 >= hi) ++i3;
         const double *r1 = rows + perm[i1] * ROW, *r2 = rows + perm[i2] * ROW, *r3 = rows + perm[i3] * ROW;
-        if (RES == CLOSURE_REG_3D3D) {
+        if (RES == CLOSURE_REG_3D3D || RES == CLOSURE_REG_3D3D_ELL) {
             double a[3][3], b[3][3];
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
@@ -415,6 +415,7 @@ cudaError_t launch_step1(int residual_type, const InstanceDesc *d_desc, int rows
     if (num_trials <= 0) return cudaSuccess;
     switch (residual_type) {
     case CLOSURE_REPROJ_2D3D: return launch_t<CLOSURE_REPROJ_2D3D>(d_desc, rows_bytes, trial_begin, num_trials, seed, out_poses, out_ok, stream);
+    case CLOSURE_REG_3D3D_ELL: return launch_t<CLOSURE_REG_3D3D_ELL>(d_desc, rows_bytes, trial_begin, num_trials, seed, out_poses, out_ok, stream);
     case CLOSURE_REG_3D3D: return launch_t<CLOSURE_REG_3D3D>(d_desc, rows_bytes, trial_begin, num_trials, seed, out_poses, out_ok, stream);
     case CLOSURE_POSE_REG: return launch_t<CLOSURE_POSE_REG>(d_desc, rows_bytes, trial_begin, num_trials, seed, out_poses, out_ok, stream);
     case CLOSURE_POSE_REG_SPLIT: return launch_t<CLOSURE_POSE_REG_SPLIT>(d_desc, rows_bytes, trial_begin, num_trials, seed, out_poses, out_ok, stream);

@@ -114,6 +114,9 @@ template <> struct Res<CLOSURE_REG_3D3D> { static constexpr int ROW = 8, BETA = 
 template <> struct Res<CLOSURE_REPROJ_2D3D> { static constexpr int ROW = 8, BETA = 5; static constexpr bool AFFINE = false; };
 template <> struct Res<CLOSURE_POSE_REG> { static constexpr int ROW = 16, BETA = 12; static constexpr bool AFFINE = true; };
 template <> struct Res<CLOSURE_POSE_REG_SPLIT> { static constexpr int ROW = 16, BETA = 14; static constexpr bool AFFINE = true; };
+// ellipse / ellipsoid norm (eq. (6)): rows [a b beta beta^2 L00 L01 L02 L11 L12 L22] and [z Z beta beta^2 L00 L01 L11]
+template <> struct Res<CLOSURE_REG_3D3D_ELL> { static constexpr int ROW = 16, BETA = 6; static constexpr bool AFFINE = false; };
+template <> struct Res<CLOSURE_REPROJ_2D3D_ELL> { static constexpr int ROW = 10, BETA = 5; static constexpr bool AFFINE = false; };
 
 __device__ __forceinline__ double frob_sq(const double (&R)[9], const double *Ri)
 {
@@ -185,6 +188,25 @@ __device__ __forceinline__ double direct_sq(const double (&R)[9], const double (
         double P0, P1, P2;
         reproj_point(R, row, P0, P1, P2);
         return reproj_sq(P0, P1, P2, t[0], t[1], t[2], row, K);      // cheirality (R-10) inside
+    } else if (RES == CLOSURE_REG_3D3D_ELL) {                        // g^T Lambda g, g = b - (R a + t)
+        const double a0 = row[0], a1 = row[1], a2 = row[2];
+        const double g0 = row[3] - (fma(R[0], a0, fma(R[1], a1, R[2] * a2)) + t[0]);
+        const double g1 = row[4] - (fma(R[3], a0, fma(R[4], a1, R[5] * a2)) + t[1]);
+        const double g2 = row[5] - (fma(R[6], a0, fma(R[7], a1, R[8] * a2)) + t[2]);
+        const double h0 = fma(row[8], g0, fma(row[9], g1, row[10] * g2));
+        const double h1 = fma(row[9], g0, fma(row[11], g1, row[12] * g2));
+        const double h2 = fma(row[10], g0, fma(row[12], g1, row[13] * g2));
+        return fma(g2, h2, fma(g1, h1, g0 * h0));
+    } else if (RES == CLOSURE_REPROJ_2D3D_ELL) {                     // g^T Lambda g, g = z - Pi(K (R Z + t))
+        const double Z0 = row[2], Z1 = row[3], Z2 = row[4];
+        const double p0 = fma(R[0], Z0, fma(R[1], Z1, R[2] * Z2)) + t[0];
+        const double p1 = fma(R[3], Z0, fma(R[4], Z1, R[5] * Z2)) + t[1];
+        const double p2 = fma(R[6], Z0, fma(R[7], Z1, R[8] * Z2)) + t[2];
+        if (!(p2 > 0.0)) return CUDART_INF;                          // cheirality (R-10)
+        const double g0 = row[0] - fma(K[0], p0 / p2, K[2]);
+        const double g1 = row[1] - fma(K[1], p1 / p2, K[3]);
+        const double h0 = fma(row[7], g0, row[8] * g1), h1 = fma(row[8], g0, row[9] * g1);
+        return fma(g1, h1, g0 * h0);
     } else {
         double s = 0.0;
         if (RES == CLOSURE_POSE_REG || part == 0) s = frob_sq(R, row);

@@ -723,6 +723,7 @@ cudaError_t launch_r(const WalkLaunch &L, int n_instances, int max_rows_bytes, i
 
 bool coop_path_available(int residual_type, int mode, int n_p, int max_n)
 {
+    if (residual_type == CLOSURE_REG_3D3D_ELL || residual_type == CLOSURE_REPROJ_2D3D_ELL) return false;   // fp64 kernels only
     return mode == CLOSURE_MODE_ROT && n_p <= 256 && max_n <= 4096;
 }
 

@@ -511,6 +511,8 @@ cudaError_t launch_walkers_coop_trans(int residual_type, const WalkLaunch &L, in
     case CLOSURE_REPROJ_2D3D: return launch_r<CLOSURE_REPROJ_2D3D>(L, n_instances, max_rows_bytes, stream);
     case CLOSURE_POSE_REG: return launch_r<CLOSURE_POSE_REG>(L, n_instances, max_rows_bytes, stream);
     case CLOSURE_POSE_REG_SPLIT: return launch_r<CLOSURE_POSE_REG_SPLIT>(L, n_instances, max_rows_bytes, stream);
+    case CLOSURE_REG_3D3D_ELL: return launch_r<CLOSURE_REG_3D3D_ELL>(L, n_instances, max_rows_bytes, stream);
+    case CLOSURE_REPROJ_2D3D_ELL: return launch_r<CLOSURE_REPROJ_2D3D_ELL>(L, n_instances, max_rows_bytes, stream);
     default: return cudaErrorInvalidValue;
     }
 }

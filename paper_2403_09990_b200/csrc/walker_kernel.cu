@@ -118,6 +118,18 @@ __global__ void __launch_bounds__(kBlock, 2) walker_kernel(const __grid_constant
                         }
                     }
                     if (STATS) { st_pp += (unsigned long long)n * kJT; st_ps += n; }
+                } else if (RES != CLOSURE_REPROJ_2D3D) {
+                    // ellipse / ellipsoid norms (eq. (6)): the residual at the perturbed translation, directly
+                    for (int i = 0; i < n; ++i) {
+                        const double *row = rows + i * ROW;
+                        const double beta = row[RS::BETA];
+#pragma unroll
+                        for (int jj = 0; jj < kJT; ++jj) {
+                            const double tj[3] = { t[0] + e0[jj], t[1] + e1[jj], t[2] + e2[jj] };
+                            dmn[jj] = dmin(dmn[jj], beta - sqrt(direct_sq<RES>(R, tj, row, K, 0)));
+                        }
+                    }
+                    if (STATS) { st_pp += (unsigned long long)n * kJT; st_ps += n; }
                 } else {
                     // REPROJ: P_i = R Z_i + t* once per constraint, then one projection per perturbation
                     for (int i = 0; i < n; ++i) {
@@ -184,6 +196,13 @@ __global__ void __launch_bounds__(kBlock, 2) walker_kernel(const __grid_constant
                         for (int k = 0; k < KCAP; ++k) {
                             const double v = fma(u0, k0[k], fma(u1, k1[k], fma(u2, k2[k], cb)));
                             if (!(v <= kdd[k])) alive &= ~(1u << k);
+                        }
+                    } else if (RES != CLOSURE_REPROJ_2D3D) {
+                        const double b2 = row[RS::BETA + 1];
+#pragma unroll
+                        for (int k = 0; k < KCAP; ++k) {
+                            const double tk[3] = { t[0] + k0[k], t[1] + k1[k], t[2] + k2[k] };
+                            if (!(direct_sq<RES>(Rm, tk, row, K, 0) <= b2)) alive &= ~(1u << k);
                         }
                     } else {
                         double P0, P1, P2;
@@ -306,6 +325,8 @@ int row_doubles(int residual_type)
     case CLOSURE_REPROJ_2D3D: return Res<CLOSURE_REPROJ_2D3D>::ROW;
     case CLOSURE_POSE_REG: return Res<CLOSURE_POSE_REG>::ROW;
     case CLOSURE_POSE_REG_SPLIT: return Res<CLOSURE_POSE_REG_SPLIT>::ROW;
+    case CLOSURE_REG_3D3D_ELL: return Res<CLOSURE_REG_3D3D_ELL>::ROW;
+    case CLOSURE_REPROJ_2D3D_ELL: return Res<CLOSURE_REPROJ_2D3D_ELL>::ROW;
     default: return 0;
     }
 }
@@ -349,6 +370,8 @@ cudaError_t launch_walkers(int residual_type, int mode, bool stats, const WalkLa
     case CLOSURE_REPROJ_2D3D: return launch_r<CLOSURE_REPROJ_2D3D>(mode, stats, L, grid, smem, stream);
     case CLOSURE_POSE_REG: return launch_r<CLOSURE_POSE_REG>(mode, stats, L, grid, smem, stream);
     case CLOSURE_POSE_REG_SPLIT: return launch_r<CLOSURE_POSE_REG_SPLIT>(mode, stats, L, grid, smem, stream);
+    case CLOSURE_REG_3D3D_ELL: return launch_r<CLOSURE_REG_3D3D_ELL>(mode, stats, L, grid, smem, stream);
+    case CLOSURE_REPROJ_2D3D_ELL: return launch_r<CLOSURE_REPROJ_2D3D_ELL>(mode, stats, L, grid, smem, stream);
     default: return cudaErrorInvalidValue;
     }
 }

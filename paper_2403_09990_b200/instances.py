@@ -24,6 +24,8 @@ REPROJ_2D3D = 1
 REG_3D3D = 2
 POSE_REG = 3
 POSE_REG_SPLIT = 4
+REG_3D3D_ELL = 5
+REPROJ_2D3D_ELL = 6
 MODE_ROT = 0
 MODE_TRANS = 1
 
@@ -187,6 +189,30 @@ def make_custom_reg(n: int, seed: int, *, noise: float = 0.05, beta: float = 0.1
     return inst
 
 
+def to_ellipsoidal(inst: Instance, seed: int = 0, lam_min: float = 0.35) -> Instance:
+    """Ellipse / ellipsoid form of a REPROJ_2D3D / REG_3D3D instance (eq. (6) with a general Lambda_i,
+    PAPER.md:58, 179-191): Lambda_i = Q_i diag(lambda) Q_i^T with a random rotation Q_i and eigenvalues uniform in
+    [lam_min, 1].  lambda <= 1 makes every constraint looser than its ball, so the generating pose and every
+    S_0 drawn for the ball form stay inside."""
+    rng = np.random.default_rng(9_000_000 + seed + inst.seed)
+    if inst.residual_type == REG_3D3D:
+        d, ty, head = 3, REG_3D3D_ELL, 6
+    elif inst.residual_type == REPROJ_2D3D:
+        d, ty, head = 2, REPROJ_2D3D_ELL, 5
+    else:
+        raise ValueError("ellipsoidal bounds exist for the residuals with point measurements")
+    lam = np.empty((inst.n, d * d))
+    for i in range(inst.n):
+        Q, _ = np.linalg.qr(rng.standard_normal((d, d)))
+        L = (Q * rng.uniform(lam_min, 1.0, d)) @ Q.T
+        lam[i] = (0.5 * (L + L.T)).reshape(-1)                      # exactly symmetric
+    meas = np.concatenate([np.asarray(inst.measurements)[:, :head], lam], axis=1)
+    out = Instance(inst.name + "_ell", ty, inst.n, meas, np.array(inst.betas, copy=True), inst.intrinsics,
+                   inst.R_gt, inst.t_gt, inst.noise_radius, inst.params, inst.num_walkers, inst.num_steps)
+    out.seed = inst.seed
+    return out
+
+
 def to_split(inst: Instance, beta_r: float = 0.11, beta_t: float = 0.03) -> Instance:
     """PURSEreg form of a POSE_REG instance: two bounds per hypothesis."""
     assert inst.residual_type == POSE_REG
@@ -210,7 +236,7 @@ def _safe_radii(inst: Instance) -> tuple[float, float]:
     slack_i = beta_i - noise_radius_i > 0 is known from how the instance was drawn.
     """
     m = inst.measurements
-    if inst.residual_type == REG_3D3D:
+    if inst.residual_type in (REG_3D3D, REG_3D3D_ELL):        # Lambda <= I: the ball form is the tighter one
         slack = float(np.min(inst.betas - inst.noise_radius))
         lever = float(np.max(np.linalg.norm(m[:, :3], axis=1)))
         # |Exp(phi) R a - R a| <= phi |a| ; residual moves by at most phi*lever + |dt|
@@ -222,7 +248,7 @@ def _safe_radii(inst: Instance) -> tuple[float, float]:
     if inst.residual_type == POSE_REG_SPLIT:
         sl = inst.betas - inst.noise_radius
         return 0.9 * float(np.min(sl[0::2])) / np.sqrt(2.0), 0.9 * float(np.min(sl[1::2]))
-    if inst.residual_type == REPROJ_2D3D:
+    if inst.residual_type in (REPROJ_2D3D, REPROJ_2D3D_ELL):
         slack = float(np.min(inst.betas - inst.noise_radius))         # pixels
         fx, fy = float(inst.intrinsics[0]), float(inst.intrinsics[1])
         lever = float(np.max(np.linalg.norm(m[:, 2:5], axis=1)))

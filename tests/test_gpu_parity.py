@@ -394,3 +394,58 @@ def test_body_pivot_api_edges():
     finally:
         for hb in hs:
             hb.closure_destroy()
+
+
+@pytest.mark.parametrize("config,mode", [(2, "rot"), (3, "rot"), (1, "rot"), (3, "trans"), (2, "trans")])
+def test_ellipsoidal_noise_bounds(config, mode):
+    """Lambda_i != I (eq. (6)): ellipsoids for Ex.2, ellipses for Ex.1, both
+    samplers, on the fp64 kernels."""
+    inst = I.to_ellipsoidal(I.make_instance(config), 3)
+    P = _small(inst.params, n_p=40, n_p_star=4, n_t=8)
+    if mode == "trans":
+        P = _small(P, mode=I.MODE_TRANS, v0=0.05 if config == 2 else P.v0, theta_p=0.03 if config == 2 else P.theta_p)
+    S0 = I.make_init_poses(inst, 32)
+    assert_parity(inst, P, S0, 160, 25, 23)
+    if mode == "rot":                                                  # and with a body pivot
+        assert_parity(inst, _small(P, pivot=(0.2, 0.1, -0.3)), S0, 96, 20, 24)
+
+
+def test_ellipsoidal_api_edges():
+    import torch
+    from oracle import step1
+    inst = I.to_ellipsoidal(I.make_instance(2), 5)
+    h = B.Closure.closure_create(inst)
+    try:
+        poses, ok = h.closure_init_sample(600, 13)                     # Step I: Arun, ellipsoid PURSE test
+        torch.cuda.synchronize()
+        o_poses, o_ok = step1.init_sample(inst, 600, 13)
+        assert np.array_equal(ok.cpu().numpy(), o_ok)
+        assert np.abs(poses.cpu().numpy() - o_poses).max() < 1e-9
+        assert o_ok.mean() > 0.2
+        n0 = h.closure_init_from_trials(600, 13, max_poses=64)
+        res = h.closure_run(2048, 40, 3)
+        assert n0 == 64 and res["count"] > 1500 and res["rot_radius"] > 0
+        with pytest.raises(B.ClosureError) as e:                       # no fp32 kernel for the ellipsoid norm
+            h.closure_set_params(_small(inst.params, precision=32))
+            h.closure_sample(64, 2, 1)
+        assert e.value.status in (B.EUNSUPPORTED, B.ECUDA, B.EINVAL)
+    finally:
+        h.closure_destroy()
+    ell3 = I.to_ellipsoidal(I.make_instance(3), 5)
+    h = B.Closure.closure_create(ell3)
+    try:
+        with pytest.raises(B.ClosureError) as e:
+            h.closure_init_sample(10, 1)
+        assert e.value.status == B.EUNSUPPORTED
+    finally:
+        h.closure_destroy()
+    for bad in ("asym", "indef"):
+        broken = I.to_ellipsoidal(I.make_instance(1), 6)
+        broken.measurements = broken.measurements.copy()
+        if bad == "asym":
+            broken.measurements[0, 7] += 1e-3                          # Lambda[0][1] != Lambda[1][0]
+        else:
+            broken.measurements[0, 6:15] = np.diag([1.0, -0.5, 1.0]).reshape(-1)
+        with pytest.raises(B.ClosureError) as e:
+            B.Closure.closure_create(broken)
+        assert e.value.status == B.EINVAL
