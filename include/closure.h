@@ -53,7 +53,7 @@ extern "C" {
  * (the ellipses / ellipsoids of PAPER.md:179-191): symmetric, positive definite
  * (CLOSURE_EINVAL otherwise).  They run on the one-walker-per-thread fp64 kernel (rotation sampler) and the
  * warp-cooperative fp64 kernel (translation sampler); there is no fp32-certified kernel and no fp32 mode for them.
- * Step I: REG_3D3D_ELL as REG_3D3D; REPROJ_2D3D_ELL is not built (CLOSURE_EUNSUPPORTED). */
+ * Step I: as for the ball forms; the 2D point of Ex.1 is then uniform in the ellipse (R-24). */
 enum { CLOSURE_REPROJ_2D3D = 1, CLOSURE_REG_3D3D = 2, CLOSURE_POSE_REG = 3, CLOSURE_POSE_REG_SPLIT = 4,
        CLOSURE_REG_3D3D_ELL = 5, CLOSURE_REPROJ_2D3D_ELL = 6 };
 

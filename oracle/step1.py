@@ -34,6 +34,7 @@ Ex.1, R-24 (the paper names a P3P solver [22] and says nothing else):
   reduce to a quartic in v (derivation at `p3p_quartic`); every positive real root with u > 0 gives depths, polished
   by three Newton steps on the three distance equations, and the pose is the rigid fit (Arun, exact for a congruent
   triangle) of Z_l -> d_l f_l;
+* ellipse form (Lambda_i != I): y_l = z_l + beta_l L^-T e_l with Lambda_l = L L^T (Cholesky), uniform in the ellipse;
 * up to four poses per trial: they are tried in ascending order of d_1 and the first that satisfies
   (PURSE2D3D) enters S_0 (one pose per trial).
 """
@@ -239,7 +240,14 @@ def p3p_trial(inst, seed: int, k: int):
     ys = []
     for l, i in enumerate(idx):
         e0, e1 = disc_point(seed, k, l)
-        ys.append((meas[i, 0] + betas[i] * e0, meas[i, 1] + betas[i] * e1))
+        if int(inst.residual_type) == REPROJ_2D3D_ELL:
+            # uniform in the ellipse (y - z)^T Lambda (y - z) <= beta^2: with Lambda = L L^T the map
+            # e -> z + beta L^-T e takes the unit disc onto it (a linear map keeps the uniform measure uniform)
+            L = np.linalg.cholesky(meas[i, 5:9].reshape(2, 2))
+            x = np.linalg.solve(L.T, np.array([e0, e1]))
+            ys.append((meas[i, 0] + betas[i] * x[0], meas[i, 1] + betas[i] * x[1]))
+        else:
+            ys.append((meas[i, 0] + betas[i] * e0, meas[i, 1] + betas[i] * e1))
     X = meas[idx, 2:5]
     ac = X - X.mean(axis=0)
     if np.linalg.norm(np.cross(ac[0], ac[1])) < 1e-8:
@@ -265,7 +273,7 @@ def init_sample(inst, num_trials: int, seed: int, trial_begin: int = 0):
             cand = arun(meas[idx, 0:3], meas[idx, 3:6])
         elif ty in (POSE_REG, POSE_REG_SPLIT):
             cand = convex_pose(meas, convex_weights(seed, k, n))
-        elif ty == REPROJ_2D3D:
+        elif ty in (REPROJ_2D3D, REPROJ_2D3D_ELL):
             if n < 3:
                 raise ValueError("RANSAG needs at least 3 correspondences")
             cand = None

@@ -475,9 +475,8 @@ int closure_init_sample(closure_t *h, long long trial_begin, long long num_trial
 {
     if (!h) return CLOSURE_EINVAL;
     if (trial_begin < 0 || num_trials < 0) return fail(h, CLOSURE_EINVAL, "negative size");
-    if (h->type == CLOSURE_REPROJ_2D3D_ELL)
-        return fail(h, CLOSURE_EUNSUPPORTED, "Step I for the ellipse-norm reprojection residual is not built");
-    if ((h->type == CLOSURE_REG_3D3D || h->type == CLOSURE_REG_3D3D_ELL || h->type == CLOSURE_REPROJ_2D3D) && h->n < 3) return fail(h, CLOSURE_EINVAL, "RANSAG needs at least 3 correspondences");
+    if ((h->type == CLOSURE_REG_3D3D || h->type == CLOSURE_REG_3D3D_ELL || h->type == CLOSURE_REPROJ_2D3D ||
+         h->type == CLOSURE_REPROJ_2D3D_ELL) && h->n < 3) return fail(h, CLOSURE_EINVAL, "RANSAG needs at least 3 correspondences");
     if (num_trials == 0) return CLOSURE_OK;
     if (!out_poses || !out_ok) return fail(h, CLOSURE_EINVAL, "output buffer is NULL");
     if (reinterpret_cast<uintptr_t>(out_poses) & 15u) return fail(h, CLOSURE_EINVAL, "pose buffer must be 16-byte aligned");

@@ -276,7 +276,7 @@ __global__ void __launch_bounds__(kStep1Block) step1_kernel(const InstanceDesc *
     double R[9], t[3];
     bool have = false;
     bool ok = false;
-    if (RES == CLOSURE_REG_3D3D || RES == CLOSURE_REG_3D3D_ELL || RES == CLOSURE_REPROJ_2D3D) {
+    if (RES == CLOSURE_REG_3D3D || RES == CLOSURE_REG_3D3D_ELL || RES == CLOSURE_REPROJ_2D3D || RES == CLOSURE_REPROJ_2D3D_ELL) {
         uint32_t x[4];
         philox4x32_10(k_lo, 0u, 0u, 2u | k_hi8, s0, s1, x);
         int i1 = (int)(x[0] % (uint32_t)n);
@@ -312,6 +312,13 @@ __global__ void __launch_bounds__(kStep1Block) step1_kernel(const InstanceDesc *
                             e0 = c0; e1 = c1; found = true;
                         }
                     }
+                }
+                if (RES == CLOSURE_REPROJ_2D3D_ELL) {
+                    // uniform in the ellipse: e <- L^-T e with Lambda = L L^T (rows hold L00 L01 L11 of Lambda at 7..9)
+                    const double l00 = sqrt(rr[l][7]), l10 = rr[l][8] / l00;
+                    const double l11 = sqrt(rr[l][9] - l10 * l10);
+                    e1 = e1 / l11;
+                    e0 = (e0 - l10 * e1) / l00;
                 }
                 const double y0 = __dadd_rn(rr[l][0], __dmul_rn(rr[l][5], e0));
                 const double y1 = __dadd_rn(rr[l][1], __dmul_rn(rr[l][5], e1));
@@ -415,6 +422,7 @@ cudaError_t launch_step1(int residual_type, const InstanceDesc *d_desc, int rows
     if (num_trials <= 0) return cudaSuccess;
     switch (residual_type) {
     case CLOSURE_REPROJ_2D3D: return launch_t<CLOSURE_REPROJ_2D3D>(d_desc, rows_bytes, trial_begin, num_trials, seed, out_poses, out_ok, stream);
+    case CLOSURE_REPROJ_2D3D_ELL: return launch_t<CLOSURE_REPROJ_2D3D_ELL>(d_desc, rows_bytes, trial_begin, num_trials, seed, out_poses, out_ok, stream);
     case CLOSURE_REG_3D3D_ELL: return launch_t<CLOSURE_REG_3D3D_ELL>(d_desc, rows_bytes, trial_begin, num_trials, seed, out_poses, out_ok, stream);
     case CLOSURE_REG_3D3D: return launch_t<CLOSURE_REG_3D3D>(d_desc, rows_bytes, trial_begin, num_trials, seed, out_poses, out_ok, stream);
     case CLOSURE_POSE_REG: return launch_t<CLOSURE_POSE_REG>(d_desc, rows_bytes, trial_begin, num_trials, seed, out_poses, out_ok, stream);

@@ -134,6 +134,13 @@ def test_p3p_trials_match_oracle():
     assert np.array_equal(full[0][150:250], part[0]) and np.array_equal(full[1][150:250], part[1])
 
 
+def test_p3p_trials_with_elliptic_bounds_match_oracle():
+    """Ex.1 with Lambda_i != I: the 2D points are uniform in the ellipses, the PURSE test uses the ellipse norm."""
+    ell = I.to_ellipsoidal(I.make_instance(3), 2)
+    ok = _compare_p3p(ell, 1500, 19)
+    assert ok.mean() > 0.02
+
+
 def test_p3p_candidates_reproject_onto_the_sampled_pixels_and_feed_the_walk():
     """Property at any size: an accepted pose maps the three selected 3D points onto the three sampled pixels
     (each within its own ellipse), and satisfies every constraint of the instance."""

@@ -239,3 +239,23 @@ def test_disc_points_and_p3p_trials_on_config_3():
                 px = np.array([K[0] * pc[0] / pc[2] + K[2], K[1] * pc[1] / pc[2] + K[3]])
                 assert pc[2] > 0 and np.abs(px - np.array(y)).max() < 1e-7
     assert n_sol > 200
+
+
+def test_p3p_points_are_uniform_in_the_ellipse_for_elliptic_bounds():
+    """Lambda_i != I (eq. (6)): the sampled pixel satisfies (y - z)^T Lambda (y - z) <= beta^2, and that normalised
+    quadratic form is distributed like r^2 of a uniform point of the unit disc (mean 1/2, P(< 1/4) = 1/4)."""
+    ell = I.to_ellipsoidal(I.make_instance(3), 2)
+    meas, betas = np.asarray(ell.measurements), np.asarray(ell.betas).reshape(-1)
+    vals = []
+    for k in range(800):
+        _, _, (idx, ys) = step1.p3p_trial(ell, 3, k)
+        for i, y in zip(idx, ys):
+            d = np.array(y) - meas[i, 0:2]
+            vals.append(d @ meas[i, 5:9].reshape(2, 2) @ d / betas[i] ** 2)
+    vals = np.array(vals)
+    assert vals.max() <= 1.0 + 1e-12
+    assert abs(vals.mean() - 0.5) < 0.02 and abs((vals < 0.25).mean() - 0.25) < 0.02
+    poses, ok = step1.init_sample(ell, 400, 3)
+    assert ok.sum() >= 5
+    for q in np.nonzero(ok)[0]:
+        assert oracle.in_purse(ell, poses[q, :9], poses[q, 9:])
