@@ -59,6 +59,14 @@ __device__ __forceinline__ uint32_t fkey(float x)
     const uint32_t b = __float_as_uint(x);
     return b ^ ((uint32_t)((int32_t)b >> 31) | 0x80000000u);
 }
+// MUFU.RSQ alone: rsqrtf() adds a rescaling path for subnormal arguments; callers pass a >= 1e-30 (normal), for
+// which both return the same bits
+__device__ __forceinline__ float rsqrt_normal(float a)
+{
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a));
+    return r;
+}
 __device__ __forceinline__ float fkey_inv(uint32_t k)
 {
     return __uint_as_float((k & 0x80000000u) ? (k ^ 0x80000000u) : ~k);

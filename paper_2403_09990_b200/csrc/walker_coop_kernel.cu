@@ -523,7 +523,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __gr
                 for (int q = 0; q < NQ; ++q) {
                     // a ~ max_i |u_i - d|^2 within E0 + 2^-22 a;  sq ~ sqrt(a) within 2^-21 relative
                     const float a = fmaxf(mx[q] + dd[q], 1e-30f);
-                    const float rr = rsqrtf(a);
+                    const float rr = rsqrt_normal(a);
                     const float sq = a * rr;
                     const float du = 1.01f * fmaf(E0, rr, (bf + sq) * kMu19);
                     unc_l = fmaxf(unc_l, du);

@@ -298,7 +298,7 @@ __global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(cons
 #pragma unroll
                     for (int q = 0; q < NQ; ++q) {
                         const float a = fmaxf(mx[q], 1e-30f);
-                        dv[q] = fminf(dv[q], bf - a * rsqrtf(a));
+                        dv[q] = fminf(dv[q], bf - a * rsqrt_normal(a));
                     }
                 }
 #pragma unroll
