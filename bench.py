@@ -40,9 +40,9 @@ FLOP_PAIR, FLOP_SETUP_A, FLOP_SETUP_L = 7.0, 26.0, 27.0
 # reprojection residual: eq. (14) pair = 4 FMA + RCP + 3 MUL + max = 13; cone pair = 8 FMA + max = 17
 FLOP_PAIR_REPROJ_A, FLOP_PAIR_REPROJ_L = 13.0, 17.0
 # DRAM traffic of the walker kernel per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the committed
-# `ncu --set full` captures of this very command line: profiles/r1_v5_final_ncu.md (C2, default arguments)
+# `ncu --set full` captures of this very command line: profiles/r1_v6_final_ncu.md (C2, default arguments)
 # and profiles/r1_v4_reproj_megb_ncu.md (--config 3).  Other workloads have no capture: null.
-NCU_TRAFFIC_BYTES = {("C2_reg_n50", "rot", 64): 494336 + 0, ("C3_reproj_n8", "rot", 64): 549376 + 776448}
+NCU_TRAFFIC_BYTES = {("C2_reg_n50", "rot", 64): 500480 + 63744, ("C3_reproj_n8", "rot", 64): 549376 + 776448}
 
 
 def _params_dict(P) -> dict:
