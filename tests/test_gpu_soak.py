@@ -1,7 +1,8 @@
 """-m gpu: randomised comparison of the certified kernels with the plain fp64 kernel (CLOSURE_FLAG_EXACT_ONLY).
 
 Random config, instance, walk parameters, |S_0|, mode and seed per run; samples and flags must agree bit for bit.
-(The same loop ran for 15 minutes at the end of round 1: 8,349 runs, 68 M walkers, no mismatch -- DESIGN.md 8.)"""
+(The same loop ran for 15 minutes twice in round 1, the second time on the final build with random bound runs and
+body pivots as below: 8,349 + 8,080 runs, 68 M + 66 M walkers, no mismatch -- DESIGN.md 8.)"""
 import copy
 
 import numpy as np
@@ -33,6 +34,11 @@ def test_random_parameters_bit_identical_to_plain_kernel(stream):
             P.theta_p = float(rng.choice([0.02, 0.1, 0.2, 0.35]))
             P.v0 = float(rng.choice([0.01, 0.05, 0.3, 2.0]))
             P.flags = int(rng.choice([0, 64]))
+        if cfg in (1, 2, 5) and rng.random() < 0.5:          # several runs of equal bounds, odd lengths
+            k = int(rng.integers(1, 5))
+            inst.betas = inst.betas * rng.choice([1.0, 1.2, 1.5, 1.9][:k], size=inst.n)
+        if P.mode != I.MODE_TRANS and cfg in (1, 2, 3, 5) and rng.random() < 0.3:
+            P.pivot = tuple(float(x) for x in rng.uniform(-0.5, 0.5, 3))      # closure_set_pivot (gpu_walk applies it)
         S0 = I.make_init_poses(inst, int(rng.choice([1, 16, 128])))
         W, S, seed = 2048, int(rng.choice([50, 150])), int(rng.integers(0, 1 << 40))
         a = gpu_walk(inst, P, S0, W, S, seed, trace=False)
