@@ -254,15 +254,19 @@ def test_fp32_mode_is_refused_where_it_does_not_exist():
     assert e.value.status == B.EUNSUPPORTED
 
 
-@pytest.mark.parametrize("kind", ["reproj", "reg", "posereg", "split"])
+@pytest.mark.parametrize("kind", ["reproj", "reg", "posereg", "split", "reproj_ell", "reg_ell"])
 def test_cooperative_translation_sampler_is_bit_identical_to_plain_kernel(kind):
     """Alg. A8 on the warp-cooperative fp64 kernel against the one-walker-per-thread kernel
     (CLOSURE_FLAG_EXACT_ONLY): same fp64 functions, so samples, flags and traces must be identical."""
-    if kind == "reproj":
+    if kind in ("reproj", "reproj_ell"):
         inst = I.make_instance(3)
+        if kind == "reproj_ell":
+            inst = I.to_ellipsoidal(inst, 1)
         P = _small(inst.params, mode=I.MODE_TRANS, v0=0.05, theta_p=0.02)
-    elif kind == "reg":
+    elif kind in ("reg", "reg_ell"):
         inst = I.make_instance(2)
+        if kind == "reg_ell":
+            inst = I.to_ellipsoidal(inst, 1)
         P = _small(inst.params, mode=I.MODE_TRANS, v0=0.1, theta_p=0.02, n_p=70, n_p_star=7)
     else:
         inst = I.make_instance(4)
