@@ -28,6 +28,10 @@
 #include "walker_common.cuh"
 #include "walker_coop_common.cuh"
 
+#ifndef CLOSURE_COOP_MIN_CTAS
+#define CLOSURE_COOP_MIN_CTAS 4   // resident CTAs per SM the register allocation aims at (128 registers per thread)
+#endif
+
 namespace closure {
 namespace {
 
@@ -290,7 +294,7 @@ __device__ __forceinline__ uint32_t eq14_constraint_major(const float4 *rowsA, c
 
 // ---------------------------------------------------------------------------------- the kernel
 template <int RES, int NQ>
-__global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_kernel(const __grid_constant__ WalkLaunch L)
+__global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_coop_kernel(const __grid_constant__ WalkLaunch L)
 {
     using RS = Res<RES>;
     constexpr int ROW = RS::ROW;

@@ -25,6 +25,10 @@
 #include "walker_common.cuh"
 #include "walker_coop_common.cuh"
 
+#ifndef CLOSURE_COOP_MIN_CTAS
+#define CLOSURE_COOP_MIN_CTAS 4   // resident CTAs per SM the register allocation aims at (128 registers per thread)
+#endif
+
 namespace closure {
 namespace {
 
@@ -138,7 +142,7 @@ __device__ __forceinline__ float cone_lo(const float4 &ra, const float4 &rb, con
 
 // ---------------------------------------------------------------------------------- the kernel
 template <int NQ>
-__global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_reproj_kernel(const __grid_constant__ WalkLaunch L)
+__global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_coop_reproj_kernel(const __grid_constant__ WalkLaunch L)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int n_runs_s;

@@ -40,6 +40,10 @@
 #include "walker_common.cuh"
 #include "walker_coop_common.cuh"
 
+#ifndef CLOSURE_COOP_MIN_CTAS
+#define CLOSURE_COOP_MIN_CTAS 4   // resident CTAs per SM the register allocation aims at (128 registers per thread)
+#endif
+
 namespace closure {
 namespace {
 
@@ -98,7 +102,7 @@ struct ExactMarginTrans {
 };
 
 template <int RES, int NQ>
-__global__ void __launch_bounds__(kCoopThreads, 4) walker_coop_trans_kernel(const __grid_constant__ WalkLaunch L)
+__global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_coop_trans_kernel(const __grid_constant__ WalkLaunch L)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
