@@ -35,6 +35,13 @@
 namespace closure {
 namespace {
 
+// Measured on B200: the registration kernel gains nothing from more resident warps (C2 +0.5 % at 5
+// or 6 CTAs), the pose-regression kernel, whose rows are twice as long, gains 3.7 % at 6 CTAs (80 registers).
+template <int RES> constexpr int coop_min_ctas()
+{
+    return (RES == CLOSURE_POSE_REG || RES == CLOSURE_POSE_REG_SPLIT) && CLOSURE_COOP_MIN_CTAS == 4 ? 6 : CLOSURE_COOP_MIN_CTAS;
+}
+
 // fp32 image of one set-up row and the bound eps on |v32 - v64| for ANY perturbation with
 // |d_c| <= t_p, where v = c - 2 u.d is evaluated as three chained FMAs:
 //   inputs: (u, c) rounded to fp32 (relative 2^-24 each); e = -2 d from pm1f (absolute 6 * 2^-24 * 2 t_p);
@@ -294,7 +301,7 @@ __device__ __forceinline__ uint32_t eq14_constraint_major(const float4 *rowsA, c
 
 // ---------------------------------------------------------------------------------- the kernel
 template <int RES, int NQ>
-__global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_coop_kernel(const __grid_constant__ WalkLaunch L)
+__global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES>()) walker_coop_kernel(const __grid_constant__ WalkLaunch L)
 {
     using RS = Res<RES>;
     constexpr int ROW = RS::ROW;
