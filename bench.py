@@ -170,6 +170,12 @@ def run_cuda(args) -> None:
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if not os.path.exists(B.LIB_PATH):      # a checkout without the built library (git-ignored): compile it once
+        if rank == 0:
+            from paper_2403_09990_b200 import build as build_mod
+            build_mod.build_library()
+        if world > 1:
+            dist.barrier()
     B.load_library()     # fails loudly if libclosure_b200.so is missing
 
     inst, S0 = _workload(args.config)
