@@ -283,6 +283,8 @@ def run_cuda(args) -> None:
         achieved = flops / walk_s / 1e12
         t_min = flops64 / peak64 + flops32 / peak32
         peak_mix = flops / t_min / 1e12
+        nom_mhz = float(clk.get("sm_max_mhz") or 1965.0)
+        nom32, nom64 = 148 * 128 * 2 * nom_mhz * 1e6, 148 * 64 * 2 * nom_mhz * 1e6
         # the integer work a flop count does not see: one Philox4x32-10 call per perturbation and iteration
         philox_calls = float(st["walker_steps"]) * (P.n_p + 1)
         t_min_rng = t_min + philox_calls / peak_philox
@@ -428,6 +430,9 @@ def run_cuda(args) -> None:
                          "fp32": {"flops_per_launch": flops32, "achieved": flops32 / walk_s / 1e12, "peak": peak32 / 1e12},
                          "fp64": {"flops_per_launch": flops64, "achieved": flops64 / walk_s / 1e12, "peak": peak64 / 1e12},
                          "flops_per_launch": flops,
+                         # the unit-count peak of SURVEY.md 8(d): 148 SMs x 128 FP32 (64 FP64) lanes x 2 x the maximum SM clock
+                         "frac_of_nominal": (flops32 / nom32 + flops64 / nom64) / walk_s,
+                         "peak_nominal": {"fp32": nom32 / 1e12, "fp64": nom64 / 1e12, "sm_mhz": nom_mhz},
                          "philox": {"calls_per_launch": philox_calls, "peak_calls_per_s": peak_philox,
                                     "note": "Philox4x32-10 calls at the rate of a kernel that does nothing else"},
                          "frac_incl_philox": t_min_rng / walk_s,
