@@ -323,29 +323,27 @@ def run_cuda(args) -> None:
         # Step I on the device (not part of the timed step): trials -> compaction -> S_0 for
         # 1,000 trials end to end, and the trial kernel alone at the 100,000 trials of the paper's pure-RANSAG
         # comparison.  Ex.1: P3P trials; Ex.2: Arun; Ex.3: convex combinations.
-        step1 = None
-        if True:
-            hs1 = B.Closure.closure_create(insts[0])
-            t_s1 = []
-            for k in range(12):
-                t1 = time.perf_counter()
-                n0_s1 = hs1.closure_init_from_trials(1000, WALK_SEED + k, 128, stream)
-                t_s1.append(1e3 * (time.perf_counter() - t1))
-            p_s1 = torch.empty((100000, 12), dtype=torch.float64, device=dev)
-            o_s1 = torch.empty((100000,), dtype=torch.uint8, device=dev)
-            k_s1 = []
-            for k in range(6):
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record(stream)
-                hs1.closure_init_sample(100000, WALK_SEED + k, p_s1, o_s1, stream)
-                e1.record(stream)
-                torch.cuda.synchronize()
-                k_s1.append(e0.elapsed_time(e1))
-            step1 = {"ms_1000_trials_to_S0_end_to_end": statistics.median(t_s1[2:]), "S0_size": n0_s1,
-                     "kernel_ms_100000_trials": statistics.median(k_s1[1:]),
-                     "accepted_fraction": float(o_s1.float().mean().item())}
-            hs1.closure_destroy()
-            del p_s1, o_s1
+        hs1 = B.Closure.closure_create(insts[0])
+        t_s1 = []
+        for k in range(12):
+            t1 = time.perf_counter()
+            n0_s1 = hs1.closure_init_from_trials(1000, WALK_SEED + k, 128, stream)
+            t_s1.append(1e3 * (time.perf_counter() - t1))
+        p_s1 = torch.empty((100000, 12), dtype=torch.float64, device=dev)
+        o_s1 = torch.empty((100000,), dtype=torch.uint8, device=dev)
+        k_s1 = []
+        for k in range(6):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            hs1.closure_init_sample(100000, WALK_SEED + k, p_s1, o_s1, stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            k_s1.append(e0.elapsed_time(e1))
+        step1 = {"ms_1000_trials_to_S0_end_to_end": statistics.median(t_s1[2:]), "S0_size": n0_s1,
+                 "kernel_ms_100000_trials": statistics.median(k_s1[1:]),
+                 "accepted_fraction": float(o_s1.float().mean().item())}
+        hs1.closure_destroy()
+        del p_s1, o_s1
 
         fp32_report = None
         if args.precision == 32:

@@ -184,7 +184,6 @@ __device__ __forceinline__ double direct_sq(const double (&R)[9], const double (
         const double g2 = row[5] - (fma(R[6], a0, fma(R[7], a1, R[8] * a2)) + t[2]);
         return fma(g2, g2, fma(g1, g1, g0 * g0));
     } else if (RES == CLOSURE_REPROJ_2D3D) {
-        const double Z0 = row[2], Z1 = row[3], Z2 = row[4];
         double P0, P1, P2;
         reproj_point(R, row, P0, P1, P2);
         return reproj_sq(P0, P1, P2, t[0], t[1], t[2], row, K);      // cheirality (R-10) inside

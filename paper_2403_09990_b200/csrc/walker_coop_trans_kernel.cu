@@ -145,7 +145,6 @@ __global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_co
     const long long local = (long long)blockIdx.x * kCoopWarps + warp;
     if (local >= L.num_walkers) return;                // no block-wide barrier below this line
     unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
-    double *pose = reinterpret_cast<double *>(wp + lay.pose);
     double *dex = reinterpret_cast<double *>(wp + lay.dex);
     double *Rc = reinterpret_cast<double *>(wp + lay.Rc);
     int *candj = reinterpret_cast<int *>(wp + lay.candj);
