@@ -78,6 +78,7 @@ __device__ __forceinline__ void exact_margins(const double (&R)[9], const double
         d[q] = rot_margin;
     }
 #pragma unroll 1
+#pragma unroll 1
     for (int i = 0; i < n; ++i) {
         const double *row = rows + i * ROW;
         double u0, u1, u2, c;
@@ -130,6 +131,7 @@ __device__ __forceinline__ bool exact_candidate_feasible(const double (&Rm)[9], 
     const double kdd = -fma(d2, d2, fma(d1, d1, d0 * d0));
     const double k0 = -2.0 * d0, k1 = -2.0 * d1, k2 = -2.0 * d2;
     bool ok = true;
+#pragma unroll 1
     for (int i = lane; i < n; i += 32) {
         const double *row = rows + i * ROW;
         double u0, u1, u2, c;
@@ -175,6 +177,7 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
     for (int e = 0; e < 3; ++e) { t[e] = pose[9 + e]; vel[e] = pose[12 + e]; }
     float eps_l = 0.f;
     double rm_l = CUDART_INF;
+#pragma unroll 1
     for (int i = lane; i < n; i += 32) {
         const double *row = rows + i * ROW;
         double u0, u1, u2, c;
@@ -217,6 +220,7 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
 #pragma unroll
             for (int e = 0; e < 9; ++e) lip = fma(dR[e], dR[e], lip);      // ||R_m - R*||_F^2
         }
+#pragma unroll 1
         for (int i = lane; i < n; i += 32) {
             const double *row = rows + i * ROW;
             double u0, u1, u2, c;
@@ -505,7 +509,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES>()) walker_coo
                     mx[0] = lane < n_p ? fkey_inv(key) : 1.0f;
                     pp = pend;
                 }
-#pragma unroll(NQ <= 2 ? 4 : 2)
+#pragma unroll(NQ <= 2 ? 4 : 1)   // measured: unrolling the NQ = 5 body further costs 2-4 % (C2, C4)
                 for (; pp < pend; ++pp) {
                     // two constraints a, b per entry: X = (f0a f0b f1a f1b), Y = (f2a f2b fca fcb)
                     const float4 X = rowsA[2 * pp], Y = rowsA[2 * pp + 1];
@@ -617,6 +621,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES>()) walker_coo
                     __syncwarp();                            // earlier readers of rowsL are done
                     float eps_l = 0.f;
                     bool rdead = false;
+#pragma unroll 1
                     for (int i = lane; i < n; i += 32) {
                         const double *row = rows + i * ROW;
                         double u0, u1, u2, c;

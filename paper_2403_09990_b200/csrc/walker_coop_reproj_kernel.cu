@@ -121,6 +121,7 @@ __device__ __forceinline__ bool exact_candidate_feasible_reproj(const double (&R
     rng.xi3(s, (uint32_t)j, 1u, x, y, z);
     const double k0 = t_p * x, k1 = t_p * y, k2 = t_p * z;
     bool ok = true;
+#pragma unroll 1
     for (int i = lane; i < n; i += 32) {
         const double *row = rows + i * ROW;
         double P0, P1, P2;
@@ -258,6 +259,7 @@ __global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_co
 #pragma unroll
             for (int e = 0; e < 4; ++e) K[e] = D->K[e];
             float unc_l = 0.f;
+#pragma unroll 1
             for (int i = lane; i < n; i += 32) {
                 const double *row = rows + i * ROW;
                 double P0, P1, P2;
@@ -290,6 +292,7 @@ __global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_co
                 b1.a = b1.b = b2.a = b2.b = make_float4(0.f, 0.f, 0.f, 0.f);
                 b1.b.z = b2.b.z = -CUDART_INF_F;            // a row that never kills
                 double lip = 0.0;
+#pragma unroll 1
                 for (int i = lane; i < n; i += 32) {
                     const double *row = rows + i * ROW;
                     double P0, P1, P2, Q0, Q1, Q2;
@@ -359,6 +362,7 @@ __global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_co
                 float mx[NQ];
 #pragma unroll
                 for (int q = 0; q < NQ; ++q) mx[q] = 0.f;
+#pragma unroll 1                         // measured: +2 % at C3 against the default unrolling
                 for (; i <= end; ++i) {
                     const float4 ra = rowsA[2 * i], rb = rowsA[2 * i + 1];
 #pragma unroll
@@ -448,6 +452,7 @@ __global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_co
                 if (full_m != m1) {
                     __syncwarp();                            // earlier readers of rowsL are done
                     float eps_l = 0.f;
+#pragma unroll 1
                     for (int i = lane; i < n; i += 32) {
                         const double *row = rows + i * ROW;
                         double Q0, Q1, Q2;
