@@ -24,7 +24,7 @@ struct CoopSmem {
 
 // Shared-memory layout; f4 = float4 words per fp32 constraint row (1: affine residuals, 2: reprojection);
 // pairs = 32-byte entries of rowsA (affine: pair-entries, runs padded to even length; otherwise n)
-__host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, int nq, int f4, int pairs)
+__host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, int nq, int f4, int pairs, int warps = kCoopWarps)
 {
     CoopSmem s;
     size_t o = 16 + (size_t)((rows_bytes + 15) & ~15);
@@ -48,7 +48,7 @@ __host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, 
     s.pose = w;  w += 18 * 8;
     s.stc = w;   w += 16 * 8;
     s.per_warp = w;
-    s.total = o + (size_t)kCoopWarps * w;
+    s.total = o + (size_t)warps * w;
     return s;
 }
 

@@ -32,6 +32,12 @@
 namespace closure {
 namespace {
 
+// One walker (warp) per CTA: the staged table is 8-10 rows, so nothing is gained by sharing it, and a CTA's slot is
+// free again as soon as its walker ends instead of when the slowest of four does (measured at C3: 474 -> 496 M
+// walker-steps/s; the affine kernels, with tables of 50-200 rows, do not gain and keep kCoopWarps = 4).
+constexpr int kReprojWarps = 1;
+constexpr int kReprojThreads = 32 * kReprojWarps;
+
 constexpr int RES = CLOSURE_REPROJ_2D3D;
 constexpr int ROW = Res<RES>::ROW;
 constexpr int BETA = Res<RES>::BETA;
@@ -143,7 +149,7 @@ __device__ __forceinline__ float cone_lo(const float4 &ra, const float4 &rb, con
 
 // ---------------------------------------------------------------------------------- the kernel
 template <int NQ>
-__global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_coop_reproj_kernel(const __grid_constant__ WalkLaunch L)
+__global__ void __launch_bounds__(kReprojThreads, CLOSURE_COOP_MIN_CTAS * (kCoopWarps / kReprojWarps)) walker_coop_reproj_kernel(const __grid_constant__ WalkLaunch L)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int n_runs_s;
@@ -155,7 +161,7 @@ __global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_co
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
     double *rows = reinterpret_cast<double *>(smem_raw + 16);
     stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
-    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 2, n);
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 2, n, kReprojWarps);
     int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
     float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
     if (warp == 0) {                                   // runs of equal bounds (rows are sorted by bound)
@@ -181,7 +187,7 @@ __global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_co
     __syncthreads();
     const int n_runs = n_runs_s;
 
-    const long long local = (long long)blockIdx.x * kCoopWarps + warp;
+    const long long local = (long long)blockIdx.x * kReprojWarps + warp;
     if (local >= L.num_walkers) return;                // no block-wide barrier below this line
     unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
     float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);   // [n][2]
@@ -533,15 +539,15 @@ __global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_co
 template <int NQ>
 cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
 {
-    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 2, max_n);
+    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 2, max_n, kReprojWarps);
     if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaFuncSetAttribute(walker_coop_reproj_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)lay.total);
     if (e != cudaSuccess) return e;
-    const long long blocks = (L.num_walkers + kCoopWarps - 1) / kCoopWarps;
+    const long long blocks = (L.num_walkers + kReprojWarps - 1) / kReprojWarps;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     dim3 grid((unsigned)blocks, (unsigned)n_instances, 1);
-    walker_coop_reproj_kernel<NQ><<<grid, kCoopThreads, lay.total, stream>>>(L);
+    walker_coop_reproj_kernel<NQ><<<grid, kReprojThreads, lay.total, stream>>>(L);
     return cudaGetLastError();
 }
 
