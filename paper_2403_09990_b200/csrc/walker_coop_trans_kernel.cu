@@ -53,9 +53,13 @@ struct TransSmem {
     size_t run_end, run_bf, warp0, per_warp, pose, dex, Rc, candj, candd, stc, rowsA, crow, betaf, Dc, krow, sT, total;
 };
 
+// Walkers (warps) per CTA: one for the reprojection residual (tables of 8-10 rows: a CTA's slot is free as soon as its
+// walker ends; measured at C3 in TRANS mode 236 -> 248 M walker-steps/s), kCoopWarps for the residuals with long tables.
+template <int RES> constexpr int kTransWarps = (RES == CLOSURE_REPROJ_2D3D) ? 1 : kCoopWarps;
+
 constexpr int kKrowMax = 512;                  // (candidate, constraint) rows of the certified ladder
 
-__host__ __device__ inline TransSmem trans_layout(int rows_bytes, int nq, int n_fast)
+__host__ __device__ inline TransSmem trans_layout(int rows_bytes, int nq, int n_fast, int warps)
 {
     TransSmem s;
     size_t o = 16 + (size_t)((rows_bytes + 15) & ~15);
@@ -76,7 +80,7 @@ __host__ __device__ inline TransSmem trans_layout(int rows_bytes, int nq, int n_
     s.krow = w;  w += (n_fast ? (size_t)kKrowMax * 16 : 0);     // cone rows of (candidate, constraint) at step 0
     s.sT = w;    w += (n_fast ? 64 * 4 : 0);                    // ladder steps dT_m in fp32
     s.per_warp = w;
-    s.total = o + (size_t)kCoopWarps * w;
+    s.total = o + (size_t)warps * w;
     return s;
 }
 
@@ -102,7 +106,7 @@ struct ExactMarginTrans {
 };
 
 template <int RES, int NQ>
-__global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_coop_trans_kernel(const __grid_constant__ WalkLaunch L)
+__global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS * (kCoopWarps / kTransWarps<RES>)) walker_coop_trans_kernel(const __grid_constant__ WalkLaunch L)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -113,7 +117,7 @@ __global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_co
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
     const double *rows = reinterpret_cast<const double *>(smem_raw + 16);
     stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
-    const TransSmem lay = trans_layout(rows_bytes, NQ, RES == CLOSURE_REPROJ_2D3D ? n : 0);
+    const TransSmem lay = trans_layout(rows_bytes, NQ, RES == CLOSURE_REPROJ_2D3D ? n : 0, kTransWarps<RES>);
     __shared__ int n_runs_s;
     int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
     float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
@@ -142,7 +146,7 @@ __global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_co
     }
     const int n_runs = (RES == CLOSURE_REPROJ_2D3D) ? n_runs_s : 0;
 
-    const long long local = (long long)blockIdx.x * kCoopWarps + warp;
+    const long long local = (long long)blockIdx.x * kTransWarps<RES> + warp;
     if (local >= L.num_walkers) return;                // no block-wide barrier below this line
     unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
     double *dex = reinterpret_cast<double *>(wp + lay.dex);
@@ -483,15 +487,15 @@ __global__ void __launch_bounds__(kCoopThreads, CLOSURE_COOP_MIN_CTAS) walker_co
 template <int RES, int NQ>
 cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, cudaStream_t stream)
 {
-    const TransSmem lay = trans_layout(max_rows_bytes, NQ, RES == CLOSURE_REPROJ_2D3D ? max_rows_bytes / (Res<RES>::ROW * 8) : 0);
+    const TransSmem lay = trans_layout(max_rows_bytes, NQ, RES == CLOSURE_REPROJ_2D3D ? max_rows_bytes / (Res<RES>::ROW * 8) : 0, kTransWarps<RES>);
     if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaFuncSetAttribute(walker_coop_trans_kernel<RES, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)lay.total);
     if (e != cudaSuccess) return e;
-    const long long blocks = (L.num_walkers + kCoopWarps - 1) / kCoopWarps;
+    const long long blocks = (L.num_walkers + kTransWarps<RES> - 1) / kTransWarps<RES>;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     dim3 grid((unsigned)blocks, (unsigned)n_instances, 1);
-    walker_coop_trans_kernel<RES, NQ><<<grid, kCoopThreads, lay.total, stream>>>(L);
+    walker_coop_trans_kernel<RES, NQ><<<grid, 32 * kTransWarps<RES>, lay.total, stream>>>(L);
     return cudaGetLastError();
 }
 
