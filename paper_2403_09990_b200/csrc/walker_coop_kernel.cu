@@ -35,11 +35,14 @@
 namespace closure {
 namespace {
 
-// Measured on B200: the registration kernel gains nothing from more resident warps (C2 +0.5 % at 5
-// or 6 CTAs), the pose-regression kernel, whose rows are twice as long, gains 3.7 % at 6 CTAs (80 registers).
-template <int RES> constexpr int coop_min_ctas()
+// Measured on B200: the pose-regression kernel, whose rows are twice as long, gains 3.7 % at 6 resident
+// CTAs (80 registers); the registration kernel gains 1 % at 5 (96 registers) in the NQ = 5 instantiation (64 < N_P <= 160: C2) and stays at 4 for
+// fewer perturbations, where the table of a C5-sized instance allows 4 CTAs anyway.
+template <int RES, int NQ> constexpr int coop_min_ctas()
 {
-    return (RES == CLOSURE_POSE_REG || RES == CLOSURE_POSE_REG_SPLIT) && CLOSURE_COOP_MIN_CTAS == 4 ? 6 : CLOSURE_COOP_MIN_CTAS;
+    if (CLOSURE_COOP_MIN_CTAS != 4) return CLOSURE_COOP_MIN_CTAS;
+    if (RES == CLOSURE_POSE_REG || RES == CLOSURE_POSE_REG_SPLIT) return 6;
+    return NQ == 5 ? 5 : 4;
 }
 
 // fp32 image of one set-up row and the bound eps on |v32 - v64| for ANY perturbation with
@@ -305,7 +308,7 @@ __device__ __forceinline__ uint32_t eq14_constraint_major(const float4 *rowsA, c
 
 // ---------------------------------------------------------------------------------- the kernel
 template <int RES, int NQ>
-__global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES>()) walker_coop_kernel(const __grid_constant__ WalkLaunch L)
+__global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker_coop_kernel(const __grid_constant__ WalkLaunch L)
 {
     using RS = Res<RES>;
     constexpr int ROW = RS::ROW;
