@@ -37,6 +37,8 @@ namespace {
 // walker-steps/s; the affine kernels, with tables of 50-200 rows, do not gain and keep kCoopWarps = 4).
 constexpr int kReprojWarps = 1;
 constexpr int kReprojThreads = 32 * kReprojWarps;
+// resident warps per SM the register allocation aims at: 20 (96 registers) measured best at C3 (16: 496, 20: 510, 24: 464 M)
+constexpr int kReprojMinCtas = (CLOSURE_COOP_MIN_CTAS == 4 ? 5 : CLOSURE_COOP_MIN_CTAS) * (kCoopWarps / kReprojWarps);
 
 constexpr int RES = CLOSURE_REPROJ_2D3D;
 constexpr int ROW = Res<RES>::ROW;
@@ -149,7 +151,7 @@ __device__ __forceinline__ float cone_lo(const float4 &ra, const float4 &rb, con
 
 // ---------------------------------------------------------------------------------- the kernel
 template <int NQ>
-__global__ void __launch_bounds__(kReprojThreads, CLOSURE_COOP_MIN_CTAS * (kCoopWarps / kReprojWarps)) walker_coop_reproj_kernel(const __grid_constant__ WalkLaunch L)
+__global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_reproj_kernel(const __grid_constant__ WalkLaunch L)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int n_runs_s;
