@@ -158,7 +158,8 @@ int closure_init_from_trials(closure_t *h, long long num_trials, unsigned long l
  *   out_trace        DEVICE or NULL, num_walkers x num_steps int32: per iteration
  *                    m_0 | (j_{k_0} << 8), 0 when nothing was feasible (parity protocol)
  * closure_sample(h, W, S, seed, samples, flags, stream) of the north star is the
- * walker_begin = 0, out_trace = NULL case. */
+ * walker_begin = 0, out_trace = NULL case.  One launch takes at most 2^31 - 1 walkers (one CTA per walker in the
+ * reprojection kernels; 258 GB of samples): more than that returns CLOSURE_ECUDA, split the range instead. */
 int closure_sample_range(closure_t *h, long long walker_begin, long long num_walkers, int num_steps,
                          unsigned long long seed, double *out_samples, unsigned char *out_on_boundary,
                          int *out_trace, void *cuda_stream);
