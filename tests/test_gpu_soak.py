@@ -2,7 +2,8 @@
 
 Random config, instance, walk parameters, |S_0|, mode and seed per run; samples and flags must agree bit for bit.
 (The same loop ran for 15 minutes twice in round 1, the second time on the final build with random bound runs and
-body pivots as below: 8,349 + 8,080 runs, 68 M + 66 M walkers, no mismatch -- DESIGN.md 8.)"""
+body pivots as below: 8,349 + 8,080 runs, 68 M + 66 M walkers, and for 10 minutes on the last build of the round: 9,720
+runs; no mismatch -- DESIGN.md 8.)"""
 import copy
 
 import numpy as np
