@@ -30,7 +30,7 @@
 extern "C" {
 #endif
 
-#define CLOSURE_ABI_VERSION 1
+#define CLOSURE_ABI_VERSION 2
 
 /* status codes */
 #define CLOSURE_OK 0
@@ -74,7 +74,8 @@ typedef struct {
     double theta_p;  /* rotation perturbation scale (the paper's R_p): rotation vector uniform on
                         [-theta_p, theta_p]^3 (R-6) */
     int precision;   /* 64: every decision is the fp64 decision (the parity path).  32: rotation sampler only --
-                        decisions are taken on the fp32 values as they are (no certificate, no fp64 fall-back);
+                        the fp32 ranking is taken as it is and a ladder candidate whose fp32 bound straddles the
+                        threshold counts as violated (no fp64 fall-back; every emitted pose is still inside S);
                         poses stay fp64.  Differs from 64 only where an fp32 error bound straddles a
                         threshold; bench.py --precision 32 reports the measured difference. */
     int flags;       /* bit 0 (CLOSURE_FLAG_EXACT_ONLY): run the plain fp64 one-walker-per-thread kernel even where
@@ -101,7 +102,11 @@ int closure_default_params(int residual_type, closure_params *p);
  *   intrinsics    host, {fx, fy, cx, cy}; required for CLOSURE_REPROJ_2D3D(_ELL), ignored (may be NULL) else
  *   p             walk parameters (copied)
  *   out           receives the handle; destroy with closure_destroy
- * Synchronous (small H2D copy).  Errors: CLOSURE_EINVAL, CLOSURE_ECUDA, CLOSURE_ENOMEM. */
+ * Synchronous (small H2D copy).  Errors: CLOSURE_EINVAL, CLOSURE_ECUDA, CLOSURE_ENOMEM; CLOSURE_EUNSUPPORTED if the
+ * constraint table (64 B per row, 128 B for pose regression) plus the ladder (2 KB per rung) exceeds the 200 KB a
+ * CTA can stage (n <= 4096 otherwise: e.g. n <= 2,700 registration rows at n_t = 15).
+ * Thread / stream safety: a handle carries per-handle device scratch (compaction tile states, statistics, closure_run's
+ * buffers).  Use one handle from one host thread and ONE stream at a time; different handles are independent. */
 int closure_create(int residual_type, const double *measurements, int n, const double *betas,
                    const double *intrinsics, const closure_params *p, closure_t **out);
 
@@ -193,7 +198,11 @@ typedef struct {
     int n_rot_support, n_trans_support;
     double host_seconds;      /* wall time of Step III inside closure_megb, device passes and copies included
                                  (reported separately) */
-    double reserved;
+    double d2h_bytes;         /* bytes closure_megb copied device -> host: the whole cloud (count x 96) on the host path;
+                                 16 per pivot + 8 d per fetched support candidate on the device path */
+    double max_pivot_seconds; /* device path: the slowest single pivot (launch + 16-byte copy + synchronise); 0 on the host path */
+    int pivots;               /* device path: farthest-point launches of both balls; 0 on the host path */
+    int pad_;
 } closure_megb_result;
 
 /* Step III (Alg. 1 l.6-7): minimum enclosing ball of {t} in R^3 and of the
@@ -226,6 +235,9 @@ typedef struct {
     unsigned long long ladder_pairs_f32;  /* pairs evaluated in certified fp32 (rung screening + full rungs), a5 */
     unsigned long long fallback_steps;  /* iterations whose fp32 ranking was not certified (fp64 re-ranking) */
     unsigned long long verified_rungs;  /* ladder rungs evaluated in full (ROT) / candidates sent to fp64 (TRANS) */
+    unsigned long long setup_cycles;    /* SM cycles the walkers' warps spent in the set-up that follows an accepted move
+                                           (cooperative rotation-sampler kernels; 0 elsewhere) */
+    unsigned long long total_cycles;    /* SM cycles of the walkers' warps from init to emit (same kernels) */
 } closure_stats;
 int closure_enable_stats(closure_t *h, int on);
 int closure_get_stats(closure_t *h, closure_stats *out);

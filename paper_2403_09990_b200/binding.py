@@ -36,7 +36,8 @@ class MegbResult(Structure):
     _fields_ = [("R", c_double * 9), ("t", c_double * 3), ("rot_radius", c_double),
                 ("trans_radius", c_double), ("rot_support", c_longlong * 5),
                 ("trans_support", c_longlong * 4), ("n_rot_support", c_int), ("n_trans_support", c_int),
-                ("host_seconds", c_double), ("reserved", c_double)]
+                ("host_seconds", c_double), ("d2h_bytes", c_double), ("max_pivot_seconds", c_double),
+                ("pivots", c_int), ("pad_", c_int)]
 
 
 class Stats(Structure):
@@ -44,7 +45,8 @@ class Stats(Structure):
                 ("perturb_setups", c_ulonglong), ("ladder_setups", c_ulonglong),
                 ("accepted_steps", c_ulonglong), ("walker_steps", c_ulonglong),
                 ("perturb_pairs_f32", c_ulonglong), ("ladder_pairs_f32", c_ulonglong),
-                ("fallback_steps", c_ulonglong), ("verified_rungs", c_ulonglong)]
+                ("fallback_steps", c_ulonglong), ("verified_rungs", c_ulonglong),
+                ("setup_cycles", c_ulonglong), ("total_cycles", c_ulonglong)]
 
 
 class ClosureError(RuntimeError):
@@ -159,7 +161,8 @@ def closure_miniball_host(points) -> tuple[np.ndarray, float, np.ndarray]:
 def _as_dict(r: MegbResult) -> dict:
     return dict(R=np.array(r.R).reshape(3, 3), t=np.array(r.t), rot_radius=r.rot_radius,
                 trans_radius=r.trans_radius, rot_support=np.array(r.rot_support[:r.n_rot_support]),
-                trans_support=np.array(r.trans_support[:r.n_trans_support]), host_seconds=r.host_seconds)
+                trans_support=np.array(r.trans_support[:r.n_trans_support]), host_seconds=r.host_seconds,
+                d2h_bytes=int(r.d2h_bytes), max_pivot_seconds=r.max_pivot_seconds, pivots=int(r.pivots))
 
 
 class Closure:

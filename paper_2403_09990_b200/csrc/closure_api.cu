@@ -306,6 +306,8 @@ int closure_set_params(closure_t *h, const closure_params *p)
     if (rc != CLOSURE_OK) return fail(h, rc, why);
     if (h->has_pivot && p->mode != CLOSURE_MODE_ROT)
         return fail(h, CLOSURE_EUNSUPPORTED, "a body pivot is set: Alg. A8 has no update_rotation (clear it with closure_set_pivot first)");
+    if (plain_kernel_smem_bytes(h->h_desc.rows_bytes, p->n_t) > kMaxStageBytes)
+        return fail(h, CLOSURE_EUNSUPPORTED, "constraint table and ladder do not fit shared memory for this n and n_t");
     h->P = *p;
     return CLOSURE_OK;
 }
@@ -320,6 +322,8 @@ int closure_create(int residual_type, const double *measurements, int n, const d
     std::string why;
     int rc = check_params(p, &why);
     if (rc != CLOSURE_OK) return rc;
+    // every instance must be stageable by the kernel of last resort (rows + per-thread ladder table)
+    if (plain_kernel_smem_bytes(n * row_doubles(residual_type) * 8, p->n_t) > kMaxStageBytes) return CLOSURE_EUNSUPPORTED;
     const int nb = residual_type == CLOSURE_POSE_REG_SPLIT ? 2 * n : n;
     if (!all_finite(measurements, (size_t)n * cols) || !all_finite(betas, nb)) return CLOSURE_EINVAL;
     for (int i = 0; i < nb; ++i)
@@ -638,6 +642,8 @@ int closure_megb(closure_t *h, const double *samples, long long count, closure_m
     double qbar[4];
     rotation_to_quat(h->h_desc.Rbar, qbar);
     Ball bt, bq;
+    double d2h_bytes = 0.0, max_pivot_s = 0.0;
+    int pivots = 0;
     const auto t0 = std::chrono::steady_clock::now();
     if (count >= kDeviceMegbMin && !(h->P.flags & CLOSURE_FLAG_HOST_MEGB)) {
         // the cloud stays on the device: one embedding pass, then one max-reduction per miniball pivot
@@ -654,6 +660,7 @@ int closure_megb(closure_t *h, const double *samples, long long count, closure_m
                         miniball_source(device_megb_quats(dm), count, 4, &bq);
         if (device_megb_status(dm) != cudaSuccess) return cuda_fail(h, device_megb_status(dm), "device MEGB pivot");
         if (!ok) return fail(h, CLOSURE_EINVAL, "miniball failed");
+        device_megb_accounting(dm, &d2h_bytes, &max_pivot_s, &pivots);
     } else {
         std::vector<double> host;
         try {
@@ -664,6 +671,7 @@ int closure_megb(closure_t *h, const double *samples, long long count, closure_m
         cudaError_t e = cudaMemcpyAsync(host.data(), samples, host.size() * sizeof(double), cudaMemcpyDeviceToHost, stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
         if (e != cudaSuccess) return cuda_fail(h, e, "copy of samples to the host");
+        d2h_bytes = (double)(host.size() * sizeof(double));
         std::vector<double> tp((size_t)count * 3), qp((size_t)count * 4);
         for (long long i = 0; i < count; ++i) {
             const double *s = host.data() + (size_t)i * 12;
@@ -693,6 +701,9 @@ int closure_megb(closure_t *h, const double *samples, long long count, closure_m
     for (int k = 0; k < bq.n_support; ++k) out->rot_support[k] = bq.support[k];
     for (int k = 0; k < bt.n_support; ++k) out->trans_support[k] = bt.support[k];
     out->host_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    out->d2h_bytes = d2h_bytes;
+    out->max_pivot_seconds = max_pivot_s;
+    out->pivots = pivots;
     return CLOSURE_OK;
 }
 
@@ -753,7 +764,7 @@ int closure_get_stats(closure_t *h, closure_stats *out)
     out->perturb_pairs = v[0]; out->ladder_pairs = v[1]; out->perturb_setups = v[2];
     out->ladder_setups = v[3]; out->accepted_steps = v[4]; out->walker_steps = v[5];
     out->perturb_pairs_f32 = v[6]; out->ladder_pairs_f32 = v[7]; out->fallback_steps = v[8];
-    out->verified_rungs = v[9];
+    out->verified_rungs = v[9]; out->setup_cycles = v[10]; out->total_cycles = v[11];
     return CLOSURE_OK;
 }
 

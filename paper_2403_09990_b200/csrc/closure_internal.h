@@ -38,7 +38,7 @@ constexpr int kMaxBatch = 96;
 constexpr int kBlock = 128;       // walkers per CTA (one per thread)
 constexpr int kMaxNT = 64;
 constexpr int kMaxKStar = 20;
-constexpr int kNumStats = 10;
+constexpr int kNumStats = 12;
 
 struct WalkLaunch {
     const InstanceDesc *desc[kMaxBatch];      // device pointers, one per instance (gridDim.y)
@@ -57,6 +57,9 @@ struct WalkLaunch {
 };
 
 int row_doubles(int residual_type);
+// shared memory of the one-walker-per-thread kernel (the kernel of last resort: every instance must fit it)
+constexpr size_t kMaxStageBytes = 200 * 1024;
+size_t plain_kernel_smem_bytes(int rows_bytes, int n_t);
 
 // walker_kernel.cu
 cudaError_t launch_walkers(int residual_type, int mode, bool stats, const WalkLaunch &L, int n_instances,
@@ -117,6 +120,7 @@ cudaError_t device_megb_prepare(DeviceMegb *m, const double *d_samples, long lon
 PointSource *device_megb_quats(DeviceMegb *m);     // cloud of aligned unit quaternions in R^4
 PointSource *device_megb_trans(DeviceMegb *m);     // cloud of translations in R^3
 cudaError_t device_megb_status(DeviceMegb *m);
+void device_megb_accounting(DeviceMegb *m, double *d2h_bytes, double *max_pivot_seconds, int *pivots);
 void device_megb_destroy(DeviceMegb *m);
 void rotation_to_quat(const double R[9], double q[4]);
 void quat_to_rotation(const double q[4], double R[9]);

@@ -13,7 +13,9 @@
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
+#include <algorithm>
 #include <array>
+#include <chrono>
 #include <unordered_map>
 #include <vector>
 
@@ -145,6 +147,9 @@ struct DeviceMegb {
     int blocks = 0, sms = 148;
     long long capacity = 0;
     cudaError_t err = cudaSuccess;
+    // accounting of one closure_megb call (closure_megb_result.d2h_bytes / pivots / max_pivot_seconds)
+    double d2h_bytes = 0.0, max_pivot_s = 0.0;
+    int pivots = 0;
 
     class Cloud : public PointSource {
     public:
@@ -152,6 +157,7 @@ struct DeviceMegb {
         bool farthest(const double *c, long long *index, double *sq_dist) override
         {
             if (m_->err != cudaSuccess) return false;
+            const auto t0 = std::chrono::steady_clock::now();
             const double c3 = d_ == 4 ? c[3] : 0.0;
             if (d_ == 4)
                 megb_farthest_kernel<4><<<m_->blocks, kFarThreads, 0, m_->stream>>>(m_->Q, m_->n, c[0], c[1], c[2], c3,
@@ -163,6 +169,9 @@ struct DeviceMegb {
             if (e == cudaSuccess) e = cudaMemcpyAsync(m_->h_out, m_->out, sizeof(FarResult), cudaMemcpyDeviceToHost, m_->stream);
             if (e == cudaSuccess) e = cudaStreamSynchronize(m_->stream);
             if (e != cudaSuccess) { m_->err = e; return false; }
+            m_->d2h_bytes += (double)sizeof(FarResult);
+            m_->pivots += 1;
+            m_->max_pivot_s = std::max(m_->max_pivot_s, std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count());
             *index = m_->h_out->idx;
             *sq_dist = m_->h_out->d2;
             return true;
@@ -176,6 +185,7 @@ struct DeviceMegb {
             cudaError_t e = cudaMemcpyAsync(m_->h_pt, src, sizeof(double) * d_, cudaMemcpyDeviceToHost, m_->stream);
             if (e == cudaSuccess) e = cudaStreamSynchronize(m_->stream);
             if (e != cudaSuccess) { m_->err = e; return nullptr; }
+            m_->d2h_bytes += (double)(sizeof(double) * d_);
             std::array<double, 4> v = { 0, 0, 0, 0 };
             for (int a = 0; a < d_; ++a) v[a] = m_->h_pt[a];
             return cache_.emplace(i, v).first->second.data();
@@ -217,6 +227,7 @@ cudaError_t device_megb_prepare(DeviceMegb *m, const double *d_samples, long lon
     m->n = count;
     m->quats.clear();
     m->trans.clear();
+    m->d2h_bytes = 0.0; m->max_pivot_s = 0.0; m->pivots = 0;
     cudaError_t e = (m->partial && m->out && m->ticket && m->h_out && m->h_pt) ? cudaSuccess : cudaErrorMemoryAllocation;
     if (e == cudaSuccess) e = cudaMemsetAsync(m->ticket, 0, sizeof(unsigned int), stream);
     if (e == cudaSuccess && count > m->capacity) {
@@ -241,6 +252,10 @@ cudaError_t device_megb_prepare(DeviceMegb *m, const double *d_samples, long lon
 PointSource *device_megb_quats(DeviceMegb *m) { return &m->quats; }
 PointSource *device_megb_trans(DeviceMegb *m) { return &m->trans; }
 cudaError_t device_megb_status(DeviceMegb *m) { return m->err; }
+void device_megb_accounting(DeviceMegb *m, double *d2h_bytes, double *max_pivot_seconds, int *pivots)
+{
+    *d2h_bytes = m->d2h_bytes; *max_pivot_seconds = m->max_pivot_s; *pivots = m->pivots;
+}
 
 void device_megb_destroy(DeviceMegb *m)
 {

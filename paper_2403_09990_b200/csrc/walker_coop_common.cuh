@@ -185,7 +185,8 @@ __device__ __forceinline__ bool topk_certified(const float (&v)[NQ], int n_ps, f
             key[NQ - 1] = 0u;
         }
     }
-    myval = fkey_inv(myg);
+    // an empty slot carries the key of -inf with its slot index in the low bits: decode it as -inf, not as the NaN those bits spell
+    myval = ((myg & ~7u) == (fkey(-CUDART_INF_F) & ~7u)) ? -CUDART_INF_F : fkey_inv(myg);
     const int myj = (__ffs(mywho) - 1) + 32 * (int)(myg & 7u);
     const bool tie = (lane <= n_ps) && ((mywho & (mywho - 1u)) != 0u) && (myval > -CUDART_INF_F);   // empty slots all look alike
     const float prev = __shfl_up_sync(FULL, myval, 1);

@@ -432,8 +432,9 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
     const bool stats = (L.stats != nullptr) && lane == 0;
     if (stats) {
-        for (int k = 0; k < 10; ++k) stc[k] = 0ull;
+        for (int k = 0; k < kNumStats; ++k) stc[k] = 0ull;
     }
+    const long long clk_begin = stats ? clock64() : 0ll;
     bool hit = false;
     bool moved = true;
     float epsA = 0.f;
@@ -446,7 +447,9 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     for (int s = 1; s <= L.num_steps; ++s) {
         // ================================================== set-up at the current pose (only after a move)
         if (moved) {
+            const long long c0 = stats ? clock64() : 0ll;
             coop_setup_on_move<RES>(smem_raw, warp, lane, rows_bytes, n, n_t, NQ, L.pairs_cap, t_p, stats);
+            if (stats) stc[10] += (unsigned long long)(clock64() - c0);
             epsA = (float)pose[16];
             rot_margin = pose[15];
             full_m = -1;
@@ -664,7 +667,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                     unsigned alive2 = __ballot_sync(FULL, mine && !dead) & cand_alive;
                     unsigned undecided = __ballot_sync(FULL, mine && !dead && !sure) & cand_alive;
                     if (L.exact_only & 2) { alive2 = cand_alive; undecided = cand_alive; }
-                    if (L.exact_only & 32) undecided = 0u;   // fp32 mode: undecided counts as satisfied
+                    if (L.exact_only & 32) { alive2 &= ~undecided; undecided = 0u; }   // fp32 mode: undecided counts as VIOLATED, so every emitted sample stays inside S (Prop. 4)
                     while (undecided != 0u) {                // rare: fp64 decides
                         const int k = __ffs(undecided) - 1;
                         undecided &= undecided - 1u;
@@ -709,7 +712,8 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
         L.out_flags[o] = hit ? 1 : 0;
         if (stats) {
             stc[5] = (unsigned long long)L.num_steps;
-            for (int k = 0; k < 10; ++k) atomicAdd(L.stats + k, stc[k]);
+            stc[11] = (unsigned long long)(clock64() - clk_begin);
+            for (int k = 0; k < kNumStats; ++k) atomicAdd(L.stats + k, stc[k]);
         }
     }
 }

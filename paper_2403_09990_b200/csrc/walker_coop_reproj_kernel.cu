@@ -248,8 +248,9 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
     unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
     const bool stats = (L.stats != nullptr) && lane == 0;
     if (stats) {
-        for (int k = 0; k < 10; ++k) stc[k] = 0ull;
+        for (int k = 0; k < kNumStats; ++k) stc[k] = 0ull;
     }
+    const long long clk_begin = stats ? clock64() : 0ll;
     bool hit = false;
     bool moved = true;
     float uncA = CUDART_INF_F;
@@ -259,6 +260,7 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
     for (int s = 1; s <= L.num_steps; ++s) {
         // ================================================== set-up at the current pose (only after a move)
         if (moved) {
+            const long long clk0 = stats ? clock64() : 0ll;
             double R[9], t[3], vel[3], K[4];
 #pragma unroll
             for (int e = 0; e < 9; ++e) R[e] = pose[e];
@@ -341,6 +343,7 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                 for (int m = n_t - 1; m >= 0; --m) { sm = fmaxf(sm, qL[m]); qL[m] = sm; }
             }
             __syncwarp();
+            if (stats) stc[10] += (unsigned long long)(clock64() - clk0);
         }
 
         // ================================================== a2: perturbations of this lane (d_j = t_p xi_j)
@@ -490,7 +493,7 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                 unsigned alive2 = __ballot_sync(FULL, mine && !dead) & cand_alive;
                 unsigned undecided = __ballot_sync(FULL, mine && !dead && !sure) & cand_alive;
                 if (L.exact_only & 2) { alive2 = cand_alive; undecided = cand_alive; }
-                if (L.exact_only & 32) undecided = 0u;       // fp32 mode: undecided counts as satisfied
+                if (L.exact_only & 32) { alive2 &= ~undecided; undecided = 0u; }   // fp32 mode: undecided counts as VIOLATED, so every emitted sample stays inside S (Prop. 4)
                 while (undecided != 0u) {                    // rare: fp64 decides
                     const int k = __ffs(undecided) - 1;
                     undecided &= undecided - 1u;
@@ -533,7 +536,8 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
         L.out_flags[o] = hit ? 1 : 0;
         if (stats) {
             stc[5] = (unsigned long long)L.num_steps;
-            for (int k = 0; k < 10; ++k) atomicAdd(L.stats + k, stc[k]);
+            stc[11] = (unsigned long long)(clock64() - clk_begin);
+            for (int k = 0; k < kNumStats; ++k) atomicAdd(L.stats + k, stc[k]);
         }
     }
 }

@@ -172,7 +172,7 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
     init_walker<CLOSURE_MODE_TRANS>(D, L, rng, w, R, t, vel);
     const bool stats = (L.stats != nullptr) && lane == 0;
     if (stats) {
-        for (int k = 0; k < 10; ++k) stc[k] = 0ull;
+        for (int k = 0; k < kNumStats; ++k) stc[k] = 0ull;
     }
     bool hit = false;
     // Reprojection residual: eq. (14) of the N_P poses in certified fp32 (see the header); needs the series of
@@ -479,7 +479,7 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
         L.out_flags[o] = hit ? 1 : 0;
         if (stats) {
             stc[5] = (unsigned long long)L.num_steps;
-            for (int k = 0; k < 10; ++k) atomicAdd(L.stats + k, stc[k]);
+            for (int k = 0; k < kNumStats; ++k) atomicAdd(L.stats + k, stc[k]);
         }
     }
 }

@@ -331,6 +331,11 @@ int row_doubles(int residual_type)
     }
 }
 
+size_t plain_kernel_smem_bytes(int rows_bytes, int n_t)
+{
+    return 16 + (size_t)((rows_bytes + 15) & ~15) + (size_t)n_t * kBlock * sizeof(double2);
+}
+
 cudaError_t launch_walkers(int residual_type, int mode, bool stats, const WalkLaunch &L, int n_instances,
                            int max_rows_bytes, cudaStream_t stream, std::string *why)
 {
@@ -341,11 +346,7 @@ cudaError_t launch_walkers(int residual_type, int mode, bool stats, const WalkLa
         return cudaErrorInvalidValue;
     }
     dim3 grid((unsigned)blocks, (unsigned)n_instances, 1);
-    const size_t smem = 16 + (size_t)((max_rows_bytes + 15) & ~15) + (size_t)L.n_t * kBlock * sizeof(double2);
-    if (smem > 200 * 1024) {
-        if (why) *why = "instance too large for shared-memory staging";
-        return cudaErrorInvalidValue;
-    }
+    const size_t smem = plain_kernel_smem_bytes(max_rows_bytes, L.n_t);
     if ((L.exact_only & 32) && !coop_path_available(residual_type, mode, L.n_p, max_rows_bytes / (row_doubles(residual_type) * 8))) {
         if (why) *why = "fp32 mode needs the cooperative kernel";
         return cudaErrorInvalidValue;
@@ -364,6 +365,12 @@ cudaError_t launch_walkers(int residual_type, int mode, bool stats, const WalkLa
     if (!(L.exact_only & 1) && mode == CLOSURE_MODE_TRANS && L.n_p <= 256) {
         const cudaError_t e = launch_walkers_coop_trans(residual_type, L, n_instances, max_rows_bytes, stream);
         if (e != cudaErrorInvalidConfiguration) return e;
+    }
+    // the one-walker-per-thread kernel: rows + a per-thread ladder table (closure_create / closure_set_params reject
+    // instances it cannot stage, so this does not fire for a handle that was created successfully)
+    if (smem > kMaxStageBytes) {
+        if (why) *why = "instance too large for shared-memory staging";
+        return cudaErrorInvalidValue;
     }
     switch (residual_type) {
     case CLOSURE_REG_3D3D: return launch_r<CLOSURE_REG_3D3D>(mode, stats, L, grid, smem, stream);

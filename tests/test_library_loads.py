@@ -26,7 +26,7 @@ def test_every_declared_symbol_is_exported(lib):
     assert declared == set(B.EXPORTS), declared ^ set(B.EXPORTS)
     for name in declared:
         assert hasattr(lib, name), name
-    assert B.closure_abi_version() == 1
+    assert B.closure_abi_version() == 2
 
 
 def test_default_params_and_strerror(lib):
