@@ -238,6 +238,10 @@ typedef struct {
     unsigned long long setup_cycles;    /* SM cycles the walkers' warps spent in the set-up that follows an accepted move
                                            (cooperative rotation-sampler kernels; 0 elsewhere) */
     unsigned long long total_cycles;    /* SM cycles of the walkers' warps from init to emit (same kernels) */
+    unsigned long long threshold_probes;   /* branch and bound of eq. (14) (affine cooperative kernel): counts taken to find the threshold */
+    unsigned long long survivors;          /* perturbations evaluated against all constraints (phase 2), summed over iterations */
+    unsigned long long reserved_;
+    unsigned long long threshold_failures; /* iterations in which no threshold separated the values (ties): fp64 on all N_P */
 } closure_stats;
 int closure_enable_stats(closure_t *h, int on);
 int closure_get_stats(closure_t *h, closure_stats *out);

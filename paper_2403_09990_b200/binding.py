@@ -46,7 +46,9 @@ class Stats(Structure):
                 ("accepted_steps", c_ulonglong), ("walker_steps", c_ulonglong),
                 ("perturb_pairs_f32", c_ulonglong), ("ladder_pairs_f32", c_ulonglong),
                 ("fallback_steps", c_ulonglong), ("verified_rungs", c_ulonglong),
-                ("setup_cycles", c_ulonglong), ("total_cycles", c_ulonglong)]
+                ("setup_cycles", c_ulonglong), ("total_cycles", c_ulonglong),
+                ("threshold_probes", c_ulonglong), ("survivors", c_ulonglong), ("reserved_", c_ulonglong),
+                ("threshold_failures", c_ulonglong)]
 
 
 class ClosureError(RuntimeError):

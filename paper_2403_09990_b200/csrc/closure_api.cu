@@ -765,6 +765,7 @@ int closure_get_stats(closure_t *h, closure_stats *out)
     out->ladder_setups = v[3]; out->accepted_steps = v[4]; out->walker_steps = v[5];
     out->perturb_pairs_f32 = v[6]; out->ladder_pairs_f32 = v[7]; out->fallback_steps = v[8];
     out->verified_rungs = v[9]; out->setup_cycles = v[10]; out->total_cycles = v[11];
+    out->threshold_probes = v[12]; out->survivors = v[13]; out->reserved_ = v[14]; out->threshold_failures = v[15];
     return CLOSURE_OK;
 }
 

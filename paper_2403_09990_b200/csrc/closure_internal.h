@@ -38,7 +38,7 @@ constexpr int kMaxBatch = 96;
 constexpr int kBlock = 128;       // walkers per CTA (one per thread)
 constexpr int kMaxNT = 64;
 constexpr int kMaxKStar = 20;
-constexpr int kNumStats = 12;
+constexpr int kNumStats = 16;
 
 struct WalkLaunch {
     const InstanceDesc *desc[kMaxBatch];      // device pointers, one per instance (gridDim.y)

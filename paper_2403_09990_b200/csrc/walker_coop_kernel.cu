@@ -1,25 +1,28 @@
 // Warp-cooperative walker kernel for the rotation-boundary sampler (Alg. 2) on
 // the residuals whose squared norm is quadratic in the translation perturbation (Ex.2 registration,
 // Ex.3 pose regression, stacked or split).  One WARP owns one walker; the 32 lanes split the work
-// that Alg. 3 tensorises per walker:
+// that Alg. 3 tensorises per walker.  Per iteration:
 //
-//   a2-a4  the N_P perturbations are dealt to the lanes (j = lane + 32 q); the per-constraint
-//          set-up u_i = b_i - (R* a_i + t*) is computed ONCE per accepted move (lane i mod 32)
-//          and broadcast through shared memory; a pair costs 3 FFMA + 1 FMNMX in fp32
-//          (packed FFMA2 + FMNMX3 in SASS).  eq. (14)'s values d~_j carry a rigorous error bound
-//          `unc`; the top-N_P* are extracted with warp reductions and the ranking is accepted only
-//          if consecutive values (and the N_P*-th against the next) are more than 2 unc apart.
-//          Otherwise the step falls back to the fp64 evaluation of the plain kernel.
-//   a5-a6  every rung m = 1..N_T is screened first (lane = (rung, half of the candidates)) against the
-//          rung's two tightest constraints and against a Lipschitz bound on what the rotation to R_m
-//          can repair; rungs with a surviving candidate are then evaluated in full, lane =
-//          (candidate, constraint chunk), in fp32 with a three-way outcome per candidate: violated
-//          for sure / satisfied for sure / undecided -> fp64.
+//   a2     the N_P perturbations are dealt to the lanes (j = lane + 32 q), Philox4x32-10 per perturbation.
+//   a3/a4  eq. (14) and the top-N_P* by exact branch and bound:
+//            phase 1  every perturbation against the few constraints that are tightest at the current pose
+//                     (a max over a subset is a lower bound of the max over all: an UPPER bound ub_j of d_j);
+//            select   a threshold U with N_P*+2 <= #{ub_j >= U} <= 32 is found by probing counts (warp sums);
+//                     no perturbation below U can be among the N_P* best once N_P* exact values above U exist;
+//            phase 2  only the survivors are evaluated against all N constraints, lane = (survivor, chunk of
+//                     the table); they are ranked by counting, and the ranking is CERTIFIED iff consecutive
+//                     values (and the N_P*-th against both the next one and U) are more than 2 unc apart,
+//                     unc being a rigorous bound on |fp32 - fp64|.  Otherwise the step falls back to the fp64
+//                     evaluation of the plain kernel.
+//          A pair costs 3 FFMA + 1 FMNMX in fp32 (packed FFMA2 + FMNMX3 in SASS); the per-constraint set-up
+//          u_i = b_i - (R* a_i + t*) is computed ONCE per accepted move and kept in shared memory.
+//   a5-a6  rungs are screened first, lane = (rung, candidate), against two tight constraint rows per rung
+//          and against a Lipschitz bound on what the rotation to R_m can repair; rungs with a surviving
+//          candidate are then evaluated in full, lane = (candidate, constraint chunk), in fp32 with a
+//          three-way outcome per candidate: violated for sure / satisfied for sure / undecided -> fp64.
 //
 // Every accept/reject decision is therefore the decision the fp64 arithmetic of walker_kernel.cu
 // takes (DESIGN.md 6.1b "Certified fp32 evaluation"); the pose itself is only ever updated in fp64.
-// Unlike the one-walker-per-thread kernel all lanes of a warp follow the same walker: no divergence
-// between walkers, the set-up is not repeated per register tile, 128 registers (16 warps per SM).
 #include <cuda_runtime.h>
 #include <math_constants.h>
 #include <stdint.h>
@@ -149,26 +152,80 @@ __device__ __forceinline__ bool exact_candidate_feasible(const double (&Rm)[9], 
     return __all_sync(FULL, ok);
 }
 
+// ---------------------------------------------------------------------------------- shared-memory layout
+constexpr int kTight = 8;     // constraints of the phase-1 table (the tightest of eight strided groups at the current pose)
+constexpr int kCset = 16;     // constraints the rung-screening rows are picked from (kTight + the tightest at a middle rung)
+
+struct AffSmem {
+    size_t run_end, run_bf, run_pend, pos, warp0, per_warp;
+    size_t rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, cand4, candj, candd, vals, sj, sv, rowsT, runT_pend, runT_bf, cset, pose, stc, total;
+};
+
+// pairs = 32-byte entries of rowsA (pair-entries, runs padded to even length)
+__host__ __device__ inline AffSmem aff_layout(int rows_bytes, int n, int n_t, int nq, int pairs, int warps = kCoopWarps)
+{
+    AffSmem s;
+    size_t o = 16 + (size_t)((rows_bytes + 15) & ~15);
+    s.run_end = o; o += (size_t)((n * 4 + 15) & ~15);
+    s.run_bf = o;  o += (size_t)((n * 4 + 15) & ~15);
+    s.run_pend = o; o += (size_t)((n * 4 + 15) & ~15);
+    s.pos = o;     o += (size_t)((n * 4 + 15) & ~15);
+    s.warp0 = o;
+    size_t w = 0;
+    s.rowsA = w; w += (size_t)pairs * 32;          // pair-transposed, runs padded to even length
+    s.rowsL = w; w += (size_t)n * 16;
+    s.pert = w;  w += (size_t)nq * 32 * 16;
+    s.ab = w;    w += (size_t)n_t * 16;
+    s.qrow = w;  w += (size_t)n_t * 32;
+    s.RmS = w;   w += (size_t)((n_t * 72 + 15) & ~15);
+    s.dex = w;   w += (size_t)nq * 32 * 8;
+    s.qL = w;    w += (size_t)((n_t * 4 + 15) & ~15);
+    s.cand4 = w; w += 32 * 16;
+    s.candj = w; w += 32 * 4;
+    s.candd = w; w += 32 * 4;
+    s.vals = w;  w += 32 * 4;
+    s.sj = w;    w += 32 * 4;
+    s.sv = w;    w += 32 * 4;
+    s.rowsT = w; w += (size_t)kTight * 32;
+    s.runT_pend = w; w += (size_t)kTight * 4;
+    s.runT_bf = w;   w += (size_t)kTight * 4;
+    s.cset = w;  w += (size_t)kCset * 4;
+    s.pose = w;  w += 20 * 8;
+    s.stc = w;   w += 16 * 8;
+    s.per_warp = w;
+    s.total = o + (size_t)warps * w;
+    return s;
+}
+
 // ---------------------------------------------------------------------------------- set-up after a move
-// Everything that depends on the pose only (DESIGN.md 6.1b "state that only changes on an accepted
-// move"): fp32 set-up rows at R* (rowsA), Exp(dT_m w) R* for every rung (RmS), per rung the two
-// tightest rows (qrow) and the Lipschitz bound (qL).  fp64-heavy and rare, so it is kept out of line:
-// its registers do not count against the per-iteration code.  Results epsA, rot_margin -> pose[16], pose[15].
+// Everything that depends on the pose only (DESIGN.md 6.1c "state that only changes on an accepted move"):
+//   rowsA   fp32 set-up rows at R* for all N constraints (fp64 set-up, then rounded: the cancellation in
+//           b - (R a + t) is taken in fp64);
+//   rowsT   the phase-1 table: the tightest constraint of each of eight strided groups of rows, as pair-entries
+//           grouped by runs of equal bound (any choice of rows is valid: a subset gives an upper bound);
+//   RmS     Exp(dT_m w) R* for every rung;
+//   qrow    per rung the two tightest rows among kCset candidate constraints (the kTight above and the tightest
+//           of each group at a middle rung) -- screening rows; any choice is valid, a violated row kills.
+// fp64-heavy and rare, so it is kept out of line.  Results epsA, rot_margin, the number of runs of rowsT
+// -> pose[16], pose[15], pose[17].  full_p1: the table is short, phase 1 runs on all of it and rowsT is not built.
 template <int RES>
-__device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int warp, int lane, int rows_bytes, int n,
-                                                int n_t, int nq, int pairs, double t_p, bool stats)
+__device__ __noinline__ void aff_setup_on_move(unsigned char *smem_raw, int warp, int lane, int rows_bytes, int n,
+                                               int n_t, int nq, int pairs, double t_p, bool full_p1, bool stats)
 {
     using RS = Res<RES>;
     constexpr int ROW = RS::ROW;
-    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, nq, 1, pairs);
+    const AffSmem lay = aff_layout(rows_bytes, n, n_t, nq, pairs);
     const double *rows = reinterpret_cast<const double *>(smem_raw + 16);
     const int *pos = reinterpret_cast<const int *>(smem_raw + lay.pos);
     unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
-    float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);
+    float *rowsA = reinterpret_cast<float *>(wp + lay.rowsA);
+    float *rowsT = reinterpret_cast<float *>(wp + lay.rowsT);
+    int *runT_pend = reinterpret_cast<int *>(wp + lay.runT_pend);
+    float *runT_bf = reinterpret_cast<float *>(wp + lay.runT_bf);
+    int *cset = reinterpret_cast<int *>(wp + lay.cset);
     const double2 *ab = reinterpret_cast<const double2 *>(wp + lay.ab);
     float4 *qrow = reinterpret_cast<float4 *>(wp + lay.qrow);
     double *RmS = reinterpret_cast<double *>(wp + lay.RmS);
-    float *qL = reinterpret_cast<float *>(wp + lay.qL);
     double *pose = reinterpret_cast<double *>(wp + lay.pose);
     unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
     const float tpf = (float)t_p * 1.0000002f;          // >= t_p
@@ -178,8 +235,24 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
     for (int e = 0; e < 9; ++e) R[e] = pose[e];
 #pragma unroll
     for (int e = 0; e < 3; ++e) { t[e] = pose[9 + e]; vel[e] = pose[12 + e]; }
+
+    // Exp(dT_m w) R* for every rung
+    for (int m = lane; m < n_t; m += 32) {
+        const double2 c2 = ab[m];
+        double Rm[9];
+        rotate_left(R, vel[0], vel[1], vel[2], c2.x, c2.y, Rm);
+#pragma unroll
+        for (int e = 0; e < 9; ++e) RmS[m * 9 + e] = Rm[e];
+    }
+    __syncwarp();
+    const int m_mid = min(n_t - 1, 4);                  // middle rung whose tight rows join the screening candidates
+    double Rq[9];
+#pragma unroll
+    for (int e = 0; e < 9; ++e) Rq[e] = RmS[m_mid * 9 + e];
+
     float eps_l = 0.f;
     double rm_l = CUDART_INF;
+    uint32_t best1 = 0u, best2 = 0u;                    // (20 key bits | row index): tightest row of this lane at R*, at R_mid
 #pragma unroll 1
     for (int i = lane; i < n; i += 32) {
         const double *row = rows + i * ROW;
@@ -189,121 +262,168 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
         screen_row(u0, u1, u2, c, tp2, tp2sq3, f0, f1, f2, fc, eps);
         {
             const int pp = pos[i], p = pp & 0x3fffffff;
-            float *A = reinterpret_cast<float *>(rowsA) + (p >> 1) * 8 + (p & 1);
+            float *A = rowsA + (p >> 1) * 8 + (p & 1);
             A[0] = f0; A[2] = f1; A[4] = f2; A[6] = fc;
             if (pp & 0x40000000) { A[1] = f0; A[3] = f1; A[5] = f2; A[7] = fc; }
         }
         eps_l = fmaxf(eps_l, eps);
-        if (RES == CLOSURE_POSE_REG_SPLIT) rm_l = dmin(rm_l, row[12] - sqrt(frob_sq(R, row)));
+        const float bfi = (float)row[RS::BETA];
+        float tk1 = sqrtf(fmaxf(fc, 0.f)) - bfi;         // larger = tighter (heuristic key only)
+        if (RES == CLOSURE_POSE_REG_SPLIT) {
+            const double rmi = row[12] - sqrt(frob_sq(R, row));
+            rm_l = dmin(rm_l, rmi);
+            tk1 = fmaxf(tk1, -(float)rmi);
+        }
+        double v0, v1, v2, cq;
+        affine_setup<RES>(Rq, t, row, v0, v1, v2, cq);
+        float tk2 = sqrtf(fmaxf((float)cq, 0.f)) - bfi;
+        if (RES == CLOSURE_POSE_REG_SPLIT) tk2 = fmaxf(tk2, sqrtf((float)frob_sq(Rq, row)) - (float)row[12]);
+        best1 = max(best1, (fkey(tk1) & 0xFFFFF000u) | (uint32_t)i);
+        best2 = max(best2, (fkey(tk2) & 0xFFFFF000u) | (uint32_t)i);
     }
     const float epsA = wmax_nonneg(eps_l);
     double rot_margin = CUDART_INF;
     if (RES == CLOSURE_POSE_REG_SPLIT) rot_margin = wmin_f64(rm_l);
-    for (int m = lane; m < n_t; m += 32) {       // Exp(dT_m w) R* for every rung
-        const double2 c2 = ab[m];
-        double Rm[9];
-        rotate_left(R, vel[0], vel[1], vel[2], c2.x, c2.y, Rm);
+    // the tightest row of each group of four lanes (rows i with (i mod 32) / 4 = g)
+    best1 = max(best1, __shfl_xor_sync(FULL, best1, 1)); best1 = max(best1, __shfl_xor_sync(FULL, best1, 2));
+    best2 = max(best2, __shfl_xor_sync(FULL, best2, 1)); best2 = max(best2, __shfl_xor_sync(FULL, best2, 2));
+    const int g8 = lane & 7;
+    const int idx1 = (int)(__shfl_sync(FULL, best1, g8 * 4) & 0xFFFu);
+    const int idx2 = (int)(__shfl_sync(FULL, best2, g8 * 4) & 0xFFFu);
+    if (lane < 8) cset[kTight + lane] = idx2;
+    // sort the eight tight rows by index (= by bound: rows are sorted by bound), lane r < 8 takes the r-th
+    int rank = 0;
 #pragma unroll
-        for (int e = 0; e < 9; ++e) RmS[m * 9 + e] = Rm[e];
+    for (int r = 0; r < 8; ++r) {
+        const int o = __shfl_sync(FULL, idx1, r);
+        rank += (o < idx1 || (o == idx1 && r < g8)) ? 1 : 0;
     }
-    __syncwarp();
-    // the two tightest constraints of every rung (largest c - beta^2 at the unperturbed
-    // translation): the rows the ladder screens each rung against while the pose stays here
-#pragma unroll 1
-    for (int m = 0; m < n_t; ++m) {
-        double Rm[9];
+    if (lane < 8) cset[rank] = idx1;
+    __syncwarp();                                        // rowsA and cset[] are complete
+    int nT_runs = 0;
+    if (!full_p1) {
+        const int myi = cset[g8];
+        const double myb = rows[myi * ROW + RS::BETA];
+        int p = 0, myp = 0;
+        bool mydup = false;
+        double prev = __shfl_sync(FULL, myb, 0);
 #pragma unroll
-        for (int e = 0; e < 9; ++e) Rm[e] = RmS[m * 9 + e];
-        float4 b1 = make_float4(0.f, 0.f, 0.f, -CUDART_INF_F), b2 = b1;
-        bool rdead = false;
-        double dR[9], lip = 0.0;                     // max_i | ||g_i(R_m, .)|| - ||g_i(R*, .)|| | <= sqrt(lip)
-#pragma unroll
-        for (int e = 0; e < 9; ++e) dR[e] = Rm[e] - R[e];
-        if (RES != CLOSURE_REG_3D3D) {
-#pragma unroll
-            for (int e = 0; e < 9; ++e) lip = fma(dR[e], dR[e], lip);      // ||R_m - R*||_F^2
+        for (int r = 0; r < 8; ++r) {
+            const double br = __shfl_sync(FULL, myb, r);
+            if (r > 0 && br != prev) {                   // close the run: odd length repeats its last row
+                if (p & 1) { if (lane == r - 1) mydup = true; ++p; }
+                if (lane == 0) { runT_pend[nT_runs] = p >> 1; runT_bf[nT_runs] = (float)prev; }
+                ++nT_runs;
+                prev = br;
+            }
+            if (lane == r) myp = p;
+            ++p;
         }
+        if (p & 1) { if (lane == 7) mydup = true; ++p; }
+        if (lane == 0) { runT_pend[nT_runs] = p >> 1; runT_bf[nT_runs] = (float)prev; }
+        ++nT_runs;
+        if (lane < 8) {
+            const int sp = pos[myi] & 0x3fffffff;
+            const float *S = rowsA + (sp >> 1) * 8 + (sp & 1);
+            float *T = rowsT + (myp >> 1) * 8 + (myp & 1);
+            const float a0 = S[0], a1 = S[2], a2 = S[4], a3 = S[6];
+            T[0] = a0; T[2] = a1; T[4] = a2; T[6] = a3;
+            if (mydup) { T[1] = a0; T[3] = a1; T[5] = a2; T[7] = a3; }
+        }
+    }
+    // screening rows of every rung: lane = (rung, candidate constraint), two rungs per pass
+    {
+        const int c = lane & 15;
+        const int ci = cset[c];
+        const double *row = rows + ci * ROW;
+        const unsigned hm = 0xFFFFu << (lane & 16);
 #pragma unroll 1
-        for (int i = lane; i < n; i += 32) {
-            const double *row = rows + i * ROW;
-            double u0, u1, u2, c;
-            affine_setup<RES>(Rm, t, row, u0, u1, u2, c);
-            if (RES == CLOSURE_REG_3D3D) {           // ||(R_m - R*) a_i||^2
-                const double q0 = dR[0] * row[0] + dR[1] * row[1] + dR[2] * row[2];
-                const double q1 = dR[3] * row[0] + dR[4] * row[1] + dR[5] * row[2];
-                const double q2 = dR[6] * row[0] + dR[7] * row[1] + dR[8] * row[2];
-                lip = dmax(lip, q0 * q0 + q1 * q1 + q2 * q2);
-            }
-            if (RES == CLOSURE_POSE_REG_SPLIT) {
-                if (!(frob_sq(Rm, row) <= row[13])) rdead = true;
-            }
+        for (int m = lane >> 4; m < n_t; m += 2) {
+            double Rm[9];
+#pragma unroll
+            for (int e = 0; e < 9; ++e) Rm[e] = RmS[m * 9 + e];
+            double u0, u1, u2, cc;
+            affine_setup<RES>(Rm, t, row, u0, u1, u2, cc);
+            bool rdead = false;
+            if (RES == CLOSURE_POSE_REG_SPLIT) rdead = !(frob_sq(Rm, row) <= row[13]);   // exact: a violated constraint kills the rung
             float g0, g1, g2, fcb, eps;
-            screen_row(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
-            const float4 r4 = make_float4(g0, g1, g2, fcb - eps);
-            if (r4.w > b1.w) { b2 = b1; b1 = r4; } else if (r4.w > b2.w) b2 = r4;
+            screen_row(u0, u1, u2, cc - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
+            float4 r4 = make_float4(g0, g1, g2, fcb - eps);
+            const uint32_t key = (fkey(r4.w) & ~15u) | (uint32_t)c;
+            const uint32_t m1 = __reduce_max_sync(hm, key);
+            const uint32_t key2 = (key == m1) ? 0u : key;
+            const uint32_t m2 = __reduce_max_sync(hm, key2);
+            if (RES == CLOSURE_POSE_REG_SPLIT) {
+                if ((__ballot_sync(hm, rdead) & hm) != 0u) r4.w = CUDART_INF_F;       // rung dead for every candidate
+            }
+            if (key == m1) qrow[2 * m] = r4;
+            if (key2 == m2) qrow[2 * m + 1] = r4;        // key2 = 0 for the winner only (keys of the others carry c != its c or are larger)
         }
-        const uint32_t k1 = fkey(b1.w);
-        const uint32_t m1 = __reduce_max_sync(FULL, k1);
-        const int src1 = __ffs(__ballot_sync(FULL, k1 == m1)) - 1;
-        const uint32_t k2 = (lane == src1) ? fkey(b2.w) : k1;
-        const uint32_t m2 = __reduce_max_sync(FULL, k2);
-        const int src2 = __ffs(__ballot_sync(FULL, k2 == m2)) - 1;
-        if (__any_sync(FULL, rdead)) b1.w = CUDART_INF_F;          // rung dead for every candidate
-        if (lane == src1) qrow[2 * m] = b1;
-        if (lane == src2) qrow[2 * m + 1] = (lane == src1) ? b2 : b1;
-        const float lf = wmax_nonneg((float)sqrt(lip));
-        if (lane == 0) qL[m] = lf * 1.001f + 1e-30f;
     }
-    if (stats) { stc[2] += n; stc[3] += (unsigned long long)n * n_t; }
-    __syncwarp();
-    if (lane == 0) {                                 // suffix maximum: qL[m] holds for every rung >= m
-        float sm = 0.f;
-        for (int m = n_t - 1; m >= 0; --m) { sm = fmaxf(sm, qL[m]); qL[m] = sm; }
-    }
-    __syncwarp();
-    if (lane == 0) { pose[15] = rot_margin; pose[16] = (double)epsA; }
+    if (stats) { stc[2] += 2 * n; stc[3] += (unsigned long long)kCset * n_t; }
+    if (lane == 0) { pose[15] = rot_margin; pose[16] = (double)epsA; pose[17] = (double)nT_runs; }
     __syncwarp();
 }
 
-// ---------------------------------------------------------------------------------- eq. (14), constraint-major
-// For N_P <= 32 (one perturbation per lane) the perturbation-major loop below leaves lanes idle and issues two
-// shared-memory loads for three FFMA2.  Here the roles are swapped for one run of equal bounds: every lane keeps
-// up to PE pair-entries of the run in registers, the perturbations are broadcast from pert[] one by one, and
-// the maximum over the constraints is a warp reduction; lane j keeps the result of perturbation j.  Same
-// products, same chain order, and a maximum does not depend on the order: bit-identical to the other loop.
-template <int PE>
-__device__ __forceinline__ uint32_t eq14_constraint_major(const float4 *rowsA, const float4 *pert, int p0, int pend,
-                                                          int n_p, int lane)
+// ---------------------------------------------------------------------------------- eq. (14), perturbation-major
+// NQ perturbations per lane in registers (packed pairs + an odd slot) against a table of pair-entries
+// (two constraints per 32-byte entry) organised in runs of equal bound: per perturbation the maximum over the
+// run's constraints of c - 2 u.d, one rsqrt per run.  dt[q] = min over runs of beta - sqrt(max + |d|^2);
+// unc_l accumulates the bound on |dt - fp64|.
+template <int NQ>
+__device__ __forceinline__ void eq14_table(const float4 *tab, int n_runs, const int *rpend, const float *rbf,
+                                           const unsigned long long (&p0)[NQ / 2 > 0 ? NQ / 2 : 1],
+                                           const unsigned long long (&p1)[NQ / 2 > 0 ? NQ / 2 : 1],
+                                           const unsigned long long (&p2)[NQ / 2 > 0 ? NQ / 2 : 1], float o0, float o1,
+                                           float o2, const float (&dd)[NQ], float E0, float (&dt)[NQ], float &unc_l)
 {
-    unsigned long long A0[PE], A1[PE], A2[PE], A3[PE];       // (f0a f0b) (f1a f1b) (f2a f2b) (fca fcb)
+    constexpr int NPK = NQ / 2;
+    constexpr bool ODD = (NQ & 1) != 0;
 #pragma unroll
-    for (int k = 0; k < PE; ++k) {
-        const int e = p0 + lane + 32 * k;
-        if (e < pend) {
-            const float4 X = rowsA[2 * e], Y = rowsA[2 * e + 1];
-            A0[k] = pk2(X.x, X.y); A1[k] = pk2(X.z, X.w); A2[k] = pk2(Y.x, Y.y); A3[k] = pk2(Y.z, Y.w);
-        } else {
-            A0[k] = A1[k] = A2[k] = pk2(0.f, 0.f);
-            A3[k] = pk2(-CUDART_INF_F, -CUDART_INF_F);
+    for (int q = 0; q < NQ; ++q) dt[q] = CUDART_INF_F;
+    int pp = 0;
+    for (int r = 0; r < n_runs; ++r) {
+        const int pend = rpend[r];
+        const float bf = rbf[r];
+        float mx[NQ];
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) mx[q] = -CUDART_INF_F;
+#pragma unroll(NQ <= 2 ? 4 : 1)   // measured: unrolling the NQ = 5 body further costs 2-4 % (C2, C4)
+        for (; pp < pend; ++pp) {
+            // two constraints a, b per entry: X = (f0a f0b f1a f1b), Y = (f2a f2b fca fcb)
+            const float4 X = tab[2 * pp], Y = tab[2 * pp + 1];
+#pragma unroll
+            for (int k = 0; k < NPK; ++k) {
+                const unsigned long long va =
+                    fma2(pk2(X.x, X.x), p0[k], fma2(pk2(X.z, X.z), p1[k], fma2(pk2(Y.x, Y.x), p2[k], pk2(Y.z, Y.z))));
+                const unsigned long long vb =
+                    fma2(pk2(X.y, X.y), p0[k], fma2(pk2(X.w, X.w), p1[k], fma2(pk2(Y.y, Y.y), p2[k], pk2(Y.w, Y.w))));
+                float la, ha, lb, hb;
+                upk2(va, la, ha);
+                upk2(vb, lb, hb);
+                mx[2 * k] = fmaxf(mx[2 * k], fmaxf(la, lb));
+                mx[2 * k + 1] = fmaxf(mx[2 * k + 1], fmaxf(ha, hb));
+            }
+            if (ODD) {                          // the odd slot takes both constraints in one packed chain
+                const unsigned long long vo = fma2(pk2(X.x, X.y), pk2(o0, o0),
+                                                   fma2(pk2(X.z, X.w), pk2(o1, o1),
+                                                        fma2(pk2(Y.x, Y.y), pk2(o2, o2), pk2(Y.z, Y.w))));
+                float lo, hi;
+                upk2(vo, lo, hi);
+                mx[NQ - 1] = fmaxf(mx[NQ - 1], fmaxf(lo, hi));
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) {
+            // a ~ max_i |u_i - d|^2 within E0 + 2^-22 a;  sq ~ sqrt(a) within 2^-21 relative
+            const float a = fmaxf(mx[q] + dd[q], 1e-30f);
+            const float rr = rsqrt_normal(a);
+            const float sq = a * rr;
+            const float du = 1.01f * fmaf(E0, rr, (bf + sq) * kMu19);
+            unc_l = fmaxf(unc_l, du);
+            dt[q] = fminf(dt[q], bf - sq);
         }
     }
-    uint32_t mine = fkey(-CUDART_INF_F);
-#pragma unroll 4
-    for (int j = 0; j < n_p; ++j) {
-        const float4 pj = pert[j];
-        float m = -CUDART_INF_F;
-#pragma unroll
-        for (int k = 0; k < PE; ++k) {
-            const unsigned long long vo =
-                fma2(A0[k], pk2(pj.x, pj.x), fma2(A1[k], pk2(pj.y, pj.y), fma2(A2[k], pk2(pj.z, pj.z), A3[k])));
-            float lo, hi;
-            upk2(vo, lo, hi);
-            m = fmaxf(m, fmaxf(lo, hi));
-        }
-        const uint32_t g = __reduce_max_sync(FULL, fkey(m));
-        if (lane == j) mine = g;
-    }
-    return mine;
 }
 
 // ---------------------------------------------------------------------------------- the kernel
@@ -313,10 +433,12 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     using RS = Res<RES>;
     constexpr int ROW = RS::ROW;
     constexpr int NPK = NQ / 2;            // packed pairs of perturbations
+    constexpr int NPK1 = NPK > 0 ? NPK : 1;
     constexpr bool ODD = (NQ & 1) != 0;    // plus one scalar slot
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ int n_runs_s, cmajor_s;
+    __shared__ int n_runs_s;
+    __shared__ float amax_s;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const InstanceDesc *__restrict__ D = L.desc[blockIdx.y];
     const int n = D->n;
@@ -325,13 +447,14 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
     double *rows = reinterpret_cast<double *>(smem_raw + 16);
     stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
-    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 1, L.pairs_cap);
+    const AffSmem lay = aff_layout(rows_bytes, n, n_t, NQ, L.pairs_cap);
     int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
     float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
     int *run_pend = reinterpret_cast<int *>(smem_raw + lay.run_pend);   // end of run r in rowsA, in PAIRS of rows
     int *pos = reinterpret_cast<int *>(smem_raw + lay.pos);             // row of constraint i in rowsA (bit 30: write it twice)
     if (warp == 0) {                                   // runs of equal bounds (rows are sorted by bound)
         int cnt = 0;
+        float am = 0.f;
         for (int base = 0; base < n; base += 32) {
             const int i = base + lane;
             bool end = false;
@@ -339,6 +462,10 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
             if (i < n) {
                 beta = rows[i * ROW + RS::BETA];
                 end = (i == n - 1) || (rows[(i + 1) * ROW + RS::BETA] != beta);
+                if (RES == CLOSURE_REG_3D3D) {
+                    const double a0 = rows[i * ROW], a1 = rows[i * ROW + 1], a2 = rows[i * ROW + 2];
+                    am = fmaxf(am, (float)sqrt(a0 * a0 + a1 * a1 + a2 * a2) * 1.000001f);
+                }
             }
             const unsigned m = __ballot_sync(FULL, end);
             if (end) {
@@ -348,29 +475,27 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
             }
             cnt += __popc(m);
         }
+        // Lipschitz constant of the residual norms in the rotation: ||(R' - R) a_i|| <= angle * max_i ||a_i|| (Ex.2);
+        // ||R' - R||_F <= sqrt(2) angle (Ex.3)
+        am = (RES == CLOSURE_REG_3D3D) ? wmax_nonneg(am) : 1.4142137f;
         __syncwarp();
         if (lane == 0) {
             // rowsA holds the fp32 set-ups two constraints per entry; a run of odd length repeats its last
             // constraint (a maximum does not see duplicates), so no pair straddles two bounds
             n_runs_s = cnt;
-            int p = 0, start = 0, longest = 0;
+            amax_s = am;
+            int p = 0, start = 0;
             for (int r = 0; r < cnt; ++r) {
                 const int end = run_end[r];
-                const int p_begin = p >> 1;
                 for (int i = start; i <= end; ++i) pos[i] = p++;
                 if (p & 1) { pos[end] |= 0x40000000; ++p; }
                 run_pend[r] = p >> 1;
-                longest = max(longest, (p >> 1) - p_begin);
                 start = end + 1;
             }
-            // constraint-major eq. (14): one perturbation per lane, enough pair-entries to fill the lanes,
-            // every run fits the registers of one pass (4 pair-entries per lane)
-            cmajor_s = (NQ == 1 && (p >> 1) >= 64 && longest <= 128) ? 1 : 0;
         }
     }
     __syncthreads();
     const int n_runs = n_runs_s;
-    const bool cmajor = NQ == 1 && cmajor_s != 0;
 
     const long long local = (long long)blockIdx.x * kCoopWarps + warp;
     if (local >= L.num_walkers) return;                // no block-wide barrier below this line
@@ -379,13 +504,19 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     float4 *rowsL = reinterpret_cast<float4 *>(wp + lay.rowsL);
     float4 *pert = reinterpret_cast<float4 *>(wp + lay.pert);
     double2 *ab = reinterpret_cast<double2 *>(wp + lay.ab);
-    float4 *qrow = reinterpret_cast<float4 *>(wp + lay.qrow);     // [rung][2]: the two tightest rows of each rung
+    float4 *qrow = reinterpret_cast<float4 *>(wp + lay.qrow);     // [rung][2]: two tight rows of each rung
     double *RmS = reinterpret_cast<double *>(wp + lay.RmS);
     double *dex = reinterpret_cast<double *>(wp + lay.dex);      // fp64 fallback: exact d_j, [q][lane]
-    float *qL = reinterpret_cast<float *>(wp + lay.qL);           // [rung]: bound on the change of any residual norm
+    float *qL = reinterpret_cast<float *>(wp + lay.qL);           // [rung]: bound on the change of any residual norm, non-increasing
     float4 *cand4 = reinterpret_cast<float4 *>(wp + lay.cand4);   // the kept perturbations (-2 d_j, -|d_j|^2), by rank
     int *candj = reinterpret_cast<int *>(wp + lay.candj);
     float *candd = reinterpret_cast<float *>(wp + lay.candd);     // upper bounds of the candidates' eq. (14) values
+    float *vals = reinterpret_cast<float *>(wp + lay.vals);       // the N_P* + 1 largest eq. (14) values, by rank
+    int *sj = reinterpret_cast<int *>(wp + lay.sj);               // survivors of the threshold: perturbation index
+    float *sv = reinterpret_cast<float *>(wp + lay.sv);           //                             and phase-1 value
+    const float4 *rowsT = reinterpret_cast<const float4 *>(wp + lay.rowsT);
+    const int *runT_pend = reinterpret_cast<const int *>(wp + lay.runT_pend);
+    const float *runT_bf = reinterpret_cast<const float *>(wp + lay.runT_bf);
     double *pose = reinterpret_cast<double *>(wp + lay.pose);     // R*(9) t*(3) omega(3): fp64, touched only on moves / fp64 paths
 
     const unsigned long long w = (unsigned long long)(L.walker_begin + local);
@@ -400,6 +531,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     {
         double R[9], t[3], vel[3];
         init_walker<CLOSURE_MODE_ROT>(D, L, rng, w, R, t, vel);
+        const double wn = sqrt(fma(vel[2], vel[2], fma(vel[1], vel[1], vel[0] * vel[0])));
         for (int m = lane; m < n_t; m += 32) {         // ladder dT_m = gamma^(m-1) by repeated multiplication
             double dT = 1.0;
             for (int q = 0; q < m; ++q) dT = dT * L.gamma;
@@ -407,6 +539,8 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
             double A, B;
             exp_coeffs(fma(p2, p2, fma(p1, p1, p0 * p0)), A, B);
             ab[m] = make_double2(A * dT, B * dT * dT);
+            // rotation angle of rung m times the Lipschitz constant (gamma <= 1: non-increasing in m)
+            qL[m] = (float)(dT * wn) * amax_s * 1.001f + 1e-30f;
         }
         if (lane == 0) {
 #pragma unroll
@@ -427,6 +561,16 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     const bool e_act = ech < NCH;
     unsigned e_mask = 0u;                               // lanes that share this lane's candidate
     for (int c = 0; c < NCH; ++c) e_mask |= 1u << (ek + c * KP);
+    const unsigned kp_all = (KP >= 32) ? FULL : ((1u << KP) - 1u);
+    const unsigned inv_kp = (65536u + (unsigned)KP - 1u) / (unsigned)KP;   // t / KP = (t * inv_kp) >> 16 for t < 3,000
+
+    // selection constants: at most s_max survivors (a power of two), at least need_lo
+    int s_max = 8;
+    while (s_max < 2 * n_ps + 4 && s_max < 32) s_max <<= 1;
+    const int need_lo = min(n_p, n_ps + 3);
+    const int r_target = n_ps + 3 + (n_ps >> 2);        // rank whose value seeds the next iteration's threshold
+    const float step0 = 0.0625f * run_bf[n_runs - 1];
+    float U_state = 0.f;
 
     // executed-work counters (closure_get_stats): in shared memory, touched by lane 0 and only when asked for
     unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
@@ -439,6 +583,8 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     bool moved = true;
     float epsA = 0.f;
     double rot_margin = CUDART_INF;
+    int nT_runs = 0;
+    const bool full_p1 = run_pend[n_runs - 1] <= kTight;   // short tables: phase 1 evaluates every constraint, no phase 2
     // cached across iterations while the pose does not move
     int full_m = -1;                                    // rung whose rows sit in rowsL
     float epsL = 0.f;
@@ -448,15 +594,16 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
         // ================================================== set-up at the current pose (only after a move)
         if (moved) {
             const long long c0 = stats ? clock64() : 0ll;
-            coop_setup_on_move<RES>(smem_raw, warp, lane, rows_bytes, n, n_t, NQ, L.pairs_cap, t_p, stats);
+            aff_setup_on_move<RES>(smem_raw, warp, lane, rows_bytes, n, n_t, NQ, L.pairs_cap, t_p, full_p1, stats);
             if (stats) stc[10] += (unsigned long long)(clock64() - c0);
             epsA = (float)pose[16];
             rot_margin = pose[15];
+            nT_runs = (int)pose[17];
             full_m = -1;
         }
 
         // ================================================== a2: perturbations of this lane
-        unsigned long long p0[NPK > 0 ? NPK : 1], p1[NPK > 0 ? NPK : 1], p2[NPK > 0 ? NPK : 1];
+        unsigned long long p0[NPK1], p1[NPK1], p2[NPK1];
         float o0 = 0.f, o1 = 0.f, o2 = 0.f;                  // the odd slot NQ-1
         float dd[NQ];
         {
@@ -489,135 +636,230 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
             if (ODD) { o0 = e0[NQ - 1]; o1 = e1[NQ - 1]; o2 = e2[NQ - 1]; }
         }
 
-        // ================================================== a3: eq. (14) in fp32 with error bound
-        float dt[NQ];
+        // ================================================== a3 / a4: eq. (14) and the top-N_P* by branch and bound
+        const float rmf = (float)rot_margin;                // +inf unless POSE_REG_SPLIT
+        const float E0 = epsA + tp2sq3 * kMu19;             // bound on |a32 - a64| up to its own rounding
         float unc_l = 0.f;
-        {
+        float ub[NQ];                                       // phase 1: upper bounds of d_j (the values themselves if full_p1)
+        const bool use_p1 = full_p1 || n_p > s_max;         // few perturbations: all of them are "survivors"
+        if (use_p1) {
+            eq14_table<NQ>(full_p1 ? rowsA : rowsT, full_p1 ? n_runs : nT_runs, full_p1 ? run_pend : runT_pend,
+                           full_p1 ? run_bf : runT_bf, p0, p1, p2, o0, o1, o2, dd, E0, ub, unc_l);
 #pragma unroll
-            for (int q = 0; q < NQ; ++q) dt[q] = CUDART_INF_F;
-            const float E0 = epsA + tp2sq3 * kMu19;          // bound on |a32 - a64| up to its own rounding
-            int pp = 0;
-            for (int r = 0; r < n_runs; ++r) {
-                const int pend = run_pend[r];
-                const float bf = run_bf[r];
-                float mx[NQ];
+            for (int q = 0; q < NQ; ++q) ub[q] = (lane + 32 * q < n_p) ? fminf(ub[q], rmf) : -CUDART_INF_F;
+            if (stats) stc[6] += (unsigned long long)(full_p1 ? n : kTight) * n_p;
+        } else {
 #pragma unroll
-                for (int q = 0; q < NQ; ++q) mx[q] = -CUDART_INF_F;
-                if (NQ == 1 && cmajor) {
-                    __syncwarp();                        // pert[] of this iteration is complete
-                    const int len = pend - pp;
-                    uint32_t key;
-                    if (len <= 32) key = eq14_constraint_major<1>(rowsA, pert, pp, pend, n_p, lane);
-                    else if (len <= 64) key = eq14_constraint_major<2>(rowsA, pert, pp, pend, n_p, lane);
-                    else if (len <= 96) key = eq14_constraint_major<3>(rowsA, pert, pp, pend, n_p, lane);
-                    else key = eq14_constraint_major<4>(rowsA, pert, pp, pend, n_p, lane);
-                    // lanes without a perturbation: any finite value (their d is masked below; -inf would blow up unc)
-                    mx[0] = lane < n_p ? fkey_inv(key) : 1.0f;
-                    pp = pend;
+            for (int q = 0; q < NQ; ++q) ub[q] = (lane + 32 * q < n_p) ? CUDART_INF_F : -CUDART_INF_F;
+        }
+
+        // ---- threshold U with need <= #{ub_j >= U} <= s_max (a NaN counts as a survivor and fails the certificate),
+        // found by probing counts; if too few of the survivors turn out to lie above U (their phase-1 values are only
+        // upper bounds) the threshold is lowered and the selection repeated (at most twice) before fp64 takes over
+        float U = -CUDART_INF_F;
+        int cnt = n_p;
+        bool found = true;
+        float lo = -CUDART_INF_F, hi = CUDART_INF_F, step = step0;
+        int need = need_lo;
+        if (n_p > s_max) U = U_state;
+        bool certified = false;
+        float myval = -CUDART_INF_F;
+        float unc = 0.f;
+#pragma unroll 1
+        for (int attempt = 0; attempt < 3; ++attempt) {
+        if (n_p > s_max) {
+            found = false;
+#pragma unroll 1
+            for (int it = 0; it < 24; ++it) {
+                int c = 0;
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) c += (!(ub[q] < U)) ? 1 : 0;
+                cnt = (int)__reduce_add_sync(FULL, (unsigned)c);
+                if (stats) stc[12] += 1;
+                if (cnt < need) hi = U;
+                else if (cnt > s_max) lo = U;
+                else { found = true; break; }
+                if (lo == -CUDART_INF_F) { U = U - step; step = step + step; }
+                else if (hi == CUDART_INF_F) { U = U + step; step = step + step; }
+                else {
+                    const float mid = 0.5f * (lo + hi);
+                    if (!(mid > lo && mid < hi)) break;      // ties: no threshold separates them
+                    U = mid;
                 }
-#pragma unroll(NQ <= 2 ? 4 : 1)   // measured: unrolling the NQ = 5 body further costs 2-4 % (C2, C4)
-                for (; pp < pend; ++pp) {
-                    // two constraints a, b per entry: X = (f0a f0b f1a f1b), Y = (f2a f2b fca fcb)
-                    const float4 X = rowsA[2 * pp], Y = rowsA[2 * pp + 1];
-#pragma unroll
-                    for (int k = 0; k < NPK; ++k) {
-                        const unsigned long long va =
-                            fma2(pk2(X.x, X.x), p0[k], fma2(pk2(X.z, X.z), p1[k], fma2(pk2(Y.x, Y.x), p2[k], pk2(Y.z, Y.z))));
-                        const unsigned long long vb =
-                            fma2(pk2(X.y, X.y), p0[k], fma2(pk2(X.w, X.w), p1[k], fma2(pk2(Y.y, Y.y), p2[k], pk2(Y.w, Y.w))));
-                        float la, ha, lb, hb;
-                        upk2(va, la, ha);
-                        upk2(vb, lb, hb);
-                        mx[2 * k] = fmaxf(mx[2 * k], fmaxf(la, lb));
-                        mx[2 * k + 1] = fmaxf(mx[2 * k + 1], fmaxf(ha, hb));
-                    }
-                    if (ODD) {                          // the odd slot takes both constraints in one packed chain
-                        const unsigned long long vo = fma2(pk2(X.x, X.y), pk2(o0, o0),
-                                                           fma2(pk2(X.z, X.w), pk2(o1, o1),
-                                                                fma2(pk2(Y.x, Y.y), pk2(o2, o2), pk2(Y.z, Y.w))));
-                        float lo, hi;
-                        upk2(vo, lo, hi);
-                        mx[NQ - 1] = fmaxf(mx[NQ - 1], fmaxf(lo, hi));
-                    }
-                }
+                if (!(fabsf(U) < 3.0e38f)) break;
+            }
+        }
+        bool ufail = false;
+        if (found) {
+            // ---- compaction of the survivors: (j, phase-1 value) by slot
+            {
+                int base = 0;
 #pragma unroll
                 for (int q = 0; q < NQ; ++q) {
-                    // a ~ max_i |u_i - d|^2 within E0 + 2^-22 a;  sq ~ sqrt(a) within 2^-21 relative
-                    const float a = fmaxf(mx[q] + dd[q], 1e-30f);
+                    const bool in = (lane + 32 * q < n_p) && !(ub[q] < U);
+                    const unsigned b = __ballot_sync(FULL, in);
+                    if (in) {
+                        const int ps = base + __popc(b & ((1u << lane) - 1u));
+                        sj[ps] = lane + 32 * q;
+                        sv[ps] = ub[q];
+                    }
+                    base += __popc(b);
+                }
+            }
+            __syncwarp();                                   // sj[], sv[], pert[] visible to all lanes
+            if (stats) stc[13] += (unsigned long long)cnt;
+            // ---- phase 2: the survivors against all constraints, lane = (survivor slot, chunk of the table)
+            int S = 1;
+            while (S < cnt) S <<= 1;
+            const int slot = lane & (S - 1);
+            const bool act = slot < cnt;
+            const int myj = act ? sj[slot] : 0;
+            float val;
+            if (full_p1) {
+                val = act ? sv[slot] : -CUDART_INF_F;
+            } else {
+                const int C = 32 / S, chunk = lane / S;
+                const float4 pj = pert[myj];
+                const unsigned long long E0p = pk2(pj.x, pj.x), E1p = pk2(pj.y, pj.y), E2p = pk2(pj.z, pj.z);
+                float v = CUDART_INF_F;
+                int pp = 0;
+                for (int r = 0; r < n_runs; ++r) {
+                    const int pend = run_pend[r];
+                    const float bf = run_bf[r];
+                    float mx = -CUDART_INF_F;
+#pragma unroll 2
+                    for (int p = pp + chunk; p < pend; p += C) {
+                        const float4 X = rowsA[2 * p], Y = rowsA[2 * p + 1];
+                        const unsigned long long vo =
+                            fma2(pk2(X.x, X.y), E0p, fma2(pk2(X.z, X.w), E1p, fma2(pk2(Y.x, Y.y), E2p, pk2(Y.z, Y.w))));
+                        float l2, h2;
+                        upk2(vo, l2, h2);
+                        mx = fmaxf(mx, fmaxf(l2, h2));
+                    }
+                    pp = pend;
+                    for (int off = S; off < 32; off <<= 1) mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, off));
+                    const float a = fmaxf(mx - pj.w, 1e-30f);          // pj.w = -|d|^2
                     const float rr = rsqrt_normal(a);
                     const float sq = a * rr;
                     const float du = 1.01f * fmaf(E0, rr, (bf + sq) * kMu19);
-                    unc_l = fmaxf(unc_l, du);
-                    dt[q] = fminf(dt[q], bf - sq);
+                    if (act) unc_l = fmaxf(unc_l, du);
+                    v = fminf(v, bf - sq);
                 }
+                val = act ? fminf(v, rmf) : -CUDART_INF_F;
+                if (stats) stc[6] += (unsigned long long)n * cnt;
             }
-            if (stats) stc[6] += (unsigned long long)n * n_p;
+            unc = wmax_nonneg(unc_l);
+            if (RES == CLOSURE_POSE_REG_SPLIT) unc += 1.2e-7f * fabsf(rmf);
+            // ---- ranking by counting (lanes 0 .. cnt-1 hold one survivor each); ties are ordered by slot and never certified
+            int rank = 0;
+            const bool nan_any = __any_sync(FULL, act && (val != val));
+#pragma unroll 4
+            for (int r = 0; r < cnt; ++r) {
+                const float xr = __shfl_sync(FULL, val, r);
+                rank += (xr > val || (xr == val && r < slot)) ? 1 : 0;
+            }
+            if (lane < cnt && rank <= n_ps) {
+                vals[rank] = val;
+                if (rank < n_ps) candj[rank] = myj;
+            }
+            // the next iteration's threshold: the value ranked r_target (the distribution is stationary while the walker stays)
+            {
+                const int rt = min(cnt - 1, r_target);
+                const unsigned bt = __ballot_sync(FULL, lane < cnt && rank == rt);
+                const float ut = __shfl_sync(FULL, val, bt ? (__ffs(bt) - 1) : 0);
+                U_state = (bt != 0u && fabsf(ut) < 3.0e38f) ? ut : U;
+            }
+            __syncwarp();
+            // ---- certificate: consecutive values more than 2 unc apart, and the N_P*-th more than 2 unc above both the
+            // next one and the threshold (every perturbation that was not evaluated has d_j <= ub_j < U + unc)
+            myval = (lane <= n_ps && lane < cnt) ? vals[lane] : -CUDART_INF_F;
+            const float prev = __shfl_up_sync(FULL, myval, 1);
+            const bool trust = (L.exact_only & 32) != 0;
+            bool ok = true;
+            if (lane < n_ps) ok = (myval > -CUDART_INF_F) && (myval < CUDART_INF_F);
+            if (lane >= 1 && lane <= n_ps) {
+                const bool none_left = (lane == n_ps) && (myval == -CUDART_INF_F);
+                const float needg = fmaf(2.0f, unc, kMu19 * (fabsf(prev) + fabsf(myval)));
+                ok = ok && (none_left || (prev - myval > needg));
+            }
+            if (trust) ok = true;                       // fp32 mode: the fp32 ranking is taken as it is
+            bool oku = true;
+            if (lane == n_ps - 1 && U > -CUDART_INF_F) {
+                const float needu = fmaf(2.0f, unc, kMu19 * (fabsf(U) + fabsf(myval)));
+                oku = trust ? (myval >= U) : (myval - U > needu);
+            }
+            if (nan_any || (L.exact_only & 4)) ok = false;
+            const bool gaps_ok = __all_sync(FULL, ok);
+            ufail = !__all_sync(FULL, oku);
+            certified = gaps_ok && !ufail;
+            if (certified && lane < n_ps) candd[lane] = myval + fmaf(1.01f, unc, kMu19 * fabsf(myval));    // >= the fp64 value d_j
+            if (certified || !gaps_ok || cnt >= s_max) break;
+            // only the threshold failed: lower it so that at least two more perturbations survive
+            if (stats) stc[14] += 1;
+            need = min(cnt + 2, s_max);
+            hi = U;
+            if (lo == -CUDART_INF_F) { U = U - step; step = step + step; } else U = 0.5f * (lo + hi);
+            __syncwarp();                                   // sj[], sv[], vals[] are rewritten by the next attempt
+        } else {
+            unc = wmax_nonneg(unc_l);
+            if (stats) stc[15] += 1;
+            break;
         }
-
-        // ================================================== a4: top-N_P* with certified ranking
-        const float rmf = (float)rot_margin;                // +inf unless POSE_REG_SPLIT
-        float dv[NQ];
-#pragma unroll
-        for (int q = 0; q < NQ; ++q) dv[q] = (lane + 32 * q < n_p) ? fminf(dt[q], rmf) : -CUDART_INF_F;
-        float unc = wmax_nonneg(unc_l), myval;
-        if (RES == CLOSURE_POSE_REG_SPLIT) unc += 1.2e-7f * fabsf(rmf);
-        // (exact_only & 4: debug, every step takes the fp64 fall-back; & 16: on all N_P perturbations)
-        if (!topk_certified<NQ>(dv, n_ps, unc, (L.exact_only & 4) != 0, (L.exact_only & 32) != 0, lane, candj, candd, myval)) {
+        }
+        if (!certified) {
+            // fp64 fall-back (near-ties, a threshold too close to the N_P*-th value, no separating threshold)
             double R[9], t[3];
 #pragma unroll
             for (int e = 0; e < 9; ++e) R[e] = pose[e];
 #pragma unroll
             for (int e = 0; e < 3; ++e) t[e] = pose[9 + e];
             const ExactMargin<RES> exact{ R, t, rows, n, rng, (uint32_t)s, t_p, rot_margin };
-            const int cnt = topk_fp64<NQ>(dv, n_p, n_ps, unc, myval, (L.exact_only & 16) != 0, lane, dex, candj, candd, exact);
-            if (stats) { stc[8] += 1; stc[0] += (unsigned long long)n * cnt; }
+            const bool all = !found || (L.exact_only & 16) != 0;
+            const int cntf = topk_fp64<NQ>(ub, n_p, n_ps, unc, myval, all, lane, dex, candj, candd, exact);
+            if (stats) { stc[8] += 1; stc[0] += (unsigned long long)n * cntf; }
         }
-        __syncwarp();                                       // pert[], candj[] visible to all lanes
+        __syncwarp();                                       // pert[], candj[], candd[] visible to all lanes
         if (lane < n_ps) cand4[lane] = pert[candj[lane]];
+        const float mycd = (lane < n_ps) ? candd[lane] : -CUDART_INF_F;
+        const float cdm = fkey_inv(__reduce_max_sync(FULL, fkey(mycd)));    // the best any candidate can be at R*
         __syncwarp();
 
         // ================================================== a5-a6: ladder, first feasible rung
         int m0 = 0;
         unsigned win = 0u;
-        bool lip_stop = false;
-        const int khalf = (KP + 1) >> 1;
-        for (int mb = 0; mb < n_t && m0 == 0 && !lip_stop; mb += 16) {
-            // ---- screening of 16 rungs, lane = (rung, half of the candidates): a candidate is dead for sure
-            // at rung m if one of the two tightest rows is violated beyond its error bound, or if its margin
-            // at R* is more negative than the rotation to R_m (or any smaller one: qL is a suffix maximum)
-            // can repair
-            const int mq = mb + (lane & 15), hq = lane >> 4;
-            const bool q_act = mq < n_t;
-            unsigned alive = 0u;
-            float Lm = CUDART_INF_F;
-            if (q_act) {
-                const float4 r0 = qrow[2 * mq], r1 = qrow[2 * mq + 1];
-                Lm = qL[mq];
-                const int k1 = min(KP, (hq + 1) * khalf);
-                for (int k = hq * khalf; k < k1; ++k) {
-                    const float4 c4 = cand4[k];
-                    const float v0 = fmaf(r0.x, c4.x, fmaf(r0.y, c4.y, fmaf(r0.z, c4.z, r0.w)));
-                    const float v1 = fmaf(r1.x, c4.x, fmaf(r1.y, c4.y, fmaf(r1.z, c4.z, r1.w)));
-                    if (!(v0 > c4.w) && !(v1 > c4.w) && !(candd[k] + Lm < 0.f)) alive |= 1u << k;
-                }
+        for (int mb = 0; mb < n_t && m0 == 0; mb += 32) {
+            // ---- rungs that the rotation can still repair: cdm + qL[m] >= 0 (qL is non-increasing in m: a prefix)
+            const int mq = mb + lane;
+            const bool lip_ok = (mq < n_t) && !(cdm + qL[min(mq, n_t - 1)] < 0.f);
+            unsigned livemask = __ballot_sync(FULL, lip_ok);
+            if (L.exact_only & 2) livemask = __ballot_sync(FULL, mq < n_t);       // debug: nothing is screened out
+            const int nlive = __popc(livemask);             // a prefix of the block
+            if (nlive == 0) break;
+            // ---- screening, lane = (rung, candidate): a candidate is dead for sure at rung m if one of the rung's two
+            // tight rows is violated beyond its error bound, or if its margin at R* is more negative than the
+            // rotation to R_m can repair
+            unsigned rmask = 0u;
+            const int tasks = nlive * KP;
+#pragma unroll 1
+            for (int tq = lane; tq < tasks; tq += 32) {
+                const int ml = (int)(((unsigned)tq * inv_kp) >> 16);
+                const int k = tq - ml * KP;
+                const int m = mb + ml;
+                const float4 r0 = qrow[2 * m], r1 = qrow[2 * m + 1];
+                const float4 c4 = cand4[k];
+                const float v0 = fmaf(r0.x, c4.x, fmaf(r0.y, c4.y, fmaf(r0.z, c4.z, r0.w)));
+                const float v1 = fmaf(r1.x, c4.x, fmaf(r1.y, c4.y, fmaf(r1.z, c4.z, r1.w)));
+                if (!(v0 > c4.w) && !(v1 > c4.w) && !(candd[k] + qL[m] < 0.f)) rmask |= 1u << ml;
             }
-            alive |= __shfl_xor_sync(FULL, alive, 16);
-            if (L.exact_only & 2) alive = q_act ? ((KP >= 32) ? FULL : ((1u << KP) - 1u)) : 0u;   // debug: nothing is screened out
-            if (mb + 16 < n_t && !(L.exact_only & 2)) {
-                // no candidate can be repaired at the last rung of this block => none at any later rung
-                float cdm = candd[0];
-                for (int k = 1; k < KP; ++k) cdm = fmaxf(cdm, candd[k]);
-                if (cdm + qL[mb + 15] < 0.f) lip_stop = true;
-            }
-            unsigned qmask = __ballot_sync(FULL, lane < 16 && alive != 0u);
-            if (stats) stc[7] += (unsigned long long)(min(n_t, mb + 16) - mb) * 2 * KP;
+            unsigned qmask = __reduce_or_sync(FULL, rmask);
+            if (L.exact_only & 2) qmask = livemask;
+            if (stats) stc[7] += (unsigned long long)tasks * 2;
 
             // ---- full evaluation of the surviving rungs, in order
             while (qmask != 0u && m0 == 0) {
                 const int l0 = __ffs(qmask) - 1;
                 qmask &= qmask - 1u;
                 const int m1 = mb + l0;
-                const unsigned cand_alive = __shfl_sync(FULL, alive, l0);
                 double Rm[9], t[3];
 #pragma unroll
                 for (int e = 0; e < 9; ++e) Rm[e] = RmS[m1 * 9 + e];
@@ -627,6 +869,8 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                     __syncwarp();                            // earlier readers of rowsL are done
                     float eps_l = 0.f;
                     bool rdead = false;
+                    float w1 = -CUDART_INF_F, w2 = -CUDART_INF_F;    // this lane's two tightest rows of the rung
+                    int i1 = 0, i2 = 0;
 #pragma unroll 1
                     for (int i = lane; i < n; i += 32) {
                         const double *row = rows + i * ROW;
@@ -637,14 +881,33 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                         }
                         float g0, g1, g2, fcb, eps;
                         screen_row(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
-                        rowsL[i] = make_float4(g0, g1, g2, fcb - eps);
+                        const float wv = fcb - eps;
+                        rowsL[i] = make_float4(g0, g1, g2, wv);
                         eps_l = fmaxf(eps_l, eps);
+                        if (wv > w1) { w2 = w1; i2 = i1; w1 = wv; i1 = i; } else if (wv > w2) { w2 = wv; i2 = i; }
                     }
                     epsL = wmax_nonneg(eps_l);
                     rdeadL = __any_sync(FULL, rdead);
                     full_m = m1;
                     if (stats) stc[3] += n;
                     __syncwarp();
+                    // the rung's screening rows become its two tightest rows among ALL constraints (they stay until the
+                    // next move): the candidate rows of the set-up let this rung through, these will not do so as easily
+                    {
+                        const uint32_t k1 = fkey(w1);
+                        const uint32_t g1m = __reduce_max_sync(FULL, k1);
+                        const int src1 = __ffs(__ballot_sync(FULL, k1 == g1m)) - 1;
+                        const uint32_t k2 = (lane == src1) ? fkey(w2) : k1;
+                        const uint32_t g2m = __reduce_max_sync(FULL, k2);
+                        const int src2 = __ffs(__ballot_sync(FULL, k2 == g2m)) - 1;
+                        if (lane == src1) {
+                            float4 r4 = rowsL[i1];
+                            if (rdeadL) r4.w = CUDART_INF_F;
+                            qrow[2 * m1] = r4;
+                        }
+                        if (lane == src2) qrow[2 * m1 + 1] = rowsL[(lane == src1) ? i2 : i1];
+                        __syncwarp();
+                    }
                 }
                 if (stats) { stc[9] += 1; stc[7] += (unsigned long long)n * KP; }
                 unsigned feas = 0u;
@@ -664,9 +927,9 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                     const bool dead = M > c4.w;
                     const bool sure = (epsL < CUDART_INF_F) && (M <= c4.w - 2.0f * epsL);
                     const bool mine = e_act && ech == 0;
-                    unsigned alive2 = __ballot_sync(FULL, mine && !dead) & cand_alive;
-                    unsigned undecided = __ballot_sync(FULL, mine && !dead && !sure) & cand_alive;
-                    if (L.exact_only & 2) { alive2 = cand_alive; undecided = cand_alive; }
+                    unsigned alive2 = __ballot_sync(FULL, mine && !dead) & kp_all;
+                    unsigned undecided = __ballot_sync(FULL, mine && !dead && !sure) & kp_all;
+                    if (L.exact_only & 2) { alive2 = kp_all; undecided = kp_all; }
                     if (L.exact_only & 32) { alive2 &= ~undecided; undecided = 0u; }   // fp32 mode: undecided counts as VIOLATED, so every emitted sample stays inside S (Prop. 4)
                     while (undecided != 0u) {                // rare: fp64 decides
                         const int k = __ffs(undecided) - 1;
@@ -679,6 +942,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                 }
                 if (feas != 0u) { m0 = m1 + 1; win = feas; }
             }
+            if (nlive < 32) break;                          // the live rungs are a prefix: none beyond this block
         }
 
         int j_win = 0;
@@ -721,7 +985,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
 template <int RES, int NQ>
 cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
 {
-    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 1, L.pairs_cap);
+    const AffSmem lay = aff_layout(max_rows_bytes, max_n, L.n_t, NQ, L.pairs_cap);
     if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaFuncSetAttribute(walker_coop_kernel<RES, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)lay.total);
