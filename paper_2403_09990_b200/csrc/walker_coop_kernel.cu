@@ -158,8 +158,27 @@ constexpr int kCset = 16;     // constraints the rung-screening rows are picked 
 
 struct AffSmem {
     size_t run_end, run_bf, run_pend, pos, warp0, per_warp;
-    size_t rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, cand4, candj, candd, vals, sj, sv, rowsT, runT_pend, runT_bf, cset, pose, stc, total;
+    size_t rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, total;
 };
+
+// Per-warp block: the small fixed-size arrays first, at compile-time offsets from the warp's base (the per-iteration
+// code addresses them without keeping pointers in registers), then the arrays sized by NQ, then those sized by the
+// instance (rowsA first: its offset is still a constant).
+constexpr size_t kOffCand4 = 0;                       // 32 x float4: the kept perturbations (-2 d_j, -|d_j|^2), by rank
+constexpr size_t kOffCandj = kOffCand4 + 32 * 16;     // 32 x int
+constexpr size_t kOffCandd = kOffCandj + 32 * 4;      // 32 x float: upper bounds of the candidates' eq. (14) values
+constexpr size_t kOffVals = kOffCandd + 32 * 4;       // 32 x float: the N_P* + 1 largest eq. (14) values, by rank
+constexpr size_t kOffSjv = kOffVals + 32 * 4;         // 32 x (int, float): survivors of the threshold (index, phase-1 value)
+constexpr size_t kOffRowsT = kOffSjv + 32 * 8;        // kTight x 32 B
+constexpr size_t kOffRunTp = kOffRowsT + (size_t)kTight * 32;
+constexpr size_t kOffRunTb = kOffRunTp + (size_t)kTight * 4;
+constexpr size_t kOffCset = kOffRunTb + (size_t)kTight * 4;
+constexpr size_t kOffPose = kOffCset + (size_t)kCset * 4;   // 20 doubles: R*(9) t*(3) omega(3) + set-up results
+constexpr size_t kOffStc = kOffPose + 20 * 8;               // 16 counters
+constexpr size_t kOffPert = kOffStc + 16 * 8;               // NQ x 32 x float4
+__host__ __device__ constexpr size_t aff_off_dex(int nq) { return kOffPert + (size_t)nq * 32 * 16; }    // NQ x 32 doubles
+__host__ __device__ constexpr size_t aff_off_rowsA(int nq) { return aff_off_dex(nq) + (size_t)nq * 32 * 8; }
+static_assert(kOffPose % 16 == 0 && kOffPert % 16 == 0 && kOffRowsT % 16 == 0, "alignment of the per-warp block");
 
 // pairs = 32-byte entries of rowsA (pair-entries, runs padded to even length)
 __host__ __device__ inline AffSmem aff_layout(int rows_bytes, int n, int n_t, int nq, int pairs, int warps = kCoopWarps)
@@ -171,27 +190,15 @@ __host__ __device__ inline AffSmem aff_layout(int rows_bytes, int n, int n_t, in
     s.run_pend = o; o += (size_t)((n * 4 + 15) & ~15);
     s.pos = o;     o += (size_t)((n * 4 + 15) & ~15);
     s.warp0 = o;
-    size_t w = 0;
+    s.pert = kOffPert;
+    s.dex = aff_off_dex(nq);
+    size_t w = aff_off_rowsA(nq);
     s.rowsA = w; w += (size_t)pairs * 32;          // pair-transposed, runs padded to even length
     s.rowsL = w; w += (size_t)n * 16;
-    s.pert = w;  w += (size_t)nq * 32 * 16;
-    s.ab = w;    w += (size_t)n_t * 16;
     s.qrow = w;  w += (size_t)n_t * 32;
     s.RmS = w;   w += (size_t)((n_t * 72 + 15) & ~15);
-    s.dex = w;   w += (size_t)nq * 32 * 8;
+    s.ab = w;    w += (size_t)n_t * 16;
     s.qL = w;    w += (size_t)((n_t * 4 + 15) & ~15);
-    s.cand4 = w; w += 32 * 16;
-    s.candj = w; w += 32 * 4;
-    s.candd = w; w += 32 * 4;
-    s.vals = w;  w += 32 * 4;
-    s.sj = w;    w += 32 * 4;
-    s.sv = w;    w += 32 * 4;
-    s.rowsT = w; w += (size_t)kTight * 32;
-    s.runT_pend = w; w += (size_t)kTight * 4;
-    s.runT_bf = w;   w += (size_t)kTight * 4;
-    s.cset = w;  w += (size_t)kCset * 4;
-    s.pose = w;  w += 20 * 8;
-    s.stc = w;   w += 16 * 8;
     s.per_warp = w;
     s.total = o + (size_t)warps * w;
     return s;
@@ -219,15 +226,15 @@ __device__ __noinline__ void aff_setup_on_move(unsigned char *smem_raw, int warp
     const int *pos = reinterpret_cast<const int *>(smem_raw + lay.pos);
     unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
     float *rowsA = reinterpret_cast<float *>(wp + lay.rowsA);
-    float *rowsT = reinterpret_cast<float *>(wp + lay.rowsT);
-    int *runT_pend = reinterpret_cast<int *>(wp + lay.runT_pend);
-    float *runT_bf = reinterpret_cast<float *>(wp + lay.runT_bf);
-    int *cset = reinterpret_cast<int *>(wp + lay.cset);
+    float *rowsT = reinterpret_cast<float *>(wp + kOffRowsT);
+    int *runT_pend = reinterpret_cast<int *>(wp + kOffRunTp);
+    float *runT_bf = reinterpret_cast<float *>(wp + kOffRunTb);
+    int *cset = reinterpret_cast<int *>(wp + kOffCset);
     const double2 *ab = reinterpret_cast<const double2 *>(wp + lay.ab);
     float4 *qrow = reinterpret_cast<float4 *>(wp + lay.qrow);
     double *RmS = reinterpret_cast<double *>(wp + lay.RmS);
-    double *pose = reinterpret_cast<double *>(wp + lay.pose);
-    unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
+    double *pose = reinterpret_cast<double *>(wp + kOffPose);
+    unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + kOffStc);
     const float tpf = (float)t_p * 1.0000002f;          // >= t_p
     const float tp2 = 2.0f * tpf, tp2sq3 = 3.0f * tpf * tpf;
     double R[9], t[3], vel[3];
@@ -502,22 +509,20 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
     float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);
     float4 *rowsL = reinterpret_cast<float4 *>(wp + lay.rowsL);
-    float4 *pert = reinterpret_cast<float4 *>(wp + lay.pert);
+    float4 *pert = reinterpret_cast<float4 *>(wp + kOffPert);
     double2 *ab = reinterpret_cast<double2 *>(wp + lay.ab);
     float4 *qrow = reinterpret_cast<float4 *>(wp + lay.qrow);     // [rung][2]: two tight rows of each rung
     double *RmS = reinterpret_cast<double *>(wp + lay.RmS);
-    double *dex = reinterpret_cast<double *>(wp + lay.dex);      // fp64 fallback: exact d_j, [q][lane]
+    double *dex = reinterpret_cast<double *>(wp + aff_off_dex(NQ));      // fp64 fallback: exact d_j, [q][lane]
     float *qL = reinterpret_cast<float *>(wp + lay.qL);           // [rung]: bound on the change of any residual norm, non-increasing
-    float4 *cand4 = reinterpret_cast<float4 *>(wp + lay.cand4);   // the kept perturbations (-2 d_j, -|d_j|^2), by rank
-    int *candj = reinterpret_cast<int *>(wp + lay.candj);
-    float *candd = reinterpret_cast<float *>(wp + lay.candd);     // upper bounds of the candidates' eq. (14) values
-    float *vals = reinterpret_cast<float *>(wp + lay.vals);       // the N_P* + 1 largest eq. (14) values, by rank
-    int *sj = reinterpret_cast<int *>(wp + lay.sj);               // survivors of the threshold: perturbation index
-    float *sv = reinterpret_cast<float *>(wp + lay.sv);           //                             and phase-1 value
-    const float4 *rowsT = reinterpret_cast<const float4 *>(wp + lay.rowsT);
-    const int *runT_pend = reinterpret_cast<const int *>(wp + lay.runT_pend);
-    const float *runT_bf = reinterpret_cast<const float *>(wp + lay.runT_bf);
-    double *pose = reinterpret_cast<double *>(wp + lay.pose);     // R*(9) t*(3) omega(3): fp64, touched only on moves / fp64 paths
+    float4 *cand4 = reinterpret_cast<float4 *>(wp + kOffCand4);   // the kept perturbations (-2 d_j, -|d_j|^2), by rank
+    int *candj = reinterpret_cast<int *>(wp + kOffCandj);
+    float *candd = reinterpret_cast<float *>(wp + kOffCandd);     // upper bounds of the candidates' eq. (14) values
+    int2 *sjv = reinterpret_cast<int2 *>(wp + kOffSjv);           // survivors of the threshold: (perturbation index, phase-1 value)
+    const float4 *rowsT = reinterpret_cast<const float4 *>(wp + kOffRowsT);
+    const int *runT_pend = reinterpret_cast<const int *>(wp + kOffRunTp);
+    const float *runT_bf = reinterpret_cast<const float *>(wp + kOffRunTb);
+    double *pose = reinterpret_cast<double *>(wp + kOffPose);     // R*(9) t*(3) omega(3): fp64, touched only on moves / fp64 paths
 
     const unsigned long long w = (unsigned long long)(L.walker_begin + local);
     const unsigned long long seed = L.seed[blockIdx.y];
@@ -562,6 +567,15 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     unsigned e_mask = 0u;                               // lanes that share this lane's candidate
     for (int c = 0; c < NCH; ++c) e_mask |= 1u << (ek + c * KP);
     const unsigned kp_all = (KP >= 32) ? FULL : ((1u << KP) - 1u);
+    unsigned sortdir = 0u;                              // bit t: this lane keeps the larger key at stage t of the bitonic network
+    {
+        int stage = 0;
+        for (int k = 2; k <= 32; k <<= 1)
+            for (int j = k >> 1; j > 0; j >>= 1) {
+                if (((lane & j) == 0) == ((lane & k) == 0)) sortdir |= 1u << stage;
+                ++stage;
+            }
+    }
     const unsigned inv_kp = (65536u + (unsigned)KP - 1u) / (unsigned)KP;   // t / KP = (t * inv_kp) >> 16 for t < 3,000
 
     // selection constants: at most s_max survivors (a power of two), at least need_lo
@@ -573,7 +587,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     float U_state = 0.f;
 
     // executed-work counters (closure_get_stats): in shared memory, touched by lane 0 and only when asked for
-    unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
+    unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + kOffStc);
     const bool stats = (L.stats != nullptr) && lane == 0;
     if (stats) {
         for (int k = 0; k < kNumStats; ++k) stc[k] = 0ull;
@@ -584,7 +598,14 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     float epsA = 0.f;
     double rot_margin = CUDART_INF;
     int nT_runs = 0;
-    const bool full_p1 = run_pend[n_runs - 1] <= kTight;   // short tables: phase 1 evaluates every constraint, no phase 2
+    const int pairs_total = run_pend[n_runs - 1];
+    const bool full_p1 = pairs_total <= kTight;          // short tables: phase 1 evaluates every constraint, no phase 2
+    // N_P <= 32 and one run of equal bounds (BASELINE config 5): best-first branch and bound, one perturbation at a time
+    // against the whole table, which the lanes keep in registers while the walker stays (up to four pair-entries each)
+    const bool best_first = NQ == 1 && n_runs == 1 && pairs_total <= 128;
+    const int pe_rt = (pairs_total + 31) >> 5;
+    unsigned long long CA0[4], CA1[4], CA2[4], CA3[4];   // (f0a f0b) (f1a f1b) (f2a f2b) (fca fcb) of entries lane + 32 k
+    float *vals = reinterpret_cast<float *>(wp + kOffVals);       // best_first: the N_P* + 1 largest eq. (14) values, by rank
     // cached across iterations while the pose does not move
     int full_m = -1;                                    // rung whose rows sit in rowsL
     float epsL = 0.f;
@@ -600,6 +621,19 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
             rot_margin = pose[15];
             nT_runs = (int)pose[17];
             full_m = -1;
+            if (NQ == 1 && best_first && !full_p1) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const int e = lane + 32 * k;
+                    if (e < pairs_total) {
+                        const float4 X = rowsA[2 * e], Y = rowsA[2 * e + 1];
+                        CA0[k] = pk2(X.x, X.y); CA1[k] = pk2(X.z, X.w); CA2[k] = pk2(Y.x, Y.y); CA3[k] = pk2(Y.z, Y.w);
+                    } else {
+                        CA0[k] = CA1[k] = CA2[k] = pk2(0.f, 0.f);
+                        CA3[k] = pk2(-CUDART_INF_F, -CUDART_INF_F);
+                    }
+                }
+            }
         }
 
         // ================================================== a2: perturbations of this lane
@@ -641,7 +675,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
         const float E0 = epsA + tp2sq3 * kMu19;             // bound on |a32 - a64| up to its own rounding
         float unc_l = 0.f;
         float ub[NQ];                                       // phase 1: upper bounds of d_j (the values themselves if full_p1)
-        const bool use_p1 = full_p1 || n_p > s_max;         // few perturbations: all of them are "survivors"
+        const bool use_p1 = full_p1 || n_p > s_max || best_first;   // few perturbations: all of them are "survivors"
         if (use_p1) {
             eq14_table<NQ>(full_p1 ? rowsA : rowsT, full_p1 ? n_runs : nT_runs, full_p1 ? run_pend : runT_pend,
                            full_p1 ? run_bf : runT_bf, p0, p1, p2, o0, o1, o2, dd, E0, ub, unc_l);
@@ -665,6 +699,84 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
         bool certified = false;
         float myval = -CUDART_INF_F;
         float unc = 0.f;
+        if (NQ == 1 && best_first) {
+            // ---- best-first branch and bound (lane j = perturbation j): the perturbation with the largest upper bound is
+            // evaluated against the whole table (lane = pair-entries, one warp maximum) until N_P* exact values lie more
+            // than 2 unc above every remaining upper bound; no other perturbation can then be among the N_P* best
+            const float ub0 = ub[0];
+            const bool valid = lane < n_p;
+            uint32_t pool = (valid && !full_p1) ? ((fkey(ub0) & ~31u) | (uint32_t)(31 - lane)) : 0u;   // not yet evaluated
+            if (valid && !full_p1 && (ub0 != ub0)) pool = 0xffffffe0u | (uint32_t)(31 - lane);             // a NaN is evaluated first
+            float dexv = (valid && full_p1) ? ub0 : -CUDART_INF_F;     // exact eq. (14) value of this lane's perturbation
+            bool evald = valid && full_p1;
+            float uncw = wmax_nonneg(unc_l);
+            const float bf0 = run_bf[0];
+            float Umax = -CUDART_INF_F;
+#pragma unroll 1
+            for (int ev = 0; ev <= n_p; ++ev) {
+                const uint32_t g = __reduce_max_sync(FULL, pool);
+                if (g == 0u) { Umax = -CUDART_INF_F; break; }           // everything is evaluated
+                Umax = fkey_inv(g | 31u);                                // >= every remaining upper bound
+                const float needl = fmaf(2.0f, uncw, 4.0f * kMu19 * (fabsf(dexv) + fabsf(Umax)));
+                const int above = __popc(__ballot_sync(FULL, evald && (dexv - Umax > needl)));
+                if (above >= n_ps) break;
+                const int jsel = 31 - (int)(g & 31u);
+                const float4 pj = pert[jsel];
+                const unsigned long long E0p = pk2(pj.x, pj.x), E1p = pk2(pj.y, pj.y), E2p = pk2(pj.z, pj.z);
+                float m = -CUDART_INF_F;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    if (k < pe_rt) {
+                        const unsigned long long vo = fma2(CA0[k], E0p, fma2(CA1[k], E1p, fma2(CA2[k], E2p, CA3[k])));
+                        float l2, h2;
+                        upk2(vo, l2, h2);
+                        m = fmaxf(m, fmaxf(l2, h2));
+                    }
+                }
+                const float mv = fkey_inv(__reduce_max_sync(FULL, fkey(m)));
+                const float a = fmaxf(mv - pj.w, 1e-30f);              // pj.w = -|d|^2
+                const float rr = rsqrt_normal(a);
+                const float sq = a * rr;
+                uncw = fmaxf(uncw, 1.01f * fmaf(E0, rr, (bf0 + sq) * kMu19));
+                if (lane == jsel) { dexv = fminf(bf0 - sq, rmf); evald = true; pool = 0u; }
+                if (stats) { stc[6] += (unsigned long long)n; stc[13] += 1; }
+            }
+            unc = uncw;
+            if (RES == CLOSURE_POSE_REG_SPLIT) unc += 1.2e-7f * fabsf(rmf);
+            // ---- rank the evaluated values by counting (a handful), the N_P* + 1 best go to vals[] / candj[]
+            const unsigned evm = __ballot_sync(FULL, evald);
+            const bool nan_any = __any_sync(FULL, evald && (dexv != dexv));
+            int rank = 0;
+            for (unsigned rem = evm; rem != 0u; rem &= rem - 1u) {
+                const int e = __ffs(rem) - 1;
+                const float xe = __shfl_sync(FULL, dexv, e);
+                rank += (xe > dexv || (xe == dexv && e < lane)) ? 1 : 0;
+            }
+            if (evald && rank <= n_ps) {
+                vals[rank] = dexv;
+                if (rank < n_ps) candj[rank] = lane;
+            }
+            __syncwarp();
+            const int nev = __popc(evm);
+            myval = (lane <= n_ps && lane < nev) ? vals[lane] : -CUDART_INF_F;
+            const float prev = __shfl_up_sync(FULL, myval, 1);
+            const bool trust = (L.exact_only & 32) != 0;
+            bool ok = true;
+            if (lane < n_ps) ok = (myval > -CUDART_INF_F) && (myval < CUDART_INF_F);
+            if (lane >= 1 && lane <= n_ps) {
+                const bool none_left = (lane == n_ps) && (myval == -CUDART_INF_F);
+                const float needg = fmaf(2.0f, unc, 4.0f * kMu19 * (fabsf(prev) + fabsf(myval)));
+                ok = ok && (none_left || (prev - myval > needg));
+            }
+            if (trust) ok = true;                       // fp32 mode: the fp32 ranking is taken as it is
+            if (lane == n_ps - 1 && Umax > -CUDART_INF_F) {
+                const float needu = fmaf(2.0f, unc, 4.0f * kMu19 * (fabsf(Umax) + fabsf(myval)));
+                ok = ok && (trust ? (myval >= Umax) : (myval - Umax > needu));
+            }
+            if (nan_any || (L.exact_only & 4)) ok = false;
+            certified = __all_sync(FULL, ok);
+            if (certified && lane < n_ps) candd[lane] = myval + fmaf(1.01f, unc, 4.0f * kMu19 * fabsf(myval));    // >= the fp64 value d_j
+        } else {
 #pragma unroll 1
         for (int attempt = 0; attempt < 3; ++attempt) {
         if (n_p > s_max) {
@@ -694,32 +806,29 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
             // ---- compaction of the survivors: (j, phase-1 value) by slot
             {
                 int base = 0;
+                const unsigned lt = (1u << lane) - 1u;
 #pragma unroll
                 for (int q = 0; q < NQ; ++q) {
                     const bool in = (lane + 32 * q < n_p) && !(ub[q] < U);
                     const unsigned b = __ballot_sync(FULL, in);
-                    if (in) {
-                        const int ps = base + __popc(b & ((1u << lane) - 1u));
-                        sj[ps] = lane + 32 * q;
-                        sv[ps] = ub[q];
-                    }
+                    if (in) sjv[base + __popc(b & lt)] = make_int2(lane + 32 * q, __float_as_int(ub[q]));
                     base += __popc(b);
                 }
             }
-            __syncwarp();                                   // sj[], sv[], pert[] visible to all lanes
+            __syncwarp();                                   // sjv[], pert[] visible to all lanes
             if (stats) stc[13] += (unsigned long long)cnt;
             // ---- phase 2: the survivors against all constraints, lane = (survivor slot, chunk of the table)
-            int S = 1;
-            while (S < cnt) S <<= 1;
+            const int lgS = 32 - __clz(max(cnt, 1) - 1);    // S = 2^lgS >= cnt survivors' slots, C = 32 / S chunks of the table
+            const int S = 1 << lgS;
             const int slot = lane & (S - 1);
             const bool act = slot < cnt;
-            const int myj = act ? sj[slot] : 0;
+            const int2 mine = sjv[act ? slot : 0];
             float val;
             if (full_p1) {
-                val = act ? sv[slot] : -CUDART_INF_F;
+                val = __int_as_float(mine.y);
             } else {
-                const int C = 32 / S, chunk = lane / S;
-                const float4 pj = pert[myj];
+                const int lgC = 5 - lgS, chunk = lane >> lgS;
+                const float4 pj = pert[mine.x];
                 const unsigned long long E0p = pk2(pj.x, pj.x), E1p = pk2(pj.y, pj.y), E2p = pk2(pj.z, pj.z);
                 float v = CUDART_INF_F;
                 int pp = 0;
@@ -727,14 +836,21 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                     const int pend = run_pend[r];
                     const float bf = run_bf[r];
                     float mx = -CUDART_INF_F;
+                    // the same trip count on every lane (a lane past the end of the run re-reads its last entry: a maximum
+                    // does not see duplicates), so that the warp stays converged
+                    const int trips = (pend - pp + (1 << lgC) - 1) >> lgC;
+                    const float4 *e = rowsA + 2 * (pp + chunk);
+                    const float4 *elast = rowsA + 2 * (pend - 1);
 #pragma unroll 2
-                    for (int p = pp + chunk; p < pend; p += C) {
-                        const float4 X = rowsA[2 * p], Y = rowsA[2 * p + 1];
+                    for (int it = 0; it < trips; ++it) {
+                        const float4 *ec = e < elast ? e : elast;
+                        const float4 X = ec[0], Y = ec[1];
                         const unsigned long long vo =
                             fma2(pk2(X.x, X.y), E0p, fma2(pk2(X.z, X.w), E1p, fma2(pk2(Y.x, Y.y), E2p, pk2(Y.z, Y.w))));
                         float l2, h2;
                         upk2(vo, l2, h2);
                         mx = fmaxf(mx, fmaxf(l2, h2));
+                        e += 2 << lgC;
                     }
                     pp = pend;
                     for (int off = S; off < 32; off <<= 1) mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, off));
@@ -745,65 +861,72 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                     if (act) unc_l = fmaxf(unc_l, du);
                     v = fminf(v, bf - sq);
                 }
-                val = act ? fminf(v, rmf) : -CUDART_INF_F;
+                val = fminf(v, rmf);
                 if (stats) stc[6] += (unsigned long long)n * cnt;
             }
             unc = wmax_nonneg(unc_l);
             if (RES == CLOSURE_POSE_REG_SPLIT) unc += 1.2e-7f * fabsf(rmf);
-            // ---- ranking by counting (lanes 0 .. cnt-1 hold one survivor each); ties are ordered by slot and never certified
-            int rank = 0;
+            // ---- ranking: a sorting network on order-preserving keys whose 5 low bits carry the slot (values move down by
+            // < 2^-18 relative: covered by the certificate); lanes 0 .. cnt-1 hold one survivor each
             const bool nan_any = __any_sync(FULL, act && (val != val));
-#pragma unroll 4
-            for (int r = 0; r < cnt; ++r) {
-                const float xr = __shfl_sync(FULL, val, r);
-                rank += (xr > val || (xr == val && r < slot)) ? 1 : 0;
+            uint32_t key = (lane < cnt) ? ((fkey(val) & ~31u) | (uint32_t)(31 - lane)) : 0u;
+            // bitonic sorting network over the 32 lanes, descending: lane r ends with the r-th largest key
+            {
+                int stage = 0;
+#pragma unroll
+                for (int k = 2; k <= 32; k <<= 1) {
+#pragma unroll
+                    for (int j = k >> 1; j > 0; j >>= 1) {
+                        const uint32_t o = __shfl_xor_sync(FULL, key, j);
+                        key = ((sortdir >> stage) & 1u) ? max(key, o) : min(key, o);
+                        ++stage;
+                    }
+                }
             }
-            if (lane < cnt && rank <= n_ps) {
-                vals[rank] = val;
-                if (rank < n_ps) candj[rank] = myj;
-            }
+            const bool have = lane < cnt;                   // this lane holds the survivor ranked `lane`
+            myval = have ? fkey_inv(key & ~31u) : -CUDART_INF_F;    // the value the key stands for (<= the survivor's value)
+            const int myj = sjv[have ? 31 - (int)(key & 31u) : 0].x;
+            if (lane < n_ps) candj[lane] = myj;
             // the next iteration's threshold: the value ranked r_target (the distribution is stationary while the walker stays)
             {
-                const int rt = min(cnt - 1, r_target);
-                const unsigned bt = __ballot_sync(FULL, lane < cnt && rank == rt);
-                const float ut = __shfl_sync(FULL, val, bt ? (__ffs(bt) - 1) : 0);
-                U_state = (bt != 0u && fabsf(ut) < 3.0e38f) ? ut : U;
+                const float ut = __shfl_sync(FULL, myval, min(cnt - 1, r_target));
+                U_state = (fabsf(ut) < 3.0e38f) ? ut : U;
             }
-            __syncwarp();
             // ---- certificate: consecutive values more than 2 unc apart, and the N_P*-th more than 2 unc above both the
             // next one and the threshold (every perturbation that was not evaluated has d_j <= ub_j < U + unc)
-            myval = (lane <= n_ps && lane < cnt) ? vals[lane] : -CUDART_INF_F;
+            if (lane > n_ps) myval = -CUDART_INF_F;
             const float prev = __shfl_up_sync(FULL, myval, 1);
             const bool trust = (L.exact_only & 32) != 0;
             bool ok = true;
             if (lane < n_ps) ok = (myval > -CUDART_INF_F) && (myval < CUDART_INF_F);
             if (lane >= 1 && lane <= n_ps) {
                 const bool none_left = (lane == n_ps) && (myval == -CUDART_INF_F);
-                const float needg = fmaf(2.0f, unc, kMu19 * (fabsf(prev) + fabsf(myval)));
+                const float needg = fmaf(2.0f, unc, 4.0f * kMu19 * (fabsf(prev) + fabsf(myval)));
                 ok = ok && (none_left || (prev - myval > needg));
             }
             if (trust) ok = true;                       // fp32 mode: the fp32 ranking is taken as it is
             bool oku = true;
             if (lane == n_ps - 1 && U > -CUDART_INF_F) {
-                const float needu = fmaf(2.0f, unc, kMu19 * (fabsf(U) + fabsf(myval)));
+                const float needu = fmaf(2.0f, unc, 4.0f * kMu19 * (fabsf(U) + fabsf(myval)));
                 oku = trust ? (myval >= U) : (myval - U > needu);
             }
             if (nan_any || (L.exact_only & 4)) ok = false;
             const bool gaps_ok = __all_sync(FULL, ok);
             ufail = !__all_sync(FULL, oku);
             certified = gaps_ok && !ufail;
-            if (certified && lane < n_ps) candd[lane] = myval + fmaf(1.01f, unc, kMu19 * fabsf(myval));    // >= the fp64 value d_j
+            if (certified && lane < n_ps) candd[lane] = myval + fmaf(1.01f, unc, 4.0f * kMu19 * fabsf(myval));    // >= the fp64 value d_j
             if (certified || !gaps_ok || cnt >= s_max) break;
             // only the threshold failed: lower it so that at least two more perturbations survive
             if (stats) stc[14] += 1;
             need = min(cnt + 2, s_max);
             hi = U;
             if (lo == -CUDART_INF_F) { U = U - step; step = step + step; } else U = 0.5f * (lo + hi);
-            __syncwarp();                                   // sj[], sv[], vals[] are rewritten by the next attempt
+            __syncwarp();                                   // sjv[], vals[] are rewritten by the next attempt
         } else {
             unc = wmax_nonneg(unc_l);
             if (stats) stc[15] += 1;
             break;
+        }
         }
         }
         if (!certified) {
