@@ -446,11 +446,18 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int n_runs_s;
     __shared__ float amax_s;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    int lane = threadIdx.x & 31;
     const InstanceDesc *__restrict__ D = L.desc[blockIdx.y];
     const int n = D->n;
     const int rows_bytes = D->rows_bytes;
-    const int n_p = L.n_p, n_ps = L.n_p_star, n_t = L.n_t;
+    int n_p = L.n_p, n_ps = L.n_p_star, n_t = L.n_t;
+    // Values the iteration uses all the time are made opaque to the compiler: under register pressure it otherwise
+    // re-derives them from special registers, the constant bank and shared memory inside the loop (measured: ~10 % of
+    // the executed instructions) instead of keeping them in a register.
+#define CLOSURE_PIN_R(x) asm volatile("" : "+r"(x))
+#define CLOSURE_PIN_F(x) asm volatile("" : "+f"(x))
+    CLOSURE_PIN_R(lane); CLOSURE_PIN_R(n_p); CLOSURE_PIN_R(n_ps); CLOSURE_PIN_R(n_t);
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
     double *rows = reinterpret_cast<double *>(smem_raw + 16);
     stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
@@ -558,8 +565,9 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
 
     const double t_p = L.t_p;
     const float tpf = (float)t_p * 1.0000002f;          // >= t_p
-    const float tp2 = 2.0f * tpf, tp2sq3 = 3.0f * tpf * tpf;
-    const float m2tp = -2.0f * (float)t_p;
+    float tp2 = 2.0f * tpf, tp2sq3 = 3.0f * tpf * tpf;
+    float m2tp = -2.0f * (float)t_p;
+    CLOSURE_PIN_F(tp2); CLOSURE_PIN_F(tp2sq3); CLOSURE_PIN_F(m2tp);
     const int KP = n_ps;                                // ladder candidates
     const int NCH = 32 / KP;                            // constraint chunks of the full evaluation
     const int ek = lane % KP, ech = lane / KP;
@@ -598,7 +606,8 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     float epsA = 0.f;
     double rot_margin = CUDART_INF;
     int nT_runs = 0;
-    const int pairs_total = run_pend[n_runs - 1];
+    int pairs_total = run_pend[n_runs - 1];
+    CLOSURE_PIN_R(pairs_total);
     const bool full_p1 = pairs_total <= kTight;          // short tables: phase 1 evaluates every constraint, no phase 2
     // N_P <= 32 and one run of equal bounds (BASELINE config 5): best-first branch and bound, one perturbation at a time
     // against the whole table, which the lanes keep in registers while the walker stays (up to four pair-entries each)
@@ -712,15 +721,13 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
             float uncw = wmax_nonneg(unc_l);
             const float bf0 = run_bf[0];
             float Umax = -CUDART_INF_F;
+            int rank = 0;                                             // of this lane's value among the evaluated ones
+            uint32_t g = __reduce_max_sync(FULL, pool);
 #pragma unroll 1
-            for (int ev = 0; ev <= n_p; ++ev) {
-                const uint32_t g = __reduce_max_sync(FULL, pool);
-                if (g == 0u) { Umax = -CUDART_INF_F; break; }           // everything is evaluated
-                Umax = fkey_inv(g | 31u);                                // >= every remaining upper bound
-                const float needl = fmaf(2.0f, uncw, 4.0f * kMu19 * (fabsf(dexv) + fabsf(Umax)));
-                const int above = __popc(__ballot_sync(FULL, evald && (dexv - Umax > needl)));
-                if (above >= n_ps) break;
+            while (g != 0u) {
                 const int jsel = 31 - (int)(g & 31u);
+                if (lane == jsel) pool = 0u;
+                const uint32_t gnext = __reduce_max_sync(FULL, pool);    // issued early: its latency hides behind the evaluation
                 const float4 pj = pert[jsel];
                 const unsigned long long E0p = pk2(pj.x, pj.x), E1p = pk2(pj.y, pj.y), E2p = pk2(pj.z, pj.z);
                 float m = -CUDART_INF_F;
@@ -738,19 +745,31 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                 const float rr = rsqrt_normal(a);
                 const float sq = a * rr;
                 uncw = fmaxf(uncw, 1.01f * fmaf(E0, rr, (bf0 + sq) * kMu19));
-                if (lane == jsel) { dexv = fminf(bf0 - sq, rmf); evald = true; pool = 0u; }
+                const float dnew = fminf(bf0 - sq, rmf);                // the same on every lane
+                // ranks are kept up to date: values below the new one move down, the new one goes below those not smaller
+                const unsigned ge = __ballot_sync(FULL, evald && !(dexv < dnew));
+                if (evald && dexv < dnew) ++rank;
+                if (lane == jsel) { dexv = dnew; evald = true; rank = __popc(ge); }
                 if (stats) { stc[6] += (unsigned long long)n; stc[13] += 1; }
+                g = gnext;
+                Umax = (g != 0u) ? fkey_inv(g | 31u) : -CUDART_INF_F;  // >= every remaining upper bound
+                const float needl = fmaf(2.0f, uncw, 4.0f * kMu19 * (fabsf(dexv) + fabsf(Umax)));
+                const int above = __popc(__ballot_sync(FULL, evald && (dexv - Umax > needl)));
+                if (above >= n_ps) break;
             }
             unc = uncw;
             if (RES == CLOSURE_POSE_REG_SPLIT) unc += 1.2e-7f * fabsf(rmf);
-            // ---- rank the evaluated values by counting (a handful), the N_P* + 1 best go to vals[] / candj[]
+            // ---- the N_P* + 1 best go to vals[] / candj[] by rank (short tables: everything was evaluated by phase 1 and
+            // is ranked by counting here)
             const unsigned evm = __ballot_sync(FULL, evald);
             const bool nan_any = __any_sync(FULL, evald && (dexv != dexv));
-            int rank = 0;
-            for (unsigned rem = evm; rem != 0u; rem &= rem - 1u) {
-                const int e = __ffs(rem) - 1;
-                const float xe = __shfl_sync(FULL, dexv, e);
-                rank += (xe > dexv || (xe == dexv && e < lane)) ? 1 : 0;
+            if (full_p1) {
+                rank = 0;
+                for (unsigned rem = evm; rem != 0u; rem &= rem - 1u) {
+                    const int e = __ffs(rem) - 1;
+                    const float xe = __shfl_sync(FULL, dexv, e);
+                    rank += (xe > dexv || (xe == dexv && e < lane)) ? 1 : 0;
+                }
             }
             if (evald && rank <= n_ps) {
                 vals[rank] = dexv;
