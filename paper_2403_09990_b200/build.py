@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libclosure_b200.so")
-SOURCES = ["walker_kernel.cu", "walker_coop_kernel.cu", "walker_coop_reproj_kernel.cu", "walker_coop_trans_kernel.cu", "compact_kernel.cu", "megb_kernels.cu", "step1_kernel.cu", "alu_peak.cu", "closure_api.cu", "miniball.cpp"]
+SOURCES = ["walker_kernel.cu", "walker_coop_kernel.cu", "walker_dense_kernel.cu", "walker_coop_reproj_kernel.cu", "walker_coop_trans_kernel.cu", "compact_kernel.cu", "megb_kernels.cu", "step1_kernel.cu", "alu_peak.cu", "closure_api.cu", "miniball.cpp"]
 HEADERS = [os.path.join(CSRC, "closure_internal.h"), os.path.join(CSRC, "walker_common.cuh"), os.path.join(CSRC, "walker_coop_common.cuh"), os.path.join(os.path.dirname(HERE), "include", "closure.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

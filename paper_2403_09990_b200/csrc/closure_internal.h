@@ -70,6 +70,10 @@ bool coop_path_available(int residual_type, int mode, int n_p, int max_n);
 cudaError_t launch_walkers_coop(int residual_type, const WalkLaunch &L, int n_instances, int max_rows_bytes,
                                 cudaStream_t stream);
 
+// walker_dense_kernel.cu: the dense variant of the above (every perturbation against every constraint), N_P > 32 on short tables
+cudaError_t launch_walkers_coop_dense(int residual_type, const WalkLaunch &L, int n_instances, int max_rows_bytes,
+                                      cudaStream_t stream);
+
 // walker_coop_reproj_kernel.cu: the same organisation for the reprojection residual (ROT mode)
 cudaError_t launch_walkers_coop_reproj(const WalkLaunch &L, int n_instances, int max_rows_bytes, cudaStream_t stream);
 

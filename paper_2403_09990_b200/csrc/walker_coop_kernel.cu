@@ -35,17 +35,20 @@
 #define CLOSURE_COOP_MIN_CTAS 4   // resident CTAs per SM the register allocation aims at (128 registers per thread)
 #endif
 
+#ifndef CLOSURE_NEED_EXTRA
+#define CLOSURE_NEED_EXTRA 3   // the threshold keeps at least N_P* + this many perturbations
+#define CLOSURE_RT_EXTRA 3     // the next threshold is the value ranked N_P* + this + (N_P* >> CLOSURE_RT_SHIFT)
+#define CLOSURE_RT_SHIFT 2
+#endif
+
 namespace closure {
 namespace {
 
-// Measured on B200: the pose-regression kernel, whose rows are twice as long, gains 3.7 % at 6 resident
-// CTAs (80 registers); the registration kernel gains 1 % at 5 (96 registers) in the NQ = 5 instantiation (64 < N_P <= 160: C2) and stays at 4 for
-// fewer perturbations, where the table of a C5-sized instance allows 4 CTAs anyway.
+// Resident CTAs per SM the register allocation aims at.  Only NQ = 1 (N_P <= 32) is built from this file; the table of a
+// C5-sized instance allows four CTAs of four warps anyway.
 template <int RES, int NQ> constexpr int coop_min_ctas()
 {
-    if (CLOSURE_COOP_MIN_CTAS != 4) return CLOSURE_COOP_MIN_CTAS;
-    if (RES == CLOSURE_POSE_REG || RES == CLOSURE_POSE_REG_SPLIT) return 6;
-    return NQ == 5 ? 5 : 4;
+    return CLOSURE_COOP_MIN_CTAS;      // 128 registers: measured at 3 / 4 / 5 on config 5 (672 / 777 / 587 M walker-steps/s)
 }
 
 // fp32 image of one set-up row and the bound eps on |v32 - v64| for ANY perturbation with
@@ -257,6 +260,7 @@ __device__ __noinline__ void aff_setup_on_move(unsigned char *smem_raw, int warp
 #pragma unroll
     for (int e = 0; e < 9; ++e) Rq[e] = RmS[m_mid * 9 + e];
 
+    const float velf0 = (float)vel[0], velf1 = (float)vel[1], velf2 = (float)vel[2];
     float eps_l = 0.f;
     double rm_l = CUDART_INF;
     uint32_t best1 = 0u, best2 = 0u;                    // (20 key bits | row index): tightest row of this lane at R*, at R_mid
@@ -281,10 +285,19 @@ __device__ __noinline__ void aff_setup_on_move(unsigned char *smem_raw, int warp
             rm_l = dmin(rm_l, rmi);
             tk1 = fmaxf(tk1, -(float)rmi);
         }
-        double v0, v1, v2, cq;
-        affine_setup<RES>(Rq, t, row, v0, v1, v2, cq);
-        float tk2 = sqrtf(fmaxf((float)cq, 0.f)) - bfi;
-        if (RES == CLOSURE_POSE_REG_SPLIT) tk2 = fmaxf(tk2, sqrtf((float)frob_sq(Rq, row)) - (float)row[12]);
+        float tk2;
+        if (RES == CLOSURE_REG_3D3D) {
+            // lever arm of R* a_i about the rotation axis, relative to the bound: a rotation by any angle moves this
+            // constraint's centre by 2 sin(angle / 2) times it, so these rows are the first to be violated at the large rungs
+            const float r0 = (float)(row[3] - t[0] - u0), r1 = (float)(row[4] - t[1] - u1), r2 = (float)(row[5] - t[2] - u2);
+            const float x0 = velf1 * r2 - velf2 * r1, x1 = velf2 * r0 - velf0 * r2, x2 = velf0 * r1 - velf1 * r0;
+            tk2 = sqrtf(fmaf(x2, x2, fmaf(x1, x1, x0 * x0))) / bfi;
+        } else {
+            double v0, v1, v2, cq;
+            affine_setup<RES>(Rq, t, row, v0, v1, v2, cq);
+            tk2 = sqrtf(fmaxf((float)cq, 0.f)) - bfi;
+            if (RES == CLOSURE_POSE_REG_SPLIT) tk2 = fmaxf(tk2, sqrtf((float)frob_sq(Rq, row)) - (float)row[12]);
+        }
         best1 = max(best1, (fkey(tk1) & 0xFFFFF000u) | (uint32_t)i);
         best2 = max(best2, (fkey(tk2) & 0xFFFFF000u) | (uint32_t)i);
     }
@@ -511,7 +524,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     __syncthreads();
     const int n_runs = n_runs_s;
 
-    const long long local = (long long)blockIdx.x * kCoopWarps + warp;
+    const long long local = (long long)blockIdx.x * (blockDim.x >> 5) + warp;   // 1, 2 or 4 walkers per CTA (launch_q)
     if (local >= L.num_walkers) return;                // no block-wide barrier below this line
     unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
     float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);
@@ -589,8 +602,8 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     // selection constants: at most s_max survivors (a power of two), at least need_lo
     int s_max = 8;
     while (s_max < 2 * n_ps + 4 && s_max < 32) s_max <<= 1;
-    const int need_lo = min(n_p, n_ps + 3);
-    const int r_target = n_ps + 3 + (n_ps >> 2);        // rank whose value seeds the next iteration's threshold
+    const int need_lo = min(n_p, n_ps + CLOSURE_NEED_EXTRA);
+    const int r_target = n_ps + CLOSURE_RT_EXTRA + (n_ps >> CLOSURE_RT_SHIFT);        // rank whose value seeds the next iteration's threshold
     const float step0 = 0.0625f * run_bf[n_runs - 1];
     float U_state = 0.f;
 
@@ -740,7 +753,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                         m = fmaxf(m, fmaxf(l2, h2));
                     }
                 }
-                const float mv = fkey_inv(__reduce_max_sync(FULL, fkey(m)));
+                const float mv = fkey_inv(__reduce_max_sync(FULL, fkey(m)));   // one warp maximum and one square root
                 const float a = fmaxf(mv - pj.w, 1e-30f);              // pj.w = -|d|^2
                 const float rr = rsqrt_normal(a);
                 const float sq = a * rr;
@@ -795,6 +808,12 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
             if (nan_any || (L.exact_only & 4)) ok = false;
             certified = __all_sync(FULL, ok);
             if (certified && lane < n_ps) candd[lane] = myval + fmaf(1.01f, unc, 4.0f * kMu19 * fabsf(myval));    // >= the fp64 value d_j
+        } else if (full_p1) {
+            // ---- short tables: phase 1 gave the exact eq. (14) value of every perturbation; the N_P* + 1 largest are
+            // extracted by rounds of warp maxima over the lanes' locally sorted keys and certified by their gaps
+            unc = wmax_nonneg(unc_l);
+            if (RES == CLOSURE_POSE_REG_SPLIT) unc += 1.2e-7f * fabsf(rmf);
+            certified = topk_certified<NQ>(ub, n_ps, unc, (L.exact_only & 4) != 0, (L.exact_only & 32) != 0, lane, candj, candd, myval);
         } else {
 #pragma unroll 1
         for (int attempt = 0; attempt < 3; ++attempt) {
@@ -861,7 +880,16 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                     const float4 *e = rowsA + 2 * (pp + chunk);
                     const float4 *elast = rowsA + 2 * (pend - 1);
 #pragma unroll 2
-                    for (int it = 0; it < trips; ++it) {
+                    for (int it = 1; it < trips; ++it) {               // all trips but the last are inside the run on every lane
+                        const float4 X = e[0], Y = e[1];
+                        const unsigned long long vo =
+                            fma2(pk2(X.x, X.y), E0p, fma2(pk2(X.z, X.w), E1p, fma2(pk2(Y.x, Y.y), E2p, pk2(Y.z, Y.w))));
+                        float l2, h2;
+                        upk2(vo, l2, h2);
+                        mx = fmaxf(mx, fmaxf(l2, h2));
+                        e += 2 << lgC;
+                    }
+                    {
                         const float4 *ec = e < elast ? e : elast;
                         const float4 X = ec[0], Y = ec[1];
                         const unsigned long long vo =
@@ -869,7 +897,6 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                         float l2, h2;
                         upk2(vo, l2, h2);
                         mx = fmaxf(mx, fmaxf(l2, h2));
-                        e += 2 << lgC;
                     }
                     pp = pend;
                     for (int off = S; off < 32; off <<= 1) mx = fmaxf(mx, __shfl_xor_sync(FULL, mx, off));
@@ -1127,25 +1154,28 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
 template <int RES, int NQ>
 cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
 {
-    const AffSmem lay = aff_layout(max_rows_bytes, max_n, L.n_t, NQ, L.pairs_cap);
+    // Walkers (warps) per CTA: four share one staged table; fewer only when four tables' worth of per-warp state does not fit.
+    int wpc = kCoopWarps;                                // measured at 1 / 2 / 4: four is best at every size, also with few walkers or iterations
+    AffSmem lay = aff_layout(max_rows_bytes, max_n, L.n_t, NQ, L.pairs_cap, wpc);
+    while (lay.total > 200 * 1024 && wpc > 1) { wpc >>= 1; lay = aff_layout(max_rows_bytes, max_n, L.n_t, NQ, L.pairs_cap, wpc); }
     if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaFuncSetAttribute(walker_coop_kernel<RES, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)lay.total);
     if (e != cudaSuccess) return e;
-    const long long blocks = (L.num_walkers + kCoopWarps - 1) / kCoopWarps;
+    const long long blocks = (L.num_walkers + wpc - 1) / wpc;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     dim3 grid((unsigned)blocks, (unsigned)n_instances, 1);
-    walker_coop_kernel<RES, NQ><<<grid, kCoopThreads, lay.total, stream>>>(L);
+    walker_coop_kernel<RES, NQ><<<grid, 32 * wpc, lay.total, stream>>>(L);
     return cudaGetLastError();
 }
 
 template <int RES>
 cudaError_t launch_r(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
 {
+    // the kernel is written for NQ perturbations per lane; only NQ = 1 (N_P <= 32) is built: launch_walkers_coop sends
+    // larger N_P to the dense kernel
     if (L.n_p <= 32) return launch_q<RES, 1>(L, n_instances, max_rows_bytes, max_n, stream);
-    if (L.n_p <= 64) return launch_q<RES, 2>(L, n_instances, max_rows_bytes, max_n, stream);
-    if (L.n_p <= 160) return launch_q<RES, 5>(L, n_instances, max_rows_bytes, max_n, stream);
-    return launch_q<RES, 8>(L, n_instances, max_rows_bytes, max_n, stream);
+    return cudaErrorInvalidConfiguration;
 }
 
 }  // namespace
@@ -1162,6 +1192,15 @@ cudaError_t launch_walkers_coop(int residual_type, const WalkLaunch &L, int n_in
     const int max_n = max_rows_bytes / (row_doubles(residual_type) * 8);
     switch (residual_type) {
     case CLOSURE_REPROJ_2D3D: return launch_walkers_coop_reproj(L, n_instances, max_rows_bytes, stream);
+    default: break;
+    }
+    // More than 32 perturbations per iteration (BASELINE configs 1, 2, 4): the dense kernel, several perturbations per
+    // lane against every constraint.  At most 32 (config 5): branch and bound (this file), one perturbation per lane.
+    // Both take the fp64 decisions bit for bit.  (Measured with N_P = 150 on tables of 30 - 200 constraints: the
+    // batched branch and bound of this file saves 2/3 of the pairs but loses 1.4 - 4x to its bookkeeping and to the
+    // fp64 fall-backs that loose phase-1 bounds cause; with N_P <= 32 the best-first form wins.)
+    if (L.n_p > 32) return launch_walkers_coop_dense(residual_type, L, n_instances, max_rows_bytes, stream);
+    switch (residual_type) {
     case CLOSURE_REG_3D3D: return launch_r<CLOSURE_REG_3D3D>(L, n_instances, max_rows_bytes, max_n, stream);
     case CLOSURE_POSE_REG: return launch_r<CLOSURE_POSE_REG>(L, n_instances, max_rows_bytes, max_n, stream);
     case CLOSURE_POSE_REG_SPLIT: return launch_r<CLOSURE_POSE_REG_SPLIT>(L, n_instances, max_rows_bytes, max_n, stream);

@@ -1,0 +1,750 @@
+// Warp-cooperative walker kernel, DENSE variant (every perturbation against every constraint), for the rotation-
+// boundary sampler (Alg. 2) on
+// the residuals whose squared norm is quadratic in the translation perturbation (Ex.2 registration,
+// Ex.3 pose regression, stacked or split).  One WARP owns one walker; the 32 lanes split the work
+// that Alg. 3 tensorises per walker:
+//
+//   a2-a4  the N_P perturbations are dealt to the lanes (j = lane + 32 q); the per-constraint
+//          set-up u_i = b_i - (R* a_i + t*) is computed ONCE per accepted move (lane i mod 32)
+//          and broadcast through shared memory; a pair costs 3 FFMA + 1 FMNMX in fp32
+//          (packed FFMA2 + FMNMX3 in SASS).  eq. (14)'s values d~_j carry a rigorous error bound
+//          `unc`; the top-N_P* are extracted with warp reductions and the ranking is accepted only
+//          if consecutive values (and the N_P*-th against the next) are more than 2 unc apart.
+//          Otherwise the step falls back to the fp64 evaluation of the plain kernel.
+//   a5-a6  every rung m = 1..N_T is screened first (lane = (rung, half of the candidates)) against the
+//          rung's two tightest constraints and against a Lipschitz bound on what the rotation to R_m
+//          can repair; rungs with a surviving candidate are then evaluated in full, lane =
+//          (candidate, constraint chunk), in fp32 with a three-way outcome per candidate: violated
+//          for sure / satisfied for sure / undecided -> fp64.
+//
+// launch_walkers_coop (walker_coop_kernel.cu) sends short tables with many perturbations here (N_P > 32 and at most 32
+// pair-entries: BASELINE configs 1, 2 and 4): the branch and bound of walker_coop_kernel.cu saves arithmetic but its
+// bookkeeping only pays on longer tables or few perturbations.
+//
+// Every accept/reject decision is therefore the decision the fp64 arithmetic of walker_kernel.cu
+// takes (DESIGN.md 6.1b "Certified fp32 evaluation"); the pose itself is only ever updated in fp64.
+// Unlike the one-walker-per-thread kernel all lanes of a warp follow the same walker: no divergence
+// between walkers, the set-up is not repeated per register tile, 128 registers (16 warps per SM).
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include <stdint.h>
+
+#include "closure_internal.h"
+#include "walker_common.cuh"
+#include "walker_coop_common.cuh"
+
+#ifndef CLOSURE_COOP_MIN_CTAS
+#define CLOSURE_COOP_MIN_CTAS 4   // resident CTAs per SM the register allocation aims at (128 registers per thread)
+#endif
+
+namespace closure {
+namespace {
+
+// Measured on B200: the pose-regression kernel, whose rows are twice as long, gains 3.7 % at 6 resident
+// CTAs (80 registers); the registration kernel gains 1 % at 5 (96 registers) in the NQ = 5 instantiation (64 < N_P <= 160: C2) and stays at 4 for
+// fewer perturbations, where the table of a C5-sized instance allows 4 CTAs anyway.
+template <int RES, int NQ> constexpr int coop_min_ctas()
+{
+    if (CLOSURE_COOP_MIN_CTAS != 4) return CLOSURE_COOP_MIN_CTAS;
+    if (RES == CLOSURE_POSE_REG || RES == CLOSURE_POSE_REG_SPLIT) return 6;
+    return NQ == 5 ? 5 : 4;
+}
+
+// fp32 image of one set-up row and the bound eps on |v32 - v64| for ANY perturbation with
+// |d_c| <= t_p, where v = c - 2 u.d is evaluated as three chained FMAs:
+//   inputs: (u, c) rounded to fp32 (relative 2^-24 each); e = -2 d from pm1f (absolute 6 * 2^-24 * 2 t_p);
+//   three FFMA roundings (2^-24 of the partial sums, each <= |c| + 2 t_p |u|_1)
+//   =>  |v32 - v64| <= 2^-24 (4 |c| + 10 * 2 t_p |u|_1).
+// eps = 2^-19 (|c| + 2 t_p |u|_1 + 3 t_p^2) leaves a factor > 3 for the roundings of eps itself,
+// of the threshold -|d|^2 in fp32 (<= 15 * 2^-24 * 3 t_p^2) and of the shifted constants c -+ eps.
+__device__ __forceinline__ void screen_row(double u0, double u1, double u2, double c, float tp2, float tp2sq3,
+                                           float &f0, float &f1, float &f2, float &fc, float &eps)
+{
+    f0 = (float)u0; f1 = (float)u1; f2 = (float)u2; fc = (float)c;
+    const float mag = fabsf(fc) + tp2 * (fabsf(f0) + fabsf(f1) + fabsf(f2)) + tp2sq3;
+    eps = mag * (kMu19 * 1.001f);
+}
+
+// The plain kernel's phase A for the NQ perturbations of this lane (same arithmetic as
+// walker_kernel.cu): exact eq. (14) margins, one sqrt per run of equal bounds.  jv[q] < 0: empty.
+template <int RES, int NJ>
+__device__ __forceinline__ void exact_margins(const double (&R)[9], const double (&t)[3], const double *rows, int n,
+                                              const Rng &rng, uint32_t s, double t_p, double rot_margin,
+                                              const int (&jv)[NJ], double (&d)[NJ])
+{
+    using RS = Res<RES>;
+    constexpr int ROW = RS::ROW;
+    uint32_t x[NJ], y[NJ], z[NJ];
+    philox_batch<NJ>(rng, s, jv, x, y, z);
+    double e0[NJ], e1[NJ], e2[NJ], dd[NJ], acc_mx[NJ];
+#pragma unroll
+    for (int q = 0; q < NJ; ++q) {
+        const double d0 = t_p * pm1(x[q]), d1 = t_p * pm1(y[q]), d2 = t_p * pm1(z[q]);
+        dd[q] = fma(d2, d2, fma(d1, d1, d0 * d0));
+        e0[q] = d0 * -2.0; e1[q] = d1 * -2.0; e2[q] = d2 * -2.0;
+        acc_mx[q] = -CUDART_INF;
+        d[q] = rot_margin;
+    }
+#pragma unroll 1
+#pragma unroll 1
+    for (int i = 0; i < n; ++i) {
+        const double *row = rows + i * ROW;
+        double u0, u1, u2, c;
+        affine_setup<RES>(R, t, row, u0, u1, u2, c);
+#pragma unroll
+        for (int q = 0; q < NJ; ++q)
+            acc_mx[q] = dmax(acc_mx[q], fma(u0, e0[q], fma(u1, e1[q], fma(u2, e2[q], c))));
+        const double beta = row[RS::BETA];
+        const bool run_ends = (i == n - 1) || (rows[(i + 1) * ROW + RS::BETA] != beta);
+        if (run_ends) {                          // warp-uniform
+#pragma unroll
+            for (int q = 0; q < NJ; ++q) {
+                d[q] = dmin(d[q], beta - sqrt(dmax(acc_mx[q] + dd[q], 0.0)));
+                acc_mx[q] = -CUDART_INF;
+            }
+        }
+    }
+}
+
+// eq. (14) of one perturbation in the plain kernel's arithmetic (functor for topk_fp64)
+template <int RES>
+struct ExactMargin {
+    const double (&R)[9];
+    const double (&t)[3];
+    const double *rows;
+    int n;
+    const Rng &rng;
+    uint32_t s;
+    double t_p, rot_margin;
+    __device__ __forceinline__ double operator()(int j) const
+    {
+        const int jv[1] = { j };
+        double d[1];
+        exact_margins<RES, 1>(R, t, rows, n, rng, s, t_p, rot_margin, jv, d);
+        return d[0];
+    }
+};
+
+// fp64 in_purse of ladder candidate (Rm, t* + d_j), constraints dealt to the lanes; the arithmetic
+// of the plain kernel's ladder.  Warp-uniform result.
+template <int RES>
+__device__ __forceinline__ bool exact_candidate_feasible(const double (&Rm)[9], const double (&t)[3], const double *rows,
+                                                         int n, const Rng &rng, uint32_t s, int j, double t_p, int lane)
+{
+    using RS = Res<RES>;
+    constexpr int ROW = RS::ROW;
+    double x, y, z;
+    rng.xi3(s, (uint32_t)j, 1u, x, y, z);
+    const double d0 = t_p * x, d1 = t_p * y, d2 = t_p * z;
+    const double kdd = -fma(d2, d2, fma(d1, d1, d0 * d0));
+    const double k0 = -2.0 * d0, k1 = -2.0 * d1, k2 = -2.0 * d2;
+    bool ok = true;
+#pragma unroll 1
+    for (int i = lane; i < n; i += 32) {
+        const double *row = rows + i * ROW;
+        double u0, u1, u2, c;
+        affine_setup<RES>(Rm, t, row, u0, u1, u2, c);
+        if (RES == CLOSURE_POSE_REG_SPLIT) {
+            if (!(frob_sq(Rm, row) <= row[13])) ok = false;
+        }
+        const double cb = c - row[RS::BETA + 1];
+        const double v = fma(u0, k0, fma(u1, k1, fma(u2, k2, cb)));
+        if (!(v <= kdd)) ok = false;
+    }
+    return __all_sync(FULL, ok);
+}
+
+// ---------------------------------------------------------------------------------- set-up after a move
+// Everything that depends on the pose only (DESIGN.md 6.1b "state that only changes on an accepted
+// move"): fp32 set-up rows at R* (rowsA), Exp(dT_m w) R* for every rung (RmS), per rung the two
+// tightest rows (qrow) and the Lipschitz bound (qL).  fp64-heavy and rare, so it is kept out of line:
+// its registers do not count against the per-iteration code.  Results epsA, rot_margin -> pose[16], pose[15].
+template <int RES>
+__device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int warp, int lane, int rows_bytes, int n,
+                                                int n_t, int nq, int pairs, double t_p, bool stats)
+{
+    using RS = Res<RES>;
+    constexpr int ROW = RS::ROW;
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, nq, 1, pairs);
+    const double *rows = reinterpret_cast<const double *>(smem_raw + 16);
+    const int *pos = reinterpret_cast<const int *>(smem_raw + lay.pos);
+    unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
+    float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);
+    const double2 *ab = reinterpret_cast<const double2 *>(wp + lay.ab);
+    float4 *qrow = reinterpret_cast<float4 *>(wp + lay.qrow);
+    double *RmS = reinterpret_cast<double *>(wp + lay.RmS);
+    float *qL = reinterpret_cast<float *>(wp + lay.qL);
+    double *pose = reinterpret_cast<double *>(wp + lay.pose);
+    unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
+    const float tpf = (float)t_p * 1.0000002f;          // >= t_p
+    const float tp2 = 2.0f * tpf, tp2sq3 = 3.0f * tpf * tpf;
+    double R[9], t[3], vel[3];
+#pragma unroll
+    for (int e = 0; e < 9; ++e) R[e] = pose[e];
+#pragma unroll
+    for (int e = 0; e < 3; ++e) { t[e] = pose[9 + e]; vel[e] = pose[12 + e]; }
+    float eps_l = 0.f;
+    double rm_l = CUDART_INF;
+#pragma unroll 1
+    for (int i = lane; i < n; i += 32) {
+        const double *row = rows + i * ROW;
+        double u0, u1, u2, c;
+        affine_setup<RES>(R, t, row, u0, u1, u2, c);
+        float f0, f1, f2, fc, eps;
+        screen_row(u0, u1, u2, c, tp2, tp2sq3, f0, f1, f2, fc, eps);
+        {
+            const int pp = pos[i], p = pp & 0x3fffffff;
+            float *A = reinterpret_cast<float *>(rowsA) + (p >> 1) * 8 + (p & 1);
+            A[0] = f0; A[2] = f1; A[4] = f2; A[6] = fc;
+            if (pp & 0x40000000) { A[1] = f0; A[3] = f1; A[5] = f2; A[7] = fc; }
+        }
+        eps_l = fmaxf(eps_l, eps);
+        if (RES == CLOSURE_POSE_REG_SPLIT) rm_l = dmin(rm_l, row[12] - sqrt(frob_sq(R, row)));
+    }
+    const float epsA = wmax_nonneg(eps_l);
+    double rot_margin = CUDART_INF;
+    if (RES == CLOSURE_POSE_REG_SPLIT) rot_margin = wmin_f64(rm_l);
+    for (int m = lane; m < n_t; m += 32) {       // Exp(dT_m w) R* for every rung
+        const double2 c2 = ab[m];
+        double Rm[9];
+        rotate_left(R, vel[0], vel[1], vel[2], c2.x, c2.y, Rm);
+#pragma unroll
+        for (int e = 0; e < 9; ++e) RmS[m * 9 + e] = Rm[e];
+    }
+    __syncwarp();
+    // the two tightest constraints of every rung (largest c - beta^2 at the unperturbed
+    // translation): the rows the ladder screens each rung against while the pose stays here
+    if (n <= 16) {
+        // short tables (Ex.1 / Ex.3 sizes): lane = (rung, constraint), two rungs per pass, so that the lanes are not
+        // left idle by a loop over 8 - 16 constraints; same rows, same bounds as the loop below
+        const int c = lane & 15;
+        const bool has = c < n;
+        const double *row = rows + (has ? c : 0) * ROW;
+        const unsigned hm = 0xFFFFu << (lane & 16);
+#pragma unroll 1
+        for (int m = lane >> 4; m < n_t; m += 2) {
+            double Rm[9], dR[9], lip = 0.0;
+#pragma unroll
+            for (int e = 0; e < 9; ++e) { Rm[e] = RmS[m * 9 + e]; dR[e] = Rm[e] - R[e]; }
+            double u0, u1, u2, cc;
+            affine_setup<RES>(Rm, t, row, u0, u1, u2, cc);
+            if (RES == CLOSURE_REG_3D3D) {           // ||(R_m - R*) a_i||^2
+                const double q0 = dR[0] * row[0] + dR[1] * row[1] + dR[2] * row[2];
+                const double q1 = dR[3] * row[0] + dR[4] * row[1] + dR[5] * row[2];
+                const double q2 = dR[6] * row[0] + dR[7] * row[1] + dR[8] * row[2];
+                lip = q0 * q0 + q1 * q1 + q2 * q2;
+            } else {
+#pragma unroll
+                for (int e = 0; e < 9; ++e) lip = fma(dR[e], dR[e], lip);      // ||R_m - R*||_F^2
+            }
+            bool rdead = false;
+            if (RES == CLOSURE_POSE_REG_SPLIT) rdead = has && !(frob_sq(Rm, row) <= row[13]);
+            float g0, g1, g2, fcb, eps;
+            screen_row(u0, u1, u2, cc - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
+            float4 r4 = make_float4(g0, g1, g2, has ? fcb - eps : -CUDART_INF_F);
+            const uint32_t key = has ? ((fkey(r4.w) & ~15u) | (uint32_t)c) : (uint32_t)c;
+            const uint32_t m1 = __reduce_max_sync(hm, key);
+            const uint32_t key2 = (key == m1) ? 0u : key;
+            const uint32_t m2 = __reduce_max_sync(hm, key2);
+            const float lf = __uint_as_float(__reduce_max_sync(hm, __float_as_uint(has ? (float)sqrt(lip) : 0.f)));
+            const bool dead_any = (__ballot_sync(hm, rdead) & hm) != 0u;
+            if (key == m1) {
+                if (dead_any) r4.w = CUDART_INF_F;                     // rung dead for every candidate
+                qrow[2 * m] = r4;
+                qL[m] = lf * 1.001f + 1e-30f;
+                if (n == 1) qrow[2 * m + 1] = r4;
+            }
+            if (key2 == m2 && n > 1) qrow[2 * m + 1] = r4;
+        }
+    } else {
+#pragma unroll 1
+    for (int m = 0; m < n_t; ++m) {
+        double Rm[9];
+#pragma unroll
+        for (int e = 0; e < 9; ++e) Rm[e] = RmS[m * 9 + e];
+        float4 b1 = make_float4(0.f, 0.f, 0.f, -CUDART_INF_F), b2 = b1;
+        bool rdead = false;
+        double dR[9], lip = 0.0;                     // max_i | ||g_i(R_m, .)|| - ||g_i(R*, .)|| | <= sqrt(lip)
+#pragma unroll
+        for (int e = 0; e < 9; ++e) dR[e] = Rm[e] - R[e];
+        if (RES != CLOSURE_REG_3D3D) {
+#pragma unroll
+            for (int e = 0; e < 9; ++e) lip = fma(dR[e], dR[e], lip);      // ||R_m - R*||_F^2
+        }
+#pragma unroll 1
+        for (int i = lane; i < n; i += 32) {
+            const double *row = rows + i * ROW;
+            double u0, u1, u2, c;
+            affine_setup<RES>(Rm, t, row, u0, u1, u2, c);
+            if (RES == CLOSURE_REG_3D3D) {           // ||(R_m - R*) a_i||^2
+                const double q0 = dR[0] * row[0] + dR[1] * row[1] + dR[2] * row[2];
+                const double q1 = dR[3] * row[0] + dR[4] * row[1] + dR[5] * row[2];
+                const double q2 = dR[6] * row[0] + dR[7] * row[1] + dR[8] * row[2];
+                lip = dmax(lip, q0 * q0 + q1 * q1 + q2 * q2);
+            }
+            if (RES == CLOSURE_POSE_REG_SPLIT) {
+                if (!(frob_sq(Rm, row) <= row[13])) rdead = true;
+            }
+            float g0, g1, g2, fcb, eps;
+            screen_row(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
+            const float4 r4 = make_float4(g0, g1, g2, fcb - eps);
+            if (r4.w > b1.w) { b2 = b1; b1 = r4; } else if (r4.w > b2.w) b2 = r4;
+        }
+        const uint32_t k1 = fkey(b1.w);
+        const uint32_t m1 = __reduce_max_sync(FULL, k1);
+        const int src1 = __ffs(__ballot_sync(FULL, k1 == m1)) - 1;
+        const uint32_t k2 = (lane == src1) ? fkey(b2.w) : k1;
+        const uint32_t m2 = __reduce_max_sync(FULL, k2);
+        const int src2 = __ffs(__ballot_sync(FULL, k2 == m2)) - 1;
+        if (__any_sync(FULL, rdead)) b1.w = CUDART_INF_F;          // rung dead for every candidate
+        if (lane == src1) qrow[2 * m] = b1;
+        if (lane == src2) qrow[2 * m + 1] = (lane == src1) ? b2 : b1;
+        const float lf = wmax_nonneg((float)sqrt(lip));
+        if (lane == 0) qL[m] = lf * 1.001f + 1e-30f;
+    }
+    }
+    if (stats) { stc[2] += n; stc[3] += (unsigned long long)n * n_t; }
+    __syncwarp();
+    if (lane == 0) {                                 // suffix maximum: qL[m] holds for every rung >= m
+        float sm = 0.f;
+        for (int m = n_t - 1; m >= 0; --m) { sm = fmaxf(sm, qL[m]); qL[m] = sm; }
+    }
+    __syncwarp();
+    if (lane == 0) { pose[15] = rot_margin; pose[16] = (double)epsA; }
+    __syncwarp();
+}
+
+// ---------------------------------------------------------------------------------- the kernel
+template <int RES, int NQ>
+__global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker_dense_kernel(const __grid_constant__ WalkLaunch L)
+{
+    using RS = Res<RES>;
+    constexpr int ROW = RS::ROW;
+    constexpr int NPK = NQ / 2;            // packed pairs of perturbations
+    constexpr bool ODD = (NQ & 1) != 0;    // plus one scalar slot
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ int n_runs_s;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const InstanceDesc *__restrict__ D = L.desc[blockIdx.y];
+    const int n = D->n;
+    const int rows_bytes = D->rows_bytes;
+    const int n_p = L.n_p, n_ps = L.n_p_star, n_t = L.n_t;
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
+    double *rows = reinterpret_cast<double *>(smem_raw + 16);
+    stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 1, L.pairs_cap);
+    int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
+    float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
+    int *run_pend = reinterpret_cast<int *>(smem_raw + lay.run_pend);   // end of run r in rowsA, in PAIRS of rows
+    int *pos = reinterpret_cast<int *>(smem_raw + lay.pos);             // row of constraint i in rowsA (bit 30: write it twice)
+    if (warp == 0) {                                   // runs of equal bounds (rows are sorted by bound)
+        int cnt = 0;
+        for (int base = 0; base < n; base += 32) {
+            const int i = base + lane;
+            bool end = false;
+            double beta = 0.0;
+            if (i < n) {
+                beta = rows[i * ROW + RS::BETA];
+                end = (i == n - 1) || (rows[(i + 1) * ROW + RS::BETA] != beta);
+            }
+            const unsigned m = __ballot_sync(FULL, end);
+            if (end) {
+                const int r = cnt + __popc(m & ((1u << lane) - 1u));
+                run_end[r] = i;
+                run_bf[r] = (float)beta;
+            }
+            cnt += __popc(m);
+        }
+        __syncwarp();
+        if (lane == 0) {
+            // rowsA holds the fp32 set-ups two constraints per entry; a run of odd length repeats its last
+            // constraint (a maximum does not see duplicates), so no pair straddles two bounds
+            n_runs_s = cnt;
+            int p = 0, start = 0, longest = 0;
+            for (int r = 0; r < cnt; ++r) {
+                const int end = run_end[r];
+                const int p_begin = p >> 1;
+                for (int i = start; i <= end; ++i) pos[i] = p++;
+                if (p & 1) { pos[end] |= 0x40000000; ++p; }
+                run_pend[r] = p >> 1;
+                longest = max(longest, (p >> 1) - p_begin);
+                start = end + 1;
+            }
+        }
+    }
+    __syncthreads();
+    const int n_runs = n_runs_s;
+
+    const long long local = (long long)blockIdx.x * kCoopWarps + warp;
+    if (local >= L.num_walkers) return;                // no block-wide barrier below this line
+    unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
+    float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);
+    float4 *rowsL = reinterpret_cast<float4 *>(wp + lay.rowsL);
+    float4 *pert = reinterpret_cast<float4 *>(wp + lay.pert);
+    double2 *ab = reinterpret_cast<double2 *>(wp + lay.ab);
+    float4 *qrow = reinterpret_cast<float4 *>(wp + lay.qrow);     // [rung][2]: the two tightest rows of each rung
+    double *RmS = reinterpret_cast<double *>(wp + lay.RmS);
+    double *dex = reinterpret_cast<double *>(wp + lay.dex);      // fp64 fallback: exact d_j, [q][lane]
+    float *qL = reinterpret_cast<float *>(wp + lay.qL);           // [rung]: bound on the change of any residual norm
+    float4 *cand4 = reinterpret_cast<float4 *>(wp + lay.cand4);   // the kept perturbations (-2 d_j, -|d_j|^2), by rank
+    int *candj = reinterpret_cast<int *>(wp + lay.candj);
+    float *candd = reinterpret_cast<float *>(wp + lay.candd);     // upper bounds of the candidates' eq. (14) values
+    double *pose = reinterpret_cast<double *>(wp + lay.pose);     // R*(9) t*(3) omega(3): fp64, touched only on moves / fp64 paths
+
+    const unsigned long long w = (unsigned long long)(L.walker_begin + local);
+    const unsigned long long seed = L.seed[blockIdx.y];
+    Rng rng;
+    rng.w_lo = (uint32_t)w;
+    rng.w_hi8 = (uint32_t)(w >> 32) << 8;
+    rng.k0 = (uint32_t)seed;
+    rng.k1 = (uint32_t)(seed >> 32);
+
+    // ---- a1: walker init, replicated on the lanes (Alg. 2 l.8-9)
+    {
+        double R[9], t[3], vel[3];
+        init_walker<CLOSURE_MODE_ROT>(D, L, rng, w, R, t, vel);
+        for (int m = lane; m < n_t; m += 32) {         // ladder dT_m = gamma^(m-1) by repeated multiplication
+            double dT = 1.0;
+            for (int q = 0; q < m; ++q) dT = dT * L.gamma;
+            const double p0 = dT * vel[0], p1 = dT * vel[1], p2 = dT * vel[2];
+            double A, B;
+            exp_coeffs(fma(p2, p2, fma(p1, p1, p0 * p0)), A, B);
+            ab[m] = make_double2(A * dT, B * dT * dT);
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int e = 0; e < 9; ++e) pose[e] = R[e];
+#pragma unroll
+            for (int e = 0; e < 3; ++e) { pose[9 + e] = t[e]; pose[12 + e] = vel[e]; }
+        }
+    }
+    __syncwarp();
+
+    const double t_p = L.t_p;
+    const float tpf = (float)t_p * 1.0000002f;          // >= t_p
+    const float tp2 = 2.0f * tpf, tp2sq3 = 3.0f * tpf * tpf;
+    const float m2tp = -2.0f * (float)t_p;
+    const int KP = n_ps;                                // ladder candidates
+    const int NCH = 32 / KP;                            // constraint chunks of the full evaluation
+    const int ek = lane % KP, ech = lane / KP;
+    const bool e_act = ech < NCH;
+    unsigned e_mask = 0u;                               // lanes that share this lane's candidate
+    for (int c = 0; c < NCH; ++c) e_mask |= 1u << (ek + c * KP);
+
+    // executed-work counters (closure_get_stats): in shared memory, touched by lane 0 and only when asked for
+    unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
+    const bool stats = (L.stats != nullptr) && lane == 0;
+    if (stats) {
+        for (int k = 0; k < kNumStats; ++k) stc[k] = 0ull;
+    }
+    const long long clk_begin = stats ? clock64() : 0ll;
+    bool hit = false;
+    bool moved = true;
+    float epsA = 0.f;
+    double rot_margin = CUDART_INF;
+    // cached across iterations while the pose does not move
+    int full_m = -1;                                    // rung whose rows sit in rowsL
+    float epsL = 0.f;
+    bool rdeadL = false;
+
+    for (int s = 1; s <= L.num_steps; ++s) {
+        // ================================================== set-up at the current pose (only after a move)
+        if (moved) {
+            const long long c0 = stats ? clock64() : 0ll;
+            coop_setup_on_move<RES>(smem_raw, warp, lane, rows_bytes, n, n_t, NQ, L.pairs_cap, t_p, stats);
+            if (stats) stc[10] += (unsigned long long)(clock64() - c0);
+            epsA = (float)pose[16];
+            rot_margin = pose[15];
+            full_m = -1;
+        }
+
+        // ================================================== a2: perturbations of this lane
+        unsigned long long p0[NPK > 0 ? NPK : 1], p1[NPK > 0 ? NPK : 1], p2[NPK > 0 ? NPK : 1];
+        float o0 = 0.f, o1 = 0.f, o2 = 0.f;                  // the odd slot NQ-1
+        float dd[NQ];
+        {
+            int jv[NQ];
+            uint32_t x[NQ], y[NQ], z[NQ];
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) jv[q] = lane + 32 * q;
+            philox_batch<NQ>(rng, (uint32_t)s, jv, x, y, z);
+            float e0[NQ], e1[NQ], e2[NQ];
+            // packed slots are produced by packed instructions so that they live in aligned register pairs
+            // (same roundings as the scalar pm1f() * m2tp)
+            const unsigned long long C1 = pk2(4.656612873077392578125e-10f, 4.656612873077392578125e-10f);
+            const unsigned long long C2 = pk2(2.3283064365386962890625e-10f - 1.0f, 2.3283064365386962890625e-10f - 1.0f);
+            const unsigned long long M2 = pk2(m2tp, m2tp);
+#pragma unroll
+            for (int k = 0; k < NPK; ++k) {
+                p0[k] = mul2(M2, fma2(pk2((float)x[2 * k], (float)x[2 * k + 1]), C1, C2));
+                p1[k] = mul2(M2, fma2(pk2((float)y[2 * k], (float)y[2 * k + 1]), C1, C2));
+                p2[k] = mul2(M2, fma2(pk2((float)z[2 * k], (float)z[2 * k + 1]), C1, C2));
+                upk2(p0[k], e0[2 * k], e0[2 * k + 1]);
+                upk2(p1[k], e1[2 * k], e1[2 * k + 1]);
+                upk2(p2[k], e2[2 * k], e2[2 * k + 1]);
+            }
+            if (ODD) { e0[NQ - 1] = m2tp * pm1f(x[NQ - 1]); e1[NQ - 1] = m2tp * pm1f(y[NQ - 1]); e2[NQ - 1] = m2tp * pm1f(z[NQ - 1]); }
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) {
+                dd[q] = 0.25f * fmaf(e2[q], e2[q], fmaf(e1[q], e1[q], e0[q] * e0[q]));
+                pert[32 * q + lane] = make_float4(e0[q], e1[q], e2[q], -dd[q]);
+            }
+            if (ODD) { o0 = e0[NQ - 1]; o1 = e1[NQ - 1]; o2 = e2[NQ - 1]; }
+        }
+
+        // ================================================== a3: eq. (14) in fp32 with error bound
+        float dt[NQ];
+        float unc_l = 0.f;
+        {
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) dt[q] = CUDART_INF_F;
+            const float E0 = epsA + tp2sq3 * kMu19;          // bound on |a32 - a64| up to its own rounding
+            int pp = 0;
+            for (int r = 0; r < n_runs; ++r) {
+                const int pend = run_pend[r];
+                const float bf = run_bf[r];
+                float mx[NQ];
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) mx[q] = -CUDART_INF_F;
+#pragma unroll(NQ <= 2 ? 4 : 1)   // measured: unrolling the NQ = 5 body further costs 2-4 % (C2, C4)
+                for (; pp < pend; ++pp) {
+                    // two constraints a, b per entry: X = (f0a f0b f1a f1b), Y = (f2a f2b fca fcb)
+                    const float4 X = rowsA[2 * pp], Y = rowsA[2 * pp + 1];
+#pragma unroll
+                    for (int k = 0; k < NPK; ++k) {
+                        const unsigned long long va =
+                            fma2(pk2(X.x, X.x), p0[k], fma2(pk2(X.z, X.z), p1[k], fma2(pk2(Y.x, Y.x), p2[k], pk2(Y.z, Y.z))));
+                        const unsigned long long vb =
+                            fma2(pk2(X.y, X.y), p0[k], fma2(pk2(X.w, X.w), p1[k], fma2(pk2(Y.y, Y.y), p2[k], pk2(Y.w, Y.w))));
+                        float la, ha, lb, hb;
+                        upk2(va, la, ha);
+                        upk2(vb, lb, hb);
+                        mx[2 * k] = fmaxf(mx[2 * k], fmaxf(la, lb));
+                        mx[2 * k + 1] = fmaxf(mx[2 * k + 1], fmaxf(ha, hb));
+                    }
+                    if (ODD) {                          // the odd slot takes both constraints in one packed chain
+                        const unsigned long long vo = fma2(pk2(X.x, X.y), pk2(o0, o0),
+                                                           fma2(pk2(X.z, X.w), pk2(o1, o1),
+                                                                fma2(pk2(Y.x, Y.y), pk2(o2, o2), pk2(Y.z, Y.w))));
+                        float lo, hi;
+                        upk2(vo, lo, hi);
+                        mx[NQ - 1] = fmaxf(mx[NQ - 1], fmaxf(lo, hi));
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < NQ; ++q) {
+                    // a ~ max_i |u_i - d|^2 within E0 + 2^-22 a;  sq ~ sqrt(a) within 2^-21 relative
+                    const float a = fmaxf(mx[q] + dd[q], 1e-30f);
+                    const float rr = rsqrt_normal(a);
+                    const float sq = a * rr;
+                    const float du = 1.01f * fmaf(E0, rr, (bf + sq) * kMu19);
+                    unc_l = fmaxf(unc_l, du);
+                    dt[q] = fminf(dt[q], bf - sq);
+                }
+            }
+            if (stats) stc[6] += (unsigned long long)n * n_p;
+        }
+
+        // ================================================== a4: top-N_P* with certified ranking
+        const float rmf = (float)rot_margin;                // +inf unless POSE_REG_SPLIT
+        float dv[NQ];
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) dv[q] = (lane + 32 * q < n_p) ? fminf(dt[q], rmf) : -CUDART_INF_F;
+        float unc = wmax_nonneg(unc_l), myval;
+        if (RES == CLOSURE_POSE_REG_SPLIT) unc += 1.2e-7f * fabsf(rmf);
+        // (exact_only & 4: debug, every step takes the fp64 fall-back; & 16: on all N_P perturbations)
+        if (!topk_certified<NQ>(dv, n_ps, unc, (L.exact_only & 4) != 0, (L.exact_only & 32) != 0, lane, candj, candd, myval)) {
+            double R[9], t[3];
+#pragma unroll
+            for (int e = 0; e < 9; ++e) R[e] = pose[e];
+#pragma unroll
+            for (int e = 0; e < 3; ++e) t[e] = pose[9 + e];
+            const ExactMargin<RES> exact{ R, t, rows, n, rng, (uint32_t)s, t_p, rot_margin };
+            const int cnt = topk_fp64<NQ>(dv, n_p, n_ps, unc, myval, (L.exact_only & 16) != 0, lane, dex, candj, candd, exact);
+            if (stats) { stc[8] += 1; stc[0] += (unsigned long long)n * cnt; }
+        }
+        __syncwarp();                                       // pert[], candj[] visible to all lanes
+        if (lane < n_ps) cand4[lane] = pert[candj[lane]];
+        __syncwarp();
+
+        // ================================================== a5-a6: ladder, first feasible rung
+        int m0 = 0;
+        unsigned win = 0u;
+        bool lip_stop = false;
+        const int khalf = (KP + 1) >> 1;
+        for (int mb = 0; mb < n_t && m0 == 0 && !lip_stop; mb += 16) {
+            // ---- screening of 16 rungs, lane = (rung, half of the candidates): a candidate is dead for sure
+            // at rung m if one of the two tightest rows is violated beyond its error bound, or if its margin
+            // at R* is more negative than the rotation to R_m (or any smaller one: qL is a suffix maximum)
+            // can repair
+            const int mq = mb + (lane & 15), hq = lane >> 4;
+            const bool q_act = mq < n_t;
+            unsigned alive = 0u;
+            float Lm = CUDART_INF_F;
+            if (q_act) {
+                const float4 r0 = qrow[2 * mq], r1 = qrow[2 * mq + 1];
+                Lm = qL[mq];
+                const int k1 = min(KP, (hq + 1) * khalf);
+                for (int k = hq * khalf; k < k1; ++k) {
+                    const float4 c4 = cand4[k];
+                    const float v0 = fmaf(r0.x, c4.x, fmaf(r0.y, c4.y, fmaf(r0.z, c4.z, r0.w)));
+                    const float v1 = fmaf(r1.x, c4.x, fmaf(r1.y, c4.y, fmaf(r1.z, c4.z, r1.w)));
+                    if (!(v0 > c4.w) && !(v1 > c4.w) && !(candd[k] + Lm < 0.f)) alive |= 1u << k;
+                }
+            }
+            alive |= __shfl_xor_sync(FULL, alive, 16);
+            if (L.exact_only & 2) alive = q_act ? ((KP >= 32) ? FULL : ((1u << KP) - 1u)) : 0u;   // debug: nothing is screened out
+            if (mb + 16 < n_t && !(L.exact_only & 2)) {
+                // no candidate can be repaired at the last rung of this block => none at any later rung
+                float cdm = candd[0];
+                for (int k = 1; k < KP; ++k) cdm = fmaxf(cdm, candd[k]);
+                if (cdm + qL[mb + 15] < 0.f) lip_stop = true;
+            }
+            unsigned qmask = __ballot_sync(FULL, lane < 16 && alive != 0u);
+            if (stats) stc[7] += (unsigned long long)(min(n_t, mb + 16) - mb) * 2 * KP;
+
+            // ---- full evaluation of the surviving rungs, in order
+            while (qmask != 0u && m0 == 0) {
+                const int l0 = __ffs(qmask) - 1;
+                qmask &= qmask - 1u;
+                const int m1 = mb + l0;
+                const unsigned cand_alive = __shfl_sync(FULL, alive, l0);
+                double Rm[9], t[3];
+#pragma unroll
+                for (int e = 0; e < 9; ++e) Rm[e] = RmS[m1 * 9 + e];
+#pragma unroll
+                for (int e = 0; e < 3; ++e) t[e] = pose[9 + e];
+                if (full_m != m1) {
+                    __syncwarp();                            // earlier readers of rowsL are done
+                    float eps_l = 0.f;
+                    bool rdead = false;
+#pragma unroll 1
+                    for (int i = lane; i < n; i += 32) {
+                        const double *row = rows + i * ROW;
+                        double u0, u1, u2, c;
+                        affine_setup<RES>(Rm, t, row, u0, u1, u2, c);
+                        if (RES == CLOSURE_POSE_REG_SPLIT) {
+                            if (!(frob_sq(Rm, row) <= row[13])) rdead = true;     // exact: no perturbation involved
+                        }
+                        float g0, g1, g2, fcb, eps;
+                        screen_row(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
+                        rowsL[i] = make_float4(g0, g1, g2, fcb - eps);
+                        eps_l = fmaxf(eps_l, eps);
+                    }
+                    epsL = wmax_nonneg(eps_l);
+                    rdeadL = __any_sync(FULL, rdead);
+                    full_m = m1;
+                    if (stats) stc[3] += n;
+                    __syncwarp();
+                }
+                if (stats) { stc[9] += 1; stc[7] += (unsigned long long)n * KP; }
+                unsigned feas = 0u;
+                if (!rdeadL) {
+                    float M = -CUDART_INF_F;
+                    float4 c4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (e_act) {
+                        c4 = cand4[ek];
+                        for (int i = ech; i < n; i += NCH) {
+                            const float4 f = rowsL[i];
+                            M = fmaxf(M, fmaf(f.x, c4.x, fmaf(f.y, c4.y, fmaf(f.z, c4.z, f.w))));
+                        }
+                        M = fkey_inv(__reduce_max_sync(e_mask, fkey(M)));
+                    }
+                    // M = max_i (v32_i - eps_i):  M > th  => some constraint violated for sure;
+                    // M + 2 eps_max <= th => every constraint satisfied for sure.
+                    const bool dead = M > c4.w;
+                    const bool sure = (epsL < CUDART_INF_F) && (M <= c4.w - 2.0f * epsL);
+                    const bool mine = e_act && ech == 0;
+                    unsigned alive2 = __ballot_sync(FULL, mine && !dead) & cand_alive;
+                    unsigned undecided = __ballot_sync(FULL, mine && !dead && !sure) & cand_alive;
+                    if (L.exact_only & 2) { alive2 = cand_alive; undecided = cand_alive; }
+                    if (L.exact_only & 32) { alive2 &= ~undecided; undecided = 0u; }   // fp32 mode: undecided counts as VIOLATED, so every emitted sample stays inside S (Prop. 4)
+                    while (undecided != 0u) {                // rare: fp64 decides
+                        const int k = __ffs(undecided) - 1;
+                        undecided &= undecided - 1u;
+                        if (!exact_candidate_feasible<RES>(Rm, t, rows, n, rng, (uint32_t)s, candj[k], t_p, lane))
+                            alive2 &= ~(1u << k);
+                        if (stats) stc[1] += n;
+                    }
+                    feas = alive2;
+                }
+                if (feas != 0u) { m0 = m1 + 1; win = feas; }
+            }
+        }
+
+        int j_win = 0;
+        if (m0) {
+            const int kw = __ffs(win) - 1;                    // lowest rank among the feasible (R-8)
+            j_win = candj[kw];
+            double x, y, z;
+            rng.xi3((uint32_t)s, (uint32_t)j_win, 1u, x, y, z);
+            const double t0 = __dadd_rn(pose[9], __dmul_rn(t_p, x));
+            const double t1 = __dadd_rn(pose[10], __dmul_rn(t_p, y));
+            const double t2 = __dadd_rn(pose[11], __dmul_rn(t_p, z));
+            const double re = (lane < 9) ? RmS[(m0 - 1) * 9 + lane] : 0.0;
+            __syncwarp();
+            if (lane < 9) pose[lane] = re;
+            if (lane == 9) { pose[9] = t0; pose[10] = t1; pose[11] = t2; }
+            if (stats) stc[4] += 1;
+        }
+        moved = (m0 != 0);
+        if (m0 != 1) hit = true;                              // R-12 (R-11: nothing feasible -> unchanged)
+        if (L.out_trace != nullptr && lane == 0)
+            L.out_trace[((size_t)blockIdx.y * L.num_walkers + local) * L.num_steps + (s - 1)] = m0 | (j_win << 8);
+        __syncwarp();                                         // RmS / pert / candj readers done before the next step writes
+    }
+
+    // ---- a7: emit
+    if (lane == 0) {
+        const size_t o = (size_t)blockIdx.y * L.num_walkers + local;
+        double2 *dst = reinterpret_cast<double2 *>(L.out_samples + 12 * o);
+#pragma unroll
+        for (int e = 0; e < 6; ++e) dst[e] = make_double2(pose[2 * e], pose[2 * e + 1]);
+        L.out_flags[o] = hit ? 1 : 0;
+        if (stats) {
+            stc[5] = (unsigned long long)L.num_steps;
+            stc[11] = (unsigned long long)(clock64() - clk_begin);
+            for (int k = 0; k < kNumStats; ++k) atomicAdd(L.stats + k, stc[k]);
+        }
+    }
+}
+
+template <int RES, int NQ>
+cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
+{
+    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 1, L.pairs_cap);
+    if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
+    cudaError_t e = cudaFuncSetAttribute(walker_dense_kernel<RES, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)lay.total);
+    if (e != cudaSuccess) return e;
+    const long long blocks = (L.num_walkers + kCoopWarps - 1) / kCoopWarps;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    dim3 grid((unsigned)blocks, (unsigned)n_instances, 1);
+    walker_dense_kernel<RES, NQ><<<grid, kCoopThreads, lay.total, stream>>>(L);
+    return cudaGetLastError();
+}
+
+template <int RES>
+cudaError_t launch_r(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
+{
+    if (L.n_p <= 64) return launch_q<RES, 2>(L, n_instances, max_rows_bytes, max_n, stream);
+    if (L.n_p <= 160) return launch_q<RES, 5>(L, n_instances, max_rows_bytes, max_n, stream);
+    return launch_q<RES, 8>(L, n_instances, max_rows_bytes, max_n, stream);
+}
+
+}  // namespace
+
+cudaError_t launch_walkers_coop_dense(int residual_type, const WalkLaunch &L, int n_instances, int max_rows_bytes,
+                                      cudaStream_t stream)
+{
+    const int max_n = max_rows_bytes / (row_doubles(residual_type) * 8);
+    switch (residual_type) {
+    case CLOSURE_REG_3D3D: return launch_r<CLOSURE_REG_3D3D>(L, n_instances, max_rows_bytes, max_n, stream);
+    case CLOSURE_POSE_REG: return launch_r<CLOSURE_POSE_REG>(L, n_instances, max_rows_bytes, max_n, stream);
+    case CLOSURE_POSE_REG_SPLIT: return launch_r<CLOSURE_POSE_REG_SPLIT>(L, n_instances, max_rows_bytes, max_n, stream);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace closure
