@@ -256,7 +256,10 @@ class Workload:
     def kernel(self) -> str:
         if self.mode == "trans":
             return "walker_coop_trans_kernel"
-        return "walker_coop_reproj_kernel" if self.inst.residual_type == 1 else "walker_coop_kernel"
+        if self.inst.residual_type == 1:
+            return "walker_coop_reproj_kernel"
+        # N_P > 32: every perturbation against every constraint; N_P <= 32: best-first branch and bound
+        return "walker_dense_kernel" if self.inst.params.n_p > 32 else "walker_coop_kernel"
 
     def walk(self, seed):
         B = self.B

@@ -325,11 +325,17 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int n_runs_s;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    int lane = threadIdx.x & 31;
     const InstanceDesc *__restrict__ D = L.desc[blockIdx.y];
     const int n = D->n;
     const int rows_bytes = D->rows_bytes;
-    const int n_p = L.n_p, n_ps = L.n_p_star, n_t = L.n_t;
+    int n_p = L.n_p, n_ps = L.n_p_star, n_t = L.n_t;
+    // Values the iteration uses all the time are made opaque to the compiler: under register pressure it otherwise
+    // re-derives them from special registers and the constant bank inside the loop instead of keeping them in a register.
+#define CLOSURE_PIN_R(x) asm volatile("" : "+r"(x))
+#define CLOSURE_PIN_F(x) asm volatile("" : "+f"(x))
+    CLOSURE_PIN_R(lane); CLOSURE_PIN_R(n_p); CLOSURE_PIN_R(n_ps); CLOSURE_PIN_R(n_t);
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
     double *rows = reinterpret_cast<double *>(smem_raw + 16);
     stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
@@ -423,8 +429,9 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
 
     const double t_p = L.t_p;
     const float tpf = (float)t_p * 1.0000002f;          // >= t_p
-    const float tp2 = 2.0f * tpf, tp2sq3 = 3.0f * tpf * tpf;
-    const float m2tp = -2.0f * (float)t_p;
+    float tp2 = 2.0f * tpf, tp2sq3 = 3.0f * tpf * tpf;
+    float m2tp = -2.0f * (float)t_p;
+    CLOSURE_PIN_F(tp2); CLOSURE_PIN_F(tp2sq3); CLOSURE_PIN_F(m2tp);
     const int KP = n_ps;                                // ladder candidates
     const int NCH = 32 / KP;                            // constraint chunks of the full evaluation
     const int ek = lane % KP, ech = lane / KP;
