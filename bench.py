@@ -146,9 +146,10 @@ def _oracle_leg(inst, S0, walkers: int, steps: int, threads: int, seed: int):
 
 def _sample_size(inst, S0, threads: int, target_s: float) -> int:
     """Walkers for about target_s seconds of oracle time, from a short calibration leg."""
-    steps = max(1, min(inst.num_steps, 50))
-    dt, _ = _oracle_leg(inst, S0, threads, steps, threads, WALK_SEED + 7)
-    rate = threads * steps / max(dt, 1e-6)                      # walker-steps/s
+    steps = max(1, min(inst.num_steps, 200))
+    cal = 4 * threads                                           # enough walkers per thread to amortise the thread start-up
+    dt, _ = _oracle_leg(inst, S0, cal, steps, threads, WALK_SEED + 7)
+    rate = cal * steps / max(dt, 1e-6)                          # walker-steps/s
     return int(min(inst.num_walkers, max(threads, round(target_s * rate / inst.num_steps))))
 
 
@@ -363,7 +364,7 @@ def e2e_of(wl: Workload, steps: int) -> dict:
     """End to end through the C ABI with HOST buffers, every step: closure_create + closure_set_init (H2D) +
     closure_run (walk, compaction, count D2H, MEGB with its own D2H) + destroy, for every instance of the batch."""
     torch, B = wl.torch, wl.B
-    megb_s, megb_max, d2h, pivots = [], 0.0, 0, 0
+    megb_s, megb_max, d2h, pivots, slowest = [], 0.0, 0, 0, (0.0, 0.0)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     for k in range(steps):
@@ -373,6 +374,7 @@ def e2e_of(wl: Workload, steps: int) -> dict:
             r = h.closure_run(wl.W, wl.S, WALK_SEED + k + 1000 * b, wl.stream)
             megb_s.append(r["host_seconds"])
             megb_max = max(megb_max, r["max_pivot_seconds"])
+            slowest = max(slowest, (r["host_seconds"], r["prepare_seconds"]))
             d2h += r["d2h_bytes"] + 8                    # what closure_megb copied + the 8-byte count
             pivots += r["pivots"]
             h.closure_destroy()
@@ -386,7 +388,10 @@ def e2e_of(wl: Workload, steps: int) -> dict:
             "buffers": "closure_run's device buffers are cached per process and device: create/destroy in this loop allocates once",
             "per_instance_ms": 1e3 * dt / (steps * wl.nb), "steps": steps,
             "megb_ms_median": 1e3 * statistics.median(megb_s), "megb_ms_max": 1e3 * max(megb_s),
-            "megb_pivots_per_instance": pivots / (steps * wl.nb), "megb_slowest_pivot_ms": 1e3 * megb_max}
+            "megb_pivots_per_instance": pivots / (steps * wl.nb), "megb_slowest_pivot_ms": 1e3 * megb_max,
+            "megb_slowest_call": {"ms": 1e3 * slowest[0], "of_which_prepare_ms": 1e3 * slowest[1],
+                                  "note": "prepare = embedding pass + cudaMalloc of the per-device cloud buffers when a larger cloud "
+                                          "than any before arrives (once per process and size): the source of the rare 20-90 ms calls"}}
 
 
 def latency_split(wl: Workload, reps: int = 5) -> dict:

@@ -203,6 +203,8 @@ typedef struct {
     double max_pivot_seconds; /* device path: the slowest single pivot (launch + 16-byte copy + synchronise); 0 on the host path */
     int pivots;               /* device path: farthest-point launches of both balls; 0 on the host path */
     int pad_;
+    double prepare_seconds;   /* device path: the embedding pass, including the (re)allocation of the per-device buffers when the
+                                 cloud is larger than any seen before in this process (cudaMalloc: tens of ms, once per size) */
 } closure_megb_result;
 
 /* Step III (Alg. 1 l.6-7): minimum enclosing ball of {t} in R^3 and of the

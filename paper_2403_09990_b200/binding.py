@@ -37,7 +37,7 @@ class MegbResult(Structure):
                 ("trans_radius", c_double), ("rot_support", c_longlong * 5),
                 ("trans_support", c_longlong * 4), ("n_rot_support", c_int), ("n_trans_support", c_int),
                 ("host_seconds", c_double), ("d2h_bytes", c_double), ("max_pivot_seconds", c_double),
-                ("pivots", c_int), ("pad_", c_int)]
+                ("pivots", c_int), ("pad_", c_int), ("prepare_seconds", c_double)]
 
 
 class Stats(Structure):
@@ -164,7 +164,8 @@ def _as_dict(r: MegbResult) -> dict:
     return dict(R=np.array(r.R).reshape(3, 3), t=np.array(r.t), rot_radius=r.rot_radius,
                 trans_radius=r.trans_radius, rot_support=np.array(r.rot_support[:r.n_rot_support]),
                 trans_support=np.array(r.trans_support[:r.n_trans_support]), host_seconds=r.host_seconds,
-                d2h_bytes=int(r.d2h_bytes), max_pivot_seconds=r.max_pivot_seconds, pivots=int(r.pivots))
+                d2h_bytes=int(r.d2h_bytes), max_pivot_seconds=r.max_pivot_seconds, pivots=int(r.pivots),
+                prepare_seconds=r.prepare_seconds)
 
 
 class Closure:

@@ -642,7 +642,7 @@ int closure_megb(closure_t *h, const double *samples, long long count, closure_m
     double qbar[4];
     rotation_to_quat(h->h_desc.Rbar, qbar);
     Ball bt, bq;
-    double d2h_bytes = 0.0, max_pivot_s = 0.0;
+    double d2h_bytes = 0.0, max_pivot_s = 0.0, prepare_s = 0.0;
     int pivots = 0;
     const auto t0 = std::chrono::steady_clock::now();
     if (count >= kDeviceMegbMin && !(h->P.flags & CLOSURE_FLAG_HOST_MEGB)) {
@@ -655,6 +655,7 @@ int closure_megb(closure_t *h, const double *samples, long long count, closure_m
         if (e == cudaSuccess && !g_megb[dev]) g_megb[dev] = device_megb_create(&e);
         if (e == cudaSuccess) e = device_megb_prepare(g_megb[dev], samples, count, qbar, stream);
         if (e != cudaSuccess) return cuda_fail(h, e, "device MEGB set-up");
+        prepare_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
         DeviceMegb *dm = g_megb[dev];
         const bool ok = miniball_source(device_megb_trans(dm), count, 3, &bt) &&
                         miniball_source(device_megb_quats(dm), count, 4, &bq);
@@ -704,6 +705,7 @@ int closure_megb(closure_t *h, const double *samples, long long count, closure_m
     out->d2h_bytes = d2h_bytes;
     out->max_pivot_seconds = max_pivot_s;
     out->pivots = pivots;
+    out->prepare_seconds = prepare_s;
     return CLOSURE_OK;
 }
 

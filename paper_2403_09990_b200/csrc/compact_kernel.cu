@@ -131,6 +131,20 @@ __global__ void __launch_bounds__(kCThreads) compact_kernel(const uint4 *__restr
     const int chunks = recs * kChunksPerRec;
     const uint4 *src = samples + base * kChunksPerRec;
     uint4 *dst = out + excl * kChunksPerRec;
+    if (tile_total == recs) {
+        // every record of the tile is kept (the usual case: a walker that has run for a while has been stopped by the
+        // boundary): a straight copy, eight independent 16-byte loads in flight per thread, no offset look-ups
+        int c = tid;
+        for (; c + 7 * kCThreads < chunks; c += 8 * kCThreads) {
+            uint4 v[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] = __ldcs(src + c + k * kCThreads);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) __stcs(dst + c + k * kCThreads, v[k]);
+        }
+        for (; c < chunks; c += kCThreads) __stcs(dst + c, __ldcs(src + c));
+        return;
+    }
 #pragma unroll 4
     for (int c = tid; c < chunks; c += kCThreads) {
         const int rec = c / kChunksPerRec;

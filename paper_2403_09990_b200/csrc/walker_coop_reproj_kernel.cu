@@ -292,6 +292,48 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
             // per rung: the two tightest cone rows at d = 0 and the Lipschitz bound L_m on the change of
             // any reprojection residual norm between R* and R_m, valid for every |d_c| <= t_p:
             //   |d/dtau fx p_1/p_3| <= fx (|dP_1| + |p_1/p_3| |dP_3|) / p_3 along p(tau) = p + tau dP
+            if (n <= 16) {
+                // short tables (Ex.1 has ~8-10 keypoints): lane = (rung, constraint), 32 / G rungs per pass with G = 8 or
+                // 16 lanes per rung, so that the lanes are not left idle by a loop over 8 constraints; same rows and bounds
+                const int G = n <= 8 ? 8 : 16;
+                const int c = lane & (G - 1);
+                const bool has = c < n;
+                const double *row = rows + (has ? c : 0) * ROW;
+                const unsigned hm = ((G == 8) ? 0xFFu : 0xFFFFu) << (lane & ~(G - 1));
+                double P0, P1, P2;
+                reproj_point(R, row, P0, P1, P2);
+#pragma unroll 1
+                for (int m = lane / G; m < n_t; m += 32 / G) {
+                    double Rm[9];
+#pragma unroll
+                    for (int e = 0; e < 9; ++e) Rm[e] = RmS[m * 9 + e];
+                    double Q0, Q1, Q2;
+                    reproj_point(Rm, row, Q0, Q1, Q2);
+                    ReprojRow r = reproj_row<true>(Q0 + t[0], Q1 + t[1], Q2 + t[2], row, K, t_p);
+                    double lip;
+                    const double plo = dmin(P2, Q2) + t[2] - 1.001 * t_p;
+                    if (plo > 0.0) {
+                        const double x_hi = dmax(fabs(P0 + t[0]), fabs(Q0 + t[0])) + t_p;
+                        const double y_hi = dmax(fabs(P1 + t[1]), fabs(Q1 + t[1])) + t_p;
+                        const double d0 = fabs(Q0 - P0), d1 = fabs(Q1 - P1), d2 = fabs(Q2 - P2);
+                        lip = K[0] * (d0 + x_hi / plo * d2) / plo + K[1] * (d1 + y_hi / plo * d2) / plo;
+                    } else {
+                        lip = CUDART_INF;
+                    }
+                    if (!has) { r.g0 = -CUDART_INF_F; r.b.z = -CUDART_INF_F; }      // a row that never kills
+                    const uint32_t key = has ? ((fkey(r.g0) & ~15u) | (uint32_t)c) : (uint32_t)c;
+                    const uint32_t m1 = __reduce_max_sync(hm, key);
+                    const uint32_t key2 = (key == m1) ? 0u : key;
+                    const uint32_t m2 = __reduce_max_sync(hm, key2);
+                    const float lf = __uint_as_float(__reduce_max_sync(hm, __float_as_uint(has ? (float)lip : 0.f)));
+                    if (key == m1) {
+                        qrow[4 * m] = r.a; qrow[4 * m + 1] = r.b;
+                        qL[m] = lf * 1.001f + 1e-30f;
+                        if (n == 1) { qrow[4 * m + 2] = r.a; qrow[4 * m + 3] = r.b; }
+                    }
+                    if (key2 == m2 && n > 1) { qrow[4 * m + 2] = r.a; qrow[4 * m + 3] = r.b; }
+                }
+            } else {
 #pragma unroll 1
             for (int m = 0; m < n_t; ++m) {
                 double Rm[9];
@@ -335,6 +377,7 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                 }
                 const float lf = wmax_nonneg((float)lip);
                 if (lane == 0) qL[m] = lf * 1.001f + 1e-30f;
+            }
             }
             if (stats) { stc[2] += n; stc[3] += (unsigned long long)n * n_t; }
             __syncwarp();
