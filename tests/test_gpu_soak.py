@@ -3,7 +3,8 @@
 Random config, instance, walk parameters, |S_0|, mode and seed per run; samples and flags must agree bit for bit.
 (The same loop ran for 15 minutes twice in round 1, the second time on the final build with random bound runs and
 body pivots as below: 8,349 + 8,080 runs, 68 M + 66 M walkers, and for 10 minutes on the last build of the round: 9,720
-runs; no mismatch -- DESIGN.md 8.)"""
+runs; no mismatch -- DESIGN.md 8.  Round 2 added streams 3 and 4 for the branch-and-bound kernel, N_P <= 32, and ran the
+loop again on the final build.)"""
 import copy
 
 import numpy as np
@@ -15,7 +16,12 @@ from tests.gpu_common import gpu_walk
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("stream", [0, 1, 2])
+def _n_p_choices(stream):
+    # streams 3 and 4: N_P <= 32, the branch-and-bound kernel (best-first on one run of equal bounds, batched otherwise)
+    return [1, 3, 8, 20, 27, 32] if stream >= 3 else [20, 33, 64, 100, 150, 160, 200, 256]
+
+
+@pytest.mark.parametrize("stream", [0, 1, 2, 3, 4])
 def test_random_parameters_bit_identical_to_plain_kernel(stream):
     rng = np.random.default_rng(1000 + stream)
     for _ in range(12):
@@ -24,7 +30,7 @@ def test_random_parameters_bit_identical_to_plain_kernel(stream):
         if cfg == 4 and rng.random() < 0.3:
             inst = I.to_split(inst)
         P = copy.copy(inst.params)
-        P.n_p = int(rng.choice([20, 33, 64, 100, 150, 160, 200, 256]))
+        P.n_p = int(rng.choice(_n_p_choices(stream)))
         P.n_p_star = int(min(P.n_p, rng.choice([1, 2, 5, 10, 16, 20])))
         P.n_t = int(rng.choice([1, 5, 10, 15, 17, 40]))
         P.t_p = float(P.t_p * rng.choice([0.1, 0.5, 1.0, 2.0]))
