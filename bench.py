@@ -352,6 +352,11 @@ def roofline_of(wl: Workload, walk_s: float, peaks: dict, seed: int = WALK_SEED)
             "philox": {"calls_per_launch": philox_calls, "peak_calls_per_s": peak_philox,
                        "note": "Philox4x32-10 calls at the rate of a kernel that does nothing else"},
             "frac_incl_philox": t_min_rng / walk_s,
+            # the branch-and-bound kernel (N_P <= 32) skips pairs that cannot matter: the same time against the arithmetic the
+            # dense evaluation of eq. (14) would need (N_P x N pairs per walker-step instead of the executed ones)
+            "frac_dense_equivalent": (t_min + max(0.0, fpa * (float(ws) * P.n_p * inst.n - st["perturb_pairs_f32"]
+                                                              - st["perturb_pairs"])) / peak32) / walk_s
+            if wl.mode != "trans" else t_min / walk_s,
             "executed_pairs_per_walker_step": pairs / ws,
             "nominal_pairs_per_walker_step": (P.n_p + P.n_p_star * P.n_t) * inst.n,
             "fp64_fallback_steps": st["fallback_steps"] / ws,
@@ -685,7 +690,7 @@ def per_config_block(B, torch, args, peaks, flush, barrier) -> list:
                      "constraint_evals_per_sec_nominal": v * (P.n_p + P.n_p_star * P.n_t) * wl.inst.n,
                      "boundary_fraction": int(wl.count.item()) / float(wl.nb * wl.W),
                      "roofline": {k: roof[k] for k in ("kernel", "achieved", "peak", "unit", "frac", "frac_of_nominal",
-                                                       "frac_incl_philox", "executed_pairs_per_walker_step",
+                                                       "frac_incl_philox", "frac_dense_equivalent", "executed_pairs_per_walker_step",
                                                        "fp64_fallback_steps", "accepted_steps", "traffic")},
                      "e2e": {k: e2e[k] for k in ("value", "unit", "per_instance_ms", "h2d_bytes_per_step",
                                                  "d2h_bytes_per_step", "megb_ms_median")}})
