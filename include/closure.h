@@ -40,6 +40,7 @@ extern "C" {
 #define CLOSURE_ECUDA (-4)    /* CUDA runtime failure (message in closure_last_error) */
 #define CLOSURE_ENOMEM (-5)
 #define CLOSURE_EUNSUPPORTED (-6) /* combination not built (e.g. n_p_star > 32) */
+#define CLOSURE_ETOOLARGE (-7)    /* closure_compact_static: n exceeds CLOSURE_COMPACT_STATIC_MAX */
 
 /* residual g(x, y_i) -- eqs. (2)-(4).  Measurement row layouts (doubles):
  *   CLOSURE_REPROJ_2D3D     [z(2) Z(3)]          g = z - Pi(K (R Z + t)), pixels; depth<=0 violates (R-10)
@@ -186,6 +187,20 @@ int closure_sample_batch(closure_t *const *handles, int n_instances, long long w
  *   out_count        DEVICE, one long long: number of kept samples */
 int closure_compact(closure_t *h, const double *samples, const unsigned char *flags, long long n,
                     double *out_compacted, long long *out_count, void *cuda_stream);
+
+/* closure_compact without any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it).  Same kernel, same result bit for bit; its scratch (8 bytes per tile of
+ * 2,048 records) is a static device array inside the library, sized for at most CLOSURE_COMPACT_STATIC_MAX records
+ * (32 KB + 8 B, held by every GPU that loads the library until exit).  Needs no handle.  ASYNC; calls no cudaMalloc,
+ * cudaFree or allocating library routine (the first call on a device resolves the array's device address, once).
+ *   samples, flags, out_compacted, out_count   DEVICE, as for closure_compact; sample buffers 16-byte aligned
+ * Errors: CLOSURE_ETOOLARGE if n > CLOSURE_COMPACT_STATIC_MAX (nothing is launched; use closure_compact),
+ * CLOSURE_EINVAL (negative n, NULL or misaligned buffers), CLOSURE_ECUDA.
+ * ALL calls on one device share the one array: it is cleared at the start of every call on the caller's stream, and
+ * two calls that can overlap on the GPU (different streams, or concurrent host threads) RACE -- serialise them. */
+#define CLOSURE_COMPACT_STATIC_MAX 8388608
+int closure_compact_static(const double *samples, const unsigned char *flags, long long n, double *out_compacted,
+                           long long *out_count, void *cuda_stream);
 
 /* Step III result.  Geodesic distance on SO(3): arccos((tr(C^T R) - 1) / 2). */
 typedef struct {

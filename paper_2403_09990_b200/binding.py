@@ -16,11 +16,12 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libclosure_b200.so")
 
-OK, EINVAL, EINIT, ENOINIT, ECUDA, ENOMEM, EUNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
+OK, EINVAL, EINIT, ENOINIT, ECUDA, ENOMEM, EUNSUPPORTED, ETOOLARGE = 0, -1, -2, -3, -4, -5, -6, -7
+COMPACT_STATIC_MAX = 8388608
 
 EXPORTS = [
     "closure_default_params", "closure_create", "closure_set_params", "closure_set_pivot", "closure_set_init",
-    "closure_sample_range", "closure_sample", "closure_sample_batch", "closure_compact", "closure_megb",
+    "closure_sample_range", "closure_sample", "closure_sample_batch", "closure_compact", "closure_compact_static", "closure_megb",
     "closure_init_sample", "closure_init_from_trials", "closure_run", "closure_enable_stats", "closure_get_stats", "closure_alu_peak", "closure_miniball_host",
     "closure_last_error", "closure_strerror", "closure_abi_version", "closure_destroy",
 ]
@@ -82,6 +83,7 @@ def load_library():
     L.closure_sample_batch.argtypes = [POINTER(c_void_p), c_int, c_longlong, c_int, POINTER(c_ulonglong),
                                        c_void_p, c_void_p, c_void_p]
     L.closure_compact.argtypes = [c_void_p, c_void_p, c_void_p, c_longlong, c_void_p, c_void_p, c_void_p]
+    L.closure_compact_static.argtypes = [c_void_p, c_void_p, c_longlong, c_void_p, c_void_p, c_void_p]
     L.closure_megb.argtypes = [c_void_p, c_void_p, c_longlong, POINTER(MegbResult), c_void_p]
     L.closure_run.argtypes = [c_void_p, c_longlong, c_int, c_ulonglong, POINTER(MegbResult),
                               POINTER(c_longlong), c_void_p]
@@ -299,6 +301,17 @@ class Closure:
             self.closure_destroy()
         except Exception:
             pass
+
+
+def closure_compact_static(samples, flags, out_compacted, out_count, stream=None):
+    """closure_compact on the library's static scratch: allocates nothing (the caller passes every buffer), at most
+    COMPACT_STATIC_MAX records; calls on one device must not overlap."""
+    rc = load_library().closure_compact_static(c_void_p(samples.data_ptr()), c_void_p(flags.data_ptr()), int(flags.shape[0]),
+                                               c_void_p(out_compacted.data_ptr()), c_void_p(out_count.data_ptr()),
+                                               _stream_ptr(stream))
+    if rc != OK:
+        raise ClosureError(rc, closure_strerror(rc))
+    return out_compacted, out_count
 
 
 def closure_sample_batch(handles: list[Closure], walkers_per_instance: int, num_steps: int, seeds,

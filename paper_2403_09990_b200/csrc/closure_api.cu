@@ -275,6 +275,7 @@ const char *closure_strerror(int status)
     case CLOSURE_ECUDA: return "CUDA failure";
     case CLOSURE_ENOMEM: return "out of memory";
     case CLOSURE_EUNSUPPORTED: return "combination not built";
+    case CLOSURE_ETOOLARGE: return "n exceeds CLOSURE_COMPACT_STATIC_MAX (8,388,608 records), the size of the static scratch of closure_compact_static: use closure_compact";
     default: return "unknown status";
     }
 }
@@ -630,6 +631,16 @@ int closure_compact(closure_t *h, const double *samples, const unsigned char *fl
                                    static_cast<cudaStream_t>(cuda_stream));
     if (e != cudaSuccess) return cuda_fail(h, e, "compaction kernel launch");
     return CLOSURE_OK;
+}
+
+int closure_compact_static(const double *samples, const unsigned char *flags, long long n, double *out_compacted,
+                           long long *out_count, void *cuda_stream)
+{
+    if (n < 0 || !out_count || (n > 0 && (!samples || !flags || !out_compacted))) return CLOSURE_EINVAL;
+    if (n > CLOSURE_COMPACT_STATIC_MAX) return CLOSURE_ETOOLARGE;
+    if ((reinterpret_cast<uintptr_t>(samples) | reinterpret_cast<uintptr_t>(out_compacted)) & 15u) return CLOSURE_EINVAL;
+    const cudaError_t e = launch_compact_static(samples, flags, n, out_compacted, out_count, static_cast<cudaStream_t>(cuda_stream));
+    return e == cudaSuccess ? CLOSURE_OK : CLOSURE_ECUDA;
 }
 
 int closure_megb(closure_t *h, const double *samples, long long count, closure_megb_result *out,

@@ -93,6 +93,9 @@ cudaError_t launch_step1(int residual_type, const InstanceDesc *d_desc, int rows
 size_t compact_scratch_bytes(long long n);
 cudaError_t launch_compact(const double *samples, const unsigned char *flags, long long n, double *out,
                            long long *out_count, void *scratch, cudaStream_t stream);
+// the same kernel on the file-scope static scratch of compact_kernel.cu (closure_compact_static: allocates nothing)
+cudaError_t launch_compact_static(const double *samples, const unsigned char *flags, long long n, double *out,
+                                  long long *out_count, cudaStream_t stream);
 
 // alu_peak.cu
 cudaError_t measure_alu_peak(int precision, double *flops_per_s, double *seconds, cudaStream_t stream);

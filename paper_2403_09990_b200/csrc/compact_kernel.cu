@@ -10,6 +10,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <mutex>
+
 #include "closure_internal.h"
 
 namespace closure {
@@ -180,6 +182,60 @@ cudaError_t launch_pivot_back(double *poses, long long n, const double *pivot, c
     const long long blocks = (n + 255) / 256;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
     pivot_back_kernel<<<(unsigned)blocks, 256, 0, stream>>>(poses, n, pivot[0], pivot[1], pivot[2]);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------- no-allocation variant
+// closure_compact_static (include/closure.h): the same kernel, with its scratch (ticket counter + one look-back state
+// per tile of 2,048 records) in a file-scope device array instead of a cudaMalloc'ed per-handle buffer, for callers that
+// cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Every GPU that loads
+// the library holds these 32 KB + 8 B until exit.  All calls on a device share the array: it keeps the last call's
+// contents (cleared at the start of every call, on the caller's stream), and two calls that overlap on the GPU race.
+namespace {
+
+constexpr long long kStaticMaxTiles = CLOSURE_COMPACT_STATIC_MAX / kTile;       // 8,388,608 records = 4,096 tiles
+static_assert(kStaticMaxTiles * kTile == CLOSURE_COMPACT_STATIC_MAX, "the static maximum is a whole number of tiles");
+static __device__ __align__(256) unsigned long long g_compact_static_scratch[kStaticMaxTiles + 1];
+
+// In HOST code the array's name is a host-side stand-in, not a device address: the address the kernel needs comes from
+// cudaGetSymbolAddress, resolved once per device with that device current and cached here.
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+unsigned long long *g_static_ptr[kStaticMaxDevices] = { nullptr };
+
+cudaError_t static_scratch_of_current_device(unsigned long long **ptr)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kStaticMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (g_static_ptr[dev] == nullptr) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_compact_static_scratch);
+        if (e != cudaSuccess) return e;
+        g_static_ptr[dev] = static_cast<unsigned long long *>(p);
+    }
+    *ptr = g_static_ptr[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+cudaError_t launch_compact_static(const double *samples, const unsigned char *flags, long long n, double *out,
+                                  long long *out_count, cudaStream_t stream)
+{
+    if (n <= 0) return cudaMemsetAsync(out_count, 0, sizeof(long long), stream);
+    if (n > CLOSURE_COMPACT_STATIC_MAX) return cudaErrorInvalidValue;             // (the C entry point reports it first)
+    const long long tiles = (n + kTile - 1) / kTile;
+    unsigned long long *scratch = nullptr;
+    cudaError_t e = static_scratch_of_current_device(&scratch);
+    if (e != cudaSuccess) return e;
+    // the ticket and the tile states of this call must start at zero: the array still holds the previous call's
+    e = cudaMemsetAsync(scratch, 0, (size_t)(tiles + 1) * sizeof(unsigned long long), stream);
+    if (e != cudaSuccess) return e;
+    compact_kernel<<<(unsigned)tiles, kCThreads, 0, stream>>>(reinterpret_cast<const uint4 *>(samples), flags, n,
+                                                             reinterpret_cast<uint4 *>(out), out_count, scratch, (int)tiles);
     return cudaGetLastError();
 }
 
