@@ -19,12 +19,15 @@ constexpr unsigned FULL = 0xffffffffu;
 constexpr float kMu19 = 1.9073486328125e-06f;   // 2^-19
 
 struct CoopSmem {
-    size_t run_end, run_bf, run_pend, pos, warp0, per_warp, rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, cand4, candj, candd, pose, stc, total;
+    size_t run_end, run_bf, run_pend, pos, af, warp0, per_warp, rowsA, rowsL, pert, ab, qrow, RmS, dex, qL, cand4, candj, candd, pose, stc, rm32, ridx, total;
 };
 
 // Shared-memory layout; f4 = float4 words per fp32 constraint row (1: affine residuals, 2: reprojection);
 // pairs = 32-byte entries of rowsA (affine: pair-entries, runs padded to even length; otherwise n)
-__host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, int nq, int f4, int pairs, int warps = kCoopWarps)
+// af_f4 > 0 (dense kernel, Ex.2: 1, Ex.3: 3): a CTA-level fp32 image of the constraints (af_f4 float4 per row) and per warp the
+// fp32 rung rotations (rm32) and the indices of each rung's screening rows (ridx), for the fp32 search of the set-up
+__host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, int nq, int f4, int pairs, int warps = kCoopWarps,
+                                                int af_f4 = 0)
 {
     CoopSmem s;
     size_t o = 16 + (size_t)((rows_bytes + 15) & ~15);
@@ -32,6 +35,7 @@ __host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, 
     s.run_bf = o;  o += (size_t)((n * 4 + 15) & ~15);
     s.run_pend = o; o += (size_t)((n * 4 + 15) & ~15);
     s.pos = o;     o += (size_t)((n * 4 + 15) & ~15);
+    s.af = o;      o += (size_t)n * 16 * af_f4;
     s.warp0 = o;
     size_t w = 0;
     s.rowsA = w; w += (size_t)pairs * 32;          // affine: pair-transposed, runs padded to even length
@@ -47,6 +51,8 @@ __host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, 
     s.candd = w; w += 32 * 4;
     s.pose = w;  w += 18 * 8;
     s.stc = w;   w += 16 * 8;
+    s.rm32 = w;  w += af_f4 > 0 ? (size_t)n_t * 48 : 0;
+    s.ridx = w;  w += af_f4 > 0 ? (size_t)((n_t * 8 + 15) & ~15) : 0;
     s.per_warp = w;
     s.total = o + (size_t)warps * w;
     return s;

@@ -154,6 +154,140 @@ __device__ __forceinline__ bool exact_candidate_feasible(const double (&Rm)[9], 
     return __all_sync(FULL, ok);
 }
 
+// float4 words per constraint of the CTA-level fp32 table behind the set-up's search for screening rows:
+// Ex.2 (a_i, beta_i^2); Ex.3 stacked (R_i row 0, beta_i^2) (R_i row 1, 0) (R_i row 2, 0); split form: none (old search)
+template <int RES> __host__ __device__ constexpr int af_width()
+{
+    return RES == CLOSURE_REG_3D3D ? 1 : (RES == CLOSURE_POSE_REG ? 3 : 0);
+}
+
+// ---------------------------------------------------------------------------------- screening rows of every rung
+// Per rung the ladder screens its candidates against two constraint rows at R_m and against a Lipschitz bound.  ANY two
+// constraints give valid rows (a violated row kills a candidate whichever row it is); the two TIGHTEST ones kill most.
+// Round 1 found them by setting up all N rows of all N_T rungs in fp64 (N N_T set-ups per move: 59 % of the warp cycles at
+// N_I = 5, where most iterations move).  Here the SEARCH runs in plain fp32 from what the set-up at R* already holds,
+//     Ex.2:  u^m_i = u*_i - (R_m - R*) a_i,    key_i = |u^m_i|^2 - beta_i^2        (9 + 3 + 3 FMA)
+//     Ex.3:  key_i = |u_i|^2 + |R_m - R_i|_F^2 - beta_i^2                            (9 SUB + 9 FMA)
+// with no error analysis (a near-tie picks another, equally valid pair), and only the two chosen rows per rung get the
+// rigorous fp64 set-up + screen_row() of before (2 N_T set-ups per move, rung m on lane m).  The Lipschitz bound of Ex.2,
+// max_i |(R_m - R*) a_i|, comes out of the same fp32 pass with a slack that covers its rounding (|g32 - g| <= 5 2^-24
+// |R_m - R*|_F |a_i| per component chain; 4e-6 |dR|_F max|a| is > 10x that); Ex.3's |R_m - R*|_F stays in fp64.
+template <int RES>
+__device__ __forceinline__ void fast_rung_rows(unsigned char *smem_raw, const CoopSmem &lay, unsigned char *wp, int lane, int n,
+                                               int n_t, const double (&R)[9], const double (&t)[3], float tp2, float tp2sq3,
+                                               float amax)
+{
+    using RS = Res<RES>;
+    constexpr int ROW = RS::ROW;
+    constexpr bool REG = RES == CLOSURE_REG_3D3D;
+    const double *rows = reinterpret_cast<const double *>(smem_raw + 16);
+    const int *pos = reinterpret_cast<const int *>(smem_raw + lay.pos);
+    const float4 *af = reinterpret_cast<const float4 *>(smem_raw + lay.af);
+    const float *rowsAf = reinterpret_cast<const float *>(wp + lay.rowsA);
+    const float4 *rm32 = reinterpret_cast<const float4 *>(wp + lay.rm32);
+    int2 *ridx = reinterpret_cast<int2 *>(wp + lay.ridx);
+    float4 *qrow = reinterpret_cast<float4 *>(wp + lay.qrow);
+    const double *RmS = reinterpret_cast<const double *>(wp + lay.RmS);
+    float *qL = reinterpret_cast<float *>(wp + lay.qL);
+
+    // key of constraint i at the rung whose fp32 rotation image is (m0, m1, m2); lipv = |(R_m - R*) a_i|^2 (Ex.2)
+    auto key_of = [&](int i, const float4 &m0, const float4 &m1, const float4 &m2, float &lipv) -> float {
+        const int sp = pos[i] & 0x3fffffff;
+        const float *S = rowsAf + (sp >> 1) * 8 + (sp & 1);
+        const float us0 = S[0], us1 = S[2], us2 = S[4];
+        if (REG) {
+            const float4 a = af[i];
+            const float g0 = fmaf(m0.z, a.z, fmaf(m0.y, a.y, m0.x * a.x));
+            const float g1 = fmaf(m1.z, a.z, fmaf(m1.y, a.y, m1.x * a.x));
+            const float g2 = fmaf(m2.z, a.z, fmaf(m2.y, a.y, m2.x * a.x));
+            lipv = fmaf(g2, g2, fmaf(g1, g1, g0 * g0));
+            const float u0 = us0 - g0, u1 = us1 - g1, u2 = us2 - g2;
+            return fmaf(u2, u2, fmaf(u1, u1, u0 * u0)) - a.w;
+        } else {
+            const float4 r0 = af[3 * i], r1 = af[3 * i + 1], r2 = af[3 * i + 2];
+            float f = fmaf(us2, us2, fmaf(us1, us1, us0 * us0)) - r0.w;
+            float d;
+            d = m0.x - r0.x; f = fmaf(d, d, f); d = m0.y - r0.y; f = fmaf(d, d, f); d = m0.z - r0.z; f = fmaf(d, d, f);
+            d = m1.x - r1.x; f = fmaf(d, d, f); d = m1.y - r1.y; f = fmaf(d, d, f); d = m1.z - r1.z; f = fmaf(d, d, f);
+            d = m2.x - r2.x; f = fmaf(d, d, f); d = m2.y - r2.y; f = fmaf(d, d, f); d = m2.z - r2.z; f = fmaf(d, d, f);
+            lipv = 0.f;
+            return f;
+        }
+    };
+
+    if (n <= 16) {
+        // lane = (rung parity, constraint): the lanes are not left idle by a loop over 8 - 16 constraints
+        const int c = lane & 15;
+        const bool has = c < n;
+        const unsigned hm = 0xFFFFu << (lane & 16);
+#pragma unroll 1
+        for (int m = lane >> 4; m < n_t; m += 2) {
+            const float4 m0 = rm32[3 * m], m1 = rm32[3 * m + 1], m2 = rm32[3 * m + 2];
+            float lipv = 0.f;
+            const float kv = key_of(has ? c : 0, m0, m1, m2, lipv);
+            const uint32_t key = has ? ((fkey(kv) & ~15u) | (uint32_t)c) : (uint32_t)c;
+            const uint32_t k1 = __reduce_max_sync(hm, key);
+            const uint32_t k2 = __reduce_max_sync(hm, key == k1 ? 0u : key);
+            const uint32_t lm = __reduce_max_sync(hm, __float_as_uint(has ? lipv : 0.f));
+            if (key == k1) {
+                ridx[m] = make_int2((int)(k1 & 15u), n > 1 ? (int)(k2 & 15u) : (int)(k1 & 15u));
+                qL[m] = __uint_as_float(lm);
+            }
+        }
+    } else {
+#pragma unroll 1
+        for (int m = 0; m < n_t; ++m) {
+            const float4 m0 = rm32[3 * m], m1 = rm32[3 * m + 1], m2 = rm32[3 * m + 2];
+            float b1 = -CUDART_INF_F, b2 = -CUDART_INF_F, lipl = 0.f;
+            int j1 = 0, j2 = 0;
+#pragma unroll 2
+            for (int i = lane; i < n; i += 32) {
+                float lipv;
+                const float kv = key_of(i, m0, m1, m2, lipv);
+                lipl = fmaxf(lipl, lipv);
+                if (kv > b1) { b2 = b1; j2 = j1; b1 = kv; j1 = i; } else if (kv > b2) { b2 = kv; j2 = i; }
+            }
+            const uint32_t q1 = fkey(b1);
+            const uint32_t g1 = __reduce_max_sync(FULL, q1);
+            const int src1 = __ffs(__ballot_sync(FULL, q1 == g1)) - 1;
+            const uint32_t q2 = (lane == src1) ? fkey(b2) : q1;
+            const uint32_t g2 = __reduce_max_sync(FULL, q2);
+            const int src2 = __ffs(__ballot_sync(FULL, q2 == g2)) - 1;
+            const int i1 = __shfl_sync(FULL, j1, src1);
+            const int i2 = __shfl_sync(FULL, src2 == src1 ? j2 : j1, src2);
+            const float lm = wmax_nonneg(lipl);
+            if (lane == 0) { ridx[m] = make_int2(i1, i2); qL[m] = lm; }
+        }
+    }
+    __syncwarp();
+    // the two chosen rows of rung m in fp64 with their error bounds, and the rung's Lipschitz bound: lane m
+    for (int m = lane; m < n_t; m += 32) {
+        double Rm[9];
+#pragma unroll
+        for (int e = 0; e < 9; ++e) Rm[e] = RmS[m * 9 + e];
+        const int2 ii = ridx[m];
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            const double *row = rows + (q ? ii.y : ii.x) * ROW;
+            double u0, u1, u2, cc;
+            affine_setup<RES>(Rm, t, row, u0, u1, u2, cc);
+            float g0, g1, g2, fcb, eps;
+            screen_row(u0, u1, u2, cc - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
+            qrow[2 * m + q] = make_float4(g0, g1, g2, fcb - eps);
+        }
+        float lf;
+        if (REG) {
+            lf = sqrtf(qL[m]) * 1.000001f + 4.0e-6f * rm32[3 * m].w * amax;
+        } else {
+            double lip = 0.0;
+#pragma unroll
+            for (int e = 0; e < 9; ++e) { const double d = Rm[e] - R[e]; lip = fma(d, d, lip); }      // |R_m - R*|_F^2
+            lf = (float)sqrt(lip);
+        }
+        qL[m] = lf * 1.001f + 1e-30f;
+    }
+}
+
 // ---------------------------------------------------------------------------------- set-up after a move
 // Everything that depends on the pose only (DESIGN.md 6.1b "state that only changes on an accepted
 // move"): fp32 set-up rows at R* (rowsA), Exp(dT_m w) R* for every rung (RmS), per rung the two
@@ -161,11 +295,12 @@ __device__ __forceinline__ bool exact_candidate_feasible(const double (&Rm)[9], 
 // its registers do not count against the per-iteration code.  Results epsA, rot_margin -> pose[16], pose[15].
 template <int RES>
 __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int warp, int lane, int rows_bytes, int n,
-                                                int n_t, int nq, int pairs, double t_p, bool stats)
+                                                int n_t, int nq, int pairs, double t_p, float amax, bool stats)
 {
     using RS = Res<RES>;
     constexpr int ROW = RS::ROW;
-    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, nq, 1, pairs);
+    constexpr bool FAST = af_width<RES>() > 0;          // fp32 search for the screening rows (below)
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, nq, 1, pairs, kCoopWarps, af_width<RES>());
     const double *rows = reinterpret_cast<const double *>(smem_raw + 16);
     const int *pos = reinterpret_cast<const int *>(smem_raw + lay.pos);
     unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
@@ -210,8 +345,24 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
         rotate_left(R, vel[0], vel[1], vel[2], c2.x, c2.y, Rm);
 #pragma unroll
         for (int e = 0; e < 9; ++e) RmS[m * 9 + e] = Rm[e];
+        if (FAST) {                                  // fp32 image for the search: R_m - R* (Ex.2), R_m (Ex.3)
+            float v[9], fro = 0.f;
+#pragma unroll
+            for (int e = 0; e < 9; ++e) {
+                v[e] = (float)(RES == CLOSURE_REG_3D3D ? Rm[e] - R[e] : Rm[e]);
+                fro = fmaf(v[e], v[e], fro);
+            }
+            float4 *rm32 = reinterpret_cast<float4 *>(wp + lay.rm32);
+            rm32[3 * m] = make_float4(v[0], v[1], v[2], sqrtf(fro));
+            rm32[3 * m + 1] = make_float4(v[3], v[4], v[5], 0.f);
+            rm32[3 * m + 2] = make_float4(v[6], v[7], v[8], 0.f);
+        }
     }
     __syncwarp();
+    if (FAST) {
+        fast_rung_rows<RES>(smem_raw, lay, wp, lane, n, n_t, R, t, tp2, tp2sq3, amax);
+        if (stats) { stc[2] += n; stc[3] += 2ull * n_t; }
+    } else {
     // the two tightest constraints of every rung (largest c - beta^2 at the unperturbed
     // translation): the rows the ladder screens each rung against while the pose stays here
     if (n <= 16) {
@@ -304,6 +455,7 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
     }
     }
     if (stats) { stc[2] += n; stc[3] += (unsigned long long)n * n_t; }
+    }
     __syncwarp();
     if (lane == 0) {                                 // suffix maximum: qL[m] holds for every rung >= m
         float sm = 0.f;
@@ -325,6 +477,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int n_runs_s;
+    __shared__ float amax_s;
     const int warp = threadIdx.x >> 5;
     int lane = threadIdx.x & 31;
     const InstanceDesc *__restrict__ D = L.desc[blockIdx.y];
@@ -339,7 +492,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
     double *rows = reinterpret_cast<double *>(smem_raw + 16);
     stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
-    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 1, L.pairs_cap);
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 1, L.pairs_cap, kCoopWarps, af_width<RES>());
     int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
     float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
     int *run_pend = reinterpret_cast<int *>(smem_raw + lay.run_pend);   // end of run r in rowsA, in PAIRS of rows
@@ -377,6 +530,28 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                 longest = max(longest, (p >> 1) - p_begin);
                 start = end + 1;
             }
+        }
+    }
+    if (af_width<RES>() > 0) {
+        // fp32 image of the constraints for the set-up's search (fast_rung_rows), and max_i |a_i| for its Lipschitz slack
+        float4 *af = reinterpret_cast<float4 *>(smem_raw + lay.af);
+        float am = 0.f;
+        for (int i = threadIdx.x; i < n; i += kCoopThreads) {
+            const double *row = rows + i * ROW;
+            const float b2 = (float)row[RS::BETA + 1];
+            if (RES == CLOSURE_REG_3D3D) {
+                af[i] = make_float4((float)row[0], (float)row[1], (float)row[2], b2);
+                am = fmaxf(am, (float)sqrt(row[0] * row[0] + row[1] * row[1] + row[2] * row[2]) * 1.000001f);
+            } else {
+                af[3 * i] = make_float4((float)row[0], (float)row[1], (float)row[2], b2);
+                af[3 * i + 1] = make_float4((float)row[3], (float)row[4], (float)row[5], 0.f);
+                af[3 * i + 2] = make_float4((float)row[6], (float)row[7], (float)row[8], 0.f);
+            }
+        }
+        if (RES == CLOSURE_REG_3D3D) {
+            if (threadIdx.x == 0) amax_s = 0.f;
+            __syncthreads();
+            atomicMax(reinterpret_cast<unsigned int *>(&amax_s), __float_as_uint(wmax_nonneg(am)));   // non-negative floats order as uints
         }
     }
     __syncthreads();
@@ -459,7 +634,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
         // ================================================== set-up at the current pose (only after a move)
         if (moved) {
             const long long c0 = stats ? clock64() : 0ll;
-            coop_setup_on_move<RES>(smem_raw, warp, lane, rows_bytes, n, n_t, NQ, L.pairs_cap, t_p, stats);
+            coop_setup_on_move<RES>(smem_raw, warp, lane, rows_bytes, n, n_t, NQ, L.pairs_cap, t_p, amax_s, stats);
             if (stats) stc[10] += (unsigned long long)(clock64() - c0);
             epsA = (float)pose[16];
             rot_margin = pose[15];
@@ -720,7 +895,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
 template <int RES, int NQ>
 cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
 {
-    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 1, L.pairs_cap);
+    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 1, L.pairs_cap, kCoopWarps, af_width<RES>());
     if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaFuncSetAttribute(walker_dense_kernel<RES, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)lay.total);
