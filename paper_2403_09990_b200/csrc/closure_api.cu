@@ -309,6 +309,8 @@ int closure_set_params(closure_t *h, const closure_params *p)
         return fail(h, CLOSURE_EUNSUPPORTED, "a body pivot is set: Alg. A8 has no update_rotation (clear it with closure_set_pivot first)");
     if (plain_kernel_smem_bytes(h->h_desc.rows_bytes, p->n_t) > kMaxStageBytes)
         return fail(h, CLOSURE_EUNSUPPORTED, "constraint table and ladder do not fit shared memory for this n and n_t");
+    if (p->precision == 32 && (h->type == CLOSURE_REG_3D3D_ELL || h->type == CLOSURE_REPROJ_2D3D_ELL))
+        return fail(h, CLOSURE_EUNSUPPORTED, "fp32 mode does not exist for the ellipse / ellipsoid norms");
     h->P = *p;
     return CLOSURE_OK;
 }
@@ -323,6 +325,7 @@ int closure_create(int residual_type, const double *measurements, int n, const d
     std::string why;
     int rc = check_params(p, &why);
     if (rc != CLOSURE_OK) return rc;
+    if (p->precision == 32 && (residual_type == CLOSURE_REG_3D3D_ELL || residual_type == CLOSURE_REPROJ_2D3D_ELL)) return CLOSURE_EUNSUPPORTED;
     // every instance must be stageable by the kernel of last resort (rows + per-thread ladder table)
     if (plain_kernel_smem_bytes(n * row_doubles(residual_type) * 8, p->n_t) > kMaxStageBytes) return CLOSURE_EUNSUPPORTED;
     const int nb = residual_type == CLOSURE_POSE_REG_SPLIT ? 2 * n : n;

@@ -27,7 +27,7 @@ struct CoopSmem {
 // af_f4 > 0 (dense kernel, Ex.2: 1, Ex.3: 3): a CTA-level fp32 image of the constraints (af_f4 float4 per row) and per warp the
 // fp32 rung rotations (rm32) and the indices of each rung's screening rows (ridx), for the fp32 search of the set-up
 __host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, int nq, int f4, int pairs, int warps = kCoopWarps,
-                                                int af_f4 = 0)
+                                                int af_f4 = 0, int af_extra_bytes = 0)
 {
     CoopSmem s;
     size_t o = 16 + (size_t)((rows_bytes + 15) & ~15);
@@ -35,7 +35,7 @@ __host__ __device__ inline CoopSmem coop_layout(int rows_bytes, int n, int n_t, 
     s.run_bf = o;  o += (size_t)((n * 4 + 15) & ~15);
     s.run_pend = o; o += (size_t)((n * 4 + 15) & ~15);
     s.pos = o;     o += (size_t)((n * 4 + 15) & ~15);
-    s.af = o;      o += (size_t)n * 16 * af_f4;
+    s.af = o;      o += (size_t)n * 16 * af_f4 + (size_t)((af_extra_bytes + 15) & ~15);
     s.warp0 = o;
     size_t w = 0;
     s.rowsA = w; w += (size_t)pairs * 32;          // affine: pair-transposed, runs padded to even length

@@ -65,6 +65,73 @@ __device__ __forceinline__ void screen_row(double u0, double u1, double u2, doub
     eps = mag * (kMu19 * 1.001f);
 }
 
+// ---------------------------------------------------------------------------------- ellipsoid norm (eq. (6), Lambda_i != I)
+// CLOSURE_REG_3D3D_ELL: |g|_L^2 = g^T L g with g = u - d, u = b - (R a + t*):
+//     (u - d)^T L (u - d) = c - 2 w.d + d^T L d,      w = L u,   c = u^T L u,
+// i.e. the affine form of Ex.2 with (w, c) in place of (u, |u|^2) plus a quadratic form in the perturbation whose six
+// coefficients are constants of the constraint.  With e = -2 d (what the lanes hold) the pair is
+//     v = c + e0 (w0 + Q00 e0 + Q01 e1 + Q02 e2) + e1 (w1 + Q11 e1 + Q12 e2) + e2 (w2 + Q22 e2),
+//     Q00 = L00/4, Q11 = L11/4, Q22 = L22/4, Q01 = L01/2, Q02 = L02/2, Q12 = L12/2              (9 FMA)
+// Error of the fp32 evaluation against the plain kernel's fp64 g^T (L g), for |e_a| <= 2 t_p, with
+// M = |c| + 2 t_p |w|_1 + (2 t_p)^2 sum|Q|:  nine FMA roundings (<= 9 2^-24 M), (w, c, Q) rounded to fp32 (<= 2^-24 M),
+// e from pm1f (6 2^-24 2 t_p per component, times |dv/de_a| <= |w_a| + 2 (2 t_p) sum_b |Q_ab|: <= 24 2^-24 M):
+// |v32 - v64| <= 34 2^-24 M.  eps = 2^-17 1.001 M leaves a factor 3.7.
+constexpr float kMu17 = 7.62939453125e-06f;   // 2^-17
+constexpr int kEll = CLOSURE_REG_3D3D_ELL;
+
+__device__ __forceinline__ void ell_setup(const double (&R)[9], const double (&t)[3], const double *row, double &w0, double &w1,
+                                          double &w2, double &c)
+{
+    const double a0 = row[0], a1 = row[1], a2 = row[2];
+    const double u0 = row[3] - (fma(R[0], a0, fma(R[1], a1, R[2] * a2)) + t[0]);
+    const double u1 = row[4] - (fma(R[3], a0, fma(R[4], a1, R[5] * a2)) + t[1]);
+    const double u2 = row[5] - (fma(R[6], a0, fma(R[7], a1, R[8] * a2)) + t[2]);
+    w0 = fma(row[8], u0, fma(row[9], u1, row[10] * u2));
+    w1 = fma(row[9], u0, fma(row[11], u1, row[12] * u2));
+    w2 = fma(row[10], u0, fma(row[12], u1, row[13] * u2));
+    c = fma(u2, w2, fma(u1, w1, u0 * w0));
+}
+
+// |Lambda_i|_F (>= its largest eigenvalue): |x|_Lambda^2 <= |Lambda|_F |x|^2, for the Lipschitz bound of a rung
+__device__ __forceinline__ double ell_lip_scale(const double *row)
+{
+    const double d = row[8] * row[8] + row[11] * row[11] + row[13] * row[13];
+    const double o = row[9] * row[9] + row[10] * row[10] + row[12] * row[12];
+    return sqrt(d + 2.0 * o) * 1.0000001;
+}
+
+// set-up of one constraint row at (R, t): (u, |u|^2 [+ |R - R_i|_F^2]) for the ball forms, (w, c) for the ellipsoid
+template <int RES>
+__device__ __forceinline__ void pair_setup(const double (&R)[9], const double (&t)[3], const double *row, double &u0, double &u1,
+                                           double &u2, double &c)
+{
+    if (RES == kEll) ell_setup(R, t, row, u0, u1, u2, c);
+    else affine_setup<RES>(R, t, row, u0, u1, u2, c);
+}
+
+// fp32 image and error bound of one row; qmag = (2 t_p)^2 sum|Q| of the constraint (ellipsoid only)
+template <int RES>
+__device__ __forceinline__ void screen_row_any(double u0, double u1, double u2, double c, float tp2, float tp2sq3, float qmag,
+                                               float &f0, float &f1, float &f2, float &fc, float &eps)
+{
+    if (RES == kEll) {
+        f0 = (float)u0; f1 = (float)u1; f2 = (float)u2; fc = (float)c;
+        const float mag = fabsf(fc) + tp2 * (fabsf(f0) + fabsf(f1) + fabsf(f2)) + qmag;
+        eps = mag * (kMu17 * 1.001f);
+    } else {
+        screen_row(u0, u1, u2, c, tp2, tp2sq3, f0, f1, f2, fc, eps);
+    }
+}
+
+// q(e) of the constraint whose coefficients are (A, B) = (Q00 Q01 Q02 Q11) (Q12 Q22 . .), plus the linear part w.e + cw
+__device__ __forceinline__ float ell_value(const float4 &r, const float4 &A, const float4 &B, const float4 &e)
+{
+    const float t0 = fmaf(A.z, e.z, fmaf(A.y, e.y, fmaf(A.x, e.x, r.x)));
+    const float t1 = fmaf(B.x, e.z, fmaf(A.w, e.y, r.y));
+    const float t2 = fmaf(B.y, e.z, r.z);
+    return fmaf(t0, e.x, fmaf(t1, e.y, fmaf(t2, e.z, r.w)));
+}
+
 // The plain kernel's phase A for the NQ perturbations of this lane (same arithmetic as
 // walker_kernel.cu): exact eq. (14) margins, one sqrt per run of equal bounds.  jv[q] < 0: empty.
 template <int RES, int NJ>
@@ -118,6 +185,19 @@ struct ExactMargin {
     double t_p, rot_margin;
     __device__ __forceinline__ double operator()(int j) const
     {
+        if (RES == kEll) {                            // the plain kernel's direct evaluation (walker_kernel.cu, non-affine branch)
+            double x, y, z;
+            rng.xi3(s, (uint32_t)j, 1u, x, y, z);
+            const double tj[3] = { t[0] + t_p * x, t[1] + t_p * y, t[2] + t_p * z };
+            const double K0[4] = { 0.0, 0.0, 0.0, 0.0 };
+            double d = rot_margin;
+#pragma unroll 1
+            for (int i = 0; i < n; ++i) {
+                const double *row = rows + i * Res<RES>::ROW;
+                d = dmin(d, row[Res<RES>::BETA] - sqrt(direct_sq<RES>(R, tj, row, K0, 0)));
+            }
+            return d;
+        }
         const int jv[1] = { j };
         double d[1];
         exact_margins<RES, 1>(R, t, rows, n, rng, s, t_p, rot_margin, jv, d);
@@ -136,6 +216,17 @@ __device__ __forceinline__ bool exact_candidate_feasible(const double (&Rm)[9], 
     double x, y, z;
     rng.xi3(s, (uint32_t)j, 1u, x, y, z);
     const double d0 = t_p * x, d1 = t_p * y, d2 = t_p * z;
+    if (RES == kEll) {                                // the plain kernel's direct ladder test
+        const double tk[3] = { t[0] + d0, t[1] + d1, t[2] + d2 };
+        const double K0[4] = { 0.0, 0.0, 0.0, 0.0 };
+        bool okl = true;
+#pragma unroll 1
+        for (int i = lane; i < n; i += 32) {
+            const double *row = rows + i * ROW;
+            if (!(direct_sq<RES>(Rm, tk, row, K0, 0) <= row[RS::BETA + 1])) okl = false;
+        }
+        return __all_sync(FULL, okl);
+    }
     const double kdd = -fma(d2, d2, fma(d1, d1, d0 * d0));
     const double k0 = -2.0 * d0, k1 = -2.0 * d1, k2 = -2.0 * d2;
     bool ok = true;
@@ -158,8 +249,10 @@ __device__ __forceinline__ bool exact_candidate_feasible(const double (&Rm)[9], 
 // Ex.2 (a_i, beta_i^2); Ex.3 stacked (R_i row 0, beta_i^2) (R_i row 1, 0) (R_i row 2, 0); split form: none (old search)
 template <int RES> __host__ __device__ constexpr int af_width()
 {
-    return RES == CLOSURE_REG_3D3D ? 1 : (RES == CLOSURE_POSE_REG ? 3 : 0);
+    return RES == CLOSURE_REG_3D3D ? 1 : (RES == CLOSURE_POSE_REG ? 3 : (RES == CLOSURE_REG_3D3D_ELL ? 2 : 0));
 }
+// ellipsoid: the table holds the quadratic-form coefficients instead, by constraint (2 float4) and by pair-entry (3 float4)
+template <int RES> __host__ __device__ constexpr int af_extra(int pairs) { return RES == CLOSURE_REG_3D3D_ELL ? pairs * 48 : 0; }
 
 // ---------------------------------------------------------------------------------- screening rows of every rung
 // Per rung the ladder screens its candidates against two constraint rows at R_m and against a Lipschitz bound.  ANY two
@@ -299,8 +392,8 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
 {
     using RS = Res<RES>;
     constexpr int ROW = RS::ROW;
-    constexpr bool FAST = af_width<RES>() > 0;          // fp32 search for the screening rows (below)
-    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, nq, 1, pairs, kCoopWarps, af_width<RES>());
+    constexpr bool FAST = RES == CLOSURE_REG_3D3D || RES == CLOSURE_POSE_REG;   // fp32 search for the screening rows (below)
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, nq, 1, pairs, kCoopWarps, af_width<RES>(), af_extra<RES>(pairs));
     const double *rows = reinterpret_cast<const double *>(smem_raw + 16);
     const int *pos = reinterpret_cast<const int *>(smem_raw + lay.pos);
     unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
@@ -313,6 +406,8 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
     unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
     const float tpf = (float)t_p * 1.0000002f;          // >= t_p
     const float tp2 = 2.0f * tpf, tp2sq3 = 3.0f * tpf * tpf;
+    const float4 *QL = reinterpret_cast<const float4 *>(smem_raw + lay.af);   // ellipsoid: (Q00 Q01 Q02 Q11) (Q12 Q22 qmag .) per constraint
+    int2 *ridx = reinterpret_cast<int2 *>(wp + lay.ridx);                      // ellipsoid: constraints of each rung's screening rows
     double R[9], t[3], vel[3];
 #pragma unroll
     for (int e = 0; e < 9; ++e) R[e] = pose[e];
@@ -324,9 +419,9 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
     for (int i = lane; i < n; i += 32) {
         const double *row = rows + i * ROW;
         double u0, u1, u2, c;
-        affine_setup<RES>(R, t, row, u0, u1, u2, c);
+        pair_setup<RES>(R, t, row, u0, u1, u2, c);
         float f0, f1, f2, fc, eps;
-        screen_row(u0, u1, u2, c, tp2, tp2sq3, f0, f1, f2, fc, eps);
+        screen_row_any<RES>(u0, u1, u2, c, tp2, tp2sq3, RES == kEll ? QL[2 * i + 1].z : 0.f, f0, f1, f2, fc, eps);
         {
             const int pp = pos[i], p = pp & 0x3fffffff;
             float *A = reinterpret_cast<float *>(rowsA) + (p >> 1) * 8 + (p & 1);
@@ -378,12 +473,13 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
 #pragma unroll
             for (int e = 0; e < 9; ++e) { Rm[e] = RmS[m * 9 + e]; dR[e] = Rm[e] - R[e]; }
             double u0, u1, u2, cc;
-            affine_setup<RES>(Rm, t, row, u0, u1, u2, cc);
-            if (RES == CLOSURE_REG_3D3D) {           // ||(R_m - R*) a_i||^2
+            pair_setup<RES>(Rm, t, row, u0, u1, u2, cc);
+            if (RES == CLOSURE_REG_3D3D || RES == kEll) {           // ||(R_m - R*) a_i||^2
                 const double q0 = dR[0] * row[0] + dR[1] * row[1] + dR[2] * row[2];
                 const double q1 = dR[3] * row[0] + dR[4] * row[1] + dR[5] * row[2];
                 const double q2 = dR[6] * row[0] + dR[7] * row[1] + dR[8] * row[2];
                 lip = q0 * q0 + q1 * q1 + q2 * q2;
+                if (RES == kEll) lip *= ell_lip_scale(row);          // ... in the norm of Lambda_i: |x|_L^2 <= |Lambda|_F |x|^2
             } else {
 #pragma unroll
                 for (int e = 0; e < 9; ++e) lip = fma(dR[e], dR[e], lip);      // ||R_m - R*||_F^2
@@ -391,7 +487,8 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
             bool rdead = false;
             if (RES == CLOSURE_POSE_REG_SPLIT) rdead = has && !(frob_sq(Rm, row) <= row[13]);
             float g0, g1, g2, fcb, eps;
-            screen_row(u0, u1, u2, cc - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
+            screen_row_any<RES>(u0, u1, u2, cc - row[RS::BETA + 1], tp2, tp2sq3, RES == kEll ? QL[2 * (has ? c : 0) + 1].z : 0.f,
+                                g0, g1, g2, fcb, eps);
             float4 r4 = make_float4(g0, g1, g2, has ? fcb - eps : -CUDART_INF_F);
             const uint32_t key = has ? ((fkey(r4.w) & ~15u) | (uint32_t)c) : (uint32_t)c;
             const uint32_t m1 = __reduce_max_sync(hm, key);
@@ -404,8 +501,9 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
                 qrow[2 * m] = r4;
                 qL[m] = lf * 1.001f + 1e-30f;
                 if (n == 1) qrow[2 * m + 1] = r4;
+                if (RES == kEll) { ridx[m].x = c; if (n == 1) ridx[m].y = c; }
             }
-            if (key2 == m2 && n > 1) qrow[2 * m + 1] = r4;
+            if (key2 == m2 && n > 1) { qrow[2 * m + 1] = r4; if (RES == kEll) ridx[m].y = c; }
         }
     } else {
 #pragma unroll 1
@@ -414,11 +512,12 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
 #pragma unroll
         for (int e = 0; e < 9; ++e) Rm[e] = RmS[m * 9 + e];
         float4 b1 = make_float4(0.f, 0.f, 0.f, -CUDART_INF_F), b2 = b1;
+        int jb1 = 0, jb2 = 0;                        // their constraints (the ellipsoid's screening needs the quadratic part)
         bool rdead = false;
         double dR[9], lip = 0.0;                     // max_i | ||g_i(R_m, .)|| - ||g_i(R*, .)|| | <= sqrt(lip)
 #pragma unroll
         for (int e = 0; e < 9; ++e) dR[e] = Rm[e] - R[e];
-        if (RES != CLOSURE_REG_3D3D) {
+        if (RES != CLOSURE_REG_3D3D && RES != kEll) {
 #pragma unroll
             for (int e = 0; e < 9; ++e) lip = fma(dR[e], dR[e], lip);      // ||R_m - R*||_F^2
         }
@@ -426,20 +525,20 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
         for (int i = lane; i < n; i += 32) {
             const double *row = rows + i * ROW;
             double u0, u1, u2, c;
-            affine_setup<RES>(Rm, t, row, u0, u1, u2, c);
-            if (RES == CLOSURE_REG_3D3D) {           // ||(R_m - R*) a_i||^2
+            pair_setup<RES>(Rm, t, row, u0, u1, u2, c);
+            if (RES == CLOSURE_REG_3D3D || RES == kEll) {           // ||(R_m - R*) a_i||^2
                 const double q0 = dR[0] * row[0] + dR[1] * row[1] + dR[2] * row[2];
                 const double q1 = dR[3] * row[0] + dR[4] * row[1] + dR[5] * row[2];
                 const double q2 = dR[6] * row[0] + dR[7] * row[1] + dR[8] * row[2];
-                lip = dmax(lip, q0 * q0 + q1 * q1 + q2 * q2);
+                lip = dmax(lip, (q0 * q0 + q1 * q1 + q2 * q2) * (RES == kEll ? ell_lip_scale(row) : 1.0));
             }
             if (RES == CLOSURE_POSE_REG_SPLIT) {
                 if (!(frob_sq(Rm, row) <= row[13])) rdead = true;
             }
             float g0, g1, g2, fcb, eps;
-            screen_row(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
+            screen_row_any<RES>(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, RES == kEll ? QL[2 * i + 1].z : 0.f, g0, g1, g2, fcb, eps);
             const float4 r4 = make_float4(g0, g1, g2, fcb - eps);
-            if (r4.w > b1.w) { b2 = b1; b1 = r4; } else if (r4.w > b2.w) b2 = r4;
+            if (r4.w > b1.w) { b2 = b1; jb2 = jb1; b1 = r4; jb1 = i; } else if (r4.w > b2.w) { b2 = r4; jb2 = i; }
         }
         const uint32_t k1 = fkey(b1.w);
         const uint32_t m1 = __reduce_max_sync(FULL, k1);
@@ -450,6 +549,11 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
         if (__any_sync(FULL, rdead)) b1.w = CUDART_INF_F;          // rung dead for every candidate
         if (lane == src1) qrow[2 * m] = b1;
         if (lane == src2) qrow[2 * m + 1] = (lane == src1) ? b2 : b1;
+        if (RES == kEll) {
+            const int i1 = __shfl_sync(FULL, jb1, src1);
+            const int i2 = __shfl_sync(FULL, src2 == src1 ? jb2 : jb1, src2);
+            if (lane == 0) ridx[m] = make_int2(i1, i2);
+        }
         const float lf = wmax_nonneg((float)sqrt(lip));
         if (lane == 0) qL[m] = lf * 1.001f + 1e-30f;
     }
@@ -492,7 +596,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
     double *rows = reinterpret_cast<double *>(smem_raw + 16);
     stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
-    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 1, L.pairs_cap, kCoopWarps, af_width<RES>());
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 1, L.pairs_cap, kCoopWarps, af_width<RES>(), af_extra<RES>(L.pairs_cap));
     int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
     float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
     int *run_pend = reinterpret_cast<int *>(smem_raw + lay.run_pend);   // end of run r in rowsA, in PAIRS of rows
@@ -532,7 +636,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
             }
         }
     }
-    if (af_width<RES>() > 0) {
+    if (RES == CLOSURE_REG_3D3D || RES == CLOSURE_POSE_REG) {
         // fp32 image of the constraints for the set-up's search (fast_rung_rows), and max_i |a_i| for its Lipschitz slack
         float4 *af = reinterpret_cast<float4 *>(smem_raw + lay.af);
         float am = 0.f;
@@ -556,6 +660,24 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     }
     __syncthreads();
     const int n_runs = n_runs_s;
+    if (RES == kEll) {
+        float4 *QLw = reinterpret_cast<float4 *>(smem_raw + lay.af);
+        float *QAw = reinterpret_cast<float *>(QLw + 2 * n);
+        const float tpq = (float)L.t_p * 1.0000002f;
+        for (int i = threadIdx.x; i < n; i += kCoopThreads) {
+            const double *row = rows + i * ROW;
+            const float q00 = (float)(0.25 * row[8]), q01 = (float)(0.5 * row[9]), q02 = (float)(0.5 * row[10]);
+            const float q11 = (float)(0.25 * row[11]), q12 = (float)(0.5 * row[12]), q22 = (float)(0.25 * row[13]);
+            const float qsum = (fabsf(q00) + fabsf(q01) + fabsf(q02) + fabsf(q11) + fabsf(q12) + fabsf(q22)) * 1.000001f;
+            QLw[2 * i] = make_float4(q00, q01, q02, q11);
+            QLw[2 * i + 1] = make_float4(q12, q22, 4.0f * tpq * tpq * qsum, 0.f);     // qmag = (2 t_p)^2 sum|Q|
+            const int pp = pos[i], p = pp & 0x3fffffff;
+            float *A = QAw + (p >> 1) * 12 + (p & 1);           // (Q00a Q00b Q01a Q01b) (Q02a Q02b Q11a Q11b) (Q12a Q12b Q22a Q22b)
+            A[0] = q00; A[2] = q01; A[4] = q02; A[6] = q11; A[8] = q12; A[10] = q22;
+            if (pp & 0x40000000) { A[1] = q00; A[3] = q01; A[5] = q02; A[7] = q11; A[9] = q12; A[11] = q22; }
+        }
+        __syncthreads();
+    }
 
     const long long local = (long long)blockIdx.x * kCoopWarps + warp;
     if (local >= L.num_walkers) return;                // no block-wide barrier below this line
@@ -572,6 +694,10 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     int *candj = reinterpret_cast<int *>(wp + lay.candj);
     float *candd = reinterpret_cast<float *>(wp + lay.candd);     // upper bounds of the candidates' eq. (14) values
     double *pose = reinterpret_cast<double *>(wp + lay.pose);     // R*(9) t*(3) omega(3): fp64, touched only on moves / fp64 paths
+    // ellipsoid norm: quadratic-form coefficients of the constraints, by constraint (QL) and by pair-entry of rowsA (QA)
+    const float4 *QL = reinterpret_cast<const float4 *>(smem_raw + lay.af);
+    const float4 *QA = QL + 2 * n;
+    const int2 *ridx = reinterpret_cast<const int2 *>(wp + lay.ridx);
 
     const unsigned long long w = (unsigned long long)(L.walker_begin + local);
     const unsigned long long seed = L.seed[blockIdx.y];
@@ -669,7 +795,8 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
             if (ODD) { e0[NQ - 1] = m2tp * pm1f(x[NQ - 1]); e1[NQ - 1] = m2tp * pm1f(y[NQ - 1]); e2[NQ - 1] = m2tp * pm1f(z[NQ - 1]); }
 #pragma unroll
             for (int q = 0; q < NQ; ++q) {
-                dd[q] = 0.25f * fmaf(e2[q], e2[q], fmaf(e1[q], e1[q], e0[q] * e0[q]));
+                // (ellipsoid: the pair carries its own quadratic form d^T Lambda_i d, nothing is added per run and thresholds are 0)
+                dd[q] = RES == kEll ? 0.f : 0.25f * fmaf(e2[q], e2[q], fmaf(e1[q], e1[q], e0[q] * e0[q]));
                 pert[32 * q + lane] = make_float4(e0[q], e1[q], e2[q], -dd[q]);
             }
             if (ODD) { o0 = e0[NQ - 1]; o1 = e1[NQ - 1]; o2 = e2[NQ - 1]; }
@@ -693,6 +820,37 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                 for (; pp < pend; ++pp) {
                     // two constraints a, b per entry: X = (f0a f0b f1a f1b), Y = (f2a f2b fca fcb)
                     const float4 X = rowsA[2 * pp], Y = rowsA[2 * pp + 1];
+                    if (RES == kEll) {
+                        // (w, c) as above plus the quadratic form: U = (Q00a Q00b Q01a Q01b) V = (Q02a Q02b Q11a Q11b) W = (Q12a Q12b Q22a Q22b)
+                        const float4 U = QA[3 * pp], V = QA[3 * pp + 1], W = QA[3 * pp + 2];
+#pragma unroll
+                        for (int k = 0; k < NPK; ++k) {
+                            const unsigned long long ta0 = fma2(pk2(V.x, V.x), p2[k], fma2(pk2(U.z, U.z), p1[k], fma2(pk2(U.x, U.x), p0[k], pk2(X.x, X.x))));
+                            const unsigned long long ta1 = fma2(pk2(W.x, W.x), p2[k], fma2(pk2(V.z, V.z), p1[k], pk2(X.z, X.z)));
+                            const unsigned long long ta2 = fma2(pk2(W.z, W.z), p2[k], pk2(Y.x, Y.x));
+                            const unsigned long long va = fma2(ta0, p0[k], fma2(ta1, p1[k], fma2(ta2, p2[k], pk2(Y.z, Y.z))));
+                            const unsigned long long tb0 = fma2(pk2(V.y, V.y), p2[k], fma2(pk2(U.w, U.w), p1[k], fma2(pk2(U.y, U.y), p0[k], pk2(X.y, X.y))));
+                            const unsigned long long tb1 = fma2(pk2(W.y, W.y), p2[k], fma2(pk2(V.w, V.w), p1[k], pk2(X.w, X.w)));
+                            const unsigned long long tb2 = fma2(pk2(W.w, W.w), p2[k], pk2(Y.y, Y.y));
+                            const unsigned long long vb = fma2(tb0, p0[k], fma2(tb1, p1[k], fma2(tb2, p2[k], pk2(Y.w, Y.w))));
+                            float la, ha, lb, hb;
+                            upk2(va, la, ha);
+                            upk2(vb, lb, hb);
+                            mx[2 * k] = fmaxf(mx[2 * k], fmaxf(la, lb));
+                            mx[2 * k + 1] = fmaxf(mx[2 * k + 1], fmaxf(ha, hb));
+                        }
+                        if (ODD) {                      // the odd slot takes both constraints in one packed chain
+                            const unsigned long long E0o = pk2(o0, o0), E1o = pk2(o1, o1), E2o = pk2(o2, o2);
+                            const unsigned long long t0 = fma2(pk2(V.x, V.y), E2o, fma2(pk2(U.z, U.w), E1o, fma2(pk2(U.x, U.y), E0o, pk2(X.x, X.y))));
+                            const unsigned long long t1 = fma2(pk2(W.x, W.y), E2o, fma2(pk2(V.z, V.w), E1o, pk2(X.z, X.w)));
+                            const unsigned long long t2 = fma2(pk2(W.z, W.w), E2o, pk2(Y.x, Y.y));
+                            const unsigned long long vo = fma2(t0, E0o, fma2(t1, E1o, fma2(t2, E2o, pk2(Y.z, Y.w))));
+                            float lo, hi;
+                            upk2(vo, lo, hi);
+                            mx[NQ - 1] = fmaxf(mx[NQ - 1], fmaxf(lo, hi));
+                        }
+                        continue;
+                    }
 #pragma unroll
                     for (int k = 0; k < NPK; ++k) {
                         const unsigned long long va =
@@ -768,11 +926,21 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                 const float4 r0 = qrow[2 * mq], r1 = qrow[2 * mq + 1];
                 Lm = qL[mq];
                 const int k1 = min(KP, (hq + 1) * khalf);
+                if (RES == kEll) {
+                    const int2 ii = ridx[mq];
+                    const float4 A0 = QL[2 * ii.x], B0 = QL[2 * ii.x + 1], A1 = QL[2 * ii.y], B1 = QL[2 * ii.y + 1];
+                    for (int k = hq * khalf; k < k1; ++k) {
+                        const float4 c4 = cand4[k];
+                        const float v0 = ell_value(r0, A0, B0, c4), v1 = ell_value(r1, A1, B1, c4);
+                        if (!(v0 > c4.w) && !(v1 > c4.w) && !(candd[k] + Lm < 0.f)) alive |= 1u << k;
+                    }
+                } else {
                 for (int k = hq * khalf; k < k1; ++k) {
                     const float4 c4 = cand4[k];
                     const float v0 = fmaf(r0.x, c4.x, fmaf(r0.y, c4.y, fmaf(r0.z, c4.z, r0.w)));
                     const float v1 = fmaf(r1.x, c4.x, fmaf(r1.y, c4.y, fmaf(r1.z, c4.z, r1.w)));
                     if (!(v0 > c4.w) && !(v1 > c4.w) && !(candd[k] + Lm < 0.f)) alive |= 1u << k;
+                }
                 }
             }
             alive |= __shfl_xor_sync(FULL, alive, 16);
@@ -805,12 +973,13 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                     for (int i = lane; i < n; i += 32) {
                         const double *row = rows + i * ROW;
                         double u0, u1, u2, c;
-                        affine_setup<RES>(Rm, t, row, u0, u1, u2, c);
+                        pair_setup<RES>(Rm, t, row, u0, u1, u2, c);
                         if (RES == CLOSURE_POSE_REG_SPLIT) {
                             if (!(frob_sq(Rm, row) <= row[13])) rdead = true;     // exact: no perturbation involved
                         }
                         float g0, g1, g2, fcb, eps;
-                        screen_row(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
+                        screen_row_any<RES>(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, RES == kEll ? QL[2 * i + 1].z : 0.f,
+                                            g0, g1, g2, fcb, eps);
                         rowsL[i] = make_float4(g0, g1, g2, fcb - eps);
                         eps_l = fmaxf(eps_l, eps);
                     }
@@ -829,7 +998,8 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                         c4 = cand4[ek];
                         for (int i = ech; i < n; i += NCH) {
                             const float4 f = rowsL[i];
-                            M = fmaxf(M, fmaf(f.x, c4.x, fmaf(f.y, c4.y, fmaf(f.z, c4.z, f.w))));
+                            if (RES == kEll) M = fmaxf(M, ell_value(f, QL[2 * i], QL[2 * i + 1], c4));
+                            else M = fmaxf(M, fmaf(f.x, c4.x, fmaf(f.y, c4.y, fmaf(f.z, c4.z, f.w))));
                         }
                         M = fkey_inv(__reduce_max_sync(e_mask, fkey(M)));
                     }
@@ -895,7 +1065,7 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
 template <int RES, int NQ>
 cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
 {
-    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 1, L.pairs_cap, kCoopWarps, af_width<RES>());
+    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 1, L.pairs_cap, kCoopWarps, af_width<RES>(), af_extra<RES>(L.pairs_cap));
     if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaFuncSetAttribute(walker_dense_kernel<RES, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)lay.total);
@@ -925,6 +1095,7 @@ cudaError_t launch_walkers_coop_dense(int residual_type, const WalkLaunch &L, in
     case CLOSURE_REG_3D3D: return launch_r<CLOSURE_REG_3D3D>(L, n_instances, max_rows_bytes, max_n, stream);
     case CLOSURE_POSE_REG: return launch_r<CLOSURE_POSE_REG>(L, n_instances, max_rows_bytes, max_n, stream);
     case CLOSURE_POSE_REG_SPLIT: return launch_r<CLOSURE_POSE_REG_SPLIT>(L, n_instances, max_rows_bytes, max_n, stream);
+    case CLOSURE_REG_3D3D_ELL: return launch_r<CLOSURE_REG_3D3D_ELL>(L, n_instances, max_rows_bytes, max_n, stream);
     default: return cudaErrorInvalidValue;
     }
 }

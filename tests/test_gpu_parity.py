@@ -438,6 +438,45 @@ def test_ellipsoidal_noise_bounds(config, mode):
         assert_parity(inst, _small(P, pivot=(0.2, 0.1, -0.3)), S0, 96, 20, 24)
 
 
+@pytest.mark.parametrize("flags", [0, 2, 4, 6, 20])
+@pytest.mark.parametrize("config,n_p,n_p_star,n_t,walkers,steps", [(2, 150, 10, 15, 2048, 100), (1, 150, 10, 15, 1024, 120),
+                                                                   (5, 20, 2, 5, 1024, 100), (2, 33, 20, 17, 512, 60)])
+def test_ellipsoid_certified_kernel_is_bit_identical_to_plain_kernel(config, n_p, n_p_star, n_t, walkers, steps, flags):
+    """Ex.2 with the ellipsoid norm on the certified fp32 kernel (walker_dense_kernel<REG_3D3D_ELL>: the pair carries the
+    quadratic form d^T Lambda_i d): outputs and traces equal the plain fp64 kernel's bit for bit -- on a long and a short table,
+    with few perturbations, a ladder longer than one screening block, and with every fp64 fall-back forced (flags 2, 4, 16)."""
+    inst = I.to_ellipsoidal(I.make_instance(config), 7)
+    S0 = I.make_init_poses(inst, 64)
+    P = _small(inst.params, n_p=n_p, n_p_star=n_p_star, n_t=n_t)
+    fast = gpu_walk(inst, _small(P, flags=flags), S0, walkers, steps, 4343)
+    plain = gpu_walk(inst, _small(P, flags=1), S0, walkers, steps, 4343)
+    for a, b in zip(fast, plain):
+        assert np.array_equal(a, b)
+    if flags == 0:                                                      # the certificates carry most iterations
+        h = B.Closure.closure_create(inst, P)
+        try:
+            h.closure_set_init(S0)
+            h.closure_enable_stats(True)
+            h.closure_sample(walkers, steps, 4343)
+            st = h.closure_get_stats()
+        finally:
+            h.closure_destroy()
+        assert st["perturb_pairs_f32"] > 0 and st["fallback_steps"] < 0.2 * st["walker_steps"], st
+
+
+def test_ellipsoid_with_several_bounds_and_a_pivot():
+    """Runs of equal bounds of odd length and a body pivot on the ellipsoid kernel, against the oracle and the plain kernel."""
+    inst = I.to_ellipsoidal(_three_bounds(77, 901, (25, 31, 21)), 8)
+    P = _small(inst.params, n_p=64, n_p_star=5, n_t=9, t_p=0.05)
+    S0 = I.make_init_poses(inst, 16)
+    assert_parity(inst, P, S0, 96, 20, 31)
+    assert_parity(inst, _small(P, pivot=(0.3, -0.2, 0.1)), S0, 64, 16, 32)
+    fast = gpu_walk(inst, P, S0, 2048, 80, 55)
+    plain = gpu_walk(inst, _small(P, flags=1), S0, 2048, 80, 55)
+    for a, b in zip(fast, plain):
+        assert np.array_equal(a, b)
+
+
 def test_ellipsoidal_api_edges():
     import torch
     from oracle import step1
