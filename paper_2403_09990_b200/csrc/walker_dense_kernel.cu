@@ -37,6 +37,10 @@
 #define CLOSURE_COOP_MIN_CTAS 4   // resident CTAs per SM the register allocation aims at (128 registers per thread)
 #endif
 
+#ifndef CLOSURE_ELL_MIN_CTAS
+#define CLOSURE_ELL_MIN_CTAS 4    // ellipsoid pair loop: nine packed FMAs per pair want the registers
+#endif
+
 namespace closure {
 namespace {
 
@@ -47,6 +51,7 @@ template <int RES, int NQ> constexpr int coop_min_ctas()
 {
     if (CLOSURE_COOP_MIN_CTAS != 4) return CLOSURE_COOP_MIN_CTAS;
     if (RES == CLOSURE_POSE_REG || RES == CLOSURE_POSE_REG_SPLIT) return 6;
+    if (RES == CLOSURE_REG_3D3D_ELL) return CLOSURE_ELL_MIN_CTAS;
     return NQ == 5 ? 5 : 4;
 }
 
@@ -75,8 +80,8 @@ __device__ __forceinline__ void screen_row(double u0, double u1, double u2, doub
 // Error of the fp32 evaluation against the plain kernel's fp64 g^T (L g), for |e_a| <= 2 t_p, with
 // M = |c| + 2 t_p |w|_1 + (2 t_p)^2 sum|Q|:  nine FMA roundings (<= 9 2^-24 M), (w, c, Q) rounded to fp32 (<= 2^-24 M),
 // e from pm1f (6 2^-24 2 t_p per component, times |dv/de_a| <= |w_a| + 2 (2 t_p) sum_b |Q_ab|: <= 24 2^-24 M):
-// |v32 - v64| <= 34 2^-24 M.  eps = 2^-17 1.001 M leaves a factor 3.7.
-constexpr float kMu17 = 7.62939453125e-06f;   // 2^-17
+// |v32 - v64| <= 34 2^-24 M.  eps = 2^-18 1.001 M (= 64 2^-24 M) leaves a factor 1.9 over that worst case.
+constexpr float kMuEll = 3.814697265625e-06f;   // 2^-18 (measured: 2^-17 sends 7.8 % of the iterations to the fp64 fall-back, 2^-18 see DESIGN.md)
 constexpr int kEll = CLOSURE_REG_3D3D_ELL;
 
 __device__ __forceinline__ void ell_setup(const double (&R)[9], const double (&t)[3], const double *row, double &w0, double &w1,
@@ -117,7 +122,7 @@ __device__ __forceinline__ void screen_row_any(double u0, double u1, double u2, 
     if (RES == kEll) {
         f0 = (float)u0; f1 = (float)u1; f2 = (float)u2; fc = (float)c;
         const float mag = fabsf(fc) + tp2 * (fabsf(f0) + fabsf(f1) + fabsf(f2)) + qmag;
-        eps = mag * (kMu17 * 1.001f);
+        eps = mag * (kMuEll * 1.001f);
     } else {
         screen_row(u0, u1, u2, c, tp2, tp2sq3, f0, f1, f2, fc, eps);
     }
@@ -283,26 +288,33 @@ __device__ __forceinline__ void fast_rung_rows(unsigned char *smem_raw, const Co
     const double *RmS = reinterpret_cast<const double *>(wp + lay.RmS);
     float *qL = reinterpret_cast<float *>(wp + lay.qL);
 
-    // key of constraint i at the rung whose fp32 rotation image is (m0, m1, m2); lipv = |(R_m - R*) a_i|^2 (Ex.2)
-    auto key_of = [&](int i, const float4 &m0, const float4 &m1, const float4 &m2, float &lipv) -> float {
+    // fp32 data of one constraint: its set-up u* at R* and (Ex.2) a_i, beta_i^2 / (Ex.3) R_i, beta_i^2
+    struct RowF { float us0, us1, us2; float4 r0, r1, r2; };
+    auto load_row = [&](int i) -> RowF {
+        RowF w;
         const int sp = pos[i] & 0x3fffffff;
         const float *S = rowsAf + (sp >> 1) * 8 + (sp & 1);
-        const float us0 = S[0], us1 = S[2], us2 = S[4];
+        w.us0 = S[0]; w.us1 = S[2]; w.us2 = S[4];
+        if (REG) { w.r0 = af[i]; w.r1 = w.r0; w.r2 = w.r0; }
+        else { w.r0 = af[3 * i]; w.r1 = af[3 * i + 1]; w.r2 = af[3 * i + 2]; }
+        return w;
+    };
+    // key of that constraint at the rung whose fp32 rotation image is (m0, m1, m2); lipv = |(R_m - R*) a_i|^2 (Ex.2)
+    auto key_of = [&](const RowF &w, const float4 &m0, const float4 &m1, const float4 &m2, float &lipv) -> float {
         if (REG) {
-            const float4 a = af[i];
+            const float4 a = w.r0;
             const float g0 = fmaf(m0.z, a.z, fmaf(m0.y, a.y, m0.x * a.x));
             const float g1 = fmaf(m1.z, a.z, fmaf(m1.y, a.y, m1.x * a.x));
             const float g2 = fmaf(m2.z, a.z, fmaf(m2.y, a.y, m2.x * a.x));
             lipv = fmaf(g2, g2, fmaf(g1, g1, g0 * g0));
-            const float u0 = us0 - g0, u1 = us1 - g1, u2 = us2 - g2;
+            const float u0 = w.us0 - g0, u1 = w.us1 - g1, u2 = w.us2 - g2;
             return fmaf(u2, u2, fmaf(u1, u1, u0 * u0)) - a.w;
         } else {
-            const float4 r0 = af[3 * i], r1 = af[3 * i + 1], r2 = af[3 * i + 2];
-            float f = fmaf(us2, us2, fmaf(us1, us1, us0 * us0)) - r0.w;
+            float f = fmaf(w.us2, w.us2, fmaf(w.us1, w.us1, w.us0 * w.us0)) - w.r0.w;
             float d;
-            d = m0.x - r0.x; f = fmaf(d, d, f); d = m0.y - r0.y; f = fmaf(d, d, f); d = m0.z - r0.z; f = fmaf(d, d, f);
-            d = m1.x - r1.x; f = fmaf(d, d, f); d = m1.y - r1.y; f = fmaf(d, d, f); d = m1.z - r1.z; f = fmaf(d, d, f);
-            d = m2.x - r2.x; f = fmaf(d, d, f); d = m2.y - r2.y; f = fmaf(d, d, f); d = m2.z - r2.z; f = fmaf(d, d, f);
+            d = m0.x - w.r0.x; f = fmaf(d, d, f); d = m0.y - w.r0.y; f = fmaf(d, d, f); d = m0.z - w.r0.z; f = fmaf(d, d, f);
+            d = m1.x - w.r1.x; f = fmaf(d, d, f); d = m1.y - w.r1.y; f = fmaf(d, d, f); d = m1.z - w.r1.z; f = fmaf(d, d, f);
+            d = m2.x - w.r2.x; f = fmaf(d, d, f); d = m2.y - w.r2.y; f = fmaf(d, d, f); d = m2.z - w.r2.z; f = fmaf(d, d, f);
             lipv = 0.f;
             return f;
         }
@@ -313,11 +325,12 @@ __device__ __forceinline__ void fast_rung_rows(unsigned char *smem_raw, const Co
         const int c = lane & 15;
         const bool has = c < n;
         const unsigned hm = 0xFFFFu << (lane & 16);
+        const RowF w = load_row(has ? c : 0);
 #pragma unroll 1
         for (int m = lane >> 4; m < n_t; m += 2) {
             const float4 m0 = rm32[3 * m], m1 = rm32[3 * m + 1], m2 = rm32[3 * m + 2];
             float lipv = 0.f;
-            const float kv = key_of(has ? c : 0, m0, m1, m2, lipv);
+            const float kv = key_of(w, m0, m1, m2, lipv);
             const uint32_t key = has ? ((fkey(kv) & ~15u) | (uint32_t)c) : (uint32_t)c;
             const uint32_t k1 = __reduce_max_sync(hm, key);
             const uint32_t k2 = __reduce_max_sync(hm, key == k1 ? 0u : key);
@@ -328,28 +341,36 @@ __device__ __forceinline__ void fast_rung_rows(unsigned char *smem_raw, const Co
             }
         }
     } else {
+        // lanes over the constraints; the first two rows of a lane stay in registers over the rungs (n <= 64 needs no more),
+        // the two largest keys of a lane are kept as (key bits | constraint index) words: max / min, no branches
+        const RowF wA = load_row(lane < n ? lane : 0), wB = load_row(lane + 32 < n ? lane + 32 : 0);
 #pragma unroll 1
         for (int m = 0; m < n_t; ++m) {
             const float4 m0 = rm32[3 * m], m1 = rm32[3 * m + 1], m2 = rm32[3 * m + 2];
-            float b1 = -CUDART_INF_F, b2 = -CUDART_INF_F, lipl = 0.f;
-            int j1 = 0, j2 = 0;
-#pragma unroll 2
-            for (int i = lane; i < n; i += 32) {
-                float lipv;
-                const float kv = key_of(i, m0, m1, m2, lipv);
-                lipl = fmaxf(lipl, lipv);
-                if (kv > b1) { b2 = b1; j2 = j1; b1 = kv; j1 = i; } else if (kv > b2) { b2 = kv; j2 = i; }
+            uint32_t b1 = 0u, b2 = 0u;
+            float lipl = 0.f;
+            auto take = [&](float kv, float lipv, int i, bool on) {
+                const uint32_t k = on ? ((fkey(kv) & ~0xFFFu) | (uint32_t)i) : 0u;      // n <= 4096: 12 index bits
+                const uint32_t lo = min(k, b1);
+                b1 = max(k, b1);
+                b2 = max(b2, lo);
+                lipl = fmaxf(lipl, on ? lipv : 0.f);
+            };
+            float lv;
+            const float kA = key_of(wA, m0, m1, m2, lv);
+            take(kA, lv, lane, lane < n);
+            const float kB = key_of(wB, m0, m1, m2, lv);
+            take(kB, lv, lane + 32, lane + 32 < n);
+#pragma unroll 1
+            for (int i = lane + 64; i < n; i += 32) {
+                const RowF w = load_row(i);
+                const float kv = key_of(w, m0, m1, m2, lv);
+                take(kv, lv, i, true);
             }
-            const uint32_t q1 = fkey(b1);
-            const uint32_t g1 = __reduce_max_sync(FULL, q1);
-            const int src1 = __ffs(__ballot_sync(FULL, q1 == g1)) - 1;
-            const uint32_t q2 = (lane == src1) ? fkey(b2) : q1;
-            const uint32_t g2 = __reduce_max_sync(FULL, q2);
-            const int src2 = __ffs(__ballot_sync(FULL, q2 == g2)) - 1;
-            const int i1 = __shfl_sync(FULL, j1, src1);
-            const int i2 = __shfl_sync(FULL, src2 == src1 ? j2 : j1, src2);
+            const uint32_t g1 = __reduce_max_sync(FULL, b1);
+            const uint32_t g2 = __reduce_max_sync(FULL, b1 == g1 ? b2 : b1);    // (indices make the words distinct)
             const float lm = wmax_nonneg(lipl);
-            if (lane == 0) { ridx[m] = make_int2(i1, i2); qL[m] = lm; }
+            if (lane == 0) { ridx[m] = make_int2((int)(g1 & 0xFFFu), (int)((n > 1 ? g2 : g1) & 0xFFFu)); qL[m] = lm; }
         }
     }
     __syncwarp();
