@@ -53,9 +53,9 @@ extern "C" {
  * Lambda_i = I for the first four (R-14).  The _ELL types carry the positive definite Lambda_i of eq. (6)
  * (the ellipses / ellipsoids of PAPER.md:179-191): symmetric, positive definite
  * (CLOSURE_EINVAL otherwise).  Rotation sampler: CLOSURE_REG_3D3D_ELL runs on the warp-cooperative certified-fp32 kernel
- * (the pair carries the quadratic form d^T Lambda_i d; same decisions as the fp64 kernel, bit for bit),
- * CLOSURE_REPROJ_2D3D_ELL on the one-walker-per-thread fp64 kernel; translation sampler: the warp-cooperative fp64
- * kernel.  There is no fp32 mode (precision = 32) for them: CLOSURE_EUNSUPPORTED.
+ * (the pair carries the quadratic form d^T Lambda_i d; same decisions as the fp64 kernel, bit for bit), and so does
+ * CLOSURE_REPROJ_2D3D_ELL (rows whitened by the Cholesky factor of Lambda_i at every set-up); translation sampler: the
+ * warp-cooperative fp64 kernel.  There is no fp32 mode (precision = 32) for them: CLOSURE_EUNSUPPORTED.
  * Step I: as for the ball forms; the 2D point of Ex.1 is then uniform in the ellipse (R-24). */
 enum { CLOSURE_REPROJ_2D3D = 1, CLOSURE_REG_3D3D = 2, CLOSURE_POSE_REG = 3, CLOSURE_POSE_REG_SPLIT = 4,
        CLOSURE_REG_3D3D_ELL = 5, CLOSURE_REPROJ_2D3D_ELL = 6 };

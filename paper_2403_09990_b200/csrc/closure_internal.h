@@ -75,7 +75,8 @@ cudaError_t launch_walkers_coop_dense(int residual_type, const WalkLaunch &L, in
                                       cudaStream_t stream);
 
 // walker_coop_reproj_kernel.cu: the same organisation for the reprojection residual (ROT mode)
-cudaError_t launch_walkers_coop_reproj(const WalkLaunch &L, int n_instances, int max_rows_bytes, cudaStream_t stream);
+cudaError_t launch_walkers_coop_reproj(int residual_type, const WalkLaunch &L, int n_instances, int max_rows_bytes,
+                                       cudaStream_t stream);
 
 // walker_coop_trans_kernel.cu: warp-cooperative fp64 kernel for TRANS mode (Alg. A8), all residuals
 cudaError_t launch_walkers_coop_trans(int residual_type, const WalkLaunch &L, int n_instances, int max_rows_bytes,

@@ -1182,7 +1182,6 @@ cudaError_t launch_r(const WalkLaunch &L, int n_instances, int max_rows_bytes, i
 
 bool coop_path_available(int residual_type, int mode, int n_p, int max_n)
 {
-    if (residual_type == CLOSURE_REPROJ_2D3D_ELL) return false;   // fp64 kernels only (the ellipse norm of Ex.1)
     return mode == CLOSURE_MODE_ROT && n_p <= 256 && max_n <= 4096;
 }
 
@@ -1191,7 +1190,8 @@ cudaError_t launch_walkers_coop(int residual_type, const WalkLaunch &L, int n_in
 {
     const int max_n = max_rows_bytes / (row_doubles(residual_type) * 8);
     switch (residual_type) {
-    case CLOSURE_REPROJ_2D3D: return launch_walkers_coop_reproj(L, n_instances, max_rows_bytes, stream);
+    case CLOSURE_REPROJ_2D3D:
+    case CLOSURE_REPROJ_2D3D_ELL: return launch_walkers_coop_reproj(residual_type, L, n_instances, max_rows_bytes, stream);
     // the ellipsoid norm of Ex.2 (eq. (6), Lambda_i != I): the dense kernel with the quadratic form in the pair, any N_P
     case CLOSURE_REG_3D3D_ELL: return launch_walkers_coop_dense(residual_type, L, n_instances, max_rows_bytes, stream);
     default: break;

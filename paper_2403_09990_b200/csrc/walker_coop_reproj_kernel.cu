@@ -40,31 +40,52 @@ constexpr int kReprojThreads = 32 * kReprojWarps;
 // resident warps per SM the register allocation aims at: 20 (96 registers) measured best at C3 (16: 496, 20: 510, 24: 464 M)
 constexpr int kReprojMinCtas = (CLOSURE_COOP_MIN_CTAS == 4 ? 5 : CLOSURE_COOP_MIN_CTAS) * (kCoopWarps / kReprojWarps);
 
-constexpr int RES = CLOSURE_REPROJ_2D3D;
-constexpr int ROW = Res<RES>::ROW;
-constexpr int BETA = Res<RES>::BETA;
+// ELL = the ellipse norm of eq. (6) (CLOSURE_REPROJ_2D3D_ELL, rows [z Z beta beta^2 L00 L01 L11]): with the Cholesky factor
+// Lambda = L L^T,  g^T Lambda g = |L^T q|^2 / p_3^2, and q' = L^T q is again affine in the perturbation,
+//     q'_0 = A'_0 + a d_0 + b d_1 + c d_2,   q'_1 = A'_1 + d' d_1 + e d_2,
+//     A'_0 = l00 A_0 + l10 A_1, A'_1 = l11 A_1,  a = -l00 fx, b = -l10 fy, c = l00 zeta_0 + l10 zeta_1, d' = -l11 fy, e = l11 zeta_1
+// (the ball form is l00 = l11 = 1, l10 = 0: a = -fx, b = 0, c = zeta_0, d' = -fy, e = zeta_1).  Rows carry a third float4 with
+// (a, b, d'); one more FMA in q'_0, so E_q0 = u (4 |A'_0| + 10 t_p (|a| + |b| + |c|)); everything else is the ball form's bound.
+template <bool ELL> struct RJ {
+    static constexpr int RES = ELL ? CLOSURE_REPROJ_2D3D_ELL : CLOSURE_REPROJ_2D3D;
+    static constexpr int ROW = Res<RES>::ROW;
+    static constexpr int BETA = Res<RES>::BETA;
+    static constexpr int F4 = ELL ? 3 : 2;          // float4 words per fp32 row
+};
 constexpr double kU = 5.9604644775390625e-08;   // 2^-24
 
 // fp32 row of one constraint at the camera-frame point P (= R Z_i + t*): (A_1, A_2, P_3 or beta P_3, zeta_1),
 // (zeta_2, beta, -E_g, rho bound) and the error constants above.
 struct ReprojRow {
-    float4 a, b;
+    float4 a, b, c;   // c = (a, b, d', .) of the whitened form (ELL only)
     float unc;      // bound on |rho32 - rho64| for eq. (14) (phase A rows)
     float g0;       // cone value at d = 0 minus E_g (ladder rows: tightness key)
 };
 
-template <bool LADDER>
+template <bool LADDER, bool ELL>
 __device__ __forceinline__ ReprojRow reproj_row(double P0, double P1, double P2, const double *row, const double (&K)[4],
                                                 double t_p)
 {
-    const double z0 = row[0] - K[2], z1 = row[1] - K[3], beta = row[BETA];
-    const double A0 = z0 * P2 - K[0] * P0, A1 = z1 * P2 - K[1] * P1;
-    const double Eq0 = kU * (3.0 * fabs(A0) + 9.0 * t_p * (fabs(z0) + K[0]));
-    const double Eq1 = kU * (3.0 * fabs(A1) + 9.0 * t_p * (fabs(z1) + K[1]));
+    constexpr int BETA = RJ<ELL>::BETA;
+    const double zz0 = row[0] - K[2], zz1 = row[1] - K[3], beta = row[BETA];
+    const double B0 = zz0 * P2 - K[0] * P0, B1 = zz1 * P2 - K[1] * P1;
+    double l00 = 1.0, l10 = 0.0, l11 = 1.0;
+    if (ELL) {                                                  // Cholesky of [[L00 L01] [L01 L11]] (positive definite: closure_create)
+        l00 = sqrt(row[7]);
+        l10 = row[8] / l00;
+        l11 = sqrt(row[9] - l10 * l10);
+    }
+    const double A0 = ELL ? l00 * B0 + l10 * B1 : B0, A1 = ELL ? l11 * B1 : B1;
+    const double ca = -l00 * K[0], cb = -l10 * K[1], cd = -l11 * K[1];          // a, b, d'
+    const double z0 = ELL ? l00 * zz0 + l10 * zz1 : zz0, z1 = ELL ? l11 * zz1 : zz1;   // c, e
+    const double s0 = fabs(ca) + fabs(cb) + fabs(z0), s1 = fabs(cd) + fabs(z1);
+    const double Eq0 = kU * ((ELL ? 4.0 : 3.0) * fabs(A0) + (ELL ? 10.0 : 9.0) * t_p * s0);
+    const double Eq1 = kU * (3.0 * fabs(A1) + 9.0 * t_p * s1);
     const double Ep = kU * (2.0 * fabs(P2) + 7.0 * t_p);       // phase A only: p_3 = P_3 + d_3
     const double plo = P2 - 1.001 * t_p;
-    const double q0hi = fabs(A0) + t_p * (fabs(z0) + K[0]), q1hi = fabs(A1) + t_p * (fabs(z1) + K[1]);
+    const double q0hi = fabs(A0) + t_p * s0, q1hi = fabs(A1) + t_p * s1;
     ReprojRow r;
+    r.c = make_float4((float)ca, (float)cb, (float)cd, 0.f);
     if (!LADDER) {
         r.a = make_float4((float)A0, (float)A1, (float)P2, (float)z0);
         r.b = make_float4((float)z1, (float)beta, 0.f, 0.f);
@@ -93,7 +114,7 @@ __device__ __forceinline__ ReprojRow reproj_row(double P0, double P1, double P2,
 }
 
 // eq. (14) of perturbation j in the plain kernel's arithmetic (functor for topk_fp64)
-struct ExactMarginReproj {
+template <bool ELL> struct ExactMarginReproj {
     const double (&R)[9];
     const double (&t)[3];
     const double (&K)[4];
@@ -108,19 +129,26 @@ struct ExactMarginReproj {
         rng.xi3(s, (uint32_t)j, 1u, x, y, z);
         const double e0 = t_p * x, e1 = t_p * y, e2 = t_p * z;
         double d = CUDART_INF;
+        const double tj[3] = { t[0] + e0, t[1] + e1, t[2] + e2 };
 #pragma unroll 1
         for (int i = 0; i < n; ++i) {
-            const double *row = rows + i * ROW;
-            double P0, P1, P2;
-            reproj_point(R, row, P0, P1, P2);
-            const double sq = reproj_sq(P0, P1, P2, t[0] + e0, t[1] + e1, t[2] + e2, row, K);
-            d = dmin(d, row[BETA] - sqrt(sq));
+            const double *row = rows + i * RJ<ELL>::ROW;
+            double sq;
+            if (ELL) {
+                sq = direct_sq<RJ<ELL>::RES>(R, tj, row, K, 0);
+            } else {
+                double P0, P1, P2;
+                reproj_point(R, row, P0, P1, P2);
+                sq = reproj_sq(P0, P1, P2, tj[0], tj[1], tj[2], row, K);
+            }
+            d = dmin(d, row[RJ<ELL>::BETA] - sqrt(sq));
         }
         return d;
     }
 };
 
 // fp64 in_purse of ladder candidate (Rm, t* + d_j), constraints dealt to the lanes (plain kernel's arithmetic)
+template <bool ELL>
 __device__ __forceinline__ bool exact_candidate_feasible_reproj(const double (&Rm)[9], const double (&t)[3],
                                                                 const double (&K)[4], const double *rows, int n,
                                                                 const Rng &rng, uint32_t s, int j, double t_p, int lane)
@@ -129,13 +157,19 @@ __device__ __forceinline__ bool exact_candidate_feasible_reproj(const double (&R
     rng.xi3(s, (uint32_t)j, 1u, x, y, z);
     const double k0 = t_p * x, k1 = t_p * y, k2 = t_p * z;
     bool ok = true;
+    const double tk[3] = { t[0] + k0, t[1] + k1, t[2] + k2 };
 #pragma unroll 1
     for (int i = lane; i < n; i += 32) {
-        const double *row = rows + i * ROW;
-        double P0, P1, P2;
-        reproj_point(Rm, row, P0, P1, P2);
-        const double sq = reproj_sq(P0, P1, P2, t[0] + k0, t[1] + k1, t[2] + k2, row, K);
-        if (!(sq <= row[BETA + 1])) ok = false;
+        const double *row = rows + i * RJ<ELL>::ROW;
+        double sq;
+        if (ELL) {
+            sq = direct_sq<RJ<ELL>::RES>(Rm, tk, row, K, 0);
+        } else {
+            double P0, P1, P2;
+            reproj_point(Rm, row, P0, P1, P2);
+            sq = reproj_sq(P0, P1, P2, tk[0], tk[1], tk[2], row, K);
+        }
+        if (!(sq <= row[RJ<ELL>::BETA + 1])) ok = false;
     }
     return __all_sync(FULL, ok);
 }
@@ -148,11 +182,26 @@ __device__ __forceinline__ float cone_lo(const float4 &ra, const float4 &rb, con
     const float w = fmaf(rb.y, c.z, ra.z);
     return fmaf(q0, q0, fmaf(q1, q1, fmaf(-w, w, rb.z)));
 }
+// the same on the whitened rows of the ellipse norm: rc = (a, b, d', .)
+__device__ __forceinline__ float cone_lo_ell(const float4 &ra, const float4 &rb, const float4 &rc, const float4 &c)
+{
+    const float q0 = fmaf(ra.w, c.z, fmaf(rc.y, c.y, fmaf(rc.x, c.x, ra.x)));
+    const float q1 = fmaf(rb.x, c.z, fmaf(rc.z, c.y, ra.y));
+    const float w = fmaf(rb.y, c.z, ra.z);
+    return fmaf(q0, q0, fmaf(q1, q1, fmaf(-w, w, rb.z)));
+}
+template <bool ELL>
+__device__ __forceinline__ float cone_row(const float4 *r, const float4 &c, float nfx, float nfy)
+{
+    if (ELL) return cone_lo_ell(r[0], r[1], r[2], c);
+    return cone_lo(r[0], r[1], c, nfx, nfy);
+}
 
 // ---------------------------------------------------------------------------------- the kernel
-template <int NQ>
+template <int NQ, bool ELL>
 __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_reproj_kernel(const __grid_constant__ WalkLaunch L)
 {
+    constexpr int ROW = RJ<ELL>::ROW, BETA = RJ<ELL>::BETA, F4 = RJ<ELL>::F4;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int n_runs_s;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -163,7 +212,7 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
     double *rows = reinterpret_cast<double *>(smem_raw + 16);
     stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
-    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 2, n, kReprojWarps);
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, F4, (n * F4 + 1) / 2, kReprojWarps);
     int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
     float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
     if (warp == 0) {                                   // runs of equal bounds (rows are sorted by bound)
@@ -192,11 +241,11 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
     const long long local = (long long)blockIdx.x * kReprojWarps + warp;
     if (local >= L.num_walkers) return;                // no block-wide barrier below this line
     unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
-    float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);   // [n][2]
-    float4 *rowsL = reinterpret_cast<float4 *>(wp + lay.rowsL);   // [n][2]
+    float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);   // [n][F4]
+    float4 *rowsL = reinterpret_cast<float4 *>(wp + lay.rowsL);   // [n][F4]
     float4 *pert = reinterpret_cast<float4 *>(wp + lay.pert);     // (d_j, 0)
     double2 *ab = reinterpret_cast<double2 *>(wp + lay.ab);
-    float4 *qrow = reinterpret_cast<float4 *>(wp + lay.qrow);     // [rung][2 rows][2]
+    float4 *qrow = reinterpret_cast<float4 *>(wp + lay.qrow);     // [rung][2 rows][F4]
     double *RmS = reinterpret_cast<double *>(wp + lay.RmS);
     double *dex = reinterpret_cast<double *>(wp + lay.dex);
     float *qL = reinterpret_cast<float *>(wp + lay.qL);
@@ -274,9 +323,10 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                 const double *row = rows + i * ROW;
                 double P0, P1, P2;
                 reproj_point(R, row, P0, P1, P2);
-                const ReprojRow r = reproj_row<false>(P0 + t[0], P1 + t[1], P2 + t[2], row, K, t_p);
-                rowsA[2 * i] = r.a;
-                rowsA[2 * i + 1] = r.b;
+                const ReprojRow r = reproj_row<false, ELL>(P0 + t[0], P1 + t[1], P2 + t[2], row, K, t_p);
+                rowsA[F4 * i] = r.a;
+                rowsA[F4 * i + 1] = r.b;
+                if (ELL) rowsA[F4 * i + 2] = r.c;
                 unc_l = fmaxf(unc_l, r.unc);
             }
             uncA = wmax_nonneg(unc_l);
@@ -302,6 +352,8 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                 const unsigned hm = ((G == 8) ? 0xFFu : 0xFFFFu) << (lane & ~(G - 1));
                 double P0, P1, P2;
                 reproj_point(R, row, P0, P1, P2);
+                // ellipse norm: | ||g_m||_L - ||g_*||_L | <= ||L^T||_2 ||g_m - g_*||_2 <= sqrt(tr Lambda) (|dg_0| + |dg_1|)
+                const double lam_scale = ELL ? sqrt(row[ELL ? 7 : 0] + row[ELL ? 9 : 0]) * 1.0000001 : 1.0;
 #pragma unroll 1
                 for (int m = lane / G; m < n_t; m += 32 / G) {
                     double Rm[9];
@@ -309,7 +361,7 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                     for (int e = 0; e < 9; ++e) Rm[e] = RmS[m * 9 + e];
                     double Q0, Q1, Q2;
                     reproj_point(Rm, row, Q0, Q1, Q2);
-                    ReprojRow r = reproj_row<true>(Q0 + t[0], Q1 + t[1], Q2 + t[2], row, K, t_p);
+                    ReprojRow r = reproj_row<true, ELL>(Q0 + t[0], Q1 + t[1], Q2 + t[2], row, K, t_p);
                     double lip;
                     const double plo = dmin(P2, Q2) + t[2] - 1.001 * t_p;
                     if (plo > 0.0) {
@@ -317,6 +369,7 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                         const double y_hi = dmax(fabs(P1 + t[1]), fabs(Q1 + t[1])) + t_p;
                         const double d0 = fabs(Q0 - P0), d1 = fabs(Q1 - P1), d2 = fabs(Q2 - P2);
                         lip = K[0] * (d0 + x_hi / plo * d2) / plo + K[1] * (d1 + y_hi / plo * d2) / plo;
+                        if (ELL) lip *= lam_scale;
                     } else {
                         lip = CUDART_INF;
                     }
@@ -327,11 +380,18 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                     const uint32_t m2 = __reduce_max_sync(hm, key2);
                     const float lf = __uint_as_float(__reduce_max_sync(hm, __float_as_uint(has ? (float)lip : 0.f)));
                     if (key == m1) {
-                        qrow[4 * m] = r.a; qrow[4 * m + 1] = r.b;
+                        qrow[2 * F4 * m] = r.a; qrow[2 * F4 * m + 1] = r.b;
+                        if (ELL) qrow[2 * F4 * m + 2] = r.c;
                         qL[m] = lf * 1.001f + 1e-30f;
-                        if (n == 1) { qrow[4 * m + 2] = r.a; qrow[4 * m + 3] = r.b; }
+                        if (n == 1) {
+                            qrow[2 * F4 * m + F4] = r.a; qrow[2 * F4 * m + F4 + 1] = r.b;
+                            if (ELL) qrow[2 * F4 * m + F4 + 2] = r.c;
+                        }
                     }
-                    if (key2 == m2 && n > 1) { qrow[4 * m + 2] = r.a; qrow[4 * m + 3] = r.b; }
+                    if (key2 == m2 && n > 1) {
+                        qrow[2 * F4 * m + F4] = r.a; qrow[2 * F4 * m + F4 + 1] = r.b;
+                        if (ELL) qrow[2 * F4 * m + F4 + 2] = r.c;
+                    }
                 }
             } else {
 #pragma unroll 1
@@ -341,7 +401,7 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                 for (int e = 0; e < 9; ++e) Rm[e] = RmS[m * 9 + e];
                 ReprojRow b1, b2;
                 b1.g0 = b2.g0 = -CUDART_INF_F;
-                b1.a = b1.b = b2.a = b2.b = make_float4(0.f, 0.f, 0.f, 0.f);
+                b1.a = b1.b = b1.c = b2.a = b2.b = b2.c = make_float4(0.f, 0.f, 0.f, 0.f);
                 b1.b.z = b2.b.z = -CUDART_INF_F;            // a row that never kills
                 double lip = 0.0;
 #pragma unroll 1
@@ -350,7 +410,7 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                     double P0, P1, P2, Q0, Q1, Q2;
                     reproj_point(R, row, P0, P1, P2);
                     reproj_point(Rm, row, Q0, Q1, Q2);
-                    const ReprojRow r = reproj_row<true>(Q0 + t[0], Q1 + t[1], Q2 + t[2], row, K, t_p);
+                    const ReprojRow r = reproj_row<true, ELL>(Q0 + t[0], Q1 + t[1], Q2 + t[2], row, K, t_p);
                     if (r.g0 > b1.g0) { b2 = b1; b1 = r; } else if (r.g0 > b2.g0) b2 = r;
                     const double plo = dmin(P2, Q2) + t[2] - 1.001 * t_p;
                     if (plo > 0.0) {
@@ -359,7 +419,7 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                         const double d0 = fabs(Q0 - P0), d1 = fabs(Q1 - P1), d2 = fabs(Q2 - P2);
                         const double lx = K[0] * (d0 + x_hi / plo * d2) / plo;
                         const double ly = K[1] * (d1 + y_hi / plo * d2) / plo;
-                        lip = dmax(lip, lx + ly);
+                        lip = dmax(lip, (lx + ly) * (ELL ? sqrt(row[ELL ? 7 : 0] + row[ELL ? 9 : 0]) * 1.0000001 : 1.0));
                     } else {
                         lip = CUDART_INF;
                     }
@@ -370,10 +430,14 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                 const uint32_t k2 = (lane == src1) ? fkey(b2.g0) : k1;
                 const uint32_t m2 = __reduce_max_sync(FULL, k2);
                 const int src2 = __ffs(__ballot_sync(FULL, k2 == m2)) - 1;
-                if (lane == src1) { qrow[4 * m] = b1.a; qrow[4 * m + 1] = b1.b; }
+                if (lane == src1) {
+                    qrow[2 * F4 * m] = b1.a; qrow[2 * F4 * m + 1] = b1.b;
+                    if (ELL) qrow[2 * F4 * m + 2] = b1.c;
+                }
                 if (lane == src2) {
-                    qrow[4 * m + 2] = (lane == src1) ? b2.a : b1.a;
-                    qrow[4 * m + 3] = (lane == src1) ? b2.b : b1.b;
+                    qrow[2 * F4 * m + F4] = (lane == src1) ? b2.a : b1.a;
+                    qrow[2 * F4 * m + F4 + 1] = (lane == src1) ? b2.b : b1.b;
+                    if (ELL) qrow[2 * F4 * m + F4 + 2] = (lane == src1) ? b2.c : b1.c;
                 }
                 const float lf = wmax_nonneg((float)lip);
                 if (lane == 0) qL[m] = lf * 1.001f + 1e-30f;
@@ -418,11 +482,14 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                 for (int q = 0; q < NQ; ++q) mx[q] = 0.f;
 #pragma unroll 1                         // measured: +2 % at C3 against the default unrolling
                 for (; i <= end; ++i) {
-                    const float4 ra = rowsA[2 * i], rb = rowsA[2 * i + 1];
+                    const float4 ra = rowsA[F4 * i], rb = rowsA[F4 * i + 1];
+                    float4 rc = make_float4(nfx, 0.f, nfy, 0.f);
+                    if (ELL) rc = rowsA[F4 * i + 2];
 #pragma unroll
                     for (int q = 0; q < NQ; ++q) {
-                        const float q0 = fmaf(ra.w, d2[q], fmaf(nfx, d0[q], ra.x));
-                        const float q1 = fmaf(rb.x, d2[q], fmaf(nfy, d1[q], ra.y));
+                        const float q0 = ELL ? fmaf(ra.w, d2[q], fmaf(rc.y, d1[q], fmaf(rc.x, d0[q], ra.x)))
+                                             : fmaf(ra.w, d2[q], fmaf(nfx, d0[q], ra.x));
+                        const float q1 = fmaf(rb.x, d2[q], fmaf(ELL ? rc.z : nfy, d1[q], ra.y));
                         float wr;
                         asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(wr) : "f"(ra.z + d2[q]));
                         mx[q] = fmaxf(mx[q], fmaf(q0, q0, q1 * q1) * (wr * wr));
@@ -450,7 +517,7 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
             for (int e = 0; e < 3; ++e) t[e] = pose[9 + e];
 #pragma unroll
             for (int e = 0; e < 4; ++e) K[e] = D->K[e];
-            const ExactMarginReproj exact{ R, t, K, rows, n, rng, (uint32_t)s, t_p };
+            const ExactMarginReproj<ELL> exact{ R, t, K, rows, n, rng, (uint32_t)s, t_p };
             const int cnt = topk_fp64<NQ>(dv, n_p, n_ps, uncA, myval, (L.exact_only & 16) != 0, lane, dex, candj, candd, exact);
             if (stats) { stc[8] += 1; stc[0] += (unsigned long long)n * cnt; }
         }
@@ -469,13 +536,15 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
             const bool q_act = mq < n_t;
             unsigned alive = 0u;
             if (q_act) {
-                const float4 r0a = qrow[4 * mq], r0b = qrow[4 * mq + 1], r1a = qrow[4 * mq + 2], r1b = qrow[4 * mq + 3];
+                float4 r0[F4], r1[F4];
+#pragma unroll
+                for (int e = 0; e < F4; ++e) { r0[e] = qrow[2 * F4 * mq + e]; r1[e] = qrow[2 * F4 * mq + F4 + e]; }
                 const float Lm = qL[mq];
                 const int k1 = min(KP, (hq + 1) * khalf);
                 for (int k = hq * khalf; k < k1; ++k) {
                     const float4 c4 = cand4[k];
-                    const float v0 = cone_lo(r0a, r0b, c4, nfx, nfy);
-                    const float v1 = cone_lo(r1a, r1b, c4, nfx, nfy);
+                    const float v0 = cone_row<ELL>(r0, c4, nfx, nfy);
+                    const float v1 = cone_row<ELL>(r1, c4, nfx, nfy);
                     if (!(v0 > 0.f) && !(v1 > 0.f) && !(candd[k] + Lm < 0.f)) alive |= 1u << k;
                 }
             }
@@ -511,9 +580,10 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                         const double *row = rows + i * ROW;
                         double Q0, Q1, Q2;
                         reproj_point(Rm, row, Q0, Q1, Q2);
-                        const ReprojRow r = reproj_row<true>(Q0 + t[0], Q1 + t[1], Q2 + t[2], row, K, t_p);
-                        rowsL[2 * i] = r.a;
-                        rowsL[2 * i + 1] = r.b;
+                        const ReprojRow r = reproj_row<true, ELL>(Q0 + t[0], Q1 + t[1], Q2 + t[2], row, K, t_p);
+                        rowsL[F4 * i] = r.a;
+                        rowsL[F4 * i + 1] = r.b;
+                        if (ELL) rowsL[F4 * i + 2] = r.c;
                         eps_l = fmaxf(eps_l, r.unc);
                     }
                     epsL = wmax_nonneg(eps_l);
@@ -525,7 +595,7 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                 float M = -CUDART_INF_F;
                 if (e_act) {
                     const float4 c4 = cand4[ek];
-                    for (int i = ech; i < n; i += NCH) M = fmaxf(M, cone_lo(rowsL[2 * i], rowsL[2 * i + 1], c4, nfx, nfy));
+                    for (int i = ech; i < n; i += NCH) M = fmaxf(M, cone_row<ELL>(rowsL + F4 * i, c4, nfx, nfy));
                     M = fkey_inv(__reduce_max_sync(e_mask, fkey(M)));
                 }
                 // M = max_i (g32_i - E_g,i):  M > 0 => some constraint violated for sure;
@@ -540,7 +610,7 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                 while (undecided != 0u) {                    // rare: fp64 decides
                     const int k = __ffs(undecided) - 1;
                     undecided &= undecided - 1u;
-                    if (!exact_candidate_feasible_reproj(Rm, t, K, rows, n, rng, (uint32_t)s, candj[k], t_p, lane))
+                    if (!exact_candidate_feasible_reproj<ELL>(Rm, t, K, rows, n, rng, (uint32_t)s, candj[k], t_p, lane))
                         alive2 &= ~(1u << k);
                     if (stats) stc[1] += n;
                 }
@@ -585,30 +655,39 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
     }
 }
 
-template <int NQ>
+template <int NQ, bool ELL>
 cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
 {
-    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 2, max_n, kReprojWarps);
+    constexpr int F4 = RJ<ELL>::F4;
+    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, F4, (max_n * F4 + 1) / 2, kReprojWarps);
     if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
-    cudaError_t e = cudaFuncSetAttribute(walker_coop_reproj_kernel<NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(walker_coop_reproj_kernel<NQ, ELL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)lay.total);
     if (e != cudaSuccess) return e;
     const long long blocks = (L.num_walkers + kReprojWarps - 1) / kReprojWarps;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     dim3 grid((unsigned)blocks, (unsigned)n_instances, 1);
-    walker_coop_reproj_kernel<NQ><<<grid, kReprojThreads, lay.total, stream>>>(L);
+    walker_coop_reproj_kernel<NQ, ELL><<<grid, kReprojThreads, lay.total, stream>>>(L);
     return cudaGetLastError();
+}
+
+template <bool ELL>
+cudaError_t launch_e(const WalkLaunch &L, int n_instances, int max_rows_bytes, cudaStream_t stream)
+{
+    const int max_n = max_rows_bytes / (RJ<ELL>::ROW * 8);
+    if (L.n_p <= 32) return launch_q<1, ELL>(L, n_instances, max_rows_bytes, max_n, stream);
+    if (L.n_p <= 64) return launch_q<2, ELL>(L, n_instances, max_rows_bytes, max_n, stream);
+    if (L.n_p <= 160) return launch_q<5, ELL>(L, n_instances, max_rows_bytes, max_n, stream);
+    return launch_q<8, ELL>(L, n_instances, max_rows_bytes, max_n, stream);
 }
 
 }  // namespace
 
-cudaError_t launch_walkers_coop_reproj(const WalkLaunch &L, int n_instances, int max_rows_bytes, cudaStream_t stream)
+cudaError_t launch_walkers_coop_reproj(int residual_type, const WalkLaunch &L, int n_instances, int max_rows_bytes,
+                                       cudaStream_t stream)
 {
-    const int max_n = max_rows_bytes / (ROW * 8);
-    if (L.n_p <= 32) return launch_q<1>(L, n_instances, max_rows_bytes, max_n, stream);
-    if (L.n_p <= 64) return launch_q<2>(L, n_instances, max_rows_bytes, max_n, stream);
-    if (L.n_p <= 160) return launch_q<5>(L, n_instances, max_rows_bytes, max_n, stream);
-    return launch_q<8>(L, n_instances, max_rows_bytes, max_n, stream);
+    if (residual_type == CLOSURE_REPROJ_2D3D_ELL) return launch_e<true>(L, n_instances, max_rows_bytes, stream);
+    return launch_e<false>(L, n_instances, max_rows_bytes, stream);
 }
 
 }  // namespace closure

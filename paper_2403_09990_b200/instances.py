@@ -117,6 +117,21 @@ def _make_reg(rng, n, noise_small, beta_small, frac_large=0.0, noise_large=0.0, 
     return meas, betas, radius, R, t
 
 
+def _make_reproj(rng, n):
+    """2D-3D keypoints of BASELINE config 3: pinhole 572.4 / 325.3 / 242.0, Z_i ~ U[-0.1, 0.1]^3 m, depth 0.8-1.2 m, pixel noise
+    uniform in a disc of 5 px.  The projection here only GENERATES the measurements."""
+    K = np.array([572.4, 572.4, 325.3, 242.0])
+    Z = rng.uniform(-0.1, 0.1, size=(n, 3))
+    R = haar_rotation(rng)
+    t = np.array([rng.uniform(-0.1, 0.1), rng.uniform(-0.1, 0.1), rng.uniform(0.8, 1.2)])
+    z = np.empty((n, 2))
+    for i in range(n):
+        p = R @ Z[i] + t
+        z[i] = np.array([K[0] * p[0] / p[2] + K[2], K[1] * p[1] / p[2] + K[3]]) \
+            + uniform_in_ball(rng, 5.0, 2)
+    return np.concatenate([z, Z], axis=1), K, R, t        # row [z(2) Z(3)]
+
+
 def make_instance(config: int, instance_index: int = 0, *, num_walkers: int | None = None,
                   num_steps: int | None = None) -> Instance:
     """BASELINE.json configs C1..C5 (1-based).  Instance seed = 1000*config + index."""
@@ -132,16 +147,7 @@ def make_instance(config: int, instance_index: int = 0, *, num_walkers: int | No
                         WalkParams(omega0=0.5, t_p=0.1), 65536, 1000)
     elif config == 3:
         n = 8
-        K = np.array([572.4, 572.4, 325.3, 242.0])
-        Z = rng.uniform(-0.1, 0.1, size=(n, 3))
-        R = haar_rotation(rng)
-        t = np.array([rng.uniform(-0.1, 0.1), rng.uniform(-0.1, 0.1), rng.uniform(0.8, 1.2)])
-        z = np.empty((n, 2))
-        for i in range(n):
-            p = R @ Z[i] + t
-            z[i] = np.array([K[0] * p[0] / p[2] + K[2], K[1] * p[1] / p[2] + K[3]]) \
-                + uniform_in_ball(rng, 5.0, 2)
-        meas = np.concatenate([z, Z], axis=1)        # row [z(2) Z(3)]
+        meas, K, R, t = _make_reproj(rng, n)
         inst = Instance("C3_reproj_n8", REPROJ_2D3D, n, meas, np.full(n, 8.0), K, R, t,
                         np.full(n, 5.0),
                         WalkParams(omega0=1.0, v0=2.0, theta_p=0.2, t_p=0.01), 262144, 1000)
@@ -185,6 +191,16 @@ def make_custom_reg(n: int, seed: int, *, noise: float = 0.05, beta: float = 0.1
         betas = betas * (1.0 + 0.5 * rng.uniform(size=n))
     inst = Instance(f"reg_n{n}_s{seed}", REG_3D3D, n, meas, betas, None, R, t, rad,
                     WalkParams(omega0=0.5, t_p=beta), 256, 50)
+    inst.seed = seed
+    return inst
+
+
+def make_custom_reproj(n: int, seed: int, *, beta: float = 8.0) -> Instance:
+    """Free-size reprojection instance for tests (a table longer than C3's 8 keypoints)."""
+    rng = np.random.default_rng(seed)
+    meas, K, R, t = _make_reproj(rng, n)
+    inst = Instance(f"reproj_n{n}_s{seed}", REPROJ_2D3D, n, meas, np.full(n, beta), K, R, t, np.full(n, 5.0),
+                    WalkParams(omega0=1.0, v0=2.0, theta_p=0.2, t_p=0.01), 256, 50)
     inst.seed = seed
     return inst
 

@@ -464,6 +464,33 @@ def test_ellipsoid_certified_kernel_is_bit_identical_to_plain_kernel(config, n_p
         assert st["perturb_pairs_f32"] > 0 and st["fallback_steps"] < 0.2 * st["walker_steps"], st
 
 
+@pytest.mark.parametrize("flags", [0, 2, 4, 6, 20])
+@pytest.mark.parametrize("n,n_p,n_p_star,n_t,walkers,steps", [(8, 150, 10, 10, 2048, 100), (8, 40, 4, 8, 1024, 60),
+                                                              (24, 150, 10, 17, 512, 60), (8, 20, 2, 5, 1024, 80)])
+def test_ellipse_certified_reprojection_kernel_is_bit_identical_to_plain_kernel(n, n_p, n_p_star, n_t, walkers, steps, flags):
+    """Ex.1 with the ellipse norm (CLOSURE_REPROJ_2D3D_ELL) on the certified fp32 kernel (walker_coop_reproj_kernel<NQ, true>:
+    rows whitened by the Cholesky factor of Lambda_i): outputs and traces equal the plain fp64 kernel's bit for bit -- C3's
+    table and a longer one (the set-up's loop over constraints, a ladder longer than one screening block), few
+    perturbations, and every fp64 fall-back forced (flags 2, 4, 16)."""
+    inst = I.to_ellipsoidal(I.make_instance(3) if n == 8 else I.make_custom_reproj(n, 977), 7)
+    S0 = I.make_init_poses(inst, 64)
+    P = _small(inst.params, n_p=n_p, n_p_star=n_p_star, n_t=n_t)
+    fast = gpu_walk(inst, _small(P, flags=flags), S0, walkers, steps, 4747)
+    plain = gpu_walk(inst, _small(P, flags=1), S0, walkers, steps, 4747)
+    for a, b in zip(fast, plain):
+        assert np.array_equal(a, b)
+    if flags == 0:                                                      # the certificates carry most iterations
+        h = B.Closure.closure_create(inst, P)
+        try:
+            h.closure_set_init(S0)
+            h.closure_enable_stats(True)
+            h.closure_sample(walkers, steps, 4747)
+            st = h.closure_get_stats()
+        finally:
+            h.closure_destroy()
+        assert st["perturb_pairs_f32"] > 0 and st["fallback_steps"] < 0.2 * st["walker_steps"], st
+
+
 def test_ellipsoid_with_several_bounds_and_a_pivot():
     """Runs of equal bounds of odd length and a body pivot on the ellipsoid kernel, against the oracle and the plain kernel."""
     inst = I.to_ellipsoidal(_three_bounds(77, 901, (25, 31, 21)), 8)
