@@ -17,6 +17,7 @@
 //   cone value g:  E_g = 2 (q1_hi E_q1 + q2_hi E_q2 + w_hi E_w) + 4 u (q1_hi^2 + q2_hi^2 + w_hi^2), x 1.5.
 // The fp64 reference of every decision is the plain kernel's arithmetic (reproj_point / reproj_sq in
 // walker_common.cuh); its own rounding (~1e-13 px) is far inside these bounds.
+// The ellipse norm of eq. (6) (CLOSURE_REPROJ_2D3D_ELL) is the <NQ, true> instantiation: see RJ below.
 #include <cuda_runtime.h>
 #include <math_constants.h>
 #include <stdint.h>
