@@ -93,6 +93,44 @@ __device__ __forceinline__ double wmin_f64(double v)
     return v;
 }
 
+// The two largest of the (distinct) keys and the maximum of a non-negative float over the aligned group of G = 8 or 16 lanes
+// this lane belongs to (gm = the group's lanes), by XOR butterflies.  REDUX with a different member mask per group is
+// serialised group by group (measured: ~30 instructions per reduction in the set-up of the short tables).
+__device__ __forceinline__ void group_top2_max(unsigned gm, int G, uint32_t key, float f, uint32_t &k1, uint32_t &k2, float &fm)
+{
+    uint32_t b1 = key, b2 = 0u, fb = __float_as_uint(f);
+#pragma unroll
+    for (int o = 1; o < 16; o <<= 1) {
+        if (o < G) {
+            const uint32_t p1 = __shfl_xor_sync(gm, b1, o), p2 = __shfl_xor_sync(gm, b2, o), pf = __shfl_xor_sync(gm, fb, o);
+            const uint32_t lo = min(b1, p1);
+            b1 = max(b1, p1);
+            b2 = max(max(b2, p2), lo);
+            fb = max(fb, pf);
+        }
+    }
+    k1 = b1; k2 = b2; fm = __uint_as_float(fb);
+}
+
+// Maximum over the lanes ek + c KP, c < NCH (the constraint chunks of one ladder candidate in the full evaluation of a rung),
+// delivered to the lane with c = 0: a tree of SHFL.DOWN on order-preserving keys (NaN stays the largest, as under REDUX.MAX).
+// Lanes beyond NCH KP pass -inf.  A REDUX with one member mask per candidate is serialised mask by mask.
+__device__ __forceinline__ float chunk_max_to_first(float M, int KP, int NCH)
+{
+    uint32_t k = fkey(M);
+    for (int off = 1; off < NCH; off <<= 1) k = max(k, __shfl_down_sync(FULL, k, off * KP));
+    return fkey_inv(k);
+}
+
+// x / d by one IMAD.HI (a division by a run-time integer is ~20 instructions): magic = ceil(2^32 / d); exact while x d < 2^32
+// (floor(x magic / 2^32) = floor(x / d + x e / 2^32) with 0 <= e < 1, and frac(x / d) <= 1 - 1/d).  d = 1 wraps magic to 0.
+struct FastDiv {
+    uint32_t magic;
+    int d;
+    __device__ __forceinline__ explicit FastDiv(int dd) : magic(0xFFFFFFFFu / (uint32_t)dd + 1u), d(dd) {}
+    __device__ __forceinline__ int div(int x) const { return d == 1 ? x : (int)__umulhi((uint32_t)x, magic); }
+};
+
 // packed fp32 pairs (FFMA2 on sm_100a)
 __device__ __forceinline__ unsigned long long pk2(float lo, float hi)
 {

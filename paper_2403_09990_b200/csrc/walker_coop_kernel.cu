@@ -370,9 +370,10 @@ __device__ __noinline__ void aff_setup_on_move(unsigned char *smem_raw, int warp
             screen_row(u0, u1, u2, cc - row[RS::BETA + 1], tp2, tp2sq3, g0, g1, g2, fcb, eps);
             float4 r4 = make_float4(g0, g1, g2, fcb - eps);
             const uint32_t key = (fkey(r4.w) & ~15u) | (uint32_t)c;
-            const uint32_t m1 = __reduce_max_sync(hm, key);
+            uint32_t m1, m2;
+            float unused;
+            group_top2_max(hm, 16, key, 0.f, m1, m2, unused);
             const uint32_t key2 = (key == m1) ? 0u : key;
-            const uint32_t m2 = __reduce_max_sync(hm, key2);
             if (RES == CLOSURE_POSE_REG_SPLIT) {
                 if ((__ballot_sync(hm, rdead) & hm) != 0u) r4.w = CUDART_INF_F;       // rung dead for every candidate
             }
@@ -585,8 +586,6 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     const int NCH = 32 / KP;                            // constraint chunks of the full evaluation
     const int ek = lane % KP, ech = lane / KP;
     const bool e_act = ech < NCH;
-    unsigned e_mask = 0u;                               // lanes that share this lane's candidate
-    for (int c = 0; c < NCH; ++c) e_mask |= 1u << (ek + c * KP);
     const unsigned kp_all = (KP >= 32) ? FULL : ((1u << KP) - 1u);
     unsigned sortdir = 0u;                              // bit t: this lane keeps the larger key at stage t of the bitonic network
     {
@@ -1089,8 +1088,8 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                             const float4 f = rowsL[i];
                             M = fmaxf(M, fmaf(f.x, c4.x, fmaf(f.y, c4.y, fmaf(f.z, c4.z, f.w))));
                         }
-                        M = fkey_inv(__reduce_max_sync(e_mask, fkey(M)));
                     }
+                    M = chunk_max_to_first(M, KP, NCH);      // valid on the lanes with ech == 0 (`mine` below)
                     // M = max_i (v32_i - eps_i):  M > th  => some constraint violated for sure;
                     // M + 2 eps_max <= th => every constraint satisfied for sure.
                     const bool dead = M > c4.w;

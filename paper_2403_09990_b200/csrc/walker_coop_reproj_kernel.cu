@@ -55,6 +55,16 @@ template <bool ELL> struct RJ {
 };
 constexpr double kU = 5.9604644775390625e-08;   // 2^-24
 
+// 1 / x for the error and Lipschitz bounds (x > 0): MUFU.RCP and one Newton step in fp64 instead of the ~20 instructions of a
+// correctly rounded fp64 division; relative error < 1e-13, far inside the 1.0001 - 1.001 slack every bound carries.  An x that
+// fp32 cannot hold gives 0 or inf from MUFU.RCP: callers get +inf ("nothing certified"), never a bound that is too small.
+__device__ __forceinline__ double bound_rcp(double x)
+{
+    const double r = (double)__frcp_rn((float)x);
+    if (!(r > 0.0) || !(r < CUDART_INF)) return CUDART_INF;
+    return r * fma(-x, r, 2.0);
+}
+
 // fp32 row of one constraint at the camera-frame point P (= R Z_i + t*): (A_1, A_2, P_3 or beta P_3, zeta_1),
 // (zeta_2, beta, -E_g, rho bound) and the error constants above.
 struct ReprojRow {
@@ -92,8 +102,9 @@ __device__ __forceinline__ ReprojRow reproj_row(double P0, double P1, double P2,
         r.b = make_float4((float)z1, (float)beta, 0.f, 0.f);
         r.g0 = 0.f;
         if (plo > 0.0) {
-            const double rho_hi = (q0hi + q1hi) / plo;
-            const double Erho = (Eq0 + Eq1) / plo + rho_hi * (Ep / plo + 1.9073486328125e-06);
+            const double inv = bound_rcp(plo);
+            const double rho_hi = (q0hi + q1hi) * inv;
+            const double Erho = (Eq0 + Eq1) * inv + rho_hi * (Ep * inv + 1.9073486328125e-06);
             r.unc = (float)(2.0 * Erho + 4.76837158203125e-07 * beta + 1e-12 * (rho_hi + beta)) * 1.0001f;
         } else {
             r.unc = CUDART_INF_F;
@@ -112,6 +123,21 @@ __device__ __forceinline__ ReprojRow reproj_row(double P0, double P1, double P2,
         r.g0 = (float)(A0 * A0 + A1 * A1 - Bp * Bp) - Egf;
     }
     return r;
+}
+
+// Lipschitz bound of one constraint between R* (camera-frame point P + t) and R_m (Q + t), valid for |d_c| <= t_p:
+//   |d/dtau fx p_1/p_3| <= fx (|dP_1| + |p_1/p_3| |dP_3|) / p_3 along p(tau) = p + tau dP
+__device__ __forceinline__ double reproj_lip(double P0, double P1, double P2, double Q0, double Q1, double Q2, const double (&t)[3],
+                                             const double (&K)[4], double t_p)
+{
+    const double plo = dmin(P2, Q2) + t[2] - 1.001 * t_p;
+    if (!(plo > 0.0)) return CUDART_INF;
+    const double inv = bound_rcp(plo);
+    if (!(inv < CUDART_INF)) return CUDART_INF;
+    const double x_hi = dmax(fabs(P0 + t[0]), fabs(Q0 + t[0])) + t_p;
+    const double y_hi = dmax(fabs(P1 + t[1]), fabs(Q1 + t[1])) + t_p;
+    const double d0 = fabs(Q0 - P0), d1 = fabs(Q1 - P1), d2i = fabs(Q2 - P2) * inv;
+    return (K[0] * fma(x_hi, d2i, d0) + K[1] * fma(y_hi, d2i, d1)) * inv;
 }
 
 // eq. (14) of perturbation j in the plain kernel's arithmetic (functor for topk_fp64)
@@ -291,8 +317,6 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
     const int NCH = 32 / KP;                            // constraint chunks of the full evaluation
     const int ek = lane % KP, ech = lane / KP;
     const bool e_act = ech < NCH;
-    unsigned e_mask = 0u;                               // lanes that share this lane's candidate
-    for (int c = 0; c < NCH; ++c) e_mask |= 1u << (ek + c * KP);
 
     // executed-work counters (closure_get_stats): in shared memory, touched by lane 0 and only when asked for
     unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
@@ -363,23 +387,14 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                     double Q0, Q1, Q2;
                     reproj_point(Rm, row, Q0, Q1, Q2);
                     ReprojRow r = reproj_row<true, ELL>(Q0 + t[0], Q1 + t[1], Q2 + t[2], row, K, t_p);
-                    double lip;
-                    const double plo = dmin(P2, Q2) + t[2] - 1.001 * t_p;
-                    if (plo > 0.0) {
-                        const double x_hi = dmax(fabs(P0 + t[0]), fabs(Q0 + t[0])) + t_p;
-                        const double y_hi = dmax(fabs(P1 + t[1]), fabs(Q1 + t[1])) + t_p;
-                        const double d0 = fabs(Q0 - P0), d1 = fabs(Q1 - P1), d2 = fabs(Q2 - P2);
-                        lip = K[0] * (d0 + x_hi / plo * d2) / plo + K[1] * (d1 + y_hi / plo * d2) / plo;
-                        if (ELL) lip *= lam_scale;
-                    } else {
-                        lip = CUDART_INF;
-                    }
+                    double lip = reproj_lip(P0, P1, P2, Q0, Q1, Q2, t, K, t_p);
+                    if (ELL) lip *= lam_scale;
                     if (!has) { r.g0 = -CUDART_INF_F; r.b.z = -CUDART_INF_F; }      // a row that never kills
                     const uint32_t key = has ? ((fkey(r.g0) & ~15u) | (uint32_t)c) : (uint32_t)c;
-                    const uint32_t m1 = __reduce_max_sync(hm, key);
+                    uint32_t m1, m2;
+                    float lf;
+                    group_top2_max(hm, G, key, has ? (float)lip : 0.f, m1, m2, lf);
                     const uint32_t key2 = (key == m1) ? 0u : key;
-                    const uint32_t m2 = __reduce_max_sync(hm, key2);
-                    const float lf = __uint_as_float(__reduce_max_sync(hm, __float_as_uint(has ? (float)lip : 0.f)));
                     if (key == m1) {
                         qrow[2 * F4 * m] = r.a; qrow[2 * F4 * m + 1] = r.b;
                         if (ELL) qrow[2 * F4 * m + 2] = r.c;
@@ -413,17 +428,8 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                     reproj_point(Rm, row, Q0, Q1, Q2);
                     const ReprojRow r = reproj_row<true, ELL>(Q0 + t[0], Q1 + t[1], Q2 + t[2], row, K, t_p);
                     if (r.g0 > b1.g0) { b2 = b1; b1 = r; } else if (r.g0 > b2.g0) b2 = r;
-                    const double plo = dmin(P2, Q2) + t[2] - 1.001 * t_p;
-                    if (plo > 0.0) {
-                        const double x_hi = dmax(fabs(P0 + t[0]), fabs(Q0 + t[0])) + t_p;
-                        const double y_hi = dmax(fabs(P1 + t[1]), fabs(Q1 + t[1])) + t_p;
-                        const double d0 = fabs(Q0 - P0), d1 = fabs(Q1 - P1), d2 = fabs(Q2 - P2);
-                        const double lx = K[0] * (d0 + x_hi / plo * d2) / plo;
-                        const double ly = K[1] * (d1 + y_hi / plo * d2) / plo;
-                        lip = dmax(lip, (lx + ly) * (ELL ? sqrt(row[ELL ? 7 : 0] + row[ELL ? 9 : 0]) * 1.0000001 : 1.0));
-                    } else {
-                        lip = CUDART_INF;
-                    }
+                    lip = dmax(lip, reproj_lip(P0, P1, P2, Q0, Q1, Q2, t, K, t_p) *
+                                        (ELL ? sqrt(row[ELL ? 7 : 0] + row[ELL ? 9 : 0]) * 1.0000001 : 1.0));
                 }
                 const uint32_t k1 = fkey(b1.g0);
                 const uint32_t m1 = __reduce_max_sync(FULL, k1);
@@ -597,8 +603,8 @@ __global__ void __launch_bounds__(kReprojThreads, kReprojMinCtas) walker_coop_re
                 if (e_act) {
                     const float4 c4 = cand4[ek];
                     for (int i = ech; i < n; i += NCH) M = fmaxf(M, cone_row<ELL>(rowsL + F4 * i, c4, nfx, nfy));
-                    M = fkey_inv(__reduce_max_sync(e_mask, fkey(M)));
                 }
+                M = chunk_max_to_first(M, KP, NCH);          // valid on the lanes with ech == 0 (`mine` below)
                 // M = max_i (g32_i - E_g,i):  M > 0 => some constraint violated for sure;
                 // M + 2 max_i E_g,i <= 0 => every constraint satisfied (and in front of the camera) for sure.
                 const bool dead = M > 0.f;

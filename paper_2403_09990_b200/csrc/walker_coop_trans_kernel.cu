@@ -200,6 +200,7 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
     bool moved = true;
     const int KP = n_ps;
     const int items = KP * n_t;                          // ladder candidates, in Alg. A8's order (m, k)
+    const FastDiv divKP(KP), divN(n);                     // items <= 20 x 64, KP n <= 20 x 4096: inside FastDiv's range
 
     for (int s = 1; s <= L.num_steps; ++s) {
         // ================================================== a2-a4: perturb, eq. (14), top-N_P*
@@ -281,6 +282,15 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
                     E[q][6] = fmaf(B, f0 * f2, -a1); E[q][7] = fmaf(B, f1 * f2, a0);  E[q][8] = -B * (s0 + s1);
                     dv[q] = CUDART_INF_F;
                 }
+                // perturbations 2k, 2k+1 share packed instructions (fma.rn.f32x2: the same roundings as the scalar chain below,
+                // which the odd slot NQ-1 keeps): 18 packed + 2 MUFU.RCP + 2 max per two pairs instead of 40 scalar instructions
+                constexpr int NPK = NQ / 2;
+                unsigned long long EP[NPK > 0 ? NPK : 1][9];
+#pragma unroll
+                for (int k = 0; k < NPK; ++k)
+#pragma unroll
+                    for (int e = 0; e < 9; ++e) EP[k][e] = pk2(E[2 * k][e], E[2 * k + 1][e]);
+                const unsigned long long NFX = pk2(nfx, nfx), NFY = pk2(nfy, nfy), ONE = pk2(1.0f, 1.0f);
                 int i = 0;
                 for (int r = 0; r < n_runs; ++r) {
                     const int end = run_end[r];
@@ -290,7 +300,27 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
                     for (; i <= end; ++i) {
                         const float4 ra = rowsA[2 * i], rb = rowsA[2 * i + 1];
 #pragma unroll
-                        for (int q = 0; q < NQ; ++q) {
+                        for (int k = 0; k < NPK; ++k) {
+                            const unsigned long long X = pk2(ra.x, ra.x), Y = pk2(ra.y, ra.y), Z = pk2(ra.z, ra.z);
+                            const unsigned long long g0 = fma2(EP[k][0], X, fma2(EP[k][1], Y, mul2(EP[k][2], Z)));   // D P
+                            const unsigned long long g1 = fma2(EP[k][3], X, fma2(EP[k][4], Y, mul2(EP[k][5], Z)));
+                            const unsigned long long g2 = fma2(EP[k][6], X, fma2(EP[k][7], Y, mul2(EP[k][8], Z)));
+                            const unsigned long long q0 = fma2(pk2(ra.w, ra.w), g2, fma2(NFX, g0, pk2(rb.y, rb.y)));
+                            const unsigned long long q1 = fma2(pk2(rb.x, rb.x), g2, fma2(NFY, g1, pk2(rb.z, rb.z)));
+                            const unsigned long long p2 = fma2(g2, ONE, pk2(rb.w, rb.w));                            // rb.w + g2
+                            float pl, ph, wl, wh;
+                            upk2(p2, pl, ph);
+                            asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(wl) : "f"(pl));
+                            asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(wh) : "f"(ph));
+                            const unsigned long long wr = pk2(wl, wh);
+                            const unsigned long long val = mul2(fma2(q0, q0, mul2(q1, q1)), mul2(wr, wr));
+                            float vl, vh;
+                            upk2(val, vl, vh);
+                            mx[2 * k] = fmaxf(mx[2 * k], vl);
+                            mx[2 * k + 1] = fmaxf(mx[2 * k + 1], vh);
+                        }
+#pragma unroll
+                        for (int q = 2 * NPK; q < NQ; ++q) {
                             const float g0 = fmaf(E[q][0], ra.x, fmaf(E[q][1], ra.y, E[q][2] * ra.z));   // D P
                             const float g1 = fmaf(E[q][3], ra.x, fmaf(E[q][4], ra.y, E[q][5] * ra.z));
                             const float g2 = fmaf(E[q][6], ra.x, fmaf(E[q][7], ra.y, E[q][8] * ra.z));
@@ -351,7 +381,7 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
             }
             __syncwarp();
             for (int pi = lane; pi < KP * n; pi += 32) {    // cone rows of (candidate k, constraint i) at step 0
-                const int k = pi / n, i = pi - k * n;
+                const int k = divN.div(pi), i = pi - k * n;
                 const float4 ra = rowsA[2 * i], rb = rowsA[2 * i + 1];
                 const float *d = Dc + 12 * k;
                 const float g0 = fmaf(d[0], ra.x, fmaf(d[1], ra.y, d[2] * ra.z));
@@ -365,7 +395,7 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
                 const int it = base + lane;
                 bool dead = true, sure = false;
                 if (it < items) {
-                    const int m = it / KP, k = it - m * KP;
+                    const int m = divKP.div(it), k = it - m * KP;
                     const float sm = sT[m];
                     float M = -CUDART_INF_F, Wmin = CUDART_INF_F;
                     for (int i = 0; i < n; ++i) {
@@ -387,7 +417,7 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
                     const int l = __ffs(alive) - 1;
                     alive &= alive - 1u;
                     const int itl = base + l;
-                    const int m = itl / KP, k = itl - m * KP;
+                    const int m = divKP.div(itl), k = itl - m * KP;
                     double x, y, z, E[9];
                     rng.xi3((uint32_t)s, (uint32_t)candj[k], 1u, x, y, z);
                     exp_so3(L.theta_p * x, L.theta_p * y, L.theta_p * z, E);
@@ -423,7 +453,7 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
             const int it = base + lane;
             bool ok = false;
             if (it < items) {
-                const int m = it / KP, k = it - m * KP;
+                const int m = divKP.div(it), k = it - m * KP;
                 double dT = 1.0;
                 for (int q = 0; q < m; ++q) dT = dT * L.gamma;          // dT_m = gamma^(m-1) by repeated multiplication
                 double tm[3], Rj[9];

@@ -332,12 +332,12 @@ __device__ __forceinline__ void fast_rung_rows(unsigned char *smem_raw, const Co
             float lipv = 0.f;
             const float kv = key_of(w, m0, m1, m2, lipv);
             const uint32_t key = has ? ((fkey(kv) & ~15u) | (uint32_t)c) : (uint32_t)c;
-            const uint32_t k1 = __reduce_max_sync(hm, key);
-            const uint32_t k2 = __reduce_max_sync(hm, key == k1 ? 0u : key);
-            const uint32_t lm = __reduce_max_sync(hm, __float_as_uint(has ? lipv : 0.f));
+            uint32_t k1, k2;
+            float lm;
+            group_top2_max(hm, 16, key, has ? lipv : 0.f, k1, k2, lm);
             if (key == k1) {
                 ridx[m] = make_int2((int)(k1 & 15u), n > 1 ? (int)(k2 & 15u) : (int)(k1 & 15u));
-                qL[m] = __uint_as_float(lm);
+                qL[m] = lm;
             }
         }
     } else {
@@ -512,10 +512,10 @@ __device__ __noinline__ void coop_setup_on_move(unsigned char *smem_raw, int war
                                 g0, g1, g2, fcb, eps);
             float4 r4 = make_float4(g0, g1, g2, has ? fcb - eps : -CUDART_INF_F);
             const uint32_t key = has ? ((fkey(r4.w) & ~15u) | (uint32_t)c) : (uint32_t)c;
-            const uint32_t m1 = __reduce_max_sync(hm, key);
+            uint32_t m1, m2;
+            float lf;
+            group_top2_max(hm, 16, key, has ? (float)sqrt(lip) : 0.f, m1, m2, lf);
             const uint32_t key2 = (key == m1) ? 0u : key;
-            const uint32_t m2 = __reduce_max_sync(hm, key2);
-            const float lf = __uint_as_float(__reduce_max_sync(hm, __float_as_uint(has ? (float)sqrt(lip) : 0.f)));
             const bool dead_any = (__ballot_sync(hm, rdead) & hm) != 0u;
             if (key == m1) {
                 if (dead_any) r4.w = CUDART_INF_F;                     // rung dead for every candidate
@@ -758,8 +758,6 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     const int NCH = 32 / KP;                            // constraint chunks of the full evaluation
     const int ek = lane % KP, ech = lane / KP;
     const bool e_act = ech < NCH;
-    unsigned e_mask = 0u;                               // lanes that share this lane's candidate
-    for (int c = 0; c < NCH; ++c) e_mask |= 1u << (ek + c * KP);
 
     // executed-work counters (closure_get_stats): in shared memory, touched by lane 0 and only when asked for
     unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
@@ -1022,8 +1020,8 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
                             if (RES == kEll) M = fmaxf(M, ell_value(f, QL[2 * i], QL[2 * i + 1], c4));
                             else M = fmaxf(M, fmaf(f.x, c4.x, fmaf(f.y, c4.y, fmaf(f.z, c4.z, f.w))));
                         }
-                        M = fkey_inv(__reduce_max_sync(e_mask, fkey(M)));
                     }
+                    M = chunk_max_to_first(M, KP, NCH);      // valid on the lanes with ech == 0 (`mine` below)
                     // M = max_i (v32_i - eps_i):  M > th  => some constraint violated for sure;
                     // M + 2 eps_max <= th => every constraint satisfied for sure.
                     const bool dead = M > c4.w;
