@@ -635,6 +635,21 @@ def run_cuda(args) -> None:
             big_gbs = big_bytes / (statistics.mean(big_ms) * 1e-3) / 1e9
             comp_big[label] = {"achieved": big_gbs, "frac": big_gbs / hbm_peak, "bytes_per_launch": big_bytes,
                                "ms": statistics.mean(big_ms)}
+        # context for the fraction above: a plain device-to-device copy of the same payload (cudaMemcpyAsync through torch),
+        # timed the same way -- what a kernel-free copy of 402.7 MB reaches of the measured peak on this box
+        copy_ms = []
+        for k in range(7):
+            flush.fill_(k)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            big_o.copy_(big_s, non_blocking=True)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            if k >= 2:
+                copy_ms.append(e0.elapsed_time(e1))
+        copy_gbs = nbig * 96 * 2 / (statistics.mean(copy_ms) * 1e-3) / 1e9
+        comp_big["memcpy_same_payload"] = {"achieved": copy_gbs, "frac": copy_gbs / hbm_peak, "bytes_per_launch": nbig * 96 * 2,
+                                           "ms": statistics.mean(copy_ms)}
         big_s = big_o = None
 
         out = {
@@ -656,7 +671,8 @@ def run_cuda(args) -> None:
                                     "bytes_per_launch": comp_bytes, "peak_source": "MEASURED_PEAKS.json hbm_gbs"
                                     if mp else "fallback 6650",
                                     "at_4194304_walkers": comp_big["all_kept"],
-                                    "at_4194304_walkers_half_kept": comp_big["half_kept"]},
+                                    "at_4194304_walkers_half_kept": comp_big["half_kept"],
+                                    "memcpy_same_payload": comp_big["memcpy_same_payload"]},
             "e2e": e2e,
             "gpu_launches": args.steps * (-(-nb // 96) + 1),     # walker launch(es) + compaction kernel per step
             "clocks": clk,
