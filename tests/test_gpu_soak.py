@@ -3,8 +3,8 @@
 Random config, instance, walk parameters, |S_0|, mode and seed per run; samples and flags must agree bit for bit.
 (The same loop ran for 15 minutes twice in round 1, the second time on the final build with random bound runs and
 body pivots as below: 8,349 + 8,080 runs, 68 M + 66 M walkers, and for 10 minutes on the last build of the round: 9,720
-runs; no mismatch -- DESIGN.md 8.  Round 2 added streams 3 and 4 for the branch-and-bound kernel, N_P <= 32, and ran the
-loop again on the final build.)"""
+runs; no mismatch -- DESIGN.md 8.  Round 2 added streams 3 and 4 for the branch-and-bound kernel, N_P <= 32, and stream 5 for
+the ellipsoid / ellipse norms, and ran the loop again on the final build.)"""
 import copy
 
 import numpy as np
@@ -18,14 +18,17 @@ pytestmark = pytest.mark.gpu
 
 def _n_p_choices(stream):
     # streams 3 and 4: N_P <= 32, the branch-and-bound kernel (best-first on one run of equal bounds, batched otherwise)
+    if stream == 5:
+        return [3, 20, 32, 33, 64, 150, 200]
     return [1, 3, 8, 20, 27, 32] if stream >= 3 else [20, 33, 64, 100, 150, 160, 200, 256]
 
 
-@pytest.mark.parametrize("stream", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("stream", [0, 1, 2, 3, 4, 5])
 def test_random_parameters_bit_identical_to_plain_kernel(stream):
     rng = np.random.default_rng(1000 + stream)
     for _ in range(12):
-        cfg = int(rng.integers(1, 6))
+        # stream 5: the ellipsoid / ellipse norms of eq. (6) (CLOSURE_REG_3D3D_ELL, CLOSURE_REPROJ_2D3D_ELL) on their certified kernels
+        cfg = int(rng.choice([1, 2, 3, 5])) if stream == 5 else int(rng.integers(1, 6))
         inst = I.make_instance(cfg, int(rng.integers(0, 50)))
         if cfg == 4 and rng.random() < 0.3:
             inst = I.to_split(inst)
@@ -44,6 +47,8 @@ def test_random_parameters_bit_identical_to_plain_kernel(stream):
         if cfg in (1, 2, 5) and rng.random() < 0.5:          # several runs of equal bounds, odd lengths
             k = int(rng.integers(1, 5))
             inst.betas = inst.betas * rng.choice([1.0, 1.2, 1.5, 1.9][:k], size=inst.n)
+        if stream == 5:
+            inst = I.to_ellipsoidal(inst, int(rng.integers(0, 100)))
         if P.mode != I.MODE_TRANS and cfg in (1, 2, 3, 5) and rng.random() < 0.3:
             P.pivot = tuple(float(x) for x in rng.uniform(-0.5, 0.5, 3))      # closure_set_pivot (gpu_walk applies it)
         S0 = I.make_init_poses(inst, int(rng.choice([1, 16, 128])))
