@@ -92,6 +92,8 @@ typedef struct {
                                         translations along their principal axes, v <- sqrtm(Cov) / sqrt(lambda_max) v
                                         (PAPER.md:324, 1074-1076); read by closure_set_init */
 #define CLOSURE_FLAG_HOST_MEGB 8    /* closure_megb: copy the cloud to the host and run the miniball there, whatever its size */
+#define CLOSURE_FLAG_ONE_WARP 128   /* rotation sampler, launches of at most 1,184 walkers: keep one warp per walker instead of the
+                                        pair of warps one iteration apart (same results bit for bit; for verification and timing) */
 
 typedef struct closure_s closure_t;   /* opaque; owns device copies of the instance and of S_0 */
 

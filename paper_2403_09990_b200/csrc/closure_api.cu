@@ -250,7 +250,7 @@ void fill_launch(const closure_t *h, WalkLaunch &L)
     L.n_p = h->P.n_p; L.n_p_star = h->P.n_p_star; L.n_t = h->P.n_t;
     L.omega0 = h->P.omega0; L.v0 = h->P.v0; L.gamma = h->P.gamma; L.t_p = h->P.t_p; L.theta_p = h->P.theta_p;
     L.pairs_cap = h->n_pairs;
-    L.exact_only = (h->P.flags & 31) | (h->P.precision == 32 ? 32 : 0);           // bit 0 documented; bits 1-2: debug switches of the screened kernel
+    L.exact_only = (h->P.flags & 31) | (h->P.precision == 32 ? 32 : 0) | (h->P.flags & CLOSURE_FLAG_ONE_WARP ? 64 : 0);           // bit 0 documented; bits 1-2: debug switches of the screened kernel
 }
 
 bool same_params(const closure_params &a, const closure_params &b)

@@ -1081,6 +1081,577 @@ __global__ void __launch_bounds__(kCoopThreads, coop_min_ctas<RES, NQ>()) walker
     }
 }
 
+// ---------------------------------------------------------------------------------- the kernel, two warps per walker
+// For launches that leave the GPU mostly empty (up to kPipeMaxWalkers walkers in all: BASELINE config 1, the paper's own 200
+// walks per instance) the time is one warp's latency per iteration, not throughput.  Here a walker owns a PAIR of warps, one
+// iteration apart: the odd warp (producer) draws the perturbations of iteration s + 1, evaluates eq. (14) and selects the
+// N_P* candidates (a2-a4: what needs the pose only) while the even warp (consumer) walks the ladder of iteration s and updates
+// the pose (a5-a6).  The candidates are handed over through two buffers in shared memory; the warps meet at one named barrier
+// per iteration.  The producer's work is speculative: it assumes that iteration s does not move the walker, which holds for a
+// walker that has reached the boundary (95 % of the iterations at config 1).  When the consumer does accept a move it redoes
+// the set-up, the producer recomputes iteration s + 1 at the new pose (two more barriers), and nothing of the discarded pass
+// is used -- so every decision is the one-warp kernel's, bit for bit (tests/test_gpu_parity.py).  Same code as above otherwise.
+constexpr int kPipeBytes = 32 * 16 + 32 * 4 + 32 * 4 + 16;    // second candidate buffer + the moved flags, per walker
+constexpr long long kPipeMaxWalkers = 148 * 8;                // two CTAs of four walker pairs per SM: everything resident at once
+
+#ifndef CLOSURE_PIPE_WALKERS
+#define CLOSURE_PIPE_WALKERS 4     // walkers (pairs of warps) per CTA
+#endif
+constexpr int kPipeWalkers = CLOSURE_PIPE_WALKERS;
+constexpr int kPipeThreads = 64 * kPipeWalkers;
+
+template <int RES, int NQ>
+__global__ void __launch_bounds__(kPipeThreads, 512 / kPipeThreads) walker_dense_pipe_kernel(const __grid_constant__ WalkLaunch L)
+{
+    using RS = Res<RES>;
+    constexpr int ROW = RS::ROW;
+    constexpr int NPK = NQ / 2;            // packed pairs of perturbations
+    constexpr bool ODD = (NQ & 1) != 0;    // plus one scalar slot
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ int n_runs_s;
+    __shared__ float amax_s;
+    const int warp_raw = threadIdx.x >> 5;
+    // warps w and w + kPipeWalkers serve walker slot w: with four slots the two warps of a walker share a scheduler (warp id mod 4)
+    // and every scheduler holds one producer and one consumer (measured: pairs on adjacent warp ids put all producers, the longer
+    // stage, on two of the four schedulers)
+    const int warp = warp_raw % kPipeWalkers;           // walker slot of the CTA
+    const bool producer = warp_raw >= kPipeWalkers;
+    int lane = threadIdx.x & 31;
+    const InstanceDesc *__restrict__ D = L.desc[blockIdx.y];
+    const int n = D->n;
+    const int rows_bytes = D->rows_bytes;
+    int n_p = L.n_p, n_ps = L.n_p_star, n_t = L.n_t;
+    // Values the iteration uses all the time are made opaque to the compiler: under register pressure it otherwise
+    // re-derives them from special registers and the constant bank inside the loop instead of keeping them in a register.
+#define CLOSURE_PIN_R(x) asm volatile("" : "+r"(x))
+#define CLOSURE_PIN_F(x) asm volatile("" : "+f"(x))
+    CLOSURE_PIN_R(lane); CLOSURE_PIN_R(n_p); CLOSURE_PIN_R(n_ps); CLOSURE_PIN_R(n_t);
+    uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
+    double *rows = reinterpret_cast<double *>(smem_raw + 16);
+    stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
+    const CoopSmem lay = coop_layout(rows_bytes, n, n_t, NQ, 1, L.pairs_cap, kCoopWarps, af_width<RES>(), af_extra<RES>(L.pairs_cap));
+    int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
+    float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
+    int *run_pend = reinterpret_cast<int *>(smem_raw + lay.run_pend);   // end of run r in rowsA, in PAIRS of rows
+    int *pos = reinterpret_cast<int *>(smem_raw + lay.pos);             // row of constraint i in rowsA (bit 30: write it twice)
+    if (warp_raw == 0) {                               // runs of equal bounds (rows are sorted by bound)
+        int cnt = 0;
+        for (int base = 0; base < n; base += 32) {
+            const int i = base + lane;
+            bool end = false;
+            double beta = 0.0;
+            if (i < n) {
+                beta = rows[i * ROW + RS::BETA];
+                end = (i == n - 1) || (rows[(i + 1) * ROW + RS::BETA] != beta);
+            }
+            const unsigned m = __ballot_sync(FULL, end);
+            if (end) {
+                const int r = cnt + __popc(m & ((1u << lane) - 1u));
+                run_end[r] = i;
+                run_bf[r] = (float)beta;
+            }
+            cnt += __popc(m);
+        }
+        __syncwarp();
+        if (lane == 0) {
+            // rowsA holds the fp32 set-ups two constraints per entry; a run of odd length repeats its last
+            // constraint (a maximum does not see duplicates), so no pair straddles two bounds
+            n_runs_s = cnt;
+            int p = 0, start = 0, longest = 0;
+            for (int r = 0; r < cnt; ++r) {
+                const int end = run_end[r];
+                const int p_begin = p >> 1;
+                for (int i = start; i <= end; ++i) pos[i] = p++;
+                if (p & 1) { pos[end] |= 0x40000000; ++p; }
+                run_pend[r] = p >> 1;
+                longest = max(longest, (p >> 1) - p_begin);
+                start = end + 1;
+            }
+        }
+    }
+    if (RES == CLOSURE_REG_3D3D || RES == CLOSURE_POSE_REG) {
+        // fp32 image of the constraints for the set-up's search (fast_rung_rows), and max_i |a_i| for its Lipschitz slack
+        float4 *af = reinterpret_cast<float4 *>(smem_raw + lay.af);
+        float am = 0.f;
+        for (int i = threadIdx.x; i < n; i += kPipeThreads) {
+            const double *row = rows + i * ROW;
+            const float b2 = (float)row[RS::BETA + 1];
+            if (RES == CLOSURE_REG_3D3D) {
+                af[i] = make_float4((float)row[0], (float)row[1], (float)row[2], b2);
+                am = fmaxf(am, (float)sqrt(row[0] * row[0] + row[1] * row[1] + row[2] * row[2]) * 1.000001f);
+            } else {
+                af[3 * i] = make_float4((float)row[0], (float)row[1], (float)row[2], b2);
+                af[3 * i + 1] = make_float4((float)row[3], (float)row[4], (float)row[5], 0.f);
+                af[3 * i + 2] = make_float4((float)row[6], (float)row[7], (float)row[8], 0.f);
+            }
+        }
+        if (RES == CLOSURE_REG_3D3D) {
+            if (threadIdx.x == 0) amax_s = 0.f;
+            __syncthreads();
+            atomicMax(reinterpret_cast<unsigned int *>(&amax_s), __float_as_uint(wmax_nonneg(am)));   // non-negative floats order as uints
+        }
+    }
+    __syncthreads();
+    const int n_runs = n_runs_s;
+    if (RES == kEll) {
+        float4 *QLw = reinterpret_cast<float4 *>(smem_raw + lay.af);
+        float *QAw = reinterpret_cast<float *>(QLw + 2 * n);
+        const float tpq = (float)L.t_p * 1.0000002f;
+        for (int i = threadIdx.x; i < n; i += kPipeThreads) {
+            const double *row = rows + i * ROW;
+            const float q00 = (float)(0.25 * row[8]), q01 = (float)(0.5 * row[9]), q02 = (float)(0.5 * row[10]);
+            const float q11 = (float)(0.25 * row[11]), q12 = (float)(0.5 * row[12]), q22 = (float)(0.25 * row[13]);
+            const float qsum = (fabsf(q00) + fabsf(q01) + fabsf(q02) + fabsf(q11) + fabsf(q12) + fabsf(q22)) * 1.000001f;
+            QLw[2 * i] = make_float4(q00, q01, q02, q11);
+            QLw[2 * i + 1] = make_float4(q12, q22, 4.0f * tpq * tpq * qsum, 0.f);     // qmag = (2 t_p)^2 sum|Q|
+            const int pp = pos[i], p = pp & 0x3fffffff;
+            float *A = QAw + (p >> 1) * 12 + (p & 1);           // (Q00a Q00b Q01a Q01b) (Q02a Q02b Q11a Q11b) (Q12a Q12b Q22a Q22b)
+            A[0] = q00; A[2] = q01; A[4] = q02; A[6] = q11; A[8] = q12; A[10] = q22;
+            if (pp & 0x40000000) { A[1] = q00; A[3] = q01; A[5] = q02; A[7] = q11; A[9] = q12; A[11] = q22; }
+        }
+        __syncthreads();
+    }
+
+    const long long local = (long long)blockIdx.x * kPipeWalkers + warp;
+    if (local >= L.num_walkers) return;                // no block-wide barrier below this line
+    unsigned char *wp = smem_raw + lay.warp0 + (size_t)warp * lay.per_warp;
+    float4 *rowsA = reinterpret_cast<float4 *>(wp + lay.rowsA);
+    float4 *rowsL = reinterpret_cast<float4 *>(wp + lay.rowsL);
+    float4 *pert = reinterpret_cast<float4 *>(wp + lay.pert);
+    double2 *ab = reinterpret_cast<double2 *>(wp + lay.ab);
+    float4 *qrow = reinterpret_cast<float4 *>(wp + lay.qrow);     // [rung][2]: the two tightest rows of each rung
+    double *RmS = reinterpret_cast<double *>(wp + lay.RmS);
+    double *dex = reinterpret_cast<double *>(wp + lay.dex);      // fp64 fallback: exact d_j, [q][lane]
+    float *qL = reinterpret_cast<float *>(wp + lay.qL);           // [rung]: bound on the change of any residual norm
+    // the kept perturbations (-2 d_j, -|d_j|^2) by rank, their indices and upper bounds of their eq. (14) values: two
+    // buffers, iteration s uses buffer s & 1
+    unsigned char *pp = smem_raw + lay.total + (size_t)warp * kPipeBytes;     // behind the one-warp kernel's layout
+    float4 *cand4_0 = reinterpret_cast<float4 *>(wp + lay.cand4), *cand4_1 = reinterpret_cast<float4 *>(pp);
+    int *candj_0 = reinterpret_cast<int *>(wp + lay.candj), *candj_1 = reinterpret_cast<int *>(pp + 512);
+    float *candd_0 = reinterpret_cast<float *>(wp + lay.candd), *candd_1 = reinterpret_cast<float *>(pp + 640);
+    volatile int *moved_flag = reinterpret_cast<volatile int *>(pp + 768);
+    const int bar_id = warp + 1;                                  // named barrier of this walker's pair of warps
+    auto pair_sync = [&]() { asm volatile("bar.sync %0, 64;" ::"r"(bar_id) : "memory"); };
+    double *pose = reinterpret_cast<double *>(wp + lay.pose);     // R*(9) t*(3) omega(3): fp64, touched only on moves / fp64 paths
+    // ellipsoid norm: quadratic-form coefficients of the constraints, by constraint (QL) and by pair-entry of rowsA (QA)
+    const float4 *QL = reinterpret_cast<const float4 *>(smem_raw + lay.af);
+    const float4 *QA = QL + 2 * n;
+    const int2 *ridx = reinterpret_cast<const int2 *>(wp + lay.ridx);
+
+    const unsigned long long w = (unsigned long long)(L.walker_begin + local);
+    const unsigned long long seed = L.seed[blockIdx.y];
+    Rng rng;
+    rng.w_lo = (uint32_t)w;
+    rng.w_hi8 = (uint32_t)(w >> 32) << 8;
+    rng.k0 = (uint32_t)seed;
+    rng.k1 = (uint32_t)(seed >> 32);
+
+    // ---- a1: walker init, replicated on the lanes (Alg. 2 l.8-9): the consumer
+    if (!producer) {
+        double R[9], t[3], vel[3];
+        init_walker<CLOSURE_MODE_ROT>(D, L, rng, w, R, t, vel);
+        for (int m = lane; m < n_t; m += 32) {         // ladder dT_m = gamma^(m-1) by repeated multiplication
+            double dT = 1.0;
+            for (int q = 0; q < m; ++q) dT = dT * L.gamma;
+            const double p0 = dT * vel[0], p1 = dT * vel[1], p2 = dT * vel[2];
+            double A, B;
+            exp_coeffs(fma(p2, p2, fma(p1, p1, p0 * p0)), A, B);
+            ab[m] = make_double2(A * dT, B * dT * dT);
+        }
+        if (lane == 0) {
+#pragma unroll
+            for (int e = 0; e < 9; ++e) pose[e] = R[e];
+#pragma unroll
+            for (int e = 0; e < 3; ++e) { pose[9 + e] = t[e]; pose[12 + e] = vel[e]; }
+        }
+    }
+    __syncwarp();
+
+    const double t_p = L.t_p;
+    const float tpf = (float)t_p * 1.0000002f;          // >= t_p
+    float tp2 = 2.0f * tpf, tp2sq3 = 3.0f * tpf * tpf;
+    float m2tp = -2.0f * (float)t_p;
+    CLOSURE_PIN_F(tp2); CLOSURE_PIN_F(tp2sq3); CLOSURE_PIN_F(m2tp);
+    const int KP = n_ps;                                // ladder candidates
+    const int NCH = 32 / KP;                            // constraint chunks of the full evaluation
+    const int ek = lane % KP, ech = lane / KP;
+    const bool e_act = ech < NCH;
+
+    // executed-work counters (closure_get_stats): in shared memory, touched by lane 0 and only when asked for
+    unsigned long long *stc = reinterpret_cast<unsigned long long *>(wp + lay.stc);
+    const bool stats = false;                           // (launches that count executed work take the one-warp kernel)
+    if (stats) {
+        for (int k = 0; k < kNumStats; ++k) stc[k] = 0ull;
+    }
+    const long long clk_begin = stats ? clock64() : 0ll;
+    bool hit = false;
+    bool moved = true;
+    float epsA = 0.f;
+    double rot_margin = CUDART_INF;
+    // cached across iterations while the pose does not move
+    int full_m = -1;                                    // rung whose rows sit in rowsL
+    float epsL = 0.f;
+    bool rdeadL = false;
+
+    pair_sync();                                        // the walker's pose, velocity and ladder are in shared memory
+    if (producer) {
+        // ============================================================ producer: a2-a4 of iteration s into buffer s & 1
+        int s = 1;
+        bool redo = false;
+        pair_sync();                                    // the first set-up is done
+        while (s <= L.num_steps) {
+            epsA = (float)pose[16];
+            rot_margin = pose[15];
+            float4 *c4b = (s & 1) ? cand4_1 : cand4_0;
+            int *cj = (s & 1) ? candj_1 : candj_0;
+            float *cd = (s & 1) ? candd_1 : candd_0;
+            // ================================================== a2: perturbations of this lane
+            unsigned long long p0[NPK > 0 ? NPK : 1], p1[NPK > 0 ? NPK : 1], p2[NPK > 0 ? NPK : 1];
+            float o0 = 0.f, o1 = 0.f, o2 = 0.f;                  // the odd slot NQ-1
+            float dd[NQ];
+            {
+                int jv[NQ];
+                uint32_t x[NQ], y[NQ], z[NQ];
+    #pragma unroll
+                for (int q = 0; q < NQ; ++q) jv[q] = lane + 32 * q;
+                philox_batch<NQ>(rng, (uint32_t)s, jv, x, y, z);
+                float e0[NQ], e1[NQ], e2[NQ];
+                // packed slots are produced by packed instructions so that they live in aligned register pairs
+                // (same roundings as the scalar pm1f() * m2tp)
+                const unsigned long long C1 = pk2(4.656612873077392578125e-10f, 4.656612873077392578125e-10f);
+                const unsigned long long C2 = pk2(2.3283064365386962890625e-10f - 1.0f, 2.3283064365386962890625e-10f - 1.0f);
+                const unsigned long long M2 = pk2(m2tp, m2tp);
+    #pragma unroll
+                for (int k = 0; k < NPK; ++k) {
+                    p0[k] = mul2(M2, fma2(pk2((float)x[2 * k], (float)x[2 * k + 1]), C1, C2));
+                    p1[k] = mul2(M2, fma2(pk2((float)y[2 * k], (float)y[2 * k + 1]), C1, C2));
+                    p2[k] = mul2(M2, fma2(pk2((float)z[2 * k], (float)z[2 * k + 1]), C1, C2));
+                    upk2(p0[k], e0[2 * k], e0[2 * k + 1]);
+                    upk2(p1[k], e1[2 * k], e1[2 * k + 1]);
+                    upk2(p2[k], e2[2 * k], e2[2 * k + 1]);
+                }
+                if (ODD) { e0[NQ - 1] = m2tp * pm1f(x[NQ - 1]); e1[NQ - 1] = m2tp * pm1f(y[NQ - 1]); e2[NQ - 1] = m2tp * pm1f(z[NQ - 1]); }
+    #pragma unroll
+                for (int q = 0; q < NQ; ++q) {
+                    // (ellipsoid: the pair carries its own quadratic form d^T Lambda_i d, nothing is added per run and thresholds are 0)
+                    dd[q] = RES == kEll ? 0.f : 0.25f * fmaf(e2[q], e2[q], fmaf(e1[q], e1[q], e0[q] * e0[q]));
+                    pert[32 * q + lane] = make_float4(e0[q], e1[q], e2[q], -dd[q]);
+                }
+                if (ODD) { o0 = e0[NQ - 1]; o1 = e1[NQ - 1]; o2 = e2[NQ - 1]; }
+            }
+
+            // ================================================== a3: eq. (14) in fp32 with error bound
+            float dt[NQ];
+            float unc_l = 0.f;
+            {
+    #pragma unroll
+                for (int q = 0; q < NQ; ++q) dt[q] = CUDART_INF_F;
+                const float E0 = epsA + tp2sq3 * kMu19;          // bound on |a32 - a64| up to its own rounding
+                int pp = 0;
+                for (int r = 0; r < n_runs; ++r) {
+                    const int pend = run_pend[r];
+                    const float bf = run_bf[r];
+                    float mx[NQ];
+    #pragma unroll
+                    for (int q = 0; q < NQ; ++q) mx[q] = -CUDART_INF_F;
+    #pragma unroll(NQ <= 2 ? 4 : 1)   // measured: unrolling the NQ = 5 body further costs 2-4 % (C2, C4)
+                    for (; pp < pend; ++pp) {
+                        // two constraints a, b per entry: X = (f0a f0b f1a f1b), Y = (f2a f2b fca fcb)
+                        const float4 X = rowsA[2 * pp], Y = rowsA[2 * pp + 1];
+                        if (RES == kEll) {
+                            // (w, c) as above plus the quadratic form: U = (Q00a Q00b Q01a Q01b) V = (Q02a Q02b Q11a Q11b) W = (Q12a Q12b Q22a Q22b)
+                            const float4 U = QA[3 * pp], V = QA[3 * pp + 1], W = QA[3 * pp + 2];
+    #pragma unroll
+                            for (int k = 0; k < NPK; ++k) {
+                                const unsigned long long ta0 = fma2(pk2(V.x, V.x), p2[k], fma2(pk2(U.z, U.z), p1[k], fma2(pk2(U.x, U.x), p0[k], pk2(X.x, X.x))));
+                                const unsigned long long ta1 = fma2(pk2(W.x, W.x), p2[k], fma2(pk2(V.z, V.z), p1[k], pk2(X.z, X.z)));
+                                const unsigned long long ta2 = fma2(pk2(W.z, W.z), p2[k], pk2(Y.x, Y.x));
+                                const unsigned long long va = fma2(ta0, p0[k], fma2(ta1, p1[k], fma2(ta2, p2[k], pk2(Y.z, Y.z))));
+                                const unsigned long long tb0 = fma2(pk2(V.y, V.y), p2[k], fma2(pk2(U.w, U.w), p1[k], fma2(pk2(U.y, U.y), p0[k], pk2(X.y, X.y))));
+                                const unsigned long long tb1 = fma2(pk2(W.y, W.y), p2[k], fma2(pk2(V.w, V.w), p1[k], pk2(X.w, X.w)));
+                                const unsigned long long tb2 = fma2(pk2(W.w, W.w), p2[k], pk2(Y.y, Y.y));
+                                const unsigned long long vb = fma2(tb0, p0[k], fma2(tb1, p1[k], fma2(tb2, p2[k], pk2(Y.w, Y.w))));
+                                float la, ha, lb, hb;
+                                upk2(va, la, ha);
+                                upk2(vb, lb, hb);
+                                mx[2 * k] = fmaxf(mx[2 * k], fmaxf(la, lb));
+                                mx[2 * k + 1] = fmaxf(mx[2 * k + 1], fmaxf(ha, hb));
+                            }
+                            if (ODD) {                      // the odd slot takes both constraints in one packed chain
+                                const unsigned long long E0o = pk2(o0, o0), E1o = pk2(o1, o1), E2o = pk2(o2, o2);
+                                const unsigned long long t0 = fma2(pk2(V.x, V.y), E2o, fma2(pk2(U.z, U.w), E1o, fma2(pk2(U.x, U.y), E0o, pk2(X.x, X.y))));
+                                const unsigned long long t1 = fma2(pk2(W.x, W.y), E2o, fma2(pk2(V.z, V.w), E1o, pk2(X.z, X.w)));
+                                const unsigned long long t2 = fma2(pk2(W.z, W.w), E2o, pk2(Y.x, Y.y));
+                                const unsigned long long vo = fma2(t0, E0o, fma2(t1, E1o, fma2(t2, E2o, pk2(Y.z, Y.w))));
+                                float lo, hi;
+                                upk2(vo, lo, hi);
+                                mx[NQ - 1] = fmaxf(mx[NQ - 1], fmaxf(lo, hi));
+                            }
+                            continue;
+                        }
+    #pragma unroll
+                        for (int k = 0; k < NPK; ++k) {
+                            const unsigned long long va =
+                                fma2(pk2(X.x, X.x), p0[k], fma2(pk2(X.z, X.z), p1[k], fma2(pk2(Y.x, Y.x), p2[k], pk2(Y.z, Y.z))));
+                            const unsigned long long vb =
+                                fma2(pk2(X.y, X.y), p0[k], fma2(pk2(X.w, X.w), p1[k], fma2(pk2(Y.y, Y.y), p2[k], pk2(Y.w, Y.w))));
+                            float la, ha, lb, hb;
+                            upk2(va, la, ha);
+                            upk2(vb, lb, hb);
+                            mx[2 * k] = fmaxf(mx[2 * k], fmaxf(la, lb));
+                            mx[2 * k + 1] = fmaxf(mx[2 * k + 1], fmaxf(ha, hb));
+                        }
+                        if (ODD) {                          // the odd slot takes both constraints in one packed chain
+                            const unsigned long long vo = fma2(pk2(X.x, X.y), pk2(o0, o0),
+                                                               fma2(pk2(X.z, X.w), pk2(o1, o1),
+                                                                    fma2(pk2(Y.x, Y.y), pk2(o2, o2), pk2(Y.z, Y.w))));
+                            float lo, hi;
+                            upk2(vo, lo, hi);
+                            mx[NQ - 1] = fmaxf(mx[NQ - 1], fmaxf(lo, hi));
+                        }
+                    }
+    #pragma unroll
+                    for (int q = 0; q < NQ; ++q) {
+                        // a ~ max_i |u_i - d|^2 within E0 + 2^-22 a;  sq ~ sqrt(a) within 2^-21 relative
+                        const float a = fmaxf(mx[q] + dd[q], 1e-30f);
+                        const float rr = rsqrt_normal(a);
+                        const float sq = a * rr;
+                        const float du = 1.01f * fmaf(E0, rr, (bf + sq) * kMu19);
+                        unc_l = fmaxf(unc_l, du);
+                        dt[q] = fminf(dt[q], bf - sq);
+                    }
+                }
+                if (stats) stc[6] += (unsigned long long)n * n_p;
+            }
+
+            // ================================================== a4: top-N_P* with certified ranking
+            const float rmf = (float)rot_margin;                // +inf unless POSE_REG_SPLIT
+            float dv[NQ];
+    #pragma unroll
+            for (int q = 0; q < NQ; ++q) dv[q] = (lane + 32 * q < n_p) ? fminf(dt[q], rmf) : -CUDART_INF_F;
+            float unc = wmax_nonneg(unc_l), myval;
+            if (RES == CLOSURE_POSE_REG_SPLIT) unc += 1.2e-7f * fabsf(rmf);
+            // (exact_only & 4: debug, every step takes the fp64 fall-back; & 16: on all N_P perturbations)
+            if (!topk_certified<NQ>(dv, n_ps, unc, (L.exact_only & 4) != 0, (L.exact_only & 32) != 0, lane, cj, cd, myval)) {
+                double R[9], t[3];
+    #pragma unroll
+                for (int e = 0; e < 9; ++e) R[e] = pose[e];
+    #pragma unroll
+                for (int e = 0; e < 3; ++e) t[e] = pose[9 + e];
+                const ExactMargin<RES> exact{ R, t, rows, n, rng, (uint32_t)s, t_p, rot_margin };
+                const int cnt = topk_fp64<NQ>(dv, n_p, n_ps, unc, myval, (L.exact_only & 16) != 0, lane, dex, cj, cd, exact);
+                if (stats) { stc[8] += 1; stc[0] += (unsigned long long)n * cnt; }
+            }
+            __syncwarp();                                       // pert[], cj[] visible to all lanes
+            if (lane < n_ps) c4b[lane] = pert[cj[lane]];
+            __syncwarp();
+            pair_sync();                                // candidates of iteration s are ready; the consumer has decided s - 1
+            if (s > 1 && !redo && moved_flag[(s - 1) & 1] != 0) {
+                pair_sync();                            // iteration s - 1 moved the walker: wait for the set-up, then redo s
+                redo = true;
+                continue;
+            }
+            redo = false;
+            ++s;
+        }
+        return;
+    }
+    // ================================================================ consumer: set-ups, a5-a6 of iteration s, pose update
+    {
+        const long long c0 = stats ? clock64() : 0ll;
+        coop_setup_on_move<RES>(smem_raw, warp, lane, rows_bytes, n, n_t, NQ, L.pairs_cap, t_p, amax_s, stats);
+        if (stats) stc[10] += (unsigned long long)(clock64() - c0);
+        epsA = (float)pose[16];
+        rot_margin = pose[15];
+        full_m = -1;
+    }
+    pair_sync();
+    for (int s = 1; s <= L.num_steps; ++s) {
+        pair_sync();                                    // candidates of iteration s are ready
+        if (s > 1 && moved) {
+            const long long c0 = stats ? clock64() : 0ll;
+            coop_setup_on_move<RES>(smem_raw, warp, lane, rows_bytes, n, n_t, NQ, L.pairs_cap, t_p, amax_s, stats);
+            if (stats) stc[10] += (unsigned long long)(clock64() - c0);
+            epsA = (float)pose[16];
+            rot_margin = pose[15];
+            full_m = -1;
+            pair_sync();                                // set-up done: the producer recomputes iteration s
+            pair_sync();                                // ... and is done
+        }
+        const float4 *c4b = (s & 1) ? cand4_1 : cand4_0;
+        const int *cj = (s & 1) ? candj_1 : candj_0;
+        const float *cd = (s & 1) ? candd_1 : candd_0;
+        // ================================================== a5-a6: ladder, first feasible rung
+        int m0 = 0;
+        unsigned win = 0u;
+        bool lip_stop = false;
+        const int khalf = (KP + 1) >> 1;
+        for (int mb = 0; mb < n_t && m0 == 0 && !lip_stop; mb += 16) {
+            // ---- screening of 16 rungs, lane = (rung, half of the candidates): a candidate is dead for sure
+            // at rung m if one of the two tightest rows is violated beyond its error bound, or if its margin
+            // at R* is more negative than the rotation to R_m (or any smaller one: qL is a suffix maximum)
+            // can repair
+            const int mq = mb + (lane & 15), hq = lane >> 4;
+            const bool q_act = mq < n_t;
+            unsigned alive = 0u;
+            float Lm = CUDART_INF_F;
+            if (q_act) {
+                const float4 r0 = qrow[2 * mq], r1 = qrow[2 * mq + 1];
+                Lm = qL[mq];
+                const int k1 = min(KP, (hq + 1) * khalf);
+                if (RES == kEll) {
+                    const int2 ii = ridx[mq];
+                    const float4 A0 = QL[2 * ii.x], B0 = QL[2 * ii.x + 1], A1 = QL[2 * ii.y], B1 = QL[2 * ii.y + 1];
+                    for (int k = hq * khalf; k < k1; ++k) {
+                        const float4 c4 = c4b[k];
+                        const float v0 = ell_value(r0, A0, B0, c4), v1 = ell_value(r1, A1, B1, c4);
+                        if (!(v0 > c4.w) && !(v1 > c4.w) && !(cd[k] + Lm < 0.f)) alive |= 1u << k;
+                    }
+                } else {
+                for (int k = hq * khalf; k < k1; ++k) {
+                    const float4 c4 = c4b[k];
+                    const float v0 = fmaf(r0.x, c4.x, fmaf(r0.y, c4.y, fmaf(r0.z, c4.z, r0.w)));
+                    const float v1 = fmaf(r1.x, c4.x, fmaf(r1.y, c4.y, fmaf(r1.z, c4.z, r1.w)));
+                    if (!(v0 > c4.w) && !(v1 > c4.w) && !(cd[k] + Lm < 0.f)) alive |= 1u << k;
+                }
+                }
+            }
+            alive |= __shfl_xor_sync(FULL, alive, 16);
+            if (L.exact_only & 2) alive = q_act ? ((KP >= 32) ? FULL : ((1u << KP) - 1u)) : 0u;   // debug: nothing is screened out
+            if (mb + 16 < n_t && !(L.exact_only & 2)) {
+                // no candidate can be repaired at the last rung of this block => none at any later rung
+                float cdm = cd[0];
+                for (int k = 1; k < KP; ++k) cdm = fmaxf(cdm, cd[k]);
+                if (cdm + qL[mb + 15] < 0.f) lip_stop = true;
+            }
+            unsigned qmask = __ballot_sync(FULL, lane < 16 && alive != 0u);
+            if (stats) stc[7] += (unsigned long long)(min(n_t, mb + 16) - mb) * 2 * KP;
+
+            // ---- full evaluation of the surviving rungs, in order
+            while (qmask != 0u && m0 == 0) {
+                const int l0 = __ffs(qmask) - 1;
+                qmask &= qmask - 1u;
+                const int m1 = mb + l0;
+                const unsigned cand_alive = __shfl_sync(FULL, alive, l0);
+                double Rm[9], t[3];
+#pragma unroll
+                for (int e = 0; e < 9; ++e) Rm[e] = RmS[m1 * 9 + e];
+#pragma unroll
+                for (int e = 0; e < 3; ++e) t[e] = pose[9 + e];
+                if (full_m != m1) {
+                    __syncwarp();                            // earlier readers of rowsL are done
+                    float eps_l = 0.f;
+                    bool rdead = false;
+#pragma unroll 1
+                    for (int i = lane; i < n; i += 32) {
+                        const double *row = rows + i * ROW;
+                        double u0, u1, u2, c;
+                        pair_setup<RES>(Rm, t, row, u0, u1, u2, c);
+                        if (RES == CLOSURE_POSE_REG_SPLIT) {
+                            if (!(frob_sq(Rm, row) <= row[13])) rdead = true;     // exact: no perturbation involved
+                        }
+                        float g0, g1, g2, fcb, eps;
+                        screen_row_any<RES>(u0, u1, u2, c - row[RS::BETA + 1], tp2, tp2sq3, RES == kEll ? QL[2 * i + 1].z : 0.f,
+                                            g0, g1, g2, fcb, eps);
+                        rowsL[i] = make_float4(g0, g1, g2, fcb - eps);
+                        eps_l = fmaxf(eps_l, eps);
+                    }
+                    epsL = wmax_nonneg(eps_l);
+                    rdeadL = __any_sync(FULL, rdead);
+                    full_m = m1;
+                    if (stats) stc[3] += n;
+                    __syncwarp();
+                }
+                if (stats) { stc[9] += 1; stc[7] += (unsigned long long)n * KP; }
+                unsigned feas = 0u;
+                if (!rdeadL) {
+                    float M = -CUDART_INF_F;
+                    float4 c4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (e_act) {
+                        c4 = c4b[ek];
+                        for (int i = ech; i < n; i += NCH) {
+                            const float4 f = rowsL[i];
+                            if (RES == kEll) M = fmaxf(M, ell_value(f, QL[2 * i], QL[2 * i + 1], c4));
+                            else M = fmaxf(M, fmaf(f.x, c4.x, fmaf(f.y, c4.y, fmaf(f.z, c4.z, f.w))));
+                        }
+                    }
+                    M = chunk_max_to_first(M, KP, NCH);      // valid on the lanes with ech == 0 (`mine` below)
+                    // M = max_i (v32_i - eps_i):  M > th  => some constraint violated for sure;
+                    // M + 2 eps_max <= th => every constraint satisfied for sure.
+                    const bool dead = M > c4.w;
+                    const bool sure = (epsL < CUDART_INF_F) && (M <= c4.w - 2.0f * epsL);
+                    const bool mine = e_act && ech == 0;
+                    unsigned alive2 = __ballot_sync(FULL, mine && !dead) & cand_alive;
+                    unsigned undecided = __ballot_sync(FULL, mine && !dead && !sure) & cand_alive;
+                    if (L.exact_only & 2) { alive2 = cand_alive; undecided = cand_alive; }
+                    if (L.exact_only & 32) { alive2 &= ~undecided; undecided = 0u; }   // fp32 mode: undecided counts as VIOLATED, so every emitted sample stays inside S (Prop. 4)
+                    while (undecided != 0u) {                // rare: fp64 decides
+                        const int k = __ffs(undecided) - 1;
+                        undecided &= undecided - 1u;
+                        if (!exact_candidate_feasible<RES>(Rm, t, rows, n, rng, (uint32_t)s, cj[k], t_p, lane))
+                            alive2 &= ~(1u << k);
+                        if (stats) stc[1] += n;
+                    }
+                    feas = alive2;
+                }
+                if (feas != 0u) { m0 = m1 + 1; win = feas; }
+            }
+        }
+
+        int j_win = 0;
+        if (m0) {
+            const int kw = __ffs(win) - 1;                    // lowest rank among the feasible (R-8)
+            j_win = cj[kw];
+            double x, y, z;
+            rng.xi3((uint32_t)s, (uint32_t)j_win, 1u, x, y, z);
+            const double t0 = __dadd_rn(pose[9], __dmul_rn(t_p, x));
+            const double t1 = __dadd_rn(pose[10], __dmul_rn(t_p, y));
+            const double t2 = __dadd_rn(pose[11], __dmul_rn(t_p, z));
+            const double re = (lane < 9) ? RmS[(m0 - 1) * 9 + lane] : 0.0;
+            __syncwarp();
+            if (lane < 9) pose[lane] = re;
+            if (lane == 9) { pose[9] = t0; pose[10] = t1; pose[11] = t2; }
+            if (stats) stc[4] += 1;
+        }
+        moved = (m0 != 0);
+        if (m0 != 1) hit = true;                              // R-12 (R-11: nothing feasible -> unchanged)
+        if (L.out_trace != nullptr && lane == 0)
+            L.out_trace[((size_t)blockIdx.y * L.num_walkers + local) * L.num_steps + (s - 1)] = m0 | (j_win << 8);
+        __syncwarp();                                         // RmS readers done before the next step writes
+        if (lane == 0) moved_flag[s & 1] = moved ? 1 : 0;
+    }
+
+    // ---- a7: emit
+    if (lane == 0) {
+        const size_t o = (size_t)blockIdx.y * L.num_walkers + local;
+        double2 *dst = reinterpret_cast<double2 *>(L.out_samples + 12 * o);
+#pragma unroll
+        for (int e = 0; e < 6; ++e) dst[e] = make_double2(pose[2 * e], pose[2 * e + 1]);
+        L.out_flags[o] = hit ? 1 : 0;
+        if (stats) {
+            stc[5] = (unsigned long long)L.num_steps;
+            stc[11] = (unsigned long long)(clock64() - clk_begin);
+            for (int k = 0; k < kNumStats; ++k) atomicAdd(L.stats + k, stc[k]);
+        }
+    }
+}
+
+
+template <int RES, int NQ>
+cudaError_t launch_pipe_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
+{
+    const CoopSmem lay = coop_layout(max_rows_bytes, max_n, L.n_t, NQ, 1, L.pairs_cap, kCoopWarps, af_width<RES>(), af_extra<RES>(L.pairs_cap));
+    const size_t smem = lay.total + (size_t)kCoopWarps * kPipeBytes;        // (laid out for kCoopWarps >= kPipeWalkers walkers)
+    if (smem > 100 * 1024) return cudaErrorInvalidConfiguration;               // two CTAs per SM
+    cudaError_t e = cudaFuncSetAttribute(walker_dense_pipe_kernel<RES, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const long long blocks = (L.num_walkers + kPipeWalkers - 1) / kPipeWalkers;
+    dim3 grid((unsigned)blocks, (unsigned)n_instances, 1);
+    walker_dense_pipe_kernel<RES, NQ><<<grid, kPipeThreads, smem, stream>>>(L);
+    return cudaGetLastError();
+}
+
 template <int RES, int NQ>
 cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
 {
@@ -1099,6 +1670,14 @@ cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, i
 template <int RES>
 cudaError_t launch_r(const WalkLaunch &L, int n_instances, int max_rows_bytes, int max_n, cudaStream_t stream)
 {
+    // launches that leave the GPU mostly empty: two warps per walker, one iteration apart (walker_dense_pipe_kernel)
+    if (L.stats == nullptr && !(L.exact_only & 64) && L.num_walkers * (long long)n_instances <= kPipeMaxWalkers) {
+        cudaError_t e = cudaErrorInvalidConfiguration;
+        if (L.n_p <= 64) e = launch_pipe_q<RES, 2>(L, n_instances, max_rows_bytes, max_n, stream);
+        else if (L.n_p <= 160) e = launch_pipe_q<RES, 5>(L, n_instances, max_rows_bytes, max_n, stream);
+        else e = launch_pipe_q<RES, 8>(L, n_instances, max_rows_bytes, max_n, stream);
+        if (e != cudaErrorInvalidConfiguration) return e;
+    }
     if (L.n_p <= 64) return launch_q<RES, 2>(L, n_instances, max_rows_bytes, max_n, stream);
     if (L.n_p <= 160) return launch_q<RES, 5>(L, n_instances, max_rows_bytes, max_n, stream);
     return launch_q<RES, 8>(L, n_instances, max_rows_bytes, max_n, stream);

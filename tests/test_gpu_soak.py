@@ -52,7 +52,8 @@ def test_random_parameters_bit_identical_to_plain_kernel(stream):
         if P.mode != I.MODE_TRANS and cfg in (1, 2, 3, 5) and rng.random() < 0.3:
             P.pivot = tuple(float(x) for x in rng.uniform(-0.5, 0.5, 3))      # closure_set_pivot (gpu_walk applies it)
         S0 = I.make_init_poses(inst, int(rng.choice([1, 16, 128])))
-        W, S, seed = 2048, int(rng.choice([50, 150])), int(rng.integers(0, 1 << 40))
+        # 1,024 walkers: the dense kernel's two-warps-per-walker form (launches of at most 1,184 walkers); 2,048: one warp per walker
+        W, S, seed = int(rng.choice([1024, 2048])), int(rng.choice([50, 150])), int(rng.integers(0, 1 << 40))
         a = gpu_walk(inst, P, S0, W, S, seed, trace=False)
         b = gpu_walk(inst, copy.copy(P).__class__(**{**vars(P), "flags": P.flags | 1}), S0, W, S, seed, trace=False)
         assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]), (cfg, inst.name, vars(P), S0.shape[0], S, seed)
