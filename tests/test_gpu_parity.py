@@ -129,6 +129,66 @@ def test_batch_members_with_different_tables():
             h.closure_destroy()
 
 
+FLAG_ONE_WARP = 128      # CLOSURE_FLAG_ONE_WARP (include/closure.h)
+
+
+@pytest.mark.parametrize("config,walkers,steps,extra", [
+    (1, 1024, 200, {}),                        # BASELINE config 1 at full size
+    (1, 1, 30, {}), (1, 3, 30, {}), (2, 5, 1, {}), (2, 7, 2, {}),          # partly filled CTAs, one and two iterations
+    (2, 1184, 40, {}), (2, 1185, 40, {}),      # the largest launch on the two-warp kernel, the first one on the one-warp kernel
+    (4, 1000, 120, {}),                        # pose regression
+    (2, 600, 60, dict(flags=2)), (2, 600, 60, dict(flags=4)), (1, 600, 60, dict(flags=20)),      # forced fp64 fall-backs
+    (2, 512, 80, dict(precision=32)),          # fp32 mode
+    (2, 700, 50, dict(n_p=40, n_p_star=4, n_t=8)), (1, 700, 50, dict(n_p=200, n_p_star=10, n_t=17)),   # NQ = 2 and 8
+    (2, 400, 60, dict(omega0=2.0, t_p=0.2)),   # many accepted moves: the producer's speculation is discarded often
+])
+def test_two_warps_per_walker_kernel_is_bit_identical_to_one_warp_kernel(config, walkers, steps, extra):
+    """Launches of at most 1,184 walkers run walker_dense_pipe_kernel (a pair of warps per walker, one iteration apart:
+    DESIGN.md 6.1b); CLOSURE_FLAG_ONE_WARP keeps walker_dense_kernel.  Samples, flags and per-iteration traces must agree
+    bit for bit, and with the plain fp64 kernel where that applies."""
+    inst = I.make_instance(config)
+    S0 = I.make_init_poses(inst, 32)
+    P = _small(inst.params, **extra)
+    pipe = gpu_walk(inst, P, S0, walkers, steps, 909)
+    one = gpu_walk(inst, _small(P, flags=P.flags | FLAG_ONE_WARP), S0, walkers, steps, 909)
+    for a, b in zip(pipe, one):
+        assert np.array_equal(a, b)
+    if getattr(P, "precision", 64) == 64:
+        plain = gpu_walk(inst, _small(P, flags=1), S0, walkers, steps, 909)
+        for a, b in zip(pipe, plain):
+            assert np.array_equal(a, b)
+
+
+def test_two_warps_per_walker_kernel_in_a_batch_and_on_the_ellipsoid_norm():
+    """closure_sample_batch with 3 x 300 walkers in all (one launch of the two-warp kernel with blockIdx.y = instance) equals the
+    members' single launches; the ellipsoid norm of Ex.2 on the two-warp kernel equals its one-warp kernel."""
+    import torch
+    insts = [I.make_instance(1, k) for k in range(3)]
+    hs = []
+    try:
+        for it in insts:
+            h = B.Closure.closure_create(it, it.params)
+            h.closure_set_init(I.make_init_poses(it, 16))
+            hs.append(h)
+        smp, flag = B.closure_sample_batch(hs, 300, 60, [11, 12, 13])
+        torch.cuda.synchronize()
+        for b, h in enumerate(hs):
+            h.closure_set_params(_small(insts[b].params, flags=FLAG_ONE_WARP))
+            s1, f1 = h.closure_sample(300, 60, 11 + b)
+            torch.cuda.synchronize()
+            assert np.array_equal(s1.cpu().numpy(), smp[b].cpu().numpy())
+            assert np.array_equal(f1.cpu().numpy(), flag[b].cpu().numpy())
+    finally:
+        for h in hs:
+            h.closure_destroy()
+    inst = I.to_ellipsoidal(I.make_instance(2), 4)
+    S0 = I.make_init_poses(inst, 32)
+    pipe = gpu_walk(inst, inst.params, S0, 900, 80, 31)
+    one = gpu_walk(inst, _small(inst.params, flags=FLAG_ONE_WARP), S0, 900, 80, 31)
+    for a, b in zip(pipe, one):
+        assert np.array_equal(a, b)
+
+
 @pytest.mark.parametrize("walkers", [1, 31, 127, 128, 129])
 def test_walker_count_edges(walkers):
     inst = I.make_instance(1)
