@@ -197,6 +197,7 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
         }
     }
     float uncA = CUDART_INF_F, tauMax = CUDART_INF_F, ewMax = CUDART_INF_F;
+    int i_tight = 0;
     bool moved = true;
     const int KP = n_ps;
     const int items = KP * n_t;                          // ladder candidates, in Alg. A8's order (m, k)
@@ -214,6 +215,7 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
                 const double th = 1.7320508075688772 * L.theta_p;
                 const double eD = 2.0 * kU * (13.5 * th + 13.0 * th * th);          // |D32 - D64| per entry
                 float unc_l = 0.f, tau_l = 0.f, ew_l = 0.f;
+                uint32_t tight_l = 0u;                                              // (key of the cone value at the pose | constraint)
                 for (int i = lane; i < n; i += 32) {
                     const double *row = rows + i * Res<RES>::ROW;
                     double P0, P1, P2;
@@ -222,6 +224,7 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
                     const double z0 = fabs(zs0), z1 = fabs(zs1);
                     const double b0 = P0 + t[0], b1 = P1 + t[1], b2 = P2 + t[2];
                     const double A0 = zs0 * b2 - K[0] * b0, A1 = zs1 * b2 - K[1] * b1;
+                    tight_l = max(tight_l, (fkey((float)(A0 * A0 + A1 * A1 - (beta * b2) * (beta * b2))) & ~0xFFFu) | (uint32_t)i);
                     const double Pn = sqrt(P0 * P0 + P1 * P1 + P2 * P2), P1n = fabs(P0) + fabs(P1) + fabs(P2);
                     const double dhi = th * Pn * 1.01;                              // |D P| <= 2 sin(th/2) |P| <= th |P|
                     const double Ed = (eD + 4.0 * kU * th) * P1n + 3.0 * kU * dhi + 1e-13;   // error of each (D P)_r
@@ -256,6 +259,7 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
                 }
                 tauMax = wmax_nonneg(tau_l);
                 ewMax = wmax_nonneg(ew_l);
+                i_tight = min((int)(__reduce_max_sync(FULL, tight_l) & 0xFFFu), n - 1);     // where the ladder's constraint loop starts
                 uncA = wmax_nonneg(unc_l);
                 __syncwarp();
             }
@@ -394,23 +398,35 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
             for (int base = 0; base < items && win < 0; base += 32) {
                 const int it = base + lane;
                 bool dead = true, sure = false;
-                if (it < items) {
-                    const int m = divKP.div(it), k = it - m * KP;
+                int done = 0;
+                {
+                    // All lanes run the constraint loop (idle ones on item 0) so that the warp can leave it together: it starts
+                    // at the constraint that is tightest at the current pose (i_tight, chosen at the set-up) and ends as soon as
+                    // every candidate of the round is violated for sure -- a maximum only grows, so the rest cannot change that.
+                    const bool act = it < items;
+                    const int itc = act ? it : 0;
+                    const int m = divKP.div(itc), k = itc - m * KP;
                     const float sm = sT[m];
                     float M = -CUDART_INF_F, Wmin = CUDART_INF_F;
-                    for (int i = 0; i < n; ++i) {
+                    int i = i_tight;
+                    while (done < n) {
                         const float4 kr = krow[i * KP + k], cr = crow[i];          // [i][k]: lanes of a round differ in k
                         const float q0 = fmaf(sm, cr.x, kr.x), q1 = fmaf(sm, cr.y, kr.y), w = fmaf(sm, cr.z, kr.z);
                         M = fmaxf(M, fmaf(q0, q0, fmaf(q1, q1, fmaf(-w, w, cr.w))));
                         Wmin = fminf(Wmin, w);
+                        ++done;
+                        if (++i == n) i = 0;
+                        if (__all_sync(FULL, !act || M > 0.f)) break;
                     }
                     // g32 - tau > 0: violated for sure (behind the camera counts as violated either way, R-10);
                     // satisfied for sure needs every g32 + tau <= 0 and beta p_3 > 0 beyond its error
-                    dead = M > 0.f;
-                    sure = (tauMax < CUDART_INF_F) && (M <= -2.0f * tauMax) && (Wmin > ewMax);
-                    if (L.exact_only & 2) { dead = false; sure = false; }
+                    if (act) {
+                        dead = M > 0.f;
+                        sure = (tauMax < CUDART_INF_F) && (M <= -2.0f * tauMax) && (Wmin > ewMax);
+                        if (L.exact_only & 2) { dead = false; sure = false; }
+                    }
                 }
-                if (stats) stc[7] += (unsigned long long)n * min(32, items - base);
+                if (stats) stc[7] += (unsigned long long)done * min(32, items - base);
                 unsigned alive = __ballot_sync(FULL, !dead);
                 const unsigned sures = __ballot_sync(FULL, sure);
                 while (alive != 0u && win < 0) {             // in Alg. A8's order; undecided ones go to fp64
