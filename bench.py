@@ -70,9 +70,12 @@ def _csrc_hash() -> str:
     return h.hexdigest()[:16]
 
 
-def _traffic(workload: str, mode: str, precision: int):
+def _traffic(workload: str, mode: str, precision: int, walkers: int, iterations: int, instances: int):
+    """DRAM bytes of the walker launch from the committed capture of this very launch (same sources, same size), else None."""
     e = NCU_TRAFFIC_BYTES.get(f"{workload}/{mode}/{precision}")
     if not e or e.get("csrc_hash") != _csrc_hash():
+        return None
+    if (e.get("walkers"), e.get("iterations"), e.get("instances")) != (walkers, iterations, instances):
         return None
     return e.get("bytes")
 
@@ -349,7 +352,7 @@ def roofline_of(wl: Workload, walk_s: float, peaks: dict, seed: int = WALK_SEED)
     t_alg = t_min + extra32 / peak32
     roof = {"bound": "alu", "kernel": wl.kernel, "achieved": flops_alg / walk_s / 1e12, "peak": flops_alg / t_alg / 1e12,
             "unit": "TFLOP/s", "frac": t_alg / walk_s,
-            "traffic": _traffic(inst.name, wl.mode, wl.precision),
+            "traffic": _traffic(inst.name, wl.mode, wl.precision, wl.W, wl.S, wl.nb),
             "definition": "achieved = algorithmic flops per launch (7 x N_P x N eq. (14) pairs per walker-step + executed ladder "
                           "pairs and set-ups) / kernel time; peak = the same flops / (fp64 flops / DFMA peak + fp32 flops / FFMA "
                           "peak), both peaks measured in this run by closure_alu_peak (register-resident FMA chains)",
