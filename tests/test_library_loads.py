@@ -93,3 +93,25 @@ def test_host_miniball_against_oracle_definition(lib):
     assert B.closure_miniball_host(np.ones((5, 3)))[1] == 0.0
     with pytest.raises(B.ClosureError):
         B.closure_miniball_host(np.zeros((3, 5)))
+
+
+def test_bench_traffic_lookup_is_keyed_to_sources_and_launch_size():
+    """bench.py's `roofline.traffic` comes from committed ncu captures: an entry counts only for the sources it was taken
+    on and for the very launch it was taken on (walkers, iterations, instances); anything else reads as null."""
+    import bench
+    from paper_2403_09990_b200 import instances as I
+    assert bench.NCU_TRAFFIC_BYTES, "profiles/ncu_traffic.json missing or unreadable"
+    h = bench._csrc_hash()
+    for key, e in bench.NCU_TRAFFIC_BYTES.items():
+        workload, mode, precision = key.split("/")
+        cfg = int(workload[1])
+        inst = I.make_instance(cfg)
+        assert inst.name == workload
+        # every entry states the full-size launch of its config
+        assert (e["walkers"], e["iterations"], e["instances"]) == (inst.num_walkers, inst.num_steps, inst.batch)
+        assert e["bytes"] == e["read"] + e["write"]
+        got = bench._traffic(workload, mode, int(precision), e["walkers"], e["iterations"], e["instances"])
+        assert got == (e["bytes"] if e["csrc_hash"] == h else None)
+        assert bench._traffic(workload, mode, int(precision), e["walkers"] // 2, e["iterations"], e["instances"]) is None
+        assert bench._traffic(workload, mode, int(precision), e["walkers"], e["iterations"] + 1, e["instances"]) is None
+    assert bench._traffic("C9_nothing", "rot", 64, 1, 1, 1) is None
