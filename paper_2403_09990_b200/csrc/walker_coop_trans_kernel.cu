@@ -59,7 +59,9 @@ template <int RES> constexpr int kTransWarps = (RES == CLOSURE_REPROJ_2D3D) ? 1 
 
 constexpr int kKrowMax = 512;                  // (candidate, constraint) rows of the certified ladder
 
-__host__ __device__ inline TransSmem trans_layout(int rows_bytes, int nq, int n_fast, int warps)
+// krows: (candidate, constraint) rows of the certified ladder that the launch can need (0: none) -- sized by N_P* x N, not by
+// kKrowMax, so that 16 one-warp CTAs of a short reprojection table fit an SM (at kKrowMax rows shared memory allowed 14)
+__host__ __device__ inline TransSmem trans_layout(int rows_bytes, int nq, int n_fast, int krows, int warps)
 {
     TransSmem s;
     size_t o = 16 + (size_t)((rows_bytes + 15) & ~15);
@@ -77,7 +79,7 @@ __host__ __device__ inline TransSmem trans_layout(int rows_bytes, int nq, int n_
     s.crow = w;  w += (size_t)n_fast * 16;       // per constraint: shift of the cone row per unit step along v, -tau
     s.betaf = w; w += (size_t)((n_fast * 4 + 15) & ~15);
     s.Dc = w;    w += (n_fast ? 32 * 12 * 4 : 0);               // D = Exp - I of the kept perturbations (fp32)
-    s.krow = w;  w += (n_fast ? (size_t)kKrowMax * 16 : 0);     // cone rows of (candidate, constraint) at step 0
+    s.krow = w;  w += (n_fast ? (size_t)krows * 16 : 0);        // cone rows of (candidate, constraint) at step 0
     s.sT = w;    w += (n_fast ? 64 * 4 : 0);                    // ladder steps dT_m in fp32
     s.per_warp = w;
     s.total = o + (size_t)warps * w;
@@ -117,7 +119,8 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
     uint64_t *bar = reinterpret_cast<uint64_t *>(smem_raw);
     const double *rows = reinterpret_cast<const double *>(smem_raw + 16);
     stage_rows(smem_raw + 16, bar, D->rows, rows_bytes);                        // a0 (TMA bulk copy)
-    const TransSmem lay = trans_layout(rows_bytes, NQ, RES == CLOSURE_REPROJ_2D3D ? n : 0, kTransWarps<RES>);
+    const TransSmem lay = trans_layout(rows_bytes, NQ, RES == CLOSURE_REPROJ_2D3D ? n : 0,
+                                       n_ps * n <= kKrowMax ? n_ps * n : 0, kTransWarps<RES>);   // as fast_ladder below
     __shared__ int n_runs_s;
     int *run_end = reinterpret_cast<int *>(smem_raw + lay.run_end);
     float *run_bf = reinterpret_cast<float *>(smem_raw + lay.run_bf);
@@ -533,7 +536,11 @@ __global__ void __launch_bounds__(32 * kTransWarps<RES>, CLOSURE_COOP_MIN_CTAS *
 template <int RES, int NQ>
 cudaError_t launch_q(const WalkLaunch &L, int n_instances, int max_rows_bytes, cudaStream_t stream)
 {
-    const TransSmem lay = trans_layout(max_rows_bytes, NQ, RES == CLOSURE_REPROJ_2D3D ? max_rows_bytes / (Res<RES>::ROW * 8) : 0, kTransWarps<RES>);
+    // the largest table of the batch bounds every instance's layout (an instance with fewer constraints needs at most as much)
+    const int n_max = max_rows_bytes / (Res<RES>::ROW * 8);
+    const long long kr = (long long)L.n_p_star * n_max;
+    const TransSmem lay = trans_layout(max_rows_bytes, NQ, RES == CLOSURE_REPROJ_2D3D ? n_max : 0,
+                                       (int)(kr < kKrowMax ? kr : kKrowMax), kTransWarps<RES>);
     if (lay.total > 200 * 1024) return cudaErrorInvalidConfiguration;
     cudaError_t e = cudaFuncSetAttribute(walker_coop_trans_kernel<RES, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)lay.total);
