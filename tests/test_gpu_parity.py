@@ -595,3 +595,33 @@ def test_ellipsoidal_api_edges():
         with pytest.raises(B.ClosureError) as e:
             B.Closure.closure_create(broken)
         assert e.value.status == B.EINVAL
+
+
+def test_trans_batch_members_with_different_reprojection_tables():
+    """Translation sampler, closure_sample_batch over reprojection instances whose tables differ in length: the launch sizes
+    the certified ladder's row buffer (N_P* x N rows) for the largest table, every member lays its own out from its own N.
+    60 constraints x N_P* = 10 exceeds the buffer's 512 rows, so that member takes the fp64 ladder inside the same launch.
+    Every member equals its own single-instance launch, and the plain fp64 kernel, bit for bit."""
+    import torch
+    insts = [I.make_custom_reproj(5, 311), I.make_instance(3, 2), I.make_custom_reproj(23, 312), I.make_custom_reproj(60, 313)]
+    P = _small(insts[1].params, mode=I.MODE_TRANS, n_p=150, n_p_star=10, n_t=10)
+    hs, hx = [], []
+    try:
+        for it in insts:
+            for flags, lst in ((0, hs), (1, hx)):
+                h = B.Closure.closure_create(it, _small(P, flags=flags))
+                h.closure_set_init(I.make_init_poses(it, 8))
+                lst.append(h)
+        smp, flag = B.closure_sample_batch(hs, 256, 30, [21, 22, 23, 24])
+        torch.cuda.synchronize()
+        for b, (h, x) in enumerate(zip(hs, hx)):
+            s1, f1 = h.closure_sample(256, 30, 21 + b)
+            s2, f2 = x.closure_sample(256, 30, 21 + b)
+            torch.cuda.synchronize()
+            assert np.array_equal(s1.cpu().numpy(), smp[b].cpu().numpy()), b
+            assert np.array_equal(f1.cpu().numpy(), flag[b].cpu().numpy()), b
+            assert np.array_equal(s2.cpu().numpy(), smp[b].cpu().numpy()), b
+            assert np.array_equal(f2.cpu().numpy(), flag[b].cpu().numpy()), b
+    finally:
+        for h in hs + hx:
+            h.closure_destroy()
