@@ -4,7 +4,8 @@ Random config, instance, walk parameters, |S_0|, mode and seed per run; samples 
 (The same loop ran for 15 minutes twice in round 1, the second time on the final build with random bound runs and
 body pivots as below: 8,349 + 8,080 runs, 68 M + 66 M walkers, and for 10 minutes on the last build of the round: 9,720
 runs; no mismatch -- DESIGN.md 8.  Round 2 added streams 3 and 4 for the branch-and-bound kernel, N_P <= 32, and stream 5 for
-the ellipsoid / ellipse norms, and ran the loop again on the final build.)"""
+the ellipsoid / ellipse norms, and ran the loop again on the final build; after the last two changes of the
+translation sampler a loop of the same kind over config 3 in TRANS mode alone ran for 8 + 9 minutes: 14,340 + 16,119 runs.)"""
 import copy
 
 import numpy as np
